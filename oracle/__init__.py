@@ -1,0 +1,181 @@
+"""CPU oracle for the TNRD hot path -- TEST INFRASTRUCTURE, not product code.
+
+Thin ctypes binding of ``oracle/tnrd_oracle.c`` (plain C, IEEE double, libm exp; the header
+of that file states what it follows in PAPER.md and what pins it).  Only ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs
+may import this package.  It imports nothing from ``paper_1503_05768_b200`` and that package
+imports nothing from here.
+
+All arrays are promoted to float64 (exact for float32 inputs) before the call; results are
+float64.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tnrd_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle_tnrd.so")
+
+SYMMETRIC_2R = 0   # reading A, the default boundary handling
+ZERO_SAME = 1      # Main Eq. 2 with K^T under zero padding -- pins only
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc -O2 (no fast-math).  Building the checker is not using it."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        dp = ctypes.POINTER(ctypes.c_double)
+        ci, cd = ctypes.c_int, ctypes.c_double
+        lib.oracle_num_threads.restype = ci
+        lib.oracle_set_num_threads.argtypes = [ci]
+        lib.oracle_mirror.argtypes = [ci, ci]
+        lib.oracle_mirror.restype = ci
+        lib.oracle_pad.argtypes = [dp, ci, ci, ci, ci, dp]
+        lib.oracle_pad.restype = None
+        lib.oracle_conv_valid.argtypes = [dp, ci, ci, dp, ci, dp]
+        lib.oracle_conv_valid.restype = None
+        lib.oracle_corr_valid.argtypes = [dp, ci, ci, dp, ci, dp]
+        lib.oracle_corr_valid.restype = None
+        lib.oracle_phi.argtypes = [dp, ctypes.c_size_t, dp, dp, ci, cd, dp]
+        lib.oracle_phi.restype = None
+        lib.oracle_stage.argtypes = [dp, dp, ci, ci, ci, ci, ci, dp, dp, dp, ci, cd, cd, dp, ci]
+        lib.oracle_stage.restype = ci
+        lib.oracle_diffuse.argtypes = [dp, dp, ci, ci, ci, ci, ci, ci, dp, dp, dp, ci, cd, dp, dp, ci]
+        lib.oracle_diffuse.restype = ci
+        _lib = lib
+    return _lib
+
+
+def _d(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _p(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    _load().oracle_set_num_threads(int(n))
+
+
+def mirror(q: int, n: int) -> int:
+    """O1 mirror map (edge pixel repeated)."""
+    return int(_load().oracle_mirror(int(q), int(n)))
+
+
+def pad(u, p: int, symmetric: bool = True):
+    u = _d(u)
+    H, W = u.shape
+    out = np.empty((H + 2 * p, W + 2 * p), dtype=np.float64)
+    _load().oracle_pad(_p(u), H, W, int(p), int(bool(symmetric)), _p(out))
+    return out
+
+
+def conv_valid(img, k):
+    """O2: true convolution, valid extent."""
+    img, k = _d(img), _d(k)
+    K = k.shape[0]
+    out = np.empty((img.shape[0] - K + 1, img.shape[1] - K + 1), dtype=np.float64)
+    _load().oracle_conv_valid(_p(img), img.shape[0], img.shape[1], _p(k), K, _p(out))
+    return out
+
+
+def corr_valid(img, k):
+    """O4: convolution with rot180(k) == correlation with k, valid extent."""
+    img, k = _d(img), _d(k)
+    K = k.shape[0]
+    out = np.empty((img.shape[0] - K + 1, img.shape[1] - K + 1), dtype=np.float64)
+    _load().oracle_corr_valid(_p(img), img.shape[0], img.shape[1], _p(k), K, _p(out))
+    return out
+
+
+def phi(z, w, mu, gamma: float):
+    """O3: Gaussian-RBF influence function, point-wise."""
+    z, w, mu = _d(z), _d(w), _d(mu)
+    out = np.empty_like(z)
+    _load().oracle_phi(_p(z), z.size, _p(w), _p(mu), mu.size, float(gamma), _p(out))
+    return out
+
+
+def _img3(a):
+    a = _d(a)
+    if a.ndim == 2:
+        a = a[None]
+    assert a.ndim == 3, "images are [B][H][W] or [H][W]"
+    return a
+
+
+def stage(f, u_in, filters_t, rbf_w_t, rbf_mu, rbf_gamma: float, lambda_t: float,
+          mode: int = SYMMETRIC_2R):
+    """One stage (O1-O5) on a batch; returns float64 [B][H][W]."""
+    f3, u3 = _img3(f), _img3(u_in)
+    k, w, mu = _d(filters_t), _d(rbf_w_t), _d(rbf_mu)
+    B, H, W = u3.shape
+    n_k, K = k.shape[0], k.shape[1]
+    assert f3.shape == u3.shape and k.shape == (n_k, K, K) and w.shape == (n_k, mu.size)
+    out = np.empty_like(u3)
+    rc = _load().oracle_stage(_p(f3), _p(u3), B, H, W, n_k, K, _p(k), _p(w), _p(mu), mu.size,
+                              float(rbf_gamma), float(lambda_t), _p(out), int(mode))
+    if rc != 0:
+        raise ValueError(f"oracle_stage failed with {rc}")
+    return out if np.ndim(u_in) == 3 else out[0]
+
+
+def diffuse(f, u0, filters, rbf_w, rbf_mu, rbf_gamma: float, lambdas, mode: int = SYMMETRIC_2R):
+    """T stages (O6); returns float64 [B][H][W]."""
+    f3, u3 = _img3(f), _img3(u0)
+    k, w, mu, lam = _d(filters), _d(rbf_w), _d(rbf_mu), _d(lambdas)
+    B, H, W = u3.shape
+    T = lam.size
+    if T > 0:
+        n_k, K = k.shape[1], k.shape[2]
+        assert k.shape == (T, n_k, K, K) and w.shape == (T, n_k, mu.size)
+    else:
+        n_k, K = 1, 1
+    assert f3.shape == u3.shape
+    out = np.empty_like(u3)
+    rc = _load().oracle_diffuse(_p(f3), _p(u3), B, H, W, T, n_k, K, _p(k), _p(w), _p(mu), mu.size,
+                                float(rbf_gamma), _p(lam), _p(out), int(mode))
+    if rc != 0:
+        raise ValueError(f"oracle_diffuse failed with {rc}")
+    return out if np.ndim(u0) == 3 else out[0]
+
+
+def diffuse_window(f, u0, filters, rbf_w, rbf_mu, rbf_gamma, lambdas, y0, x0, h, w):
+    """u_T restricted to the window [y0,y0+h) x [x0,x0+w) of ONE image, from a crop.
+
+    The update is local: u_T inside a window depends only on u0, f within 2r*T pixels of it
+    (mirror-extended at true image borders).  The crop keeps a 2r*T margin and cuts it off
+    only where it reaches a real image border (where the crop border IS the image border, so
+    the mirror extension is the true one).  Everything is still computed by diffuse().
+    """
+    f2, u2 = _d(f), _d(u0)
+    assert f2.ndim == 2
+    H, W = f2.shape
+    T = int(np.size(lambdas))
+    K = int(np.shape(filters)[-1])
+    m = (K - 1) * T            # 2 r T
+    ya, yb = max(0, y0 - m), min(H, y0 + h + m)
+    xa, xb = max(0, x0 - m), min(W, x0 + w + m)
+    res = diffuse(f2[ya:yb, xa:xb], u2[ya:yb, xa:xb], filters, rbf_w, rbf_mu, rbf_gamma, lambdas)
+    return res[y0 - ya:y0 - ya + h, x0 - xa:x0 - xa + w]

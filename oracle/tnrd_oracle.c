@@ -1,0 +1,241 @@
+/*
+ * tnrd_oracle.c -- CPU ORACLE for the TNRD inference hot path.  TEST INFRASTRUCTURE ONLY.
+ *
+ * Plain, slow, double-precision transcription of the stage update of
+ *   Chen, Yu, Pock, "On learning optimized reaction diffusion processes for effective
+ *   image restoration" (arXiv 1503.05768), Main Eq. 7 with the boundary
+ *   handling of Supp. Sec. 1:
+ *
+ *     u_t = u_{t-1} - ( sum_i  kbar_i^t * phi_i^t( k_i^t * u_{t-1} )  +  lambda^t (u_{t-1} - f) )
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may build, link or call this file.  It shares no code, header, table or helper with the
+ * CUDA library (paper_1503_05768_b200/csrc) and neither includes the other.
+ *
+ * The method is its own definition, so the oracle follows it step by step (O1..O6 below,
+ * DESIGN.md "Readings"), every intermediate image materialised, no tiling, no fusion, no
+ * lookup table, no truncation of the 63-term sum, libm exp(), IEEE double, no -ffast-math.
+ * The only concession to run time is an OpenMP "parallel for" over rows of an image; it
+ * does not change the order of any floating-point sum.
+ *
+ * Pins (tests/test_oracle_pins.py, all "-m 'not gpu'"): P1 delta response, P2 constant
+ * image invariant, P3 closed form of phi for one non-zero weight, P4 adjoint identity under
+ * zero padding, P5 finite-difference of the FoE energy (erf closed form), P6 linear-phi
+ * special case against scipy.signal, P7 dense-matrix brute force on 8x8, P8 literal
+ * pad-omega/crop procedure for several omega, P9 flip/transpose equivariance, P12 degenerate
+ * parameters, P13 interior shift-equivariance.  Absolute end-to-end values for the
+ * BASELINE.json configs are "parity unpinned by the paper" (no printed example, no weights).
+ *
+ * Layouts: images row-major [B][H][W] (x fastest); filters [N_k][K][K] with k[a][b],
+ * a = row, b = column; rbf_w [N_k][M]; rbf_mu [M].
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORACLE_OK 0
+#define ORACLE_ERR_ARG (-1)
+#define ORACLE_ERR_MEM (-2)
+
+/* mode of boundary handling */
+#define ORACLE_SYMMETRIC_2R 0 /* reading A (default): mirror-extend u by 2r, two valid convolutions, crop */
+#define ORACLE_ZERO_SAME 1    /* Main Eq. 2 with K^T under zero padding; used by pins P1, P4, P5 only */
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void oracle_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* O1 mirror map (PAPER.md:383 "pad ... with mirror reflections of itself"; :387 "symmetric
+ * boundary condition").  Half-sample symmetric, edge pixel repeated:  ... b a | a b ...
+ * valid for -n <= q < 2n. */
+int oracle_mirror(int q, int n)
+{
+    if (q < 0) return -1 - q;
+    if (q >= n) return 2 * n - 1 - q;
+    return q;
+}
+
+/* Extend an H x W image by p pixels on every side.  symmetric != 0: mirror map; else zeros.
+ * up has (H+2p) x (W+2p) elements. */
+void oracle_pad(const double *u, int H, int W, int p, int symmetric, double *up)
+{
+    const int Hp = H + 2 * p, Wp = W + 2 * p;
+    for (int y = 0; y < Hp; ++y) {
+        for (int x = 0; x < Wp; ++x) {
+            const int sy = y - p, sx = x - p;
+            double val;
+            if (symmetric) {
+                val = u[(size_t)oracle_mirror(sy, H) * W + oracle_mirror(sx, W)];
+            } else {
+                val = (sy >= 0 && sy < H && sx >= 0 && sx < W) ? u[(size_t)sy * W + sx] : 0.0;
+            }
+            up[(size_t)y * Wp + x] = val;
+        }
+    }
+}
+
+/* O2 forward filter: TRUE 2-D convolution (kernel flipped), "valid" extent (PAPER.md:70,
+ * "K_i u <=> k_i * u").  in is Hin x Win, out is (Hin-K+1) x (Win-K+1):
+ *   out[y][x] = sum_{a,b} k[a][b] * in[y + (K-1) - a][x + (K-1) - b]                    */
+void oracle_conv_valid(const double *in, int Hin, int Win, const double *k, int K, double *out)
+{
+    const int Ho = Hin - K + 1, Wo = Win - K + 1;
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < Ho; ++y) {
+        for (int x = 0; x < Wo; ++x) {
+            double acc = 0.0;
+            for (int a = 0; a < K; ++a)
+                for (int b = 0; b < K; ++b)
+                    acc += k[a * K + b] * in[(size_t)(y + (K - 1) - a) * Win + (x + (K - 1) - b)];
+            out[(size_t)y * Wo + x] = acc;
+        }
+    }
+}
+
+/* O4 transposed filter: convolution with kbar = rot180(k), i.e. correlation
+ * with k, "valid" extent:
+ *   out[y][x] = sum_{a,b} k[a][b] * in[y + a][x + b]                                    */
+void oracle_corr_valid(const double *in, int Hin, int Win, const double *k, int K, double *out)
+{
+    const int Ho = Hin - K + 1, Wo = Win - K + 1;
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < Ho; ++y) {
+        for (int x = 0; x < Wo; ++x) {
+            double acc = 0.0;
+            for (int a = 0; a < K; ++a)
+                for (int b = 0; b < K; ++b)
+                    acc += k[a * K + b] * in[(size_t)(y + a) * Win + (x + b)];
+            out[(size_t)y * Wo + x] = acc;
+        }
+    }
+}
+
+/* O3 influence function, Gaussian RBF mixture (PAPER.md:113-117 Eq. 6; :553 phi_g):
+ *   phi(z) = sum_{j=1..M} w_j exp( -(z - mu_j)^2 / (2 gamma^2) )                        */
+double oracle_phi1(double z, const double *w, const double *mu, int M, double gamma)
+{
+    double acc = 0.0;
+    for (int j = 0; j < M; ++j) {
+        const double d = z - mu[j];
+        acc += w[j] * exp(-(d * d) / (2.0 * gamma * gamma));
+    }
+    return acc;
+}
+
+void oracle_phi(const double *z, size_t n, const double *w, const double *mu, int M, double gamma,
+                double *v)
+{
+#pragma omp parallel for schedule(static)
+    for (long long p = 0; p < (long long)n; ++p) v[p] = oracle_phi1(z[p], w, mu, M, gamma);
+}
+
+/* One stage for one image (O1..O5). */
+static int stage_one(const double *f, const double *u, int H, int W, int N_k, int K,
+                     const double *filters, const double *rbf_w, const double *rbf_mu, int M,
+                     double gamma, double lambda, double *u_out, int mode)
+{
+    const int r = (K - 1) / 2;
+    int Hu, Wu, Hz, Wz; /* extended u; z and v maps */
+    if (mode == ORACLE_SYMMETRIC_2R) {
+        Hu = H + 4 * r; Wu = W + 4 * r; Hz = H + 2 * r; Wz = W + 2 * r;
+    } else {
+        Hu = H + 2 * r; Wu = W + 2 * r; Hz = H; Wz = W;
+    }
+    const int Hv = H + 2 * r, Wv = W + 2 * r; /* v as seen by the transposed filter */
+    double *ue = (double *)malloc(sizeof(double) * (size_t)Hu * Wu);
+    double *z = (double *)malloc(sizeof(double) * (size_t)Hz * Wz);
+    double *v = (double *)malloc(sizeof(double) * (size_t)Hz * Wz);
+    double *ve = (double *)malloc(sizeof(double) * (size_t)Hv * Wv);
+    double *si = (double *)malloc(sizeof(double) * (size_t)H * W);
+    double *s = (double *)calloc((size_t)H * W, sizeof(double));
+    if (!ue || !z || !v || !ve || !si || !s) {
+        free(ue); free(z); free(v); free(ve); free(si); free(s);
+        return ORACLE_ERR_MEM;
+    }
+    /* O1 */
+    if (mode == ORACLE_SYMMETRIC_2R) oracle_pad(u, H, W, 2 * r, 1, ue);
+    else oracle_pad(u, H, W, r, 0, ue);
+
+    for (int i = 0; i < N_k; ++i) {
+        const double *k = filters + (size_t)i * K * K;
+        oracle_conv_valid(ue, Hu, Wu, k, K, z);                              /* O2 */
+        oracle_phi(z, (size_t)Hz * Wz, rbf_w + (size_t)i * M, rbf_mu, M, gamma, v); /* O3 */
+        const double *vin = v;
+        if (mode == ORACLE_ZERO_SAME) { /* v = 0 outside the image: this is K_i^T v */
+            oracle_pad(v, H, W, r, 0, ve);
+            vin = ve;
+        }
+        oracle_corr_valid(vin, Hv, Wv, k, K, si);                            /* O4 */
+        for (size_t p = 0; p < (size_t)H * W; ++p) s[p] += si[p];            /* sum over i */
+    }
+    /* O5 */
+    for (size_t p = 0; p < (size_t)H * W; ++p) u_out[p] = u[p] - (s[p] + lambda * (u[p] - f[p]));
+
+    free(ue); free(z); free(v); free(ve); free(si); free(s);
+    return ORACLE_OK;
+}
+
+static int check_shape(int B, int H, int W, int N_k, int K, int M)
+{
+    if (B < 1 || H < 1 || W < 1 || N_k < 1 || M < 1) return ORACLE_ERR_ARG;
+    if (K < 1 || (K % 2) == 0) return ORACLE_ERR_ARG;
+    if (H < K - 1 || W < K - 1) return ORACLE_ERR_ARG; /* mirror source must exist: min(H,W) >= 2r */
+    return ORACLE_OK;
+}
+
+/* One stage on a batch.  u_out must not alias u_in or f. */
+int oracle_stage(const double *f, const double *u_in, int B, int H, int W, int N_k, int K,
+                 const double *filters_t, const double *rbf_w_t, const double *rbf_mu, int M,
+                 double gamma, double lambda_t, double *u_out, int mode)
+{
+    if (!f || !u_in || !filters_t || !rbf_w_t || !rbf_mu || !u_out) return ORACLE_ERR_ARG;
+    if (check_shape(B, H, W, N_k, K, M) != ORACLE_OK || !(gamma > 0.0)) return ORACLE_ERR_ARG;
+    for (int b = 0; b < B; ++b) {
+        const size_t off = (size_t)b * H * W;
+        int rc = stage_one(f + off, u_in + off, H, W, N_k, K, filters_t, rbf_w_t, rbf_mu, M, gamma,
+                           lambda_t, u_out + off, mode);
+        if (rc != ORACLE_OK) return rc;
+    }
+    return ORACLE_OK;
+}
+
+/* O6: T stages with per-stage parameters Theta_t.  T = 0 copies u0. */
+int oracle_diffuse(const double *f, const double *u0, int B, int H, int W, int T, int N_k, int K,
+                   const double *filters, const double *rbf_w, const double *rbf_mu, int M,
+                   double gamma, const double *lambda, double *out, int mode)
+{
+    if (!f || !u0 || !out || T < 0) return ORACLE_ERR_ARG;
+    if (T > 0 && (!filters || !rbf_w || !rbf_mu || !lambda)) return ORACLE_ERR_ARG;
+    if (check_shape(B, H, W, N_k, K, M) != ORACLE_OK || !(gamma > 0.0)) return ORACLE_ERR_ARG;
+    const size_t n = (size_t)B * H * W;
+    double *cur = (double *)malloc(sizeof(double) * n);
+    double *nxt = (double *)malloc(sizeof(double) * n);
+    if (!cur || !nxt) { free(cur); free(nxt); return ORACLE_ERR_MEM; }
+    memcpy(cur, u0, sizeof(double) * n);
+    for (int t = 0; t < T; ++t) {
+        int rc = oracle_stage(f, cur, B, H, W, N_k, K, filters + (size_t)t * N_k * K * K,
+                              rbf_w + (size_t)t * N_k * M, rbf_mu, M, gamma, lambda[t], nxt, mode);
+        if (rc != ORACLE_OK) { free(cur); free(nxt); return rc; }
+        double *tmp = cur; cur = nxt; nxt = tmp;
+    }
+    memcpy(out, cur, sizeof(double) * n);
+    free(cur); free(nxt);
+    return ORACLE_OK;
+}
