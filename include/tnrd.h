@@ -1,0 +1,124 @@
+/*
+ * tnrd.h -- C ABI of libtnrd: the inference hot path of the trained nonlinear
+ * reaction-diffusion model (TNRD) of Chen, Yu & Pock, arXiv 1503.05768, on NVIDIA B200 (sm_100a).
+ *
+ * The library computes, per stage t = 1..T (Main Eq. 7; Supp. Eq. 2):
+ *
+ *     u_t = u_{t-1} - ( sum_{i=1..N_k} kbar_i^t * phi_i^t( k_i^t * u_{t-1} ) + lambda^t (u_{t-1} - f) )
+ *
+ *   k_i * u      true 2-D convolution with the ksize x ksize filter k_i
+ *   phi_i(z)     = sum_{j=1..63} w_ij exp( -(z - mu_j)^2 / (2 gamma^2) )        (Main Eq. 6, :113-117; :553)
+ *   kbar_i       = k_i rotated by 180 degrees
+ *   boundary     u_{t-1} is extended by 2r (r = (ksize-1)/2) with mirror reflections (edge pixel
+ *                repeated), both filterings are "valid", the result is the H x W centre -- the
+ *                pad / diffuse / crop procedure of Supp. Sec. 1, which is the same
+ *                for every pad width omega >= 2r (reading S1).
+ *
+ * All arithmetic is IEEE fp32 (FMA contraction, any summation order, ex2.approx for the exponential);
+ * results are deterministic run to run.  Nothing here allocates or reads through PyTorch; callers hand
+ * in raw pointers.
+ *
+ * Conventions common to all entry points
+ *   - Images are dense row-major float32 [B][H][W] (x fastest).  filters [T][N_k][ksize][ksize] with
+ *     k[a][b], a = row, b = column.  rbf_w [T][N_k][63].  rbf_mu [63].  lambda [T].
+ *   - "device pointer": memory of the CURRENT CUDA device (cudaMalloc / torch allocator), 4-byte aligned.
+ *     "host pointer": ordinary or pinned host memory.
+ *   - Ownership: the caller owns every buffer and keeps device buffers alive until the work queued on
+ *     `stream` has completed.  The library owns only an internal per-device scratch (one ping-pong plane of
+ *     B*H*W floats plus a parameter staging block), grown on demand and released by tnrd_shutdown().
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device entry points
+ *     are asynchronous on `stream` and never synchronise the device.
+ *   - Every function returning int returns TNRD_OK (0) or a negative tnrd_status.  Nothing throws.
+ *     Errors found while validating or launching are returned; asynchronous faults surface at the
+ *     caller's next synchronisation.  On error no output is written.
+ *   - Shapes: B,H,W >= 1, B*H*W < 2^31; ksize in {3,5,7,9}; 1 <= N_k <= 128; min(H,W) >= ksize-1 (the
+ *     mirror source must lie inside the image); T >= 0.
+ */
+#ifndef TNRD_H_
+#define TNRD_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TNRD_NUM_RBF 63 /* M, PAPER.md:176 ("63 Gaussian RBFs") -- fixed by the model family */
+#define TNRD_MAX_FILTERS 128
+#define TNRD_VERSION 100 /* 0.1.0 */
+
+typedef enum {
+    TNRD_OK = 0,
+    TNRD_ERR_NULL = -1,        /* a required pointer is NULL */
+    TNRD_ERR_SHAPE = -2,       /* B/H/W/T/N_k out of range, image smaller than the 2r halo, too many pixels */
+    TNRD_ERR_UNSUPPORTED = -3, /* ksize not in {3,5,7,9}; unknown option */
+    TNRD_ERR_ALIAS = -4,       /* output aliases an input it must not alias */
+    TNRD_ERR_CUDA = -5,        /* a CUDA call failed; see tnrd_last_cuda_error() */
+    TNRD_ERR_PARAM = -6        /* rbf_gamma not finite or <= 0 */
+} tnrd_status;
+
+/*
+ * One stage (rows a1-a5 of the hot path; Main Eq. 7).
+ *   f, u_in     device, [B][H][W]   noisy image f_n and previous iterate u_{t-1}
+ *   filters_t   device, [N_k][ksize][ksize]      k_i^t
+ *   rbf_w_t     device, [N_k][63]                w_ij^t
+ *   rbf_mu      device, [63]                     mu_j (any values; equidistant in the paper, :117)
+ *   rbf_gamma   by value, > 0 and finite         shared width gamma (:117 "unified scaling", :553)
+ *   lambda_t    by value                          reaction weight lambda^t
+ *   u_out       device, [B][H][W]   u_t; must not be u_in or f (halo reads) -> TNRD_ERR_ALIAS on pointer
+ *               equality; partial overlap is undefined behaviour.
+ */
+int tnrd_stage(const float* f, const float* u_in, int B, int H, int W, int N_k, int ksize,
+               const float* filters_t, const float* rbf_w_t, const float* rbf_mu, float rbf_gamma,
+               float lambda_t, float* u_out, void* stream);
+
+/*
+ * T stages with per-stage parameters Theta_t = {lambda^t, phi_i^t, k_i^t} (row a6).
+ *   f, u0       device, [B][H][W]; the paper starts from u0 = f (Main Fig. 2)
+ *   filters     device, [T][N_k][ksize][ksize];  rbf_w device [T][N_k][63];  rbf_mu device [63]
+ *   lambda      device, [T]  (device so that the call needs no host sync and can be graph-captured)
+ *   out         device, [B][H][W]; receives u_T.  out may equal u0 (in place); out must not equal f.
+ *   T = 0 copies u0 to out.
+ * Stages ping-pong between `out` and the internal scratch so that the last stage writes `out`.
+ */
+int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, int N_k, int ksize,
+                 const float* filters, const float* rbf_w, const float* rbf_mu, float rbf_gamma,
+                 const float* lambda, float* out, void* stream);
+
+/*
+ * End-to-end variant with HOST buffers: every pointer below is a host pointer (pinned memory makes the
+ * copies asynchronous).  Copies f, u0 and the parameters to the device, runs tnrd_diffuse on `stream`,
+ * copies u_T back to `out` and synchronises `stream` before returning.  f == u0 (same host pointer) is
+ * uploaded once.  Device staging buffers are cached in the library scratch.
+ */
+int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int T, int N_k, int ksize,
+                      const float* filters, const float* rbf_w, const float* rbf_mu, float rbf_gamma,
+                      const float* lambda, float* out, void* stream);
+
+/*
+ * Kernel selection, for tests and profiling.  which = 0: automatic (default); 1: the plain one-thread-per-
+ * pixel reference kernel (global memory only); 2: the fused tiled stage kernel.  Returns TNRD_ERR_UNSUPPORTED
+ * for other values.  Process-wide.
+ */
+int tnrd_set_kernel(int which);
+
+/* Number of kernels this library has launched since load (or since the last tnrd_reset_launch_count). */
+unsigned long long tnrd_launch_count(void);
+void tnrd_reset_launch_count(void);
+
+/*
+ * Roofline denominators measured on the current device: register-only micro-kernels
+ * timed with CUDA events on `stream`; synchronises `stream`.
+ *   which = 0: FP32 FFMA rate      -> *rate = FMA lane-operations per second (x2 = FLOP/s)
+ *   which = 1: MUFU.EX2 rate       -> *rate = ex2 evaluations per second
+ *   which = 2: the phi inner loop (FADD, FMUL, MUFU.EX2, FFMA per term) -> RBF terms per second
+ */
+int tnrd_microbench(int which, double* rate, void* stream);
+
+const char* tnrd_strerror(int status);
+const char* tnrd_last_cuda_error(void); /* message of the last failing CUDA call on this thread, "" if none */
+int tnrd_version(void);
+void tnrd_shutdown(void); /* frees the cached scratch of every device; the library stays usable */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TNRD_H_ */

@@ -1,0 +1,155 @@
+"""paper_1503_05768_b200 -- thin Python binding of libtnrd (include/tnrd.h).
+
+The hot path of the trained nonlinear reaction-diffusion model (Chen, Yu, Pock, arXiv 1503.05768, Main
+Eq. 7) runs entirely inside the hand-written sm_100a kernels of ``libtnrd.so``.  This module
+only marshals arguments: it loads the shared library with ``ctypes`` and passes ``tensor.data_ptr()`` and the
+current CUDA stream.  PyTorch supplies device memory and streams, nothing else.  There is NO CPU fallback:
+if the library is missing, loading fails loudly.
+
+Function names and argument order are those of the C ABI.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtnrd.so")
+NUM_RBF = 63
+
+OK, ERR_NULL, ERR_SHAPE, ERR_UNSUPPORTED, ERR_ALIAS, ERR_CUDA, ERR_PARAM = 0, -1, -2, -3, -4, -5, -6
+
+_lib = None
+
+
+class TnrdError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"libtnrd status {status}: {msg}")
+        self.status = status
+
+
+def build(verbose: bool = False) -> str:
+    """Compile libtnrd.so in-tree for sm_100a (nvcc cross-compiles without a GPU)."""
+    import importlib
+    _b = importlib.import_module(__name__ + ".build")   # the submodule, not this function
+    return _b.build(verbose=verbose)
+
+
+def lib() -> ctypes.CDLL:
+    """Load libtnrd.so (raises if it has not been built -- never falls back to anything else)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_1503_05768_b200.build` "
+                "(there is no CPU fallback for the TNRD hot path)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, ci, cf = ctypes.c_void_p, ctypes.c_int, ctypes.c_float
+        L.tnrd_stage.argtypes = [vp, vp, ci, ci, ci, ci, ci, vp, vp, vp, cf, cf, vp, vp]
+        L.tnrd_stage.restype = ci
+        dargs = [vp, vp, ci, ci, ci, ci, ci, ci, vp, vp, vp, cf, vp, vp, vp]
+        L.tnrd_diffuse.argtypes = dargs
+        L.tnrd_diffuse.restype = ci
+        L.tnrd_diffuse_host.argtypes = dargs
+        L.tnrd_diffuse_host.restype = ci
+        L.tnrd_set_kernel.argtypes = [ci]
+        L.tnrd_set_kernel.restype = ci
+        L.tnrd_launch_count.restype = ctypes.c_ulonglong
+        L.tnrd_reset_launch_count.restype = None
+        L.tnrd_microbench.argtypes = [ci, ctypes.POINTER(ctypes.c_double), vp]
+        L.tnrd_microbench.restype = ci
+        L.tnrd_strerror.argtypes = [ci]
+        L.tnrd_strerror.restype = ctypes.c_char_p
+        L.tnrd_last_cuda_error.restype = ctypes.c_char_p
+        L.tnrd_version.restype = ci
+        L.tnrd_shutdown.restype = None
+        _lib = L
+    return _lib
+
+
+def _ptr(x):
+    """Raw address of a torch tensor / numpy array / int / None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if hasattr(x, "ctypes"):
+        return x.ctypes.data
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream
+
+
+def _check(rc: int):
+    if rc != 0:
+        L = lib()
+        msg = L.tnrd_strerror(rc).decode()
+        if rc == ERR_CUDA:
+            msg += " -- " + L.tnrd_last_cuda_error().decode()
+        raise TnrdError(rc, msg)
+
+
+def tnrd_stage(f, u_in, B, H, W, N_k, ksize, filters_t, rbf_w_t, rbf_mu, rbf_gamma, lambda_t, u_out,
+               stream=None):
+    """One stage on device buffers (include/tnrd.h: tnrd_stage)."""
+    _check(lib().tnrd_stage(_ptr(f), _ptr(u_in), B, H, W, N_k, ksize, _ptr(filters_t), _ptr(rbf_w_t),
+                            _ptr(rbf_mu), float(rbf_gamma), float(lambda_t), _ptr(u_out), _stream(stream)))
+    return u_out
+
+
+def tnrd_diffuse(f, u0, B, H, W, T, N_k, ksize, filters, rbf_w, rbf_mu, rbf_gamma, lam, out, stream=None):
+    """T stages on device buffers (include/tnrd.h: tnrd_diffuse)."""
+    _check(lib().tnrd_diffuse(_ptr(f), _ptr(u0), B, H, W, T, N_k, ksize, _ptr(filters), _ptr(rbf_w),
+                              _ptr(rbf_mu), float(rbf_gamma), _ptr(lam), _ptr(out), _stream(stream)))
+    return out
+
+
+def tnrd_diffuse_host(f, u0, B, H, W, T, N_k, ksize, filters, rbf_w, rbf_mu, rbf_gamma, lam, out,
+                      stream=None):
+    """T stages on HOST buffers, copies included (include/tnrd.h: tnrd_diffuse_host)."""
+    _check(lib().tnrd_diffuse_host(_ptr(f), _ptr(u0), B, H, W, T, N_k, ksize, _ptr(filters), _ptr(rbf_w),
+                                   _ptr(rbf_mu), float(rbf_gamma), _ptr(lam), _ptr(out), _stream(stream)))
+    return out
+
+
+def tnrd_set_kernel(which: int):
+    _check(lib().tnrd_set_kernel(int(which)))
+
+
+def tnrd_launch_count() -> int:
+    return int(lib().tnrd_launch_count())
+
+
+def tnrd_reset_launch_count():
+    lib().tnrd_reset_launch_count()
+
+
+def tnrd_microbench(which: int, stream=None) -> float:
+    r = ctypes.c_double(0.0)
+    _check(lib().tnrd_microbench(int(which), ctypes.byref(r), _stream(stream)))
+    return r.value
+
+
+def tnrd_strerror(status: int) -> str:
+    return lib().tnrd_strerror(int(status)).decode()
+
+
+def tnrd_last_cuda_error() -> str:
+    return lib().tnrd_last_cuda_error().decode()
+
+
+def tnrd_version() -> int:
+    return int(lib().tnrd_version())
+
+
+def tnrd_shutdown():
+    lib().tnrd_shutdown()
