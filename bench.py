@@ -1,0 +1,279 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of libtnrd on B200:  Mpixel-stages/s of the 48-filter 7x7, T=5 TNRD model.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--size 4096] [--T 5]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 ... bench.py --gpus N
+
+A "step" is one pass of the whole hot path (rows a1-a6 of DESIGN.md: T fused stage launches of
+tnrd_diffuse) over one synthetic noisy image of BASELINE.json configs[3] (size x size, sigma 25).  One process
+per GPU; with N > 1 every rank runs the same workload on its own image (independent problems, no data-path
+collective -> weak scaling); the time is the max over ranks of a CUDA-event interval bracketed by barrier +
+synchronize.  Prints ONE JSON line on rank 0.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the box's host cores on a bounded sample of
+the same workload; see DESIGN.md "Measurement".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import tnrd_gen  # noqa: E402
+
+METRIC = "Mpixel-stages/s"
+N_K, KSIZE, M = 48, 7, 63
+EX2_PER_PX_STAGE = N_K * M                       # 3024 MUFU.EX2 per pixel-stage (dense phi)
+FMA_PER_PX_STAGE = 2 * N_K * KSIZE * KSIZE       # 4704 FFMA of filtering
+FLOP_PER_PX_STAGE = 2 * FMA_PER_PX_STAGE + 5 * EX2_PER_PX_STAGE   # per RBF term: sub, mul, ex2, fma(2) -> 24528
+NOMINAL_SM_MHZ, NOMINAL_SMS, MUFU_PER_CLK_SM = 1965.0, 148, 16
+# dram bytes per fused-stage launch from profiles/ (ncu --set full); None until captured
+TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def read_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return {}
+
+
+class ClockSampler:
+    """Samples nvidia-smi SM clock and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+                for nm, val in zip(names, r[3:7]):
+                    if val.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        # keep samples taken under load (clock above idle); fall back to all samples
+        busy = [c for c in sm if c > 0.6 * mx] or sm
+        return {"sm_mhz": float(np.median(busy)) if busy else None, "sm_max_mhz": mx or None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(cfg, cores_hint=None, target_s=12.0):
+    """Time the oracle on a bounded crop of the workload; returns (Mpx-stages/s, cores, sample text, seconds)."""
+    import oracle
+    cores = oracle.num_threads()
+    T = cfg["T"]
+    per_core = 50e-6                                   # ~47 us per 48x7x7 px-stage per core
+    px = max(48 * 48, int(target_s * cores / per_core / T))
+    side = int(min(cfg["H"], cfg["W"], max(48, int(px ** 0.5))))
+    y0, x0 = (cfg["H"] - side) // 2, (cfg["W"] - side) // 2
+    f = cfg["f"][0, y0:y0 + side, x0:x0 + side]
+    t0 = time.perf_counter()
+    out = oracle.diffuse(f, f, cfg["filters"], cfg["rbf_w"], cfg["rbf_mu"], cfg["rbf_gamma"], cfg["lambda"])
+    dt = time.perf_counter() - t0
+    assert np.all(np.isfinite(out))
+    val = side * side * T / dt / 1e6
+    return val, cores, f"centre {side}x{side} crop of the {cfg['H']}x{cfg['W']} image, all T={T} stages, {dt:.1f} s", dt
+
+
+def run_reference(args, rank):
+    """--impl reference: the oracle as it stands on the host cores; rank 0 only."""
+    if rank != 0:
+        return
+    cfg = tnrd_gen.make_config(4, size=args.size, T=args.T)
+    vals, secs, sample, cores = [], [], "", 1
+    for i in range(args.warmup + args.steps):
+        v, cores, sample, dt = oracle_sample(cfg, target_s=args.ref_seconds)
+        if i >= args.warmup:
+            vals.append(v); secs.append(dt)
+    value = float(np.mean(vals))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "Mpixel-stages/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(secs)),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"C4 {args.size}x{args.size} T={args.T} N_k=48 7x7 (BASELINE.json configs[3])",
+                   "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "Mpixel-stages/s", "cores": cores, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": "Mpixel-stages/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--size", type=int, default=4096)
+    ap.add_argument("--T", type=int, default=5)
+    ap.add_argument("--ref-seconds", type=float, default=8.0, help="CPU seconds per oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_1503_05768_b200 as tnrd
+    from paper_1503_05768_b200.shard import max_over_ranks, sum_over_ranks
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the TNRD hot path has no CPU fallback")
+    tnrd.build()
+    tnrd.lib()
+    torch.cuda.set_device(local_rank)
+    devs = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=devs)
+    warmup = max(args.warmup, 3)
+
+    cfg = tnrd_gen.make_config(4, size=args.size, T=args.T)
+    B, H, W, T = cfg["B"], cfg["H"], cfg["W"], cfg["T"]
+    f = torch.from_numpy(cfg["f"]).to(devs)
+    out = torch.empty_like(f)
+    k, w = torch.from_numpy(cfg["filters"]).to(devs), torch.from_numpy(cfg["rbf_w"]).to(devs)
+    mu, lam = torch.from_numpy(cfg["rbf_mu"]).to(devs), torch.from_numpy(cfg["lambda"]).to(devs)
+    gamma = cfg["rbf_gamma"]
+    stream = torch.cuda.current_stream()
+
+    def step():
+        tnrd.tnrd_diffuse(f, f, B, H, W, T, N_K, KSIZE, k, w, mu, gamma, lam, out, stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(warmup):
+        step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    tnrd.tnrd_reset_launch_count()
+    with ClockSampler(local_rank) as clocks:
+        e0.record(stream)
+        for _ in range(args.steps):
+            step()
+        e1.record(stream)
+        barrier()
+    launches = tnrd.tnrd_launch_count()
+    ms = max_over_ranks(e0.elapsed_time(e1), devs)
+    px_stages_all = sum_over_ranks(float(B) * H * W * T * args.steps, devs)
+    value = px_stages_all / (ms * 1e-3) / 1e6
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region -------------
+    hf = torch.from_numpy(cfg["f"]).pin_memory()
+    hout = torch.empty_like(hf).pin_memory()
+    hp = [cfg["filters"], cfg["rbf_w"], cfg["rbf_mu"], cfg["lambda"]]
+
+    def step_host():
+        tnrd.tnrd_diffuse_host(hf, hf, B, H, W, T, N_K, KSIZE, hp[0], hp[1], hp[2], gamma, hp[3], hout, stream)
+
+    step_host()
+    barrier()
+    e2e_steps = max(1, min(args.steps, 5))
+    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2.record(stream)
+    for _ in range(e2e_steps):
+        step_host()
+    e3.record(stream)
+    barrier()
+    ms_e2e = max_over_ranks(e2.elapsed_time(e3), devs)
+    e2e_value = sum_over_ranks(float(B) * H * W * T * e2e_steps, devs) / (ms_e2e * 1e-3) / 1e6
+    h2d = hf.numel() * 4 + sum(int(a.nbytes) for a in hp)
+    d2h = hout.numel() * 4
+    same = bool(torch.equal(hout.to(devs), out))
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (stage_fused_kernel): XU pipe, one MUFU.EX2 per RBF term ------------
+    launch_s = (ms * 1e-3) / (args.steps * T)           # step time / T: the staging kernel (~us) is charged too
+    achieved = EX2_PER_PX_STAGE * float(B) * H * W / launch_s / 1e12
+    peak_nominal = NOMINAL_SMS * MUFU_PER_CLK_SM * NOMINAL_SM_MHZ * 1e6 / 1e12
+    mb = {n: tnrd.tnrd_microbench(i) / 1e12 for i, n in enumerate(["ffma_T_per_s", "ex2_T_per_s", "phi_terms_T_per_s"])}
+    roofline = {
+        "bound": "alu", "pipe": "xu (MUFU.EX2)", "achieved": achieved, "peak": peak_nominal, "unit": "Tex2/s",
+        "frac": achieved / peak_nominal, "traffic": TRAFFIC_BYTES_PER_LAUNCH,
+        "peak_source": "148 SM x 16 MUFU/clk/SM x 1.965 GHz (DESIGN.md Roofline); measured by tnrd_microbench: "
+                       f"{mb['ex2_T_per_s']:.3f} Tex2/s",
+        "frac_of_measured_ex2": achieved / mb["ex2_T_per_s"], "microbench": mb,
+        "useful_tflops": FLOP_PER_PX_STAGE * float(B) * H * W / launch_s / 1e12,
+        "hbm_gbs_algorithmic": 12.0 * B * H * W / launch_s / 1e9, "hbm_peak_gbs": read_peaks().get("hbm_gbs"),
+        "launch_ms": launch_s * 1e3,
+    }
+    line = {
+        "metric": METRIC, "value": value, "unit": "Mpixel-stages/s", "n_gpus": world, "steps": args.steps,
+        "warmup": warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"C4 {H}x{W} T={T} N_k=48 7x7 M=63 (BASELINE.json configs[3]), one image per GPU",
+                   "global_batch": world * B, "parallelism": f"dp{world} (independent images, no collective)",
+                   "l2": "inputs larger than L2 (3 planes x %d MB)" % (H * W * 4 // 2 ** 20)},
+        "roofline": roofline, "clocks": clocks.summary(),
+        "e2e": {"value": e2e_value, "unit": "Mpixel-stages/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": e2e_steps, "matches_device_path": same},
+        "gpu_launches": int(launches),
+        "paper_context": "GTX 780 Ti: 54.2 Mpixel-stages/s at 3072^2 (PAPER.md:253), other hardware, LUT phi",
+    }
+    if not args.no_cpu_baseline and world == 1:
+        v, cores, sample, _ = oracle_sample(cfg, target_s=args.ref_seconds)
+        line["cpu_baseline"] = {"value": v, "unit": "Mpixel-stages/s", "cores": cores, "kind": "oracle",
+                                "sample": sample}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,220 @@
+"""GPU parity: libtnrd (through the C ABI binding) against the double-precision CPU oracle, element by
+element on the same seeded inputs.  Tolerance (BASELINE.json north_star (d)): max-abs <= 1e-2 and
+RMS <= 1e-3 on the 0..255 scale after all T stages."""
+import numpy as np
+import pytest
+
+import oracle
+import tnrd_gen
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+MAX_ABS, RMS = 1e-2, 1e-3
+
+
+@pytest.fixture(scope="module")
+def tnrd():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1503_05768_b200 as t
+    t.lib()                      # fails loudly if libtnrd.so is missing: no fallback
+    t.tnrd_set_kernel(0)
+    return t
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_gpu(tnrd, c, kernel=0, T=None, out=None, u0=None):
+    """tnrd_diffuse on config dict c; returns float64 numpy [B][H][W]."""
+    tnrd.tnrd_set_kernel(kernel)
+    T = c["T"] if T is None else T
+    f = dev(c["f"]); u0 = dev(c["u0"]) if u0 is None else u0
+    k, w, mu, lam = dev(c["filters"]), dev(c["rbf_w"]), dev(c["rbf_mu"]), dev(c["lambda"])
+    out = torch.empty_like(f) if out is None else out
+    tnrd.tnrd_diffuse(f, u0, c["B"], c["H"], c["W"], T, c["N_k"], c["ksize"], k, w, mu, c["rbf_gamma"], lam, out)
+    torch.cuda.synchronize()
+    tnrd.tnrd_set_kernel(0)
+    return out.cpu().numpy().astype(np.float64)
+
+
+def run_oracle(c, T=None):
+    T = c["T"] if T is None else T
+    return oracle.diffuse(c["f"], c["u0"], c["filters"][:T], c["rbf_w"][:T], c["rbf_mu"], c["rbf_gamma"],
+                          c["lambda"][:T])
+
+
+def check(got, want, what=""):
+    err = got - want
+    mx, rms = float(np.max(np.abs(err))), float(np.sqrt(np.mean(err ** 2)))
+    assert np.all(np.isfinite(got)), what
+    assert mx <= MAX_ABS and rms <= RMS, f"{what}: max-abs {mx:.3e} rms {rms:.3e}"
+    return mx, rms
+
+
+# --- small and ragged shapes, every ksize, both kernels: element by element ---------------------------------
+SMALL = [  # seed, B, H, W, T, N_k, ksize
+    (1, 1, 8, 8, 1, 3, 3), (2, 2, 13, 29, 2, 8, 3), (3, 1, 4, 4, 2, 4, 5), (4, 3, 37, 23, 2, 6, 5),
+    (5, 1, 6, 6, 1, 5, 7), (6, 2, 70, 50, 2, 7, 7), (7, 1, 8, 8, 1, 2, 9), (8, 1, 45, 61, 2, 4, 9),
+    (9, 1, 131, 140, 1, 5, 7), (10, 1, 2, 300, 1, 3, 3), (11, 1, 300, 2, 1, 3, 3), (12, 1, 64, 64, 1, 128, 3),
+]
+
+
+@pytest.mark.parametrize("kernel", [1, 2])
+@pytest.mark.parametrize("case", SMALL, ids=[f"s{c[0]}" for c in SMALL])
+def test_small_cases_match_oracle(tnrd, case, kernel):
+    seed, B, H, W, T, n_k, K = case
+    c = tnrd_gen.make_small(seed, B, H, W, T, n_k, K)
+    check(run_gpu(tnrd, c, kernel=kernel), run_oracle(c), f"case {case} kernel {kernel}")
+
+
+# --- BASELINE.json configs 1-3 in full ------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_configs_1_to_3_full_image(tnrd, cfg):
+    c = tnrd_gen.make_config(cfg)
+    want = run_oracle(c)
+    mx, rms = check(run_gpu(tnrd, c), want, f"config {cfg}")
+    print(f"config {cfg}: max-abs {mx:.3e} rms {rms:.3e}")
+    if cfg == 2:   # transposed orientation of the stand-in image (reading S14)
+        ct = dict(c, H=c["W"], W=c["H"], f=np.ascontiguousarray(c["f"].transpose(0, 2, 1)),
+                  u0=np.ascontiguousarray(c["u0"].transpose(0, 2, 1)),
+                  filters=np.ascontiguousarray(np.swapaxes(c["filters"], -1, -2)))
+        check(run_gpu(tnrd, ct).transpose(0, 2, 1), want, "config 2 transposed")
+
+
+# --- full sizes in the launch configuration bench.py times: sampled windows the oracle computes one by one --------
+def _windows(H, W, size, n_random, seed):
+    ys = [0, (H - size) // 2, H - size]
+    xs = [0, (W - size) // 2, W - size]
+    wins = [(y, x) for y in ys for x in xs]                      # 4 corners, 4 edge mid-points, centre
+    r = np.random.default_rng([7, seed])
+    wins += [(int(r.integers(0, H - size + 1)), int(r.integers(0, W - size + 1))) for _ in range(n_random)]
+    return wins
+
+
+def test_config4_4096_T5_sampled_windows(tnrd):
+    c = tnrd_gen.make_config(4, size=4096, T=5)
+    got = run_gpu(tnrd, c)[0]
+    assert np.all(np.isfinite(got))
+    worst = 0.0
+    for (y0, x0) in _windows(4096, 4096, 24, 4, 4):
+        want = oracle.diffuse_window(c["f"][0], c["u0"][0], c["filters"], c["rbf_w"], c["rbf_mu"],
+                                     c["rbf_gamma"], c["lambda"], y0, x0, 24, 24)
+        mx, _ = check(got[y0:y0 + 24, x0:x0 + 24], want, f"C4 window {(y0, x0)}")
+        worst = max(worst, mx)
+    print(f"config 4 (4096^2, T=5): worst window max-abs {worst:.3e}")
+    # tile seams: a window straddling the first tile boundaries in both directions
+    for (y0, x0) in [(110, 110), (121 * 17 - 12, 121 * 5 - 12)]:
+        want = oracle.diffuse_window(c["f"][0], c["u0"][0], c["filters"], c["rbf_w"], c["rbf_mu"],
+                                     c["rbf_gamma"], c["lambda"], y0, x0, 24, 24)
+        check(got[y0:y0 + 24, x0:x0 + 24], want, f"C4 seam window {(y0, x0)}")
+
+
+def test_config4_1024_T8_sampled_windows_and_T5_prefix(tnrd):
+    c8 = tnrd_gen.make_config(4, size=1024, T=8)
+    got8 = run_gpu(tnrd, c8)[0]
+    got5 = run_gpu(tnrd, c8, T=5)[0]
+    for (y0, x0) in _windows(1024, 1024, 20, 1, 8)[::3]:
+        for T, got in ((8, got8), (5, got5)):
+            want = oracle.diffuse_window(c8["f"][0], c8["u0"][0], c8["filters"][:T], c8["rbf_w"][:T], c8["rbf_mu"],
+                                         c8["rbf_gamma"], c8["lambda"][:T], y0, x0, 20, 20)
+            check(got[y0:y0 + 20, x0:x0 + 20], want, f"C4-1024 T={T} window {(y0, x0)}")
+
+
+def test_config5_batch_sampled_and_independent(tnrd):
+    c = tnrd_gen.make_config(5)
+    got = run_gpu(tnrd, c)
+    assert got.shape == (128, 321, 481) and np.all(np.isfinite(got))
+    for b in (0, 63, 127):
+        for (y0, x0) in [(0, 0), (321 - 24, 481 - 24), (150, 230)]:
+            want = oracle.diffuse_window(c["f"][b], c["u0"][b], c["filters"], c["rbf_w"], c["rbf_mu"],
+                                         c["rbf_gamma"], c["lambda"], y0, x0, 24, 24)
+            check(got[b, y0:y0 + 24, x0:x0 + 24], want, f"C5 image {b} window {(y0, x0)}")
+    # P10: an image processed alone is bit-identical to the same image inside the batch
+    one = dict(c, B=1, f=c["f"][5:6], u0=c["u0"][5:6])
+    assert np.array_equal(run_gpu(tnrd, one)[0], got[5])
+
+
+# --- properties that hold at any size ----------------------------------------------------------------------------
+def test_P2_constant_image_gpu(tnrd):
+    c = tnrd_gen.make_config(3)
+    u0 = np.full_like(c["f"], 93.25)
+    got = run_gpu(tnrd, dict(c, u0=u0), T=1)
+    lam = float(c["lambda"][0])
+    want = u0.astype(np.float64) - lam * (u0.astype(np.float64) - c["f"])
+    assert np.max(np.abs(got - want)) <= 2e-4          # zero-mean DCT filters: sum_i kbar_i * const = O(eps)
+
+
+def test_P12_degenerate_parameters_gpu(tnrd):
+    c = tnrd_gen.make_small(21, 2, 40, 52, 2, 6, 5)
+    z = dict(c, rbf_w=np.zeros_like(c["rbf_w"]))
+    u, f = c["u0"].astype(np.float64), c["f"].astype(np.float64)
+    want = u - float(c["lambda"][0]) * (u - f)
+    assert np.max(np.abs(run_gpu(tnrd, z, T=1) - want)) <= 1e-4
+    one = dict(z, **{"lambda": np.ones_like(c["lambda"])})
+    assert np.max(np.abs(run_gpu(tnrd, one, T=1) - f)) <= 1e-4          # lambda = 1, w = 0 => u_1 = f
+    assert np.array_equal(run_gpu(tnrd, c, T=0), u)                      # T = 0 copies u0
+
+
+def test_P9_flip_equivariance_gpu(tnrd):
+    c = tnrd_gen.make_small(22, 1, 150, 139, 2, 8, 7)
+    base = run_gpu(tnrd, c)
+    fl = dict(c, f=np.ascontiguousarray(c["f"][..., ::-1]), u0=np.ascontiguousarray(c["u0"][..., ::-1]),
+              filters=np.ascontiguousarray(c["filters"][..., ::-1]))
+    assert np.max(np.abs(run_gpu(tnrd, fl)[..., ::-1] - base)) <= 2e-3   # fp32 summation order differs
+
+
+# --- API semantics (P11, aliasing, host entry point, determinism) -------------------------------------------------
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_diffuse_equals_repeated_stage_and_inplace(tnrd, kernel):
+    for T in (1, 2, 3, 4):
+        c = tnrd_gen.make_small(30 + T, 2, 33, 47, T, 5, 5)
+        ref = run_gpu(tnrd, c, kernel=kernel)
+        tnrd.tnrd_set_kernel(kernel)
+        f, u = dev(c["f"]), dev(c["u0"])
+        k, w, mu = dev(c["filters"]), dev(c["rbf_w"]), dev(c["rbf_mu"])
+        for t in range(T):
+            nxt = torch.empty_like(u)
+            tnrd.tnrd_stage(f, u, 2, 33, 47, 5, 5, k[t], w[t], mu, c["rbf_gamma"], float(c["lambda"][t]), nxt)
+            u = nxt
+        torch.cuda.synchronize()
+        tnrd.tnrd_set_kernel(0)
+        assert np.array_equal(u.cpu().numpy().astype(np.float64), ref), f"T={T}: diffuse != T x stage"
+        u0 = dev(c["u0"])                                   # in place: out == u0
+        assert np.array_equal(run_gpu(tnrd, c, kernel=kernel, out=u0, u0=u0), ref), f"T={T}: in-place differs"
+
+
+def test_host_entry_point_and_determinism(tnrd):
+    c = tnrd_gen.make_small(40, 3, 90, 77, 3, 9, 7)
+    ref = run_gpu(tnrd, c)
+    assert np.array_equal(run_gpu(tnrd, c), ref)           # run-to-run deterministic
+    f = torch.from_numpy(c["f"]).pin_memory()
+    out = torch.empty_like(f).pin_memory()
+    tnrd.tnrd_diffuse_host(f, f, 3, 90, 77, 3, 9, 7, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"],
+                           c["lambda"], out)
+    assert np.array_equal(out.numpy().astype(np.float64), ref)
+    out2 = np.empty_like(c["f"])                            # pageable numpy buffers work too
+    tnrd.tnrd_diffuse_host(c["f"], c["u0"], 3, 90, 77, 3, 9, 7, c["filters"], c["rbf_w"], c["rbf_mu"],
+                           c["rbf_gamma"], c["lambda"], out2)
+    assert np.array_equal(out2.astype(np.float64), ref)
+
+
+def test_side_stream_and_launch_count(tnrd):
+    c = tnrd_gen.make_small(41, 1, 60, 60, 2, 4, 3)
+    ref = run_gpu(tnrd, c)
+    s = torch.cuda.Stream()
+    tnrd.tnrd_reset_launch_count()
+    with torch.cuda.stream(s):
+        got = run_gpu(tnrd, c)
+    assert np.array_equal(got, ref)
+    assert tnrd.tnrd_launch_count() == 1 + c["T"]          # one staging kernel + one fused kernel per stage
+    tnrd.tnrd_shutdown()
+    assert np.array_equal(run_gpu(tnrd, c), ref)            # usable after shutdown
+
+
+def test_microbench_rates_are_sane(tnrd):
+    ffma, mufu, phi = (tnrd.tnrd_microbench(i) for i in range(3))
+    print(f"FFMA {ffma / 1e12:.2f} T/s  MUFU.EX2 {mufu / 1e12:.2f} T/s  phi terms {phi / 1e12:.2f} T/s")
+    assert 5e12 < ffma < 60e12 and 1e12 < mufu < 12e12 and 0.5e12 < phi <= mufu * 1.05
