@@ -155,6 +155,8 @@ int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, in
         if ((rc = run_stage(sc, a, st)) != TNRD_OK) return rc;
         src = dst;
     }
+    if (src != out)  // T == 1 in place: the single stage went to the second plane
+        TNRD_CUDA(cudaMemcpyAsync(out, src, n * sizeof(float), cudaMemcpyDeviceToDevice, st));
     return TNRD_OK;
 }
 

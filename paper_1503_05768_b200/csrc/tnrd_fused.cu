@@ -16,6 +16,8 @@
 //
 // The path is bound by the XU (MUFU) pipe: 3024 ex2 per pixel-stage for the 48 x 7x7 model against 4704 FFMA of
 // filtering; tensor cores are not used.
+#include <cstdlib>
+
 #include "tnrd_internal.h"
 
 namespace tnrd {
@@ -29,7 +31,7 @@ __device__ __forceinline__ float ex2_approx(float x)
     return y;
 }
 
-template <int KS, int RW, int RH, int NT>
+template <int KS, int RW, int RH, int NT, int MINB = 1>
 struct Cfg {
     static constexpr int R = (KS - 1) / 2;
     static constexpr int US = RW + 8;                   // u tile row stride (floats)
@@ -118,11 +120,11 @@ __device__ __forceinline__ void phi_block(const float2* __restrict__ mw, const f
     }
 }
 
-template <int KS, int RW, int RH, int NT>
-__global__ void __launch_bounds__(NT, 1)
+template <int KS, int RW, int RH, int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB)
 stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
 {
-    using C = Cfg<KS, RW, RH, NT>;
+    using C = Cfg<KS, RW, RH, NT, MINB>;
     constexpr int R = C::R;
     extern __shared__ __align__(16) float smem[];
     float* us = smem;                              // [UH][US]
@@ -232,13 +234,13 @@ inline void split(int n, int maxt, int* nt, int* tsz)
     *tsz = (n + *nt - 1) / *nt;
 }
 
-template <int KS, int RW, int RH, int NT>
+template <int KS, int RW, int RH, int NT, int MINB>
 cudaError_t launch_cfg(const StageArgs& a, cudaStream_t st)
 {
-    using C = Cfg<KS, RW, RH, NT>;
+    using C = Cfg<KS, RW, RH, NT, MINB>;
     static bool attr_done = false;  // per-process; the attribute is per-function and sticky
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<KS, RW, RH, NT>,
+        cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<KS, RW, RH, NT, MINB>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
         if (e != cudaSuccess) return e;
         attr_done = true;
@@ -248,20 +250,39 @@ cudaError_t launch_cfg(const StageArgs& a, cudaStream_t st)
     split(a.H, RH - 2 * C::R, &nty, &th);
     const long long grid = (long long)ntx * nty * a.B;
     if (grid > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    stage_fused_kernel<KS, RW, RH, NT><<<(unsigned)grid, NT, C::SMEM, st>>>(a, tw, th, ntx, nty);
+    stage_fused_kernel<KS, RW, RH, NT, MINB><<<(unsigned)grid, NT, C::SMEM, st>>>(a, tw, th, ntx, nty);
     return cudaGetLastError();
+}
+
+// TNRD_TILE=<id> (environment, read once) forces a tile configuration; a tuning knob, not part of the ABI.
+inline int forced_tile()
+{
+    static int v = -1;
+    if (v < 0) {
+        const char* e = getenv("TNRD_TILE");
+        v = e ? atoi(e) : 0;
+    }
+    return v;
 }
 
 template <int KS>
 cudaError_t launch_ks(const StageArgs& a, int num_sms, cudaStream_t st)
 {
-    // Large tiles (less halo recompute) when they still fill the machine, small tiles otherwise.
-    int ntx, nty, tw, th;
-    split(a.W, 128 - (KS - 1), &ntx, &tw);
-    split(a.H, 128 - (KS - 1), &nty, &th);
-    const long long big_tiles = (long long)ntx * nty * a.B;
-    if (big_tiles >= 2LL * num_sms) return launch_cfg<KS, 128, 128, 512>(a, st);
-    return launch_cfg<KS, 64, 32, 256>(a, st);
+    int id = forced_tile();
+    if (id == 0) {
+        // Large tiles (less halo recompute) when they still fill the machine, small tiles otherwise.
+        int ntx, nty, tw, th;
+        split(a.W, 128 - (KS - 1), &ntx, &tw);
+        split(a.H, 128 - (KS - 1), &nty, &th);
+        id = ((long long)ntx * nty * a.B >= 2LL * num_sms) ? 1 : 2;
+    }
+    switch (id) {
+        case 1: return launch_cfg<KS, 128, 128, 512, 1>(a, st);
+        case 2: return launch_cfg<KS, 64, 32, 256, 2>(a, st);
+        case 3: return launch_cfg<KS, 128, 64, 256, 2>(a, st);
+        case 4: return launch_cfg<KS, 64, 128, 256, 2>(a, st);
+        default: return cudaErrorInvalidValue;
+    }
 }
 
 }  // namespace
