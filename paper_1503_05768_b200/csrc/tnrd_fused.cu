@@ -6,7 +6,7 @@
 //   a1  the u tile with its 2r halo is gathered through the mirror index map into shared
 //       memory -- the padded image is never materialised;
 //   then, one filter i at a time (streamed, so that only two influence maps live on chip):
-//   a2  z' = k'_i * u~ on the (tw+2r) x (th+2r) "phi region", in registers, 4x2 pixels per thread-block-of-work,
+//   a2  z' = k'_i * u~ on the (tw+2r) x (th+2r) "phi region", in registers, 4x2 pixels per unit of work,
 //   a3  v = sum_j w'_ij 2^{-(z' - mu'_j)^2}, all 63 terms, one MUFU.EX2 each (ex2.approx.ftz), in registers,
 //       written once to a double-buffered shared-memory map,
 //   a4  the rot180 taps of filter i-1 are applied to the map finished in the previous iteration and summed into
@@ -15,7 +15,13 @@
 // One __syncthreads() per filter.  HBM traffic is the algorithmic 12 B per pixel-stage plus the halo re-read.
 //
 // The path is bound by the XU (MUFU) pipe: 3024 ex2 per pixel-stage for the 48 x 7x7 model against 4704 FFMA of
-// filtering; tensor cores are not used.
+// filtering; tensor cores are not used.  Two things keep the XU pipe fed
+// (profiles/r01_*.md):
+//   * software pipelining inside a thread: the 63-term phi loop of block n is interleaved, row-step by row-step, with
+//     the forward filter of the NEXT block (a2) and the transposed filter of block n for the previous filter (a4), so
+//     every warp always carries a mix of MUFU and FMA work instead of all warps of a CTA filtering in lock-step;
+//   * packed fp32x2 arithmetic (FADD2 / FMUL2 / FFMA2, sm_100): the two output rows of a 4x2 block form the two
+//     halves of one register pair, which halves the issue slots of everything that is not a MUFU.
 #include <cstdlib>
 
 #include "tnrd_internal.h"
@@ -24,10 +30,11 @@ namespace tnrd {
 
 namespace {
 
-__device__ __forceinline__ float ex2_approx(float x)
+// 2^{-x}: the negation rides on the MUFU operand
+__device__ __forceinline__ float ex2_neg(float x)
 {
     float y;
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(-x));
     return y;
 }
 
@@ -38,86 +45,59 @@ struct Cfg {
     static constexpr int UH = RH + 2 * R;               // u tile rows
     static constexpr int VS = RW;                       // phi map row stride
     static constexpr int VPLANE = RH * RW + 16;         // one phi map (+ overrun pad for masked pixels)
+    static constexpr int TS = prm_ts(KS);               // floats per row of tap pairs
     static constexpr int PRM = prm_stride(KS);          // floats per staged record
     static constexpr int NB = ((RW / 4) * (RH / 2) + NT - 1) / NT;  // 4x2 work blocks per thread (max)
-    static constexpr size_t SMEM = sizeof(float) * ((size_t)UH * US + 2 * (size_t)VPLANE + 3 * (size_t)PRM);
+    static constexpr int NG = TNRD_MP / 8;              // phi steps of 8 terms
+    static constexpr size_t SMEM = sizeof(float) * ((size_t)UH * US + 2 * (size_t)VPLANE + 4 * (size_t)PRM);
 };
 
-// forward filter (a2): z[j][p] += sum_{a,b} k[a][b] * U[py0 + j + 2r - a][px0 + p + 2r - b]
-// `uw` points at U[py0][px0]; `taps` at the staged record (rows of TS floats, but stored densely a*KS+b)
-template <int KS, int US>
-__device__ __forceinline__ void conv_fwd_block(const float* __restrict__ uw, const float* __restrict__ taps,
-                                               float (&z)[2][4])
+template <int N>
+__device__ __forceinline__ void lds_vec(const float* __restrict__ p, float (&d)[N])
 {
-    constexpr int WC = 4 + KS - 1, NV = (WC + 3) / 4;
 #pragma unroll
-    for (int wr = 0; wr < KS + 1; ++wr) {
-        float row[NV * 4];
-#pragma unroll
-        for (int q = 0; q < NV; ++q) {
-            const float4 t = *reinterpret_cast<const float4*>(uw + wr * US + 4 * q);
-            row[4 * q + 0] = t.x; row[4 * q + 1] = t.y; row[4 * q + 2] = t.z; row[4 * q + 3] = t.w;
-        }
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            const int a = j + (KS - 1) - wr;
-            if (a < 0 || a >= KS) continue;
-#pragma unroll
-            for (int b = 0; b < KS; ++b) {
-                const float k = taps[a * KS + b];
-#pragma unroll
-                for (int p = 0; p < 4; ++p) z[j][p] = fmaf(k, row[p + (KS - 1) - b], z[j][p]);
-            }
-        }
+    for (int q = 0; q < N / 4; ++q) {
+        const float4 t = *reinterpret_cast<const float4*>(p + 4 * q);
+        d[4 * q + 0] = t.x; d[4 * q + 1] = t.y; d[4 * q + 2] = t.z; d[4 * q + 3] = t.w;
     }
 }
 
-// transposed filter (a4): s[j][p] += sum_{a,b} k[a][b] * V[oy0 + j + a][ox0 + p + b]; `vw` points at V[oy0][ox0]
-template <int KS, int VS>
-__device__ __forceinline__ void conv_bwd_block(const float* __restrict__ vw, const float* __restrict__ taps,
-                                               float (&s)[2][4])
+// One window row of either filtering for a 4x2 block.  acc[p] holds the two output rows of column p as one pair;
+// trow = row of tap pairs P[rho][b] = (k[rho-1][b], k[rho][b]).  REV = false: forward filter (a2), pair = (row 0,
+// row 1), rho = KS - wr, source column p + 2r - b.  REV = true: transposed filter (a4), pair = (row 1, row 0),
+// rho = wr, source column p + b.
+template <int KS, bool REV>
+__device__ __forceinline__ void rowstep(const float* __restrict__ srow, const float* __restrict__ trow,
+                                        float2 (&acc)[4])
 {
-    constexpr int WC = 4 + KS - 1, NV = (WC + 3) / 4;
+    constexpr int TS = prm_ts(KS), NV = (4 + KS - 1 + 3) / 4;
+    float row[NV * 4], kp[TS];
+    lds_vec(srow, row);
+    lds_vec(trow, kp);
 #pragma unroll
-    for (int wr = 0; wr < KS + 1; ++wr) {
-        float row[NV * 4];
+    for (int b = 0; b < KS; ++b)
 #pragma unroll
-        for (int q = 0; q < NV; ++q) {
-            const float4 t = *reinterpret_cast<const float4*>(vw + wr * VS + 4 * q);
-            row[4 * q + 0] = t.x; row[4 * q + 1] = t.y; row[4 * q + 2] = t.z; row[4 * q + 3] = t.w;
+        for (int p = 0; p < 4; ++p) {
+            const float x = REV ? row[p + b] : row[p + (KS - 1) - b];
+            acc[p] = __ffma2_rn(make_float2(kp[2 * b], kp[2 * b + 1]), make_float2(x, x), acc[p]);
         }
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            const int a = wr - j;
-            if (a < 0 || a >= KS) continue;
-#pragma unroll
-            for (int b = 0; b < KS; ++b) {
-                const float k = taps[a * KS + b];
-#pragma unroll
-                for (int p = 0; p < 4; ++p) s[j][p] = fmaf(k, row[p + b], s[j][p]);
-            }
-        }
-    }
 }
 
-// influence function (a3) on 8 responses held in registers; mw = 64 pairs (mu'_j, w'_ij)
-__device__ __forceinline__ void phi_block(const float2* __restrict__ mw, const float (&z)[2][4], float (&v)[2][4])
+// 8 RBF terms for the 8 responses of a block: 4 x LDS.128 of (-mu', w') pairs, then per term and response pair
+// FADD2, FMUL2, 2 x MUFU.EX2, FFMA2
+__device__ __forceinline__ void phi_step8(const float* __restrict__ mw, const float2 (&z)[4], float2 (&v)[4])
 {
+    float c[16];
+    lds_vec(mw, c);
 #pragma unroll
-    for (int j = 0; j < 2; ++j)
+    for (int m = 0; m < 8; ++m)
 #pragma unroll
-        for (int p = 0; p < 4; ++p) v[j][p] = 0.0f;
-#pragma unroll 4
-    for (int m = 0; m < TNRD_MP; ++m) {
-        const float2 c = mw[m];
-#pragma unroll
-        for (int j = 0; j < 2; ++j)
-#pragma unroll
-            for (int p = 0; p < 4; ++p) {
-                const float d = z[j][p] - c.x;
-                v[j][p] = fmaf(ex2_approx(-d * d), c.y, v[j][p]);
-            }
-    }
+        for (int p = 0; p < 4; ++p) {
+            const float2 d = __fadd2_rn(z[p], make_float2(c[2 * m], c[2 * m]));
+            const float2 t = __fmul2_rn(d, d);
+            const float2 e = make_float2(ex2_neg(t.x), ex2_neg(t.y));
+            v[p] = __ffma2_rn(e, make_float2(c[2 * m + 1], c[2 * m + 1]), v[p]);
+        }
 }
 
 template <int KS, int RW, int RH, int NT, int MINB>
@@ -125,11 +105,11 @@ __global__ void __launch_bounds__(NT, MINB)
 stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
 {
     using C = Cfg<KS, RW, RH, NT, MINB>;
-    constexpr int R = C::R;
+    constexpr int R = C::R, TS = C::TS, KKP = prm_kkp(KS);
     extern __shared__ __align__(16) float smem[];
-    float* us = smem;                              // [UH][US]
-    float* vs = us + C::UH * C::US;                // [2][VPLANE]
-    float* ps = vs + 2 * C::VPLANE;                // [3][PRM]
+    float* us = smem;                              // [UH][US]   u tile with 2r halo
+    float* vs = us + C::UH * C::US;                // [2][VPLANE] influence maps of filters i and i-1
+    float* ps = vs + 2 * C::VPLANE;                // [4][PRM]   staged records of filters i-1 .. i+2
 
     const int tid = threadIdx.x;
     int t = blockIdx.x;
@@ -138,6 +118,7 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
     const int img = t;
     const int X0 = tx * tw, Y0 = ty * th;          // image coordinates of the output tile origin
     const float* __restrict__ u_img = a.u_in + (size_t)img * a.H * a.W;
+    const int N_k = a.N_k;
 
     // ---- a1: gather the u tile through the mirror map ----------------------------------------------------
     for (int idx = tid; idx < C::UH * C::US; idx += NT) {
@@ -145,64 +126,94 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
         const int gy = mirror_clamp(Y0 - 2 * R + uy, a.H), gx = mirror_clamp(X0 - 2 * R + ux, a.W);
         us[idx] = __ldg(u_img + (size_t)gy * a.W + gx);
     }
-    for (int idx = tid; idx < C::PRM; idx += NT) ps[idx] = __ldg(a.prm + idx);
+    for (int idx = tid; idx < 2 * C::PRM; idx += NT)
+        if (idx < N_k * C::PRM) ps[idx] = __ldg(a.prm + idx);          // records 0 and 1
 
     // ---- work decomposition: 4x2 pixel blocks, NB per thread ----------------------------------------------
     const int nbx = (tw + 2 * R + 3) >> 2, nby = (th + 2 * R + 1) >> 1;   // phi region
     const int nbxo = (tw + 3) >> 2, nbyo = (th + 1) >> 1;                  // output tile
-    int offA[C::NB], offC[C::NB];   // offsets of the block origin (row*stride + col), -1 = no work
+    int uoff[C::NB], voff[C::NB], coff[C::NB];   // block origins in us / a phi map (phi side) / a phi map (output side)
 #pragma unroll
     for (int n = 0; n < C::NB; ++n) {
         const int blk = tid + n * NT;
         const int by = blk / nbx, bx = blk - by * nbx;
-        offA[n] = (by < nby) ? ((2 * by) << 16 | (4 * bx)) : -1;
+        uoff[n] = (by < nby) ? (2 * by) * C::US + 4 * bx : -1;
+        voff[n] = (2 * by) * C::VS + 4 * bx;
         const int cy = blk / nbxo, cx = blk - cy * nbxo;
-        offC[n] = (cy < nbyo) ? ((2 * cy) << 16 | (4 * cx)) : -1;
+        coff[n] = (cy < nbyo) ? (2 * cy) * C::VS + 4 * cx : -1;
     }
-    float acc[C::NB][2][4];
+    float2 acc[C::NB][4];                          // (row 1, row 0) of the transposed-filter sum, per block column
 #pragma unroll
     for (int n = 0; n < C::NB; ++n)
 #pragma unroll
-        for (int j = 0; j < 2; ++j)
-#pragma unroll
-            for (int p = 0; p < 4; ++p) acc[n][j][p] = 0.0f;
+        for (int p = 0; p < 4; ++p) acc[n][p] = make_float2(0.f, 0.f);
 
     __syncthreads();
 
-    // ---- filter loop: a2 + a3 for filter i, a4 for filter i-1 ---------------------------------------------
-    for (int i = 0; i <= a.N_k; ++i) {
-        if (i + 1 < a.N_k) {  // stage the next record (triple buffer: i-1 is still read by a4)
-            const float* src = a.prm + (size_t)(i + 1) * C::PRM;
-            float* dst = ps + ((i + 1) % 3) * C::PRM;
+    // prologue: responses of filter 0 on this thread's first block
+    float2 zc[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
+    if (uoff[0] >= 0) {
+#pragma unroll
+        for (int wr = 0; wr <= KS; ++wr) rowstep<KS, false>(us + uoff[0] + wr * C::US, ps + (KS - wr) * TS, zc);
+    }
+
+    // ---- filter loop ------------------------------------------------------------------------------------------
+    for (int i = 0; i < N_k; ++i) {
+        if (i + 2 < N_k) {                                    // stage record i+2 (read from iteration i+1 on)
+            const float* src = a.prm + (size_t)(i + 2) * C::PRM;
+            float* dst = ps + ((i + 2) & 3) * C::PRM;
             for (int idx = tid; idx < C::PRM; idx += NT) dst[idx] = __ldg(src + idx);
         }
-        if (i < a.N_k) {
-            const float* rec = ps + (i % 3) * C::PRM;
-            float* vcur = vs + (i & 1) * C::VPLANE;
-#pragma unroll 1
-            for (int n = 0; n < C::NB; ++n) {
-                if (offA[n] < 0) continue;
-                const int py = offA[n] >> 16, px = offA[n] & 0xffff;
-                float z[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-                conv_fwd_block<KS, C::US>(us + py * C::US + px, rec, z);
-                float v[2][4];
-                phi_block(reinterpret_cast<const float2*>(rec + prm_kkp(KS)), z, v);
-                *reinterpret_cast<float4*>(vcur + py * C::VS + px) = make_float4(v[0][0], v[0][1], v[0][2], v[0][3]);
-                *reinterpret_cast<float4*>(vcur + (py + 1) * C::VS + px) =
-                    make_float4(v[1][0], v[1][1], v[1][2], v[1][3]);
-            }
-        }
-        if (i > 0) {
-            const float* rec = ps + ((i - 1) % 3) * C::PRM;
-            const float* vprev = vs + ((i - 1) & 1) * C::VPLANE;
+        const float* rec = ps + (i & 3) * C::PRM;             // filter i: phi pairs, a2 of blocks 1..NB-1
+        const float* recn = ps + ((i + 1) & 3) * C::PRM;      // filter i+1: a2 of block 0
+        const float* recp = ps + ((i + 3) & 3) * C::PRM;      // filter i-1: a4
+        float* vcur = vs + (i & 1) * C::VPLANE;
+        const float* vprev = vs + ((i + 1) & 1) * C::VPLANE;
 #pragma unroll
-            for (int n = 0; n < C::NB; ++n) {
-                if (offC[n] < 0) continue;
-                const int oy = offC[n] >> 16, ox = offC[n] & 0xffff;
-                conv_bwd_block<KS, C::VS>(vprev + oy * C::VS + ox, rec, acc[n]);
+        for (int n = 0; n < C::NB; ++n) {
+            const bool last = (n == C::NB - 1);
+            const int un = last ? uoff[0] : uoff[(n + 1) % C::NB];
+            const bool hasB = uoff[n] >= 0;                               // phi of block n
+            const bool hasN = un >= 0 && (!last || i + 1 < N_k);          // forward filter of the next block
+            const bool hasC = i > 0 && coff[n] >= 0;                      // transposed filter of output block n
+            const float* tapsN = last ? recn : rec;
+            const float* uwn = us + (un >= 0 ? un : 0);
+            const float* vw = vprev + (coff[n] >= 0 ? coff[n] : 0);
+            float2 v[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
+            float2 zn[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
+#pragma unroll 1
+            for (int g = 0; g < C::NG; ++g) {
+                if (hasB) phi_step8(rec + KKP + 16 * g, zc, v);
+                if (g <= KS) {
+                    if (hasN) rowstep<KS, false>(uwn + g * C::US, tapsN + (KS - g) * TS, zn);
+                    if (hasC) rowstep<KS, true>(vw + g * C::VS, recp + g * TS, acc[n]);
+                }
+                if (KS + 1 > C::NG && g + C::NG <= KS) {      // ksize 9: ten row-steps in eight phi steps
+                    const int g2 = g + C::NG;
+                    if (hasN) rowstep<KS, false>(uwn + g2 * C::US, tapsN + (KS - g2) * TS, zn);
+                    if (hasC) rowstep<KS, true>(vw + g2 * C::VS, recp + g2 * TS, acc[n]);
+                }
             }
+            if (hasB) {
+                *reinterpret_cast<float4*>(vcur + voff[n]) = make_float4(v[0].x, v[1].x, v[2].x, v[3].x);
+                *reinterpret_cast<float4*>(vcur + voff[n] + C::VS) = make_float4(v[0].y, v[1].y, v[2].y, v[3].y);
+            }
+#pragma unroll
+            for (int p = 0; p < 4; ++p) zc[p] = zn[p];
         }
         __syncthreads();
+    }
+
+    // ---- a4 of the last filter --------------------------------------------------------------------------------
+    {
+        const float* recp = ps + ((N_k - 1) & 3) * C::PRM;
+        const float* vprev = vs + ((N_k - 1) & 1) * C::VPLANE;
+#pragma unroll
+        for (int n = 0; n < C::NB; ++n) {
+            if (coff[n] < 0) continue;
+#pragma unroll
+            for (int wr = 0; wr <= KS; ++wr) rowstep<KS, true>(vprev + coff[n] + wr * C::VS, recp + wr * TS, acc[n]);
+        }
     }
 
     // ---- a5: reaction term and update ------------------------------------------------------------------------
@@ -211,8 +222,8 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
     float* __restrict__ o_img = a.u_out + (size_t)img * a.H * a.W;
 #pragma unroll
     for (int n = 0; n < C::NB; ++n) {
-        if (offC[n] < 0) continue;
-        const int oy = offC[n] >> 16, ox = offC[n] & 0xffff;
+        if (coff[n] < 0) continue;
+        const int oy = coff[n] / C::VS, ox = coff[n] - oy * C::VS;
 #pragma unroll
         for (int j = 0; j < 2; ++j)
 #pragma unroll
@@ -220,8 +231,9 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
                 const int ly = oy + j, lx = ox + p, gy = Y0 + ly, gx = X0 + lx;
                 if (ly < th && lx < tw && gy < a.H && gx < a.W) {
                     const float uu = us[(ly + 2 * R) * C::US + lx + 2 * R];
+                    const float s = j ? acc[n][p].x : acc[n][p].y;
                     const size_t g = (size_t)gy * a.W + gx;
-                    o_img[g] = uu - (acc[n][j][p] + lambda * (uu - __ldg(f_img + g)));
+                    o_img[g] = uu - (s + lambda * (uu - __ldg(f_img + g)));
                 }
             }
     }
@@ -279,8 +291,7 @@ cudaError_t launch_ks(const StageArgs& a, int num_sms, cudaStream_t st)
     switch (id) {
         case 1: return launch_cfg<KS, 128, 128, 512, 1>(a, st);
         case 2: return launch_cfg<KS, 64, 32, 256, 2>(a, st);
-        case 3: return launch_cfg<KS, 128, 64, 256, 2>(a, st);
-        case 4: return launch_cfg<KS, 64, 128, 256, 2>(a, st);
+        case 3: return launch_cfg<KS, 128, 96, 512, 1>(a, st);
         default: return cudaErrorInvalidValue;
     }
 }

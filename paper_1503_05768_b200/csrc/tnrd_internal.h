@@ -10,12 +10,17 @@ namespace tnrd {
 
 // ---- staged ("prepped") parameters ---------------------------------------------------------------
 // For every stage t and filter i the prep kernel writes one record of prm_stride(ksize) floats:
-//   [0 .. KK)            k'_i[a][b] = s * k_i[a][b],  s = sqrt(log2(e) / (2 gamma^2))
-//   [KKP .. KKP + 128)   pairs (mu'_j, w'_ij) = (s * mu_j, w_ij / s), j = 0..63 (pair 63 = (0, 0))
+//   taps     (ksize + 1) rows rho = 0..ksize of prm_ts(ksize) floats; row rho holds the ksize PAIRS
+//            P[rho][b] = (k'[rho-1][b], k'[rho][b]),  k'_i[a][b] = s * k_i[a][b],  k'[-1] = k'[ksize] = 0,
+//            s = sqrt(log2(e) / (2 gamma^2)).  A pair feeds one packed FFMA2 that updates the two output rows of a
+//            4x2 pixel block at once: forward filter at window row wr uses row rho = ksize - wr, transposed filter
+//            at window row wr uses row rho = wr.
+//   pairs    at offset prm_kkp: 64 pairs (-mu'_j, w'_ij) = (-s * mu_j, w_ij / s), pair 63 = (0, 0)
 // so that phi_i(k_i * u) = sum_j w_ij 2^{-(z' - mu'_j)^2} with z' = k'_i * u, and the transposed bank
 // sum_i kbar_i * v_i = sum_i kbar'_i * (v_i / s) re-uses the same scaled taps.
-// After the T*N_k records: lambda[T] is read directly from the caller's array.
-__host__ __device__ constexpr int prm_kkp(int ksize) { return ((ksize * ksize + 3) / 4) * 4; }
+__host__ __device__ constexpr int prm_ts(int ksize) { return ((2 * ksize + 3) / 4) * 4; }
+__host__ __device__ constexpr int prm_tap(int ksize, int a, int b) { return (a + 1) * prm_ts(ksize) + 2 * b; }
+__host__ __device__ constexpr int prm_kkp(int ksize) { return (ksize + 1) * prm_ts(ksize); }
 __host__ __device__ constexpr int prm_stride(int ksize) { return prm_kkp(ksize) + 2 * TNRD_MP; }
 
 // Half-sample symmetric mirror map, edge pixel repeated, then clamped so that

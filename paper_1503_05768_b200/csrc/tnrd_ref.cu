@@ -20,17 +20,18 @@ __global__ void prep_params_kernel(const float* __restrict__ filters, const floa
                                    const float* __restrict__ rbf_mu, float gamma, int TN, int ksize,
                                    float* __restrict__ prm)
 {
-    const int KK = ksize * ksize, KKP = prm_kkp(ksize), S = prm_stride(ksize);
+    const int KK = ksize * ksize, KKP = prm_kkp(ksize), S = prm_stride(ksize), TS = prm_ts(ksize);
     const float s = sqrtf(1.4426950408889634f / (2.0f * gamma * gamma));
     const int total = TN * S;
     for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
         const int rec = idx / S, e = idx - rec * S;
         float val = 0.0f;
-        if (e < KK) {
-            val = s * filters[(size_t)rec * KK + e];
-        } else if (e >= KKP) {
+        if (e < KKP) {
+            const int rho = e / TS, c = e - rho * TS, b = c >> 1, a = rho - 1 + (c & 1);
+            if (a >= 0 && a < ksize && b < ksize) val = s * filters[(size_t)rec * KK + a * ksize + b];
+        } else {
             const int j = (e - KKP) >> 1, which = (e - KKP) & 1;
-            if (j < TNRD_M) val = which ? rbf_w[(size_t)rec * TNRD_M + j] / s : s * rbf_mu[j];
+            if (j < TNRD_M) val = which ? rbf_w[(size_t)rec * TNRD_M + j] / s : -s * rbf_mu[j];
         }
         prm[idx] = val;
     }
@@ -68,11 +69,11 @@ __global__ void ref_phi_kernel(StageArgs a, float* __restrict__ vbuf)
         float z = 0.0f;
         for (int ka = 0; ka < K; ++ka)
             for (int kb = 0; kb < K; ++kb)
-                z = fmaf(rec[ka * K + kb],
+                z = fmaf(rec[prm_tap(K, ka, kb)],
                          u[(size_t)mirror_clamp(y + r - ka, a.H) * a.W + mirror_clamp(x + r - kb, a.W)], z);
         float acc = 0.0f;
         for (int j = 0; j < TNRD_M; ++j) {
-            const float d = z - rec[KKP + 2 * j];
+            const float d = z + rec[KKP + 2 * j];
             acc = fmaf(ex2_approx(-d * d), rec[KKP + 2 * j + 1], acc);
         }
         vbuf[idx] = acc;
@@ -97,7 +98,7 @@ __global__ void ref_update_kernel(StageArgs a, const float* __restrict__ vbuf)
             const float* v = vbuf + ((size_t)b * a.N_k + i) * Hv * Wv;
             for (int ka = 0; ka < K; ++ka)
                 for (int kb = 0; kb < K; ++kb)
-                    s = fmaf(rec[ka * K + kb], v[(size_t)(y + ka) * Wv + (x + kb)], s);
+                    s = fmaf(rec[prm_tap(K, ka, kb)], v[(size_t)(y + ka) * Wv + (x + kb)], s);
         }
         const float uu = a.u_in[idx];
         a.u_out[idx] = uu - (s + lambda * (uu - a.f[idx]));
