@@ -36,8 +36,8 @@ EX2_PER_PX_STAGE = N_K * M                       # 3024 MUFU.EX2 per pixel-stage
 FMA_PER_PX_STAGE = 2 * N_K * KSIZE * KSIZE       # 4704 FFMA of filtering
 FLOP_PER_PX_STAGE = 2 * FMA_PER_PX_STAGE + 5 * EX2_PER_PX_STAGE   # per RBF term: sub, mul, ex2, fma(2) -> 24528
 NOMINAL_SM_MHZ, NOMINAL_SMS, MUFU_PER_CLK_SM = 1965.0, 148, 16
-# dram bytes per fused-stage launch from profiles/ (ncu --set full); None until captured
-TRAFFIC_BYTES_PER_LAUNCH = None
+# dram__bytes_read.sum + dram__bytes_write.sum per fused-stage launch at 4096^2 (profiles/r01_fused_stage_ncu.md)
+TRAFFIC_BYTES_PER_LAUNCH = {4096: 92.5e6}
 
 
 def read_peaks():
@@ -103,7 +103,7 @@ def oracle_sample(cfg, cores_hint=None, target_s=12.0):
     import oracle
     cores = oracle.num_threads()
     T = cfg["T"]
-    per_core = 50e-6                                   # ~47 us per 48x7x7 px-stage per core
+    per_core = 20e-6                                   # measured on the B200 host: ~20 us per 48x7x7 px-stage per core
     px = max(48 * 48, int(target_s * cores / per_core / T))
     side = int(min(cfg["H"], cfg["W"], max(48, int(px ** 0.5))))
     y0, x0 = (cfg["H"] - side) // 2, (cfg["W"] - side) // 2
@@ -149,7 +149,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--size", type=int, default=4096)
     ap.add_argument("--T", type=int, default=5)
-    ap.add_argument("--ref-seconds", type=float, default=8.0, help="CPU seconds per oracle sample")
+    ap.add_argument("--ref-seconds", type=float, default=10.0, help="CPU seconds per oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
@@ -245,7 +245,7 @@ def main():
     mb = {n: tnrd.tnrd_microbench(i) / 1e12 for i, n in enumerate(["ffma_T_per_s", "ex2_T_per_s", "phi_terms_T_per_s"])}
     roofline = {
         "bound": "alu", "pipe": "xu (MUFU.EX2)", "achieved": achieved, "peak": peak_nominal, "unit": "Tex2/s",
-        "frac": achieved / peak_nominal, "traffic": TRAFFIC_BYTES_PER_LAUNCH,
+        "frac": achieved / peak_nominal, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(H if H == W else -1),
         "peak_source": "148 SM x 16 MUFU/clk/SM x 1.965 GHz (DESIGN.md Roofline); measured by tnrd_microbench: "
                        f"{mb['ex2_T_per_s']:.3f} Tex2/s",
         "frac_of_measured_ex2": achieved / mb["ex2_T_per_s"], "microbench": mb,
