@@ -31,7 +31,7 @@ sys.path.insert(0, ROOT)
 import tnrd_gen  # noqa: E402
 
 METRIC = "Mpixel-stages/s"
-N_K, KSIZE, M = 48, 7, 63
+N_K, KSIZE, M = 48, 7, 63                          # headline model; main() re-derives them per workload
 EX2_PER_PX_STAGE = N_K * M                       # 3024 MUFU.EX2 per pixel-stage (dense phi)
 FMA_PER_PX_STAGE = 2 * N_K * KSIZE * KSIZE       # 4704 FFMA of filtering
 FLOP_PER_PX_STAGE = 2 * FMA_PER_PX_STAGE + 5 * EX2_PER_PX_STAGE   # per RBF term: sub, mul, ex2, fma(2) -> 24528
@@ -147,6 +147,8 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5"],
+                    help="BASELINE.json config; c4 (default) is the headline, the others are for exploration")
     ap.add_argument("--size", type=int, default=4096)
     ap.add_argument("--T", type=int, default=5)
     ap.add_argument("--ref-seconds", type=float, default=10.0, help="CPU seconds per oracle sample")
@@ -176,8 +178,12 @@ def main():
         dist.init_process_group("nccl", device_id=devs)
     warmup = max(args.warmup, 3)
 
-    cfg = tnrd_gen.make_config(4, size=args.size, T=args.T)
+    cfg = (tnrd_gen.make_config(4, size=args.size, T=args.T) if args.workload == "c4"
+           else tnrd_gen.make_config(int(args.workload[1])))
     B, H, W, T = cfg["B"], cfg["H"], cfg["W"], cfg["T"]
+    N_K, KSIZE = cfg["N_k"], cfg["ksize"]
+    EX2_PER_PX_STAGE, FMA_PER_PX_STAGE = N_K * M, 2 * N_K * KSIZE * KSIZE
+    FLOP_PER_PX_STAGE = 2 * FMA_PER_PX_STAGE + 5 * EX2_PER_PX_STAGE
     f = torch.from_numpy(cfg["f"]).to(devs)
     out = torch.empty_like(f)
     k, w = torch.from_numpy(cfg["filters"]).to(devs), torch.from_numpy(cfg["rbf_w"]).to(devs)
@@ -245,7 +251,7 @@ def main():
     mb = {n: tnrd.tnrd_microbench(i) / 1e12 for i, n in enumerate(["ffma_T_per_s", "ex2_T_per_s", "phi_terms_T_per_s"])}
     roofline = {
         "bound": "alu", "pipe": "xu (MUFU.EX2)", "achieved": achieved, "peak": peak_nominal, "unit": "Tex2/s",
-        "frac": achieved / peak_nominal, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(H if H == W else -1),
+        "frac": achieved / peak_nominal, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(H if (H == W and args.workload == "c4") else -1),
         "peak_source": "148 SM x 16 MUFU/clk/SM x 1.965 GHz (DESIGN.md Roofline); measured by tnrd_microbench: "
                        f"{mb['ex2_T_per_s']:.3f} Tex2/s",
         "frac_of_measured_ex2": achieved / mb["ex2_T_per_s"], "microbench": mb,
@@ -257,9 +263,11 @@ def main():
         "metric": METRIC, "value": value, "unit": "Mpixel-stages/s", "n_gpus": world, "steps": args.steps,
         "warmup": warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"C4 {H}x{W} T={T} N_k=48 7x7 M=63 (BASELINE.json configs[3]), one image per GPU",
+        "config": {"workload": f"C{args.workload[1]} {B}x{H}x{W} T={T} N_k={N_K} {KSIZE}x{KSIZE} M=63 "
+                               f"(BASELINE.json configs[{int(args.workload[1]) - 1}]), one such batch per GPU",
                    "global_batch": world * B, "parallelism": f"dp{world} (independent images, no collective)",
-                   "l2": "inputs larger than L2 (3 planes x %d MB)" % (H * W * 4 // 2 ** 20)},
+                   "l2": ("inputs larger than L2 (3 planes x %d MB)" % (B * H * W * 4 // 2 ** 20)) if 3 * B * H * W * 4 > 126e6
+                   else "working set fits L2 (exploration workload)"},
         "roofline": roofline, "clocks": clocks.summary(),
         "e2e": {"value": e2e_value, "unit": "Mpixel-stages/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "matches_device_path": same},

@@ -83,14 +83,15 @@ __device__ __forceinline__ void rowstep(const float* __restrict__ srow, const fl
         }
 }
 
-// 8 RBF terms for the 8 responses of a block: 4 x LDS.128 of (-mu', w') pairs, then per term and response pair
-// FADD2, FMUL2, 2 x MUFU.EX2, FFMA2
-__device__ __forceinline__ void phi_step8(const float* __restrict__ mw, const float2 (&z)[4], float2 (&v)[4])
+// NTERM (8, or 7 in the last step: 63 = 7 * 8 + 7) RBF terms for the 8 responses of a block: 4 x LDS.128 of
+// (-mu', w') pairs, then per term and response pair FADD2, FMUL2, 2 x MUFU.EX2, FFMA2
+template <int NTERM>
+__device__ __forceinline__ void phi_step(const float* __restrict__ mw, const float2 (&z)[4], float2 (&v)[4])
 {
     float c[16];
     lds_vec(mw, c);
 #pragma unroll
-    for (int m = 0; m < 8; ++m)
+    for (int m = 0; m < NTERM; ++m)
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
             const float2 d = __fadd2_rn(z[p], make_float2(c[2 * m], c[2 * m]));
@@ -120,18 +121,22 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
     const float* __restrict__ u_img = a.u_in + (size_t)img * a.H * a.W;
     const int N_k = a.N_k;
 
-    // ---- a1: gather the u tile through the mirror map ----------------------------------------------------
-    for (int idx = tid; idx < C::UH * C::US; idx += NT) {
-        const int uy = idx / C::US, ux = idx - uy * C::US;
-        const int gy = mirror_clamp(Y0 - 2 * R + uy, a.H), gx = mirror_clamp(X0 - 2 * R + ux, a.W);
-        us[idx] = __ldg(u_img + (size_t)gy * a.W + gx);
+    // ---- work decomposition: 4x2 pixel blocks, NB per thread ----------------------------------------------
+    const int nbx = (tw + 2 * R + 3) >> 2, nby = (th + 2 * R + 1) >> 1;   // phi region
+    const int nbxo = (tw + 3) >> 2, nbyo = (th + 1) >> 1;                  // output tile
+
+    // ---- a1: gather the u tile through the mirror map (only the rows / columns some block will read) -----
+    {
+        const int nr = min(C::UH, 2 * nby + 2 * R), nc = min(C::US, 4 * nbx + 2 * R + 4);
+        for (int uy = tid >> 5; uy < nr; uy += NT / 32) {
+            const float* __restrict__ grow = u_img + (size_t)mirror_clamp(Y0 - 2 * R + uy, a.H) * a.W;
+            for (int ux = tid & 31; ux < nc; ux += 32)
+                us[uy * C::US + ux] = __ldg(grow + mirror_clamp(X0 - 2 * R + ux, a.W));
+        }
     }
     for (int idx = tid; idx < 2 * C::PRM; idx += NT)
         if (idx < N_k * C::PRM) ps[idx] = __ldg(a.prm + idx);          // records 0 and 1
 
-    // ---- work decomposition: 4x2 pixel blocks, NB per thread ----------------------------------------------
-    const int nbx = (tw + 2 * R + 3) >> 2, nby = (th + 2 * R + 1) >> 1;   // phi region
-    const int nbxo = (tw + 3) >> 2, nbyo = (th + 1) >> 1;                  // output tile
     int uoff[C::NB], voff[C::NB], coff[C::NB];   // block origins in us / a phi map (phi side) / a phi map (output side)
 #pragma unroll
     for (int n = 0; n < C::NB; ++n) {
@@ -182,8 +187,8 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
             float2 v[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
             float2 zn[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
 #pragma unroll 1
-            for (int g = 0; g < C::NG; ++g) {
-                if (hasB) phi_step8(rec + KKP + 16 * g, zc, v);
+            for (int g = 0; g < C::NG - 1; ++g) {
+                if (hasB) phi_step<8>(rec + KKP + 16 * g, zc, v);
                 if (g <= KS) {
                     if (hasN) rowstep<KS, false>(uwn + g * C::US, tapsN + (KS - g) * TS, zn);
                     if (hasC) rowstep<KS, true>(vw + g * C::VS, recp + g * TS, acc[n]);
@@ -192,6 +197,14 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
                     const int g2 = g + C::NG;
                     if (hasN) rowstep<KS, false>(uwn + g2 * C::US, tapsN + (KS - g2) * TS, zn);
                     if (hasC) rowstep<KS, true>(vw + g2 * C::VS, recp + g2 * TS, acc[n]);
+                }
+            }
+            {   // last step: the remaining 63 - 56 = 7 terms
+                constexpr int g = C::NG - 1;
+                if (hasB) phi_step<TNRD_M - 8 * g>(rec + KKP + 16 * g, zc, v);
+                if (g <= KS) {
+                    if (hasN) rowstep<KS, false>(uwn + g * C::US, tapsN + (KS - g) * TS, zn);
+                    if (hasC) rowstep<KS, true>(vw + g * C::VS, recp + g * TS, acc[n]);
                 }
             }
             if (hasB) {
@@ -239,15 +252,39 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
     }
 }
 
-// balanced tile edge: the fewest tiles of at most `maxt` that cover n, all of (nearly) equal size
-inline void split(int n, int maxt, int* nt, int* tsz)
+// ---- host side: tile plan and launch ------------------------------------------------------------------------------
+struct Plan {
+    int ntx, nty, tw, th;
+    long long cost;   // estimated time in thread-rounds per SM (see plan_tiles)
+    long long work;   // thread-rounds of one CTA (critical path; tie-break)
+};
+
+// Tile plan for one kernel configuration.  The path is XU-bound, so an SM's time is proportional to the phi work
+// assigned to it: (CTAs per SM) x (rounds of 4x2 blocks per thread, 1..NB) x (threads per CTA).  Try the fewest equal
+// tiles that cover the image and a few more in each direction (a smaller tile can save a whole round), keep the cheapest.
+template <int KS, int RW, int RH, int NT>
+Plan plan_tiles(const StageArgs& a, int num_sms)
 {
-    *nt = (n + maxt - 1) / maxt;
-    *tsz = (n + *nt - 1) / *nt;
+    constexpr int R = (KS - 1) / 2;
+    Plan best{0, 0, 0, 0, -1, 0};
+    const int ntx0 = (a.W + RW - 2 * R - 1) / (RW - 2 * R), nty0 = (a.H + RH - 2 * R - 1) / (RH - 2 * R);
+    for (int dx = 0; dx < 3; ++dx)
+        for (int dy = 0; dy < 3; ++dy) {
+            const int ntx = ntx0 + dx, nty = nty0 + dy;
+            if (ntx > a.W || nty > a.H) continue;
+            const int tw = (a.W + ntx - 1) / ntx, th = (a.H + nty - 1) / nty;
+            const long long blocks = (long long)((tw + 2 * R + 3) / 4) * ((th + 2 * R + 1) / 2);
+            const long long rounds = (blocks + NT - 1) / NT;
+            const long long ctas = (long long)ntx * nty * a.B;
+            const long long cost = ((ctas + num_sms - 1) / num_sms) * rounds * NT;
+            if (best.cost < 0 || cost < best.cost || (cost == best.cost && rounds * NT < best.work))
+                best = Plan{ntx, nty, tw, th, cost, rounds * NT};
+        }
+    return best;
 }
 
 template <int KS, int RW, int RH, int NT, int MINB>
-cudaError_t launch_cfg(const StageArgs& a, cudaStream_t st)
+cudaError_t launch_cfg(const StageArgs& a, const Plan& pl, cudaStream_t st)
 {
     using C = Cfg<KS, RW, RH, NT, MINB>;
     static bool attr_done = false;  // per-process; the attribute is per-function and sticky
@@ -257,16 +294,13 @@ cudaError_t launch_cfg(const StageArgs& a, cudaStream_t st)
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    int ntx, nty, tw, th;
-    split(a.W, RW - 2 * C::R, &ntx, &tw);
-    split(a.H, RH - 2 * C::R, &nty, &th);
-    const long long grid = (long long)ntx * nty * a.B;
+    const long long grid = (long long)pl.ntx * pl.nty * a.B;
     if (grid > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    stage_fused_kernel<KS, RW, RH, NT, MINB><<<(unsigned)grid, NT, C::SMEM, st>>>(a, tw, th, ntx, nty);
+    stage_fused_kernel<KS, RW, RH, NT, MINB><<<(unsigned)grid, NT, C::SMEM, st>>>(a, pl.tw, pl.th, pl.ntx, pl.nty);
     return cudaGetLastError();
 }
 
-// TNRD_TILE=<id> (environment, read once) forces a tile configuration; a tuning knob, not part of the ABI.
+// TNRD_TILE=<id> (environment, read once) forces a kernel configuration; a tuning knob, not part of the ABI.
 inline int forced_tile()
 {
     static int v = -1;
@@ -280,18 +314,22 @@ inline int forced_tile()
 template <int KS>
 cudaError_t launch_ks(const StageArgs& a, int num_sms, cudaStream_t st)
 {
+    // 1: 128x128 phi region, 512 threads, 1 CTA/SM (least halo); 2: 64x32, 256 threads, 2 CTAs/SM (small images);
+    // 3: 64x64, 256 threads, 2 CTAs/SM.  Cheapest estimated plan wins; ties go to the shorter CTA.
+    const Plan p1 = plan_tiles<KS, 128, 128, 512>(a, num_sms);
+    const Plan p2 = plan_tiles<KS, 64, 32, 256>(a, num_sms);
+    const Plan p3 = plan_tiles<KS, 64, 64, 256>(a, num_sms);
     int id = forced_tile();
     if (id == 0) {
-        // Large tiles (less halo recompute) when they still fill the machine, small tiles otherwise.
-        int ntx, nty, tw, th;
-        split(a.W, 128 - (KS - 1), &ntx, &tw);
-        split(a.H, 128 - (KS - 1), &nty, &th);
-        id = ((long long)ntx * nty * a.B >= 2LL * num_sms) ? 1 : 2;
+        id = 1;
+        Plan b = p1;
+        if (p3.cost < b.cost || (p3.cost == b.cost && p3.work < b.work)) { id = 3; b = p3; }
+        if (p2.cost < b.cost || (p2.cost == b.cost && p2.work < b.work)) { id = 2; b = p2; }
     }
     switch (id) {
-        case 1: return launch_cfg<KS, 128, 128, 512, 1>(a, st);
-        case 2: return launch_cfg<KS, 64, 32, 256, 2>(a, st);
-        case 3: return launch_cfg<KS, 128, 96, 512, 1>(a, st);
+        case 1: return launch_cfg<KS, 128, 128, 512, 1>(a, p1, st);
+        case 2: return launch_cfg<KS, 64, 32, 256, 2>(a, p2, st);
+        case 3: return launch_cfg<KS, 64, 64, 256, 2>(a, p3, st);
         default: return cudaErrorInvalidValue;
     }
 }
