@@ -54,6 +54,8 @@ def lib() -> ctypes.CDLL:
         L.tnrd_diffuse_host.restype = ci
         L.tnrd_set_kernel.argtypes = [ci]
         L.tnrd_set_kernel.restype = ci
+        L.tnrd_set_phi_mode.argtypes = [ci]
+        L.tnrd_set_phi_mode.restype = ci
         L.tnrd_launch_count.restype = ctypes.c_ulonglong
         L.tnrd_reset_launch_count.restype = None
         L.tnrd_microbench.argtypes = [ci, ctypes.POINTER(ctypes.c_double), vp]
@@ -123,6 +125,11 @@ def tnrd_diffuse_host(f, u0, B, H, W, T, N_k, ksize, filters, rbf_w, rbf_mu, rbf
 
 def tnrd_set_kernel(which: int):
     _check(lib().tnrd_set_kernel(int(which)))
+
+
+def tnrd_set_phi_mode(mode: int):
+    """0 = dense 63-term phi (default), 1 = windowed evaluator (include/tnrd.h: tnrd_set_phi_mode)."""
+    _check(lib().tnrd_set_phi_mode(int(mode)))
 
 
 def tnrd_launch_count() -> int:

@@ -15,6 +15,7 @@ namespace {
 thread_local char g_cuda_err[512] = "";
 unsigned long long g_launches = 0;
 int g_kernel = 0;  // 0 auto, 1 reference, 2 fused
+int g_phi_mode = 0;  // 0 dense 63-term phi, 1 windowed evaluator (dense fallback decided on the device)
 std::mutex g_mu;
 
 int cuda_fail(cudaError_t e, const char* what)
@@ -92,7 +93,7 @@ int run_stage(Scratch* sc, const tnrd::StageArgs& a, cudaStream_t st)
         if (rc != TNRD_OK) return rc;
         TNRD_CUDA(tnrd::launch_stage_ref(a, sc->refv.p, st, &g_launches));
     } else {
-        TNRD_CUDA(tnrd::launch_stage_fused(a, sc->num_sms, st, &g_launches));
+        TNRD_CUDA(tnrd::launch_stage_fused(a, sc->num_sms, g_phi_mode, st, &g_launches));
     }
     return TNRD_OK;
 }
@@ -207,6 +208,13 @@ int tnrd_set_kernel(int which)
 {
     if (which < 0 || which > 2) return TNRD_ERR_UNSUPPORTED;
     g_kernel = which;
+    return TNRD_OK;
+}
+
+int tnrd_set_phi_mode(int mode)
+{
+    if (mode < 0 || mode > 1) return TNRD_ERR_UNSUPPORTED;
+    g_phi_mode = mode;
     return TNRD_OK;
 }
 

@@ -101,7 +101,43 @@ __device__ __forceinline__ void phi_step(const float* __restrict__ mw, const flo
         }
 }
 
-template <int KS, int RW, int RH, int NT, int MINB>
+// ---- windowed phi evaluator (PHI = 1) -------------------------------------------------------------------------------
+// With equidistant centres (spacing delta' in scaled units) and gamma <= delta, every centre farther than 6.5 gamma from
+// a response z contributes less than e^{-21.1} = 6.7e-10 of its weight -- below fp32 rounding of the sum.  Each response
+// therefore evaluates only the 16 consecutive centres j0 .. j0+15 (j0 a multiple of 4) that contain [jc-6, jc+6], jc =
+// nearest centre: 16 MUFU.EX2 instead of 63, weights gathered per lane from the plain w' row of the staged record.
+// win_setup: per response the offset d = z' - mu'_{j0} and the byte offset of w'_{j0} inside the record.
+__device__ __forceinline__ void win_setup1(float z, float inv_delta, float mu0, float delta, float& d, int& wofs)
+{
+    const float tq = (z - mu0) * inv_delta;
+    int jc = __float2int_rn(fminf(fmaxf(tq, 0.0f), 62.0f));
+    int j0 = min(max(jc - 6, 0) & ~3, 48);
+    d = (z - mu0) - (float)j0 * delta;
+    wofs = j0 * 4;
+}
+
+// one step = two consecutive centres (2g, 2g+1 of the window) for the 8 responses of a block; dd is advanced by the
+// caller.  wsec = shared-memory byte address of w'_{i,0} + 8 g.
+__device__ __forceinline__ void phi_win_step(unsigned wsec, const int (&wofs)[4][2], float delta, float2 (&dd)[4],
+                                             float2 (&v)[4])
+{
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+        float2 wa, wb;
+        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(wa.x), "=f"(wa.y) : "r"(wsec + wofs[p][0]));
+        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(wb.x), "=f"(wb.y) : "r"(wsec + wofs[p][1]));
+        const float2 d0 = dd[p];
+        const float2 d1 = __fadd2_rn(d0, make_float2(-delta, -delta));
+        const float2 t0 = __fmul2_rn(d0, d0), t1 = __fmul2_rn(d1, d1);
+        const float2 e0 = make_float2(ex2_neg(t0.x), ex2_neg(t0.y));
+        const float2 e1 = make_float2(ex2_neg(t1.x), ex2_neg(t1.y));
+        v[p] = __ffma2_rn(e0, make_float2(wa.x, wb.x), v[p]);
+        v[p] = __ffma2_rn(e1, make_float2(wa.y, wb.y), v[p]);
+        dd[p] = __fadd2_rn(d1, make_float2(-delta, -delta));
+    }
+}
+
+template <int KS, int RW, int RH, int NT, int MINB, int PHI>
 __global__ void __launch_bounds__(NT, MINB)
 stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
 {
@@ -120,6 +156,12 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
     const int X0 = tx * tw, Y0 = ty * th;          // image coordinates of the output tile origin
     const float* __restrict__ u_img = a.u_in + (size_t)img * a.H * a.W;
     const int N_k = a.N_k;
+    // The windowed evaluator runs only if the staging kernel found the centres equidistant; when it is selected both
+    // kernels are launched and the one that does not apply returns at once (no host synchronisation needed).
+    const float win_ok = __ldg(a.prm + prm_hdr(KS) + 3);
+    if (PHI == 1 ? (win_ok == 0.0f) : (a.dense_is_fallback && win_ok != 0.0f)) return;
+    const float w_inv_delta = __ldg(a.prm + prm_hdr(KS) + 0), w_mu0 = __ldg(a.prm + prm_hdr(KS) + 1),
+                w_delta = __ldg(a.prm + prm_hdr(KS) + 2);
 
     // ---- work decomposition: 4x2 pixel blocks, NB per thread ----------------------------------------------
     const int nbx = (tw + 2 * R + 3) >> 2, nby = (th + 2 * R + 1) >> 1;   // phi region
@@ -186,9 +228,23 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
             const float* vw = vprev + (coff[n] >= 0 ? coff[n] : 0);
             float2 v[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
             float2 zn[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
+            float2 dd[4];
+            int wofs[4][2];
+            unsigned wsec = 0;
+            if (PHI == 1) {
+#pragma unroll
+                for (int p = 0; p < 4; ++p) {
+                    win_setup1(zc[p].x, w_inv_delta, w_mu0, w_delta, dd[p].x, wofs[p][0]);
+                    win_setup1(zc[p].y, w_inv_delta, w_mu0, w_delta, dd[p].y, wofs[p][1]);
+                }
+                wsec = (unsigned)__cvta_generic_to_shared(rec + prm_wplain(KS));
+            }
 #pragma unroll 1
             for (int g = 0; g < C::NG - 1; ++g) {
-                if (hasB) phi_step<8>(rec + KKP + 16 * g, zc, v);
+                if (hasB) {
+                    if (PHI == 1) phi_win_step(wsec + 8 * g, wofs, w_delta, dd, v);
+                    else phi_step<8>(rec + KKP + 16 * g, zc, v);
+                }
                 if (g <= KS) {
                     if (hasN) rowstep<KS, false>(uwn + g * C::US, tapsN + (KS - g) * TS, zn);
                     if (hasC) rowstep<KS, true>(vw + g * C::VS, recp + g * TS, acc[n]);
@@ -199,9 +255,12 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
                     if (hasC) rowstep<KS, true>(vw + g2 * C::VS, recp + g2 * TS, acc[n]);
                 }
             }
-            {   // last step: the remaining 63 - 56 = 7 terms
+            {   // last step: the remaining 63 - 56 = 7 terms (dense) / window centres 14, 15
                 constexpr int g = C::NG - 1;
-                if (hasB) phi_step<TNRD_M - 8 * g>(rec + KKP + 16 * g, zc, v);
+                if (hasB) {
+                    if (PHI == 1) phi_win_step(wsec + 8 * g, wofs, w_delta, dd, v);
+                    else phi_step<TNRD_M - 8 * g>(rec + KKP + 16 * g, zc, v);
+                }
                 if (g <= KS) {
                     if (hasN) rowstep<KS, false>(uwn + g * C::US, tapsN + (KS - g) * TS, zn);
                     if (hasC) rowstep<KS, true>(vw + g * C::VS, recp + g * TS, acc[n]);
@@ -283,20 +342,20 @@ Plan plan_tiles(const StageArgs& a, int num_sms)
     return best;
 }
 
-template <int KS, int RW, int RH, int NT, int MINB>
+template <int KS, int RW, int RH, int NT, int MINB, int PHI>
 cudaError_t launch_cfg(const StageArgs& a, const Plan& pl, cudaStream_t st)
 {
     using C = Cfg<KS, RW, RH, NT, MINB>;
     static bool attr_done = false;  // per-process; the attribute is per-function and sticky
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<KS, RW, RH, NT, MINB>,
+        cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<KS, RW, RH, NT, MINB, PHI>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
     const long long grid = (long long)pl.ntx * pl.nty * a.B;
     if (grid > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    stage_fused_kernel<KS, RW, RH, NT, MINB><<<(unsigned)grid, NT, C::SMEM, st>>>(a, pl.tw, pl.th, pl.ntx, pl.nty);
+    stage_fused_kernel<KS, RW, RH, NT, MINB, PHI><<<(unsigned)grid, NT, C::SMEM, st>>>(a, pl.tw, pl.th, pl.ntx, pl.nty);
     return cudaGetLastError();
 }
 
@@ -311,7 +370,7 @@ inline int forced_tile()
     return v;
 }
 
-template <int KS>
+template <int KS, int PHI>
 cudaError_t launch_ks(const StageArgs& a, int num_sms, cudaStream_t st)
 {
     // 1: 128x128 phi region, 512 threads, 1 CTA/SM (least halo); 2: 64x32, 256 threads, 2 CTAs/SM (small images);
@@ -327,9 +386,9 @@ cudaError_t launch_ks(const StageArgs& a, int num_sms, cudaStream_t st)
         if (p2.cost < b.cost || (p2.cost == b.cost && p2.work < b.work)) { id = 2; b = p2; }
     }
     switch (id) {
-        case 1: return launch_cfg<KS, 128, 128, 512, 1>(a, p1, st);
-        case 2: return launch_cfg<KS, 64, 32, 256, 2>(a, p2, st);
-        case 3: return launch_cfg<KS, 64, 64, 256, 2>(a, p3, st);
+        case 1: return launch_cfg<KS, 128, 128, 512, 1, PHI>(a, p1, st);
+        case 2: return launch_cfg<KS, 64, 32, 256, 2, PHI>(a, p2, st);
+        case 3: return launch_cfg<KS, 64, 64, 256, 2, PHI>(a, p3, st);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -338,16 +397,29 @@ cudaError_t launch_ks(const StageArgs& a, int num_sms, cudaStream_t st)
 
 cudaError_t fused_init() { return cudaSuccess; }
 
-cudaError_t launch_stage_fused(const StageArgs& a, int num_sms, cudaStream_t st, unsigned long long* launches)
+template <int PHI>
+cudaError_t launch_phi(const StageArgs& a, int num_sms, cudaStream_t st)
 {
-    cudaError_t e;
     switch (a.ksize) {
-        case 3: e = launch_ks<3>(a, num_sms, st); break;
-        case 5: e = launch_ks<5>(a, num_sms, st); break;
-        case 7: e = launch_ks<7>(a, num_sms, st); break;
-        case 9: e = launch_ks<9>(a, num_sms, st); break;
+        case 3: return launch_ks<3, PHI>(a, num_sms, st);
+        case 5: return launch_ks<5, PHI>(a, num_sms, st);
+        case 7: return launch_ks<7, PHI>(a, num_sms, st);
+        case 9: return launch_ks<9, PHI>(a, num_sms, st);
         default: return cudaErrorInvalidValue;
     }
+}
+
+cudaError_t launch_stage_fused(const StageArgs& a_in, int num_sms, int phi_mode, cudaStream_t st,
+                               unsigned long long* launches)
+{
+    StageArgs a = a_in;
+    a.dense_is_fallback = (phi_mode == 1);
+    if (phi_mode == 1) {            // windowed evaluator; exits at once when the centres are not equidistant ...
+        cudaError_t e = launch_phi<1>(a, num_sms, st);
+        ++*launches;
+        if (e != cudaSuccess) return e;
+    }
+    cudaError_t e = launch_phi<0>(a, num_sms, st);   // ... in which case this dense launch does the work (else it exits)
     ++*launches;
     return e;
 }

@@ -16,12 +16,18 @@ namespace tnrd {
 //            4x2 pixel block at once: forward filter at window row wr uses row rho = ksize - wr, transposed filter
 //            at window row wr uses row rho = wr.
 //   pairs    at offset prm_kkp: 64 pairs (-mu'_j, w'_ij) = (-s * mu_j, w_ij / s), pair 63 = (0, 0)
+//   wplain   at offset prm_wplain: w'_ij, j = 0..63 (w'_i63 = 0), for the windowed phi evaluator's per-lane gathers
+//   hdr      at offset prm_hdr: (1/delta', mu'_0, delta', ok) -- centre spacing in scaled units and ok = 1.0f when the
+//            centres are equidistant (|mu_j - mu_0 - j delta| <= 1e-4 delta) and gamma <= delta (window of 16 centres
+//            then holds every centre within 6.5 gamma of any z); the same four floats in every record
 // so that phi_i(k_i * u) = sum_j w_ij 2^{-(z' - mu'_j)^2} with z' = k'_i * u, and the transposed bank
 // sum_i kbar_i * v_i = sum_i kbar'_i * (v_i / s) re-uses the same scaled taps.
 __host__ __device__ constexpr int prm_ts(int ksize) { return ((2 * ksize + 3) / 4) * 4; }
 __host__ __device__ constexpr int prm_tap(int ksize, int a, int b) { return (a + 1) * prm_ts(ksize) + 2 * b; }
 __host__ __device__ constexpr int prm_kkp(int ksize) { return (ksize + 1) * prm_ts(ksize); }
-__host__ __device__ constexpr int prm_stride(int ksize) { return prm_kkp(ksize) + 2 * TNRD_MP; }
+__host__ __device__ constexpr int prm_wplain(int ksize) { return prm_kkp(ksize) + 2 * TNRD_MP; }
+__host__ __device__ constexpr int prm_hdr(int ksize) { return prm_wplain(ksize) + TNRD_MP; }
+__host__ __device__ constexpr int prm_stride(int ksize) { return prm_hdr(ksize) + 4; }
 
 // Half-sample symmetric mirror map, edge pixel repeated, then clamped so that
 // coordinates beyond the 2r halo (ragged tiles) still address memory inside the image.
@@ -41,6 +47,7 @@ struct StageArgs {
     const float* lambda_ptr; // device pointer to lambda_t, or nullptr -> lambda_val
     float lambda_val;
     int B, H, W, N_k, ksize;
+    int dense_is_fallback;  // set by the launcher: the dense kernel returns at once when the windowed one applies
 };
 
 // launchers (each returns the cudaError_t of the launch; *launches += kernels launched)
@@ -48,7 +55,8 @@ cudaError_t launch_prep(const float* filters, const float* rbf_w, const float* r
                         int T, int N_k, int ksize, float* prm, cudaStream_t st, unsigned long long* launches);
 cudaError_t launch_stage_ref(const StageArgs& a, float* vbuf, cudaStream_t st, unsigned long long* launches);
 size_t ref_scratch_floats(int B, int H, int W, int N_k, int ksize);
-cudaError_t launch_stage_fused(const StageArgs& a, int num_sms, cudaStream_t st, unsigned long long* launches);
+cudaError_t launch_stage_fused(const StageArgs& a, int num_sms, int phi_mode, cudaStream_t st,
+                               unsigned long long* launches);   // phi_mode: 0 dense, 1 windowed (with dense fallback)
 cudaError_t fused_init();   // opt-in shared memory attributes; idempotent
 cudaError_t run_microbench(int which, double* rate, cudaStream_t st, unsigned long long* launches);
 

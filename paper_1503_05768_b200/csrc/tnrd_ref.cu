@@ -29,9 +29,25 @@ __global__ void prep_params_kernel(const float* __restrict__ filters, const floa
         if (e < KKP) {
             const int rho = e / TS, c = e - rho * TS, b = c >> 1, a = rho - 1 + (c & 1);
             if (a >= 0 && a < ksize && b < ksize) val = s * filters[(size_t)rec * KK + a * ksize + b];
-        } else {
+        } else if (e < KKP + 2 * TNRD_MP) {
             const int j = (e - KKP) >> 1, which = (e - KKP) & 1;
             if (j < TNRD_M) val = which ? rbf_w[(size_t)rec * TNRD_M + j] / s : -s * rbf_mu[j];
+        } else if (e < KKP + 3 * TNRD_MP) {
+            const int j = e - KKP - 2 * TNRD_MP;
+            if (j < TNRD_M) val = rbf_w[(size_t)rec * TNRD_M + j] / s;
+        } else {
+            // header: spacing of the centres in scaled units and the "windowed evaluator is valid" flag
+            const float mu0 = rbf_mu[0], delta = (rbf_mu[TNRD_M - 1] - mu0) / (float)(TNRD_M - 1);
+            const int h = e - KKP - 3 * TNRD_MP;
+            if (h == 0) val = 1.0f / (s * delta);
+            else if (h == 1) val = s * mu0;
+            else if (h == 2) val = s * delta;
+            else {
+                bool ok = delta > 0.0f && gamma <= delta * 1.000001f;
+                for (int j = 0; j < TNRD_M && ok; ++j)
+                    ok = fabsf(rbf_mu[j] - (mu0 + (float)j * delta)) <= 1e-4f * delta;
+                val = ok ? 1.0f : 0.0f;
+            }
         }
         prm[idx] = val;
     }

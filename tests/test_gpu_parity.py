@@ -218,3 +218,62 @@ def test_microbench_rates_are_sane(tnrd):
     ffma, mufu, phi = (tnrd.tnrd_microbench(i) for i in range(3))
     print(f"FFMA {ffma / 1e12:.2f} T/s  MUFU.EX2 {mufu / 1e12:.2f} T/s  phi terms {phi / 1e12:.2f} T/s")
     assert 5e12 < ffma < 60e12 and 1e12 < mufu < 12e12 and 0.5e12 < phi <= mufu * 1.05
+
+
+# --- windowed phi evaluator (tnrd_set_phi_mode(1)): same oracle, same tolerance ------------------------------------
+def run_gpu_window(tnrd, c, **kw):
+    tnrd.tnrd_set_phi_mode(1)
+    try:
+        return run_gpu(tnrd, c, **kw)
+    finally:
+        tnrd.tnrd_set_phi_mode(0)
+
+
+@pytest.mark.parametrize("case", SMALL, ids=[f"s{c[0]}" for c in SMALL])
+def test_window_phi_small_cases(tnrd, case):
+    seed, B, H, W, T, n_k, K = case
+    c = tnrd_gen.make_small(seed, B, H, W, T, n_k, K)
+    check(run_gpu_window(tnrd, c), run_oracle(c), f"window case {case}")
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_window_phi_configs(tnrd, cfg):
+    c = tnrd_gen.make_config(cfg)
+    got = run_gpu_window(tnrd, c)
+    mx, rms = check(got, run_oracle(c), f"window config {cfg}")
+    dense = run_gpu(tnrd, c)
+    print(f"window config {cfg}: max-abs {mx:.3e} rms {rms:.3e}; vs dense GPU {np.max(np.abs(got - dense)):.3e}")
+    assert np.max(np.abs(got - dense)) <= 2e-4     # truncated mass < 1e-9 w: only fp32 rounding differs
+
+
+def test_window_phi_extreme_responses(tnrd):
+    # responses far outside [mu_1, mu_63] and large weights on the outermost centres: the clamped window must hold
+    c = tnrd_gen.make_small(50, 1, 40, 44, 1, 6, 5)
+    c["f"] = (c["f"] * 6.0 - 400.0).astype(np.float32); c["u0"] = c["f"].copy()     # z up to ~ +-1000
+    w = c["rbf_w"].copy(); w[..., :3] = 0.5; w[..., -3:] = -0.5; c["rbf_w"] = w
+    check(run_gpu_window(tnrd, c), run_oracle(c), "window extreme")
+
+
+def test_window_phi_falls_back_to_dense(tnrd):
+    c = tnrd_gen.make_small(51, 2, 50, 61, 2, 5, 7)
+    for change in ("jitter", "gamma"):
+        d = dict(c)
+        if change == "jitter":                      # centres not equidistant
+            mu = c["rbf_mu"].copy(); mu[10] += 2.0; d["rbf_mu"] = mu
+        else:                                       # gamma > delta: 16 centres no longer cover 6.5 gamma
+            d["rbf_gamma"] = 14.0
+        dense = run_gpu(tnrd, d)
+        tnrd.tnrd_reset_launch_count()
+        got = run_gpu_window(tnrd, d)
+        assert tnrd.tnrd_launch_count() == 1 + 2 * d["T"]      # both kernels launched, one returns at once
+        assert np.array_equal(got, dense), change               # ... and the dense one did the work
+        check(got, run_oracle(d), f"fallback {change}")
+
+
+def test_window_phi_full_size_windows(tnrd):
+    c = tnrd_gen.make_config(4, size=2048, T=5)
+    got = run_gpu_window(tnrd, c)[0]
+    for (y0, x0) in _windows(2048, 2048, 24, 2, 9)[::2]:
+        want = oracle.diffuse_window(c["f"][0], c["u0"][0], c["filters"], c["rbf_w"], c["rbf_mu"],
+                                     c["rbf_gamma"], c["lambda"], y0, x0, 24, 24)
+        check(got[y0:y0 + 24, x0:x0 + 24], want, f"window C4-2048 {(y0, x0)}")
