@@ -158,10 +158,15 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
     const int N_k = a.N_k;
     // The windowed evaluator runs only if the staging kernel found the centres equidistant; when it is selected both
     // kernels are launched and the one that does not apply returns at once (no host synchronisation needed).
-    const float win_ok = __ldg(a.prm + prm_hdr(KS) + 3);
-    if (PHI == 1 ? (win_ok == 0.0f) : (a.dense_is_fallback && win_ok != 0.0f)) return;
-    const float w_inv_delta = __ldg(a.prm + prm_hdr(KS) + 0), w_mu0 = __ldg(a.prm + prm_hdr(KS) + 1),
-                w_delta = __ldg(a.prm + prm_hdr(KS) + 2);
+    float w_inv_delta = 0.f, w_mu0 = 0.f, w_delta = 0.f;
+    if (PHI == 1) {
+        if (__ldg(a.prm + prm_hdr(KS) + 3) == 0.0f) return;
+        w_inv_delta = __ldg(a.prm + prm_hdr(KS) + 0);
+        w_mu0 = __ldg(a.prm + prm_hdr(KS) + 1);
+        w_delta = __ldg(a.prm + prm_hdr(KS) + 2);
+    } else if (a.dense_is_fallback) {
+        if (__ldg(a.prm + prm_hdr(KS) + 3) != 0.0f) return;
+    }
 
     // ---- work decomposition: 4x2 pixel blocks, NB per thread ----------------------------------------------
     const int nbx = (tw + 2 * R + 3) >> 2, nby = (th + 2 * R + 1) >> 1;   // phi region

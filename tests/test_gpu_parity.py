@@ -18,6 +18,7 @@ def tnrd():
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     import paper_1503_05768_b200 as t
+    t.build()                    # compiles libtnrd.so with nvcc if it is stale or absent (not a fallback)
     t.lib()                      # fails loudly if libtnrd.so is missing: no fallback
     t.tnrd_set_kernel(0)
     return t
