@@ -179,3 +179,56 @@ def diffuse_window(f, u0, filters, rbf_w, rbf_mu, rbf_gamma, lambdas, y0, x0, h,
     xa, xb = max(0, x0 - m), min(W, x0 + w + m)
     res = diffuse(f2[ya:yb, xa:xb], u2[ya:yb, xa:xb], filters, rbf_w, rbf_mu, rbf_gamma, lambdas)
     return res[y0 - ya:y0 - ya + h, x0 - xa:x0 - xa + w]
+
+
+# ---- JPEG-deblocking stage (Main Eq. 9; Supp. Eq. 26-29) -----------------------------------------------------
+def _load_deblock():
+    lib = _load()
+    if not getattr(lib, "_deblock_ready", False):
+        dp, ci, cd = ctypes.POINTER(ctypes.c_double), ctypes.c_int, ctypes.c_double
+        lib.oracle_block_dct8.argtypes = [dp, ci, ci, ci, dp]
+        lib.oracle_block_dct8.restype = ci
+        lib.oracle_qcs_project.argtypes = [dp, ci, ci, dp, dp, dp]
+        lib.oracle_qcs_project.restype = ci
+        lib.oracle_deblock_stage.argtypes = [dp, ci, ci, ci, ci, ci, dp, dp, dp, ci, cd, dp, dp, dp]
+        lib.oracle_deblock_stage.restype = ci
+        lib.oracle_deblock_diffuse.argtypes = [dp, ci, ci, ci, ci, ci, ci, dp, dp, dp, ci, cd, dp, dp, dp]
+        lib.oracle_deblock_diffuse.restype = ci
+        lib._deblock_ready = True
+    return lib
+
+
+def block_dct8(img, inverse: bool = False):
+    """Orthonormal 2-D DCT-II (inverse: DCT-III) of every 8x8 block of one image; coefficient layout in place."""
+    a = _d(img)
+    out = np.empty_like(a)
+    rc = _load_deblock().oracle_block_dct8(_p(a), a.shape[0], a.shape[1], int(bool(inverse)), _p(out))
+    if rc != 0:
+        raise ValueError(f"oracle_block_dct8 failed with {rc}")
+    return out
+
+
+def qcs_project(y, lo, hi):
+    """u = D^T eta(D y) for one image (Supp. Eq. 26-27)."""
+    y, lo, hi = _d(y), _d(lo), _d(hi)
+    out = np.empty_like(y)
+    rc = _load_deblock().oracle_qcs_project(_p(y), y.shape[0], y.shape[1], _p(lo), _p(hi), _p(out))
+    if rc != 0:
+        raise ValueError(f"oracle_qcs_project failed with {rc}")
+    return out
+
+
+def deblock_diffuse(u0, filters, rbf_w, rbf_mu, rbf_gamma: float, qcs_lo, qcs_hi):
+    """T deblocking stages (Supp. Eq. 28-29); T = filters.shape[0]; returns float64 [B][H][W]."""
+    u3, lo, hi = _img3(u0), _img3(qcs_lo), _img3(qcs_hi)
+    k, w, mu = _d(filters), _d(rbf_w), _d(rbf_mu)
+    B, H, W = u3.shape
+    T = k.shape[0]
+    n_k, K = (k.shape[1], k.shape[2]) if T > 0 else (1, 1)
+    assert lo.shape == u3.shape and hi.shape == u3.shape
+    out = np.empty_like(u3)
+    rc = _load_deblock().oracle_deblock_diffuse(_p(u3), B, H, W, T, n_k, K, _p(k), _p(w), _p(mu), mu.size,
+                                                float(rbf_gamma), _p(lo), _p(hi), _p(out))
+    if rc != 0:
+        raise ValueError(f"oracle_deblock_diffuse failed with {rc}")
+    return out if np.ndim(u0) == 3 else out[0]

@@ -239,3 +239,115 @@ int oracle_diffuse(const double *f, const double *u0, int B, int H, int W, int T
     free(cur); free(nxt);
     return ORACLE_OK;
 }
+
+/* =====================================================================================================
+ * JPEG-deblocking stage (Main Eq. 9; Supp. Eq. 26-29):
+ *     y = u_{t-1} - sum_i kbar_i * phi_i(k_i * u_{t-1})      (diffusion term only, no reaction term)
+ *     z = D y            D = orthonormal 2-D DCT-II of every 8x8 block ("D^T D = D D^T = I")
+ *     v = eta(z)         point-wise projection onto the box [a_p, b_p] (QCS, Supp. Eq. 26)
+ *     u_t = D^T v
+ * Coefficient (p, q) of block (by, bx) is stored at pixel position (8 by + p, 8 bx + q); a, b use the same
+ * layout.  H and W must be multiples of 8.  The paper pads by omega = 8: a whole block, so the
+ * block grid of the padded image coincides with the image's own and, with re-padding every stage
+ * (u_tp = P_T u_t), the centre H x W result is exactly the above with the diffusion term of O1-O4
+ * (reading D1).
+ * Pins (tests/test_oracle_deblock.py): D against scipy.fft.dctn(norm="ortho"), orthogonality / Parseval,
+ * closed forms (constant block, single cosine), projection properties, reduction to the pinned denoising
+ * stage when the box is infinite.
+ * ===================================================================================================== */
+
+/* 2-D DCT-II (inverse != 0: DCT-III, its transpose) of every 8x8 block, by the definition:
+ *   c[p][q] = alpha_p alpha_q sum_{y,x} in[y][x] cos(pi (2y+1) p / 16) cos(pi (2x+1) q / 16),
+ *   alpha_0 = sqrt(1/8), alpha_p = sqrt(2/8).                                                          */
+int oracle_block_dct8(const double *in, int H, int W, int inverse, double *out)
+{
+    if (!in || !out || H < 8 || W < 8 || (H % 8) || (W % 8)) return ORACLE_ERR_ARG;
+    const double pi = 3.14159265358979323846;
+    double cs[8][8]; /* cs[p][y] = alpha_p cos(pi (2y+1) p / 16) */
+    for (int p = 0; p < 8; ++p)
+        for (int y = 0; y < 8; ++y)
+            cs[p][y] = (p == 0 ? sqrt(1.0 / 8.0) : sqrt(2.0 / 8.0)) * cos(pi * (2.0 * y + 1.0) * p / 16.0);
+#pragma omp parallel for schedule(static)
+    for (int by = 0; by < H / 8; ++by) {
+        for (int bx = 0; bx < W / 8; ++bx) {
+            const double *src = in + (size_t)(8 * by) * W + 8 * bx;
+            double *dst = out + (size_t)(8 * by) * W + 8 * bx;
+            double tmp[8][8];
+            for (int p = 0; p < 8; ++p)
+                for (int q = 0; q < 8; ++q) {
+                    double acc = 0.0;
+                    for (int y = 0; y < 8; ++y)
+                        for (int x = 0; x < 8; ++x) {
+                            const double basis = inverse ? cs[y][p] * cs[x][q] : cs[p][y] * cs[q][x];
+                            acc += src[(size_t)y * W + x] * basis;
+                        }
+                    tmp[p][q] = acc;
+                }
+            for (int p = 0; p < 8; ++p)
+                for (int q = 0; q < 8; ++q) dst[(size_t)p * W + q] = tmp[p][q];
+        }
+    }
+    return ORACLE_OK;
+}
+
+/* u = D^T eta(D y): projection of one image onto the QCS in the DCT domain (Supp. Eq. 26-27). */
+int oracle_qcs_project(const double *y, int H, int W, const double *lo, const double *hi, double *u)
+{
+    if (!y || !lo || !hi || !u) return ORACLE_ERR_ARG;
+    const size_t n = (size_t)H * W;
+    double *z = (double *)malloc(sizeof(double) * n);
+    if (!z) return ORACLE_ERR_MEM;
+    int rc = oracle_block_dct8(y, H, W, 0, z);
+    if (rc == ORACLE_OK) {
+        for (size_t p = 0; p < n; ++p) { /* eta, Supp. Eq. 26 */
+            if (z[p] > hi[p]) z[p] = hi[p];
+            else if (z[p] < lo[p]) z[p] = lo[p];
+        }
+        rc = oracle_block_dct8(z, H, W, 1, u);
+    }
+    free(z);
+    return rc;
+}
+
+/* One deblocking stage on a batch (Supp. Eq. 29).  lo / hi are [B][H][W]. */
+int oracle_deblock_stage(const double *u_in, int B, int H, int W, int N_k, int K, const double *filters_t,
+                         const double *rbf_w_t, const double *rbf_mu, int M, double gamma, const double *lo,
+                         const double *hi, double *u_out)
+{
+    if (!u_in || !lo || !hi || !u_out) return ORACLE_ERR_ARG;
+    if ((H % 8) || (W % 8)) return ORACLE_ERR_ARG;
+    const size_t n = (size_t)H * W;
+    double *y = (double *)malloc(sizeof(double) * n);
+    if (!y) return ORACLE_ERR_MEM;
+    int rc = ORACLE_OK;
+    for (int b = 0; b < B && rc == ORACLE_OK; ++b) {
+        /* y = u - sum_i kbar_i * phi_i(k_i * u): the denoising stage with lambda = 0 (f is then irrelevant) */
+        rc = oracle_stage(u_in + b * n, u_in + b * n, 1, H, W, N_k, K, filters_t, rbf_w_t, rbf_mu, M, gamma, 0.0, y,
+                          ORACLE_SYMMETRIC_2R);
+        if (rc == ORACLE_OK) rc = oracle_qcs_project(y, H, W, lo + b * n, hi + b * n, u_out + b * n);
+    }
+    free(y);
+    return rc;
+}
+
+/* T deblocking stages with per-stage parameters Theta_t = {phi_i^t, k_i^t}. */
+int oracle_deblock_diffuse(const double *u0, int B, int H, int W, int T, int N_k, int K, const double *filters,
+                           const double *rbf_w, const double *rbf_mu, int M, double gamma, const double *lo,
+                           const double *hi, double *out)
+{
+    if (!u0 || !out || T < 0) return ORACLE_ERR_ARG;
+    const size_t n = (size_t)B * H * W;
+    double *cur = (double *)malloc(sizeof(double) * n);
+    double *nxt = (double *)malloc(sizeof(double) * n);
+    if (!cur || !nxt) { free(cur); free(nxt); return ORACLE_ERR_MEM; }
+    memcpy(cur, u0, sizeof(double) * n);
+    int rc = ORACLE_OK;
+    for (int t = 0; t < T && rc == ORACLE_OK; ++t) {
+        rc = oracle_deblock_stage(cur, B, H, W, N_k, K, filters + (size_t)t * N_k * K * K,
+                                  rbf_w + (size_t)t * N_k * M, rbf_mu, M, gamma, lo, hi, nxt);
+        double *tmp = cur; cur = nxt; nxt = tmp;
+    }
+    if (rc == ORACLE_OK) memcpy(out, cur, sizeof(double) * n);
+    free(cur); free(nxt);
+    return rc;
+}

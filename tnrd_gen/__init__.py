@@ -1,4 +1,4 @@
-"""Seeded synthetic inputs and parameters for the TNRD hot path (NumPy only).
+"""Seeded synthetic inputs and parameters for the TNRD hot path (NumPy; SciPy only for the JPEG-like codec simulator).
 
 This module serves BOTH the CPU oracle (``oracle/``) and the CUDA library
 (``paper_1503_05768_b200``).  It holds none of the method's arithmetic: no
@@ -222,5 +222,53 @@ def make_small(seed: int, B: int, H: int, W: int, T: int, n_k: int, ksize: int,
                       for _ in range(B)], axis=0)
     f = np.ascontiguousarray(add_noise(clean, sigma, rng), dtype=np.float32)
     out = dict(B=B, H=H, W=W, cfg=0, f=f, u0=f.copy(), clean=clean.astype(np.float32))
+    out.update(prm)
+    return out
+
+
+# --------------------------------------------------------------------------
+# JPEG-deblocking inputs: a synthetic compress / decompress round trip
+# --------------------------------------------------------------------------
+def synthetic_quant_table(strength: float) -> np.ndarray:
+    """8x8 quantisation steps growing with frequency, Q[i][j] = strength * (1 + 0.6 (i + j) + 0.15 i j).
+
+    A stand-in for a JPEG luminance table at some quality (the real tables and JPEG files are not available
+    here); `strength` plays the role of the quality factor (larger = coarser)."""
+    i = np.arange(8, dtype=np.float64)[:, None]
+    j = np.arange(8, dtype=np.float64)[None, :]
+    return strength * (1.0 + 0.6 * (i + j) + 0.15 * i * j)
+
+
+def jpeg_like_roundtrip(clean: np.ndarray, qtable: np.ndarray):
+    """Block-DCT, quantise, dequantise, inverse DCT of one image (H, W multiples of 8).
+
+    Returns (decoded image, qcs_lo, qcs_hi): the decoder output u0 and the quantisation constraint set
+    S = [Q (d - 1/2), Q (d + 1/2)] in block-coefficient layout.  Uses scipy's DCT: this is data
+    synthesis (a codec simulator), not the method under test."""
+    import scipy.fft as sfft
+    H, W = clean.shape
+    assert H % 8 == 0 and W % 8 == 0
+    blocks = clean.reshape(H // 8, 8, W // 8, 8).transpose(0, 2, 1, 3)
+    coef = sfft.dctn(blocks, type=2, norm="ortho", axes=(2, 3))
+    d = np.rint(coef / qtable)
+    lo, hi = qtable * (d - 0.5), qtable * (d + 0.5)
+    dec = sfft.idctn(qtable * d, type=2, norm="ortho", axes=(2, 3))
+    back = lambda a: a.transpose(0, 2, 1, 3).reshape(H, W)  # noqa: E731
+    return back(dec), back(lo), back(hi)
+
+
+def make_deblock(seed: int, B: int, H: int, W: int, T: int, n_k: int, ksize: int,
+                 strength: float = 6.0) -> dict:
+    """Deblocking case: decoded images u0, QCS bounds and per-stage parameters (no lambda: PAPER.md:716)."""
+    rng = rng_for(2000 + seed, 0, 0)
+    prm = make_params(2000 + seed, T, n_k, ksize)
+    q = synthetic_quant_table(strength)
+    u0, lo, hi, clean = [], [], [], []
+    for _ in range(B):
+        c = image_field_texture(H, W, rng, blur_sigma=max(2.0, min(12.0, H / 16.0)))
+        d, a, b = jpeg_like_roundtrip(c, q)
+        clean.append(c); u0.append(d); lo.append(a); hi.append(b)
+    f32 = lambda xs: np.ascontiguousarray(np.stack(xs), dtype=np.float32)  # noqa: E731
+    out = dict(B=B, H=H, W=W, u0=f32(u0), qcs_lo=f32(lo), qcs_hi=f32(hi), clean=f32(clean))
     out.update(prm)
     return out
