@@ -94,6 +94,26 @@ int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int 
                       const float* lambda, float* out, void* stream);
 
 /*
+ * JPEG-deblocking variant (Main Eq. 9; Supp. Eq. 26-29).  Per stage
+ *     y = u_{t-1} - sum_i kbar_i^t * phi_i^t(k_i^t * u_{t-1})        (the diffusion term of tnrd_stage, no reaction term)
+ *     u_t = D^T eta(D y)                                              (projection onto the quantisation constraint set)
+ * D is the orthonormal 2-D DCT-II of every 8x8 block (D^T D = I; the block grid starts at pixel (0,0)),
+ * eta clamps coefficient p to [qcs_lo_p, qcs_hi_p] (Supp. Eq. 26).  Coefficient (p, q) of block (by, bx) lives at pixel
+ * (8 by + p, 8 bx + q) of a [B][H][W] array; qcs_lo / qcs_hi use that layout and refer to the DCT of u itself (no level
+ * shift).  H and W must be multiples of 8 (TNRD_ERR_SHAPE otherwise); the paper's pad width omega = 8 is
+ * one whole block, so with the 2r mirror halo of the diffusion term the H x W result is the paper's (D1).
+ *   u0, qcs_lo, qcs_hi, out   device, [B][H][W];  filters [T][N_k][ksize][ksize], rbf_w [T][N_k][63], rbf_mu [63] device
+ *   out may equal u0; out must not equal qcs_lo or qcs_hi.  T = 0 copies u0.  Asynchronous on `stream`.
+ */
+int tnrd_deblock_diffuse(const float* u0, int B, int H, int W, int T, int N_k, int ksize, const float* filters,
+                         const float* rbf_w, const float* rbf_mu, float rbf_gamma, const float* qcs_lo,
+                         const float* qcs_hi, float* out, void* stream);
+
+/* u_out = D^T eta(D y) alone (all device, [B][H][W]; u_out may equal y).  Asynchronous on `stream`. */
+int tnrd_qcs_project(const float* y, int B, int H, int W, const float* qcs_lo, const float* qcs_hi, float* u_out,
+                     void* stream);
+
+/*
  * Kernel selection, for tests and profiling.  which = 0: automatic (default); 1: the plain one-thread-per-
  * pixel reference kernel (global memory only); 2: the fused tiled stage kernel.  Returns TNRD_ERR_UNSUPPORTED
  * for other values.  Process-wide.

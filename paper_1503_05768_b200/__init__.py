@@ -52,6 +52,10 @@ def lib() -> ctypes.CDLL:
         L.tnrd_diffuse.restype = ci
         L.tnrd_diffuse_host.argtypes = dargs
         L.tnrd_diffuse_host.restype = ci
+        L.tnrd_deblock_diffuse.argtypes = [vp, ci, ci, ci, ci, ci, ci, vp, vp, vp, cf, vp, vp, vp, vp]
+        L.tnrd_deblock_diffuse.restype = ci
+        L.tnrd_qcs_project.argtypes = [vp, ci, ci, ci, vp, vp, vp, vp]
+        L.tnrd_qcs_project.restype = ci
         L.tnrd_set_kernel.argtypes = [ci]
         L.tnrd_set_kernel.restype = ci
         L.tnrd_set_phi_mode.argtypes = [ci]
@@ -121,6 +125,20 @@ def tnrd_diffuse_host(f, u0, B, H, W, T, N_k, ksize, filters, rbf_w, rbf_mu, rbf
     _check(lib().tnrd_diffuse_host(_ptr(f), _ptr(u0), B, H, W, T, N_k, ksize, _ptr(filters), _ptr(rbf_w),
                                    _ptr(rbf_mu), float(rbf_gamma), _ptr(lam), _ptr(out), _stream(stream)))
     return out
+
+
+def tnrd_deblock_diffuse(u0, B, H, W, T, N_k, ksize, filters, rbf_w, rbf_mu, rbf_gamma, qcs_lo, qcs_hi, out,
+                         stream=None):
+    """T JPEG-deblocking stages on device buffers (include/tnrd.h: tnrd_deblock_diffuse)."""
+    _check(lib().tnrd_deblock_diffuse(_ptr(u0), B, H, W, T, N_k, ksize, _ptr(filters), _ptr(rbf_w), _ptr(rbf_mu),
+                                      float(rbf_gamma), _ptr(qcs_lo), _ptr(qcs_hi), _ptr(out), _stream(stream)))
+    return out
+
+
+def tnrd_qcs_project(y, B, H, W, qcs_lo, qcs_hi, u_out, stream=None):
+    """u_out = D^T eta(D y) on device buffers (include/tnrd.h: tnrd_qcs_project)."""
+    _check(lib().tnrd_qcs_project(_ptr(y), B, H, W, _ptr(qcs_lo), _ptr(qcs_hi), _ptr(u_out), _stream(stream)))
+    return u_out
 
 
 def tnrd_set_kernel(which: int):

@@ -204,6 +204,59 @@ int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int 
     return TNRD_OK;
 }
 
+int tnrd_qcs_project(const float* y, int B, int H, int W, const float* qcs_lo, const float* qcs_hi, float* u_out,
+                     void* stream)
+{
+    if (!y || !qcs_lo || !qcs_hi || !u_out) return TNRD_ERR_NULL;
+    if (B < 1 || H < 8 || W < 8 || (H % 8) || (W % 8) || (long long)B * H * W >= (1LL << 31)) return TNRD_ERR_SHAPE;
+    if (u_out == qcs_lo || u_out == qcs_hi) return TNRD_ERR_ALIAS;
+    TNRD_CUDA(tnrd::launch_qcs_project(y, qcs_lo, qcs_hi, u_out, B, H, W, (cudaStream_t)stream, &g_launches));
+    return TNRD_OK;
+}
+
+int tnrd_deblock_diffuse(const float* u0, int B, int H, int W, int T, int N_k, int ksize, const float* filters,
+                         const float* rbf_w, const float* rbf_mu, float rbf_gamma, const float* qcs_lo,
+                         const float* qcs_hi, float* out, void* stream)
+{
+    if (!u0 || !out || !qcs_lo || !qcs_hi) return TNRD_ERR_NULL;
+    if (T < 0) return TNRD_ERR_SHAPE;
+    if (T > 0 && (!filters || !rbf_w || !rbf_mu)) return TNRD_ERR_NULL;
+    int rc = check_shape(B, H, W, N_k, ksize);
+    if (rc != TNRD_OK) return rc;
+    if ((H % 8) || (W % 8)) return TNRD_ERR_SHAPE;
+    if ((rc = check_gamma(rbf_gamma)) != TNRD_OK) return rc;
+    if (out == qcs_lo || out == qcs_hi) return TNRD_ERR_ALIAS;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)B * H * W;
+    if (T == 0) {
+        if (out != u0) TNRD_CUDA(cudaMemcpyAsync(out, u0, n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        return TNRD_OK;
+    }
+    Scratch* sc = nullptr;
+    if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
+    const size_t rec = (size_t)N_k * tnrd::prm_stride(ksize);
+    if ((rc = grow(sc->prm, (size_t)T * rec, st)) != TNRD_OK) return rc;
+    const bool inplace_odd = (out == u0) && (T & 1);
+    if (T > 1 && (rc = grow(sc->plane[0], n, st)) != TNRD_OK) return rc;
+    if (inplace_odd && (rc = grow(sc->plane[1], n, st)) != TNRD_OK) return rc;
+    TNRD_CUDA(tnrd::launch_prep(filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, sc->prm.p, st, &g_launches));
+    // Same ping-pong as tnrd_diffuse.  Per stage (Supp. Eq. 29): the fused kernel with lambda = 0 writes
+    // y = u - sum_i kbar_i * phi_i(k_i * u) to the destination plane (f is then irrelevant: u itself is passed),
+    // the projection kernel turns it into u_t = D^T eta(D y) in place.
+    const float* src = u0;
+    for (int t = 1; t <= T; ++t) {
+        float* dst;
+        if (t == 1 && inplace_odd) dst = sc->plane[1].p;
+        else dst = ((T - t) & 1) ? sc->plane[0].p : out;
+        tnrd::StageArgs a{src, src, dst, sc->prm.p + (size_t)(t - 1) * rec, nullptr, 0.0f, B, H, W, N_k, ksize};
+        if ((rc = run_stage(sc, a, st)) != TNRD_OK) return rc;
+        TNRD_CUDA(tnrd::launch_qcs_project(dst, qcs_lo, qcs_hi, dst, B, H, W, st, &g_launches));
+        src = dst;
+    }
+    if (src != out) TNRD_CUDA(cudaMemcpyAsync(out, src, n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    return TNRD_OK;
+}
+
 int tnrd_set_kernel(int which)
 {
     if (which < 0 || which > 2) return TNRD_ERR_UNSUPPORTED;

@@ -57,6 +57,8 @@ cudaError_t launch_stage_ref(const StageArgs& a, float* vbuf, cudaStream_t st, u
 size_t ref_scratch_floats(int B, int H, int W, int N_k, int ksize);
 cudaError_t launch_stage_fused(const StageArgs& a, int num_sms, int phi_mode, cudaStream_t st,
                                unsigned long long* launches);   // phi_mode: 0 dense, 1 windowed (with dense fallback)
+cudaError_t launch_qcs_project(const float* y, const float* lo, const float* hi, float* u, int B, int H, int W,
+                               cudaStream_t st, unsigned long long* launches);   // u may alias y
 cudaError_t fused_init();   // opt-in shared memory attributes; idempotent
 cudaError_t run_microbench(int which, double* rate, cudaStream_t st, unsigned long long* launches);
 

@@ -75,6 +75,13 @@ def test_argument_validation_without_gpu(L):
     assert L.tnrd_stage(p, p + 64, 1, 8, 8, 4, 3, p, p, p, 10.0, 0.1, p + 64, st) == tnrd.ERR_ALIAS
     assert L.tnrd_stage(p, p + 64, 1, 8, 8, 4, 3, p, p, p, 10.0, 0.1, p, st) == tnrd.ERR_ALIAS
     assert L.tnrd_diffuse(p, p + 64, 1, 8, 8, 2, 4, 3, p, p, p, 10.0, p, p, st) == tnrd.ERR_ALIAS
+    # deblocking: H, W multiples of 8; bounds may not be the output
+    assert L.tnrd_deblock_diffuse(p, 1, 12, 16, 1, 4, 3, p, p, p, 10.0, p, p, p + 64, st) == tnrd.ERR_SHAPE
+    assert L.tnrd_deblock_diffuse(p, 1, 16, 16, 1, 4, 3, p, p, p, 10.0, p, n, p + 64, st) == tnrd.ERR_NULL
+    assert L.tnrd_deblock_diffuse(p, 1, 16, 16, 1, 4, 3, p, p, p, 10.0, p, p + 64, p + 64, st) == tnrd.ERR_ALIAS
+    assert L.tnrd_qcs_project(p, 1, 16, 20, p, p, p + 64, st) == tnrd.ERR_SHAPE
+    assert L.tnrd_qcs_project(p, 1, 16, 16, p + 64, p, p + 64, st) == tnrd.ERR_ALIAS
+    assert L.tnrd_set_phi_mode(3) == tnrd.ERR_UNSUPPORTED and L.tnrd_set_phi_mode(0) == tnrd.OK
     # options
     assert L.tnrd_set_kernel(7) == tnrd.ERR_UNSUPPORTED
     assert L.tnrd_set_kernel(0) == tnrd.OK
