@@ -147,7 +147,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5"],
+    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5", "deblock"],
                     help="BASELINE.json config; c4 (default) is the headline, the others are for exploration")
     ap.add_argument("--size", type=int, default=4096)
     ap.add_argument("--T", type=int, default=5)
@@ -179,8 +179,14 @@ def main():
         dist.init_process_group("nccl", device_id=devs)
     warmup = max(args.warmup, 3)
 
-    cfg = (tnrd_gen.make_config(4, size=args.size, T=args.T) if args.workload == "c4"
-           else tnrd_gen.make_config(int(args.workload[1])))
+    deblock = args.workload == "deblock"
+    if deblock:      # TRD^4_{7x7} JPEG deblocking at 1024^2, the size the paper times it at
+        cfg = tnrd_gen.make_deblock(9, 1, 1024, 1024, 4, 48, 7)
+        cfg["f"], cfg["lambda"] = cfg["u0"], np.zeros(4, dtype=np.float32)
+        args.no_window = True
+    else:
+        cfg = (tnrd_gen.make_config(4, size=args.size, T=args.T) if args.workload == "c4"
+               else tnrd_gen.make_config(int(args.workload[1])))
     B, H, W, T = cfg["B"], cfg["H"], cfg["W"], cfg["T"]
     N_K, KSIZE = cfg["N_k"], cfg["ksize"]
     EX2_PER_PX_STAGE, FMA_PER_PX_STAGE = N_K * M, 2 * N_K * KSIZE * KSIZE
@@ -192,8 +198,14 @@ def main():
     gamma = cfg["rbf_gamma"]
     stream = torch.cuda.current_stream()
 
+    if deblock:
+        qlo, qhi = torch.from_numpy(cfg["qcs_lo"]).to(devs), torch.from_numpy(cfg["qcs_hi"]).to(devs)
+
     def step():
-        tnrd.tnrd_diffuse(f, f, B, H, W, T, N_K, KSIZE, k, w, mu, gamma, lam, out, stream)
+        if deblock:
+            tnrd.tnrd_deblock_diffuse(f, B, H, W, T, N_K, KSIZE, k, w, mu, gamma, qlo, qhi, out, stream)
+        else:
+            tnrd.tnrd_diffuse(f, f, B, H, W, T, N_K, KSIZE, k, w, mu, gamma, lam, out, stream)
 
     def barrier():
         torch.cuda.synchronize()
@@ -222,8 +234,18 @@ def main():
     hout = torch.empty_like(hf).pin_memory()
     hp = [cfg["filters"], cfg["rbf_w"], cfg["rbf_mu"], cfg["lambda"]]
 
+    if deblock:
+        hq = [torch.from_numpy(cfg["qcs_lo"]).pin_memory(), torch.from_numpy(cfg["qcs_hi"]).pin_memory()]
+        dq = [torch.empty_like(f), torch.empty_like(f), torch.empty_like(f), torch.empty_like(f)]
+
     def step_host():
-        tnrd.tnrd_diffuse_host(hf, hf, B, H, W, T, N_K, KSIZE, hp[0], hp[1], hp[2], gamma, hp[3], hout, stream)
+        if deblock:   # no host entry point for this variant: explicit pinned copies around the device call
+            dq[0].copy_(hf, non_blocking=True); dq[1].copy_(hq[0], non_blocking=True); dq[2].copy_(hq[1], non_blocking=True)
+            tnrd.tnrd_deblock_diffuse(dq[0], B, H, W, T, N_K, KSIZE, k, w, mu, gamma, dq[1], dq[2], dq[3], stream)
+            hout.copy_(dq[3], non_blocking=True)
+            stream.synchronize()
+        else:
+            tnrd.tnrd_diffuse_host(hf, hf, B, H, W, T, N_K, KSIZE, hp[0], hp[1], hp[2], gamma, hp[3], hout, stream)
 
     step_host()
     barrier()
@@ -236,7 +258,7 @@ def main():
     barrier()
     ms_e2e = max_over_ranks(e2.elapsed_time(e3), devs)
     e2e_value = sum_over_ranks(float(B) * H * W * T * e2e_steps, devs) / (ms_e2e * 1e-3) / 1e6
-    h2d = hf.numel() * 4 + sum(int(a.nbytes) for a in hp)
+    h2d = hf.numel() * 4 * (3 if deblock else 1) + (0 if deblock else sum(int(a.nbytes) for a in hp))
     d2h = hout.numel() * 4
     same = bool(torch.equal(hout.to(devs), out))
 
@@ -281,8 +303,9 @@ def main():
         "metric": METRIC, "value": value, "unit": "Mpixel-stages/s", "n_gpus": world, "steps": args.steps,
         "warmup": warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"C{args.workload[1]} {B}x{H}x{W} T={T} N_k={N_K} {KSIZE}x{KSIZE} M=63 "
-                               f"(BASELINE.json configs[{int(args.workload[1]) - 1}]), one such batch per GPU",
+        "config": {"workload": (f"JPEG deblocking TRD^4_7x7 {B}x{H}x{W} (PAPER.md:287), synthetic QCS" if deblock else
+                                f"C{args.workload[1]} {B}x{H}x{W} T={T} N_k={N_K} {KSIZE}x{KSIZE} M=63 "
+                                f"(BASELINE.json configs[{int(args.workload[1]) - 1}]), one such batch per GPU"),
                    "global_batch": world * B, "parallelism": f"dp{world} (independent images, no collective)",
                    "l2": ("inputs larger than L2 (3 planes x %d MB)" % (B * H * W * 4 // 2 ** 20)) if 3 * B * H * W * 4 > 126e6
                    else "working set fits L2 (exploration workload)"},
