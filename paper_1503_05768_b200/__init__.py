@@ -28,11 +28,10 @@ class TnrdError(RuntimeError):
         self.status = status
 
 
-def build(verbose: bool = False) -> str:
+def build(verbose: bool = False, force: bool = False) -> str:
     """Compile libtnrd.so in-tree for sm_100a (nvcc cross-compiles without a GPU)."""
-    import importlib
-    _b = importlib.import_module(__name__ + ".build")   # the submodule, not this function
-    return _b.build(verbose=verbose)
+    from . import _build
+    return _build.build(verbose=verbose, force=force)
 
 
 def lib() -> ctypes.CDLL:
@@ -41,7 +40,7 @@ def lib() -> ctypes.CDLL:
     if _lib is None:
         if not os.path.exists(LIB_PATH):
             raise FileNotFoundError(
-                f"{LIB_PATH} is missing: build it with `python -m paper_1503_05768_b200.build` "
+                f"{LIB_PATH} is missing: build it with `python -m paper_1503_05768_b200._build` "
                 "(there is no CPU fallback for the TNRD hot path)")
         L = ctypes.CDLL(LIB_PATH)
         vp, ci, cf = ctypes.c_void_p, ctypes.c_int, ctypes.c_float

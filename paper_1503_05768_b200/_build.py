@@ -1,4 +1,4 @@
-"""Build libtnrd.so in-tree for sm_100a:  python -m paper_1503_05768_b200.build [-v]"""
+"""Build libtnrd.so in-tree for sm_100a:  python -m paper_1503_05768_b200._build [-v]"""
 from __future__ import annotations
 
 import glob
