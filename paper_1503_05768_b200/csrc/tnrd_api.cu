@@ -41,6 +41,7 @@ struct Scratch {
     cudaStream_t st = nullptr;
     int num_sms = 0;
     Buf prm, plane[2], refv;          // staged parameters, ping-pong planes, reference-path phi maps
+    Buf split;                        // small-image path: tile counters (kept zero between launches) + partial sums
     Buf h_f, h_u, h_out, h_par;       // device staging of the host entry point
 };
 std::vector<Scratch*> g_scratch;
@@ -93,7 +94,13 @@ int run_stage(Scratch* sc, const tnrd::StageArgs& a, cudaStream_t st)
         if (rc != TNRD_OK) return rc;
         TNRD_CUDA(tnrd::launch_stage_ref(a, sc->refv.p, st, &g_launches));
     } else {
-        TNRD_CUDA(tnrd::launch_stage_fused(a, sc->num_sms, g_phi_mode, st, &g_launches));
+        const tnrd::FusedPlan pl = tnrd::plan_stage_fused(a, sc->num_sms);
+        if (pl.split_floats > sc->split.cap) {
+            int rc = grow(sc->split, pl.split_floats, st);
+            if (rc != TNRD_OK) return rc;
+            TNRD_CUDA(cudaMemsetAsync(sc->split.p, 0, sc->split.cap * sizeof(float), st));
+        }
+        TNRD_CUDA(tnrd::launch_stage_fused(a, pl, sc->split.p, g_phi_mode, st, &g_launches));
     }
     return TNRD_OK;
 }
@@ -306,7 +313,7 @@ void tnrd_shutdown(void)
     (void)cudaGetDevice(&cur);
     for (Scratch* s : g_scratch) {
         (void)cudaSetDevice(s->dev);
-        Buf* bufs[] = {&s->prm, &s->plane[0], &s->plane[1], &s->refv, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
+        Buf* bufs[] = {&s->prm, &s->plane[0], &s->plane[1], &s->refv, &s->split, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
         for (Buf* b : bufs)
             if (b->p) (void)cudaFree(b->p);   // synchronising free: the stream may be gone by now
         delete s;

@@ -22,6 +22,7 @@
 //     every warp always carries a mix of MUFU and FMA work instead of all warps of a CTA filtering in lock-step;
 //   * packed fp32x2 arithmetic (FADD2 / FMUL2 / FFMA2, sm_100): the two output rows of a 4x2 block form the two
 //     halves of one register pair, which halves the issue slots of everything that is not a MUFU.
+#include <cstdio>
 #include <cstdlib>
 
 #include "tnrd_internal.h"
@@ -37,6 +38,10 @@ __device__ __forceinline__ float ex2_neg(float x)
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(-x));
     return y;
 }
+
+// small-image path: the scratch starts with this many tile counters (a fixed area, so that launches with different
+// tile counts never see each other's partial sums as counters), followed by the partial sums
+constexpr int SPLIT_COUNTERS = 4096;
 
 template <int KS, int RW, int RH, int NT, int MINB = 1>
 struct Cfg {
@@ -139,7 +144,7 @@ __device__ __forceinline__ void phi_win_step(unsigned wsec, const int (&wofs)[4]
 
 template <int KS, int RW, int RH, int NT, int MINB, int PHI>
 __global__ void __launch_bounds__(NT, MINB)
-stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
+stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty, int nsplit, float* __restrict__ split)
 {
     using C = Cfg<KS, RW, RH, NT, MINB>;
     constexpr int R = C::R, TS = C::TS, KKP = prm_kkp(KS);
@@ -149,13 +154,14 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
     float* ps = vs + 2 * C::VPLANE;                // [4][PRM]   staged records of filters i-1 .. i+2
 
     const int tid = threadIdx.x;
-    int t = blockIdx.x;
+    int t = blockIdx.x;                            // tile; blockIdx.y = this CTA's chunk of the filter bank
     const int tx = t % ntx; t /= ntx;
     const int ty = t % nty; t /= nty;
     const int img = t;
     const int X0 = tx * tw, Y0 = ty * th;          // image coordinates of the output tile origin
     const float* __restrict__ u_img = a.u_in + (size_t)img * a.H * a.W;
-    const int N_k = a.N_k;
+    const int f0 = (int)(blockIdx.y * a.N_k / nsplit);
+    const int N_k = (int)((blockIdx.y + 1) * a.N_k / nsplit) - f0;          // filters f0 .. f0 + N_k - 1
     // The windowed evaluator runs only if the staging kernel found the centres equidistant; when it is selected both
     // kernels are launched and the one that does not apply returns at once (no host synchronisation needed).
     float w_inv_delta = 0.f, w_mu0 = 0.f, w_delta = 0.f;
@@ -171,18 +177,24 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
     // ---- work decomposition: 4x2 pixel blocks, NB per thread ----------------------------------------------
     const int nbx = (tw + 2 * R + 3) >> 2, nby = (th + 2 * R + 1) >> 1;   // phi region
     const int nbxo = (tw + 3) >> 2, nbyo = (th + 1) >> 1;                  // output tile
+    const int nrounds = (nbx * nby + NT - 1) / NT;   // rounds of blocks this tile needs (<= NB): the software pipeline
+                                                     // wraps from the last USED round to block 0 of the next filter
 
     // ---- a1: gather the u tile through the mirror map (only the rows / columns some block will read) -----
     {
         const int nr = min(C::UH, 2 * nby + 2 * R), nc = min(C::US, 4 * nbx + 2 * R + 4);
+#pragma unroll 2
         for (int uy = tid >> 5; uy < nr; uy += NT / 32) {
             const float* __restrict__ grow = u_img + (size_t)mirror_clamp(Y0 - 2 * R + uy, a.H) * a.W;
-            for (int ux = tid & 31; ux < nc; ux += 32)
-                us[uy * C::US + ux] = __ldg(grow + mirror_clamp(X0 - 2 * R + ux, a.W));
+#pragma unroll
+            for (int q = 0; q < (C::US + 31) / 32; ++q) {          // all loads of a row issued before the first store
+                const int ux = (tid & 31) + 32 * q;
+                if (ux < nc) us[uy * C::US + ux] = __ldg(grow + mirror_clamp(X0 - 2 * R + ux, a.W));
+            }
         }
     }
     for (int idx = tid; idx < 2 * C::PRM; idx += NT)
-        if (idx < N_k * C::PRM) ps[idx] = __ldg(a.prm + idx);          // records 0 and 1
+        if (idx < N_k * C::PRM) ps[idx] = __ldg(a.prm + (size_t)f0 * C::PRM + idx);   // records 0 and 1
 
     int uoff[C::NB], voff[C::NB], coff[C::NB];   // block origins in us / a phi map (phi side) / a phi map (output side)
 #pragma unroll
@@ -212,7 +224,7 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
     // ---- filter loop ------------------------------------------------------------------------------------------
     for (int i = 0; i < N_k; ++i) {
         if (i + 2 < N_k) {                                    // stage record i+2 (read from iteration i+1 on)
-            const float* src = a.prm + (size_t)(i + 2) * C::PRM;
+            const float* src = a.prm + (size_t)((int)(blockIdx.y * a.N_k / nsplit) + i + 2) * C::PRM;
             float* dst = ps + ((i + 2) & 3) * C::PRM;
             for (int idx = tid; idx < C::PRM; idx += NT) dst[idx] = __ldg(src + idx);
         }
@@ -223,7 +235,8 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
         const float* vprev = vs + ((i + 1) & 1) * C::VPLANE;
 #pragma unroll
         for (int n = 0; n < C::NB; ++n) {
-            const bool last = (n == C::NB - 1);
+            if (n >= nrounds) break;
+            const bool last = (n == nrounds - 1);
             const int un = last ? uoff[0] : uoff[(n + 1) % C::NB];
             const bool hasB = uoff[n] >= 0;                               // phi of block n
             const bool hasN = un >= 0 && (!last || i + 1 < N_k);          // forward filter of the next block
@@ -293,6 +306,53 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
         }
     }
 
+    // ---- small-image path: the nsplit CTAs of a tile meet in scratch; the last one to arrive adds the partial
+    // sums in fixed order (deterministic) and goes on to a5, the others are done ---------------------------------
+    if (nsplit > 1) {
+        __shared__ int s_last;
+        unsigned* counters = reinterpret_cast<unsigned*>(split);
+        const int tile = blockIdx.x, part = blockIdx.y;
+        float* part0 = split + SPLIT_COUNTERS + (size_t)tile * nsplit * (C::NB * NT * 8);
+        float* mine = part0 + (size_t)part * (C::NB * NT * 8);
+#pragma unroll
+        for (int n = 0; n < C::NB; ++n) {
+            if (coff[n] < 0) continue;
+            float4* d = reinterpret_cast<float4*>(mine + ((size_t)n * NT + tid) * 8);
+            __stcg(d, make_float4(acc[n][0].x, acc[n][0].y, acc[n][1].x, acc[n][1].y));
+            __stcg(d + 1, make_float4(acc[n][2].x, acc[n][2].y, acc[n][3].x, acc[n][3].y));
+        }
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) {
+            const unsigned prev = atomicAdd(counters + tile, 1u);
+            s_last = (prev == (unsigned)nsplit - 1);
+            if (s_last) counters[tile] = 0;                    // ready for the next launch
+        }
+        __syncthreads();
+        if (!s_last) return;
+        __threadfence();
+#pragma unroll
+        for (int n = 0; n < C::NB; ++n) {
+            if (coff[n] < 0) continue;
+#pragma unroll
+            for (int p = 0; p < 4; ++p) acc[n][p] = make_float2(0.f, 0.f);
+            const float4* sp = reinterpret_cast<const float4*>(part0 + ((size_t)n * NT + tid) * 8);
+            constexpr size_t QS = (size_t)C::NB * NT * 2;            // float4s between the partial sums of two CTAs
+            for (int q0 = 0; q0 < nsplit; q0 += 4) {                 // loads in batches of 4 CTAs, adds in CTA order
+                float4 lo[4], hi[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if (q0 + j < nsplit) { lo[j] = __ldcg(sp + (q0 + j) * QS); hi[j] = __ldcg(sp + (q0 + j) * QS + 1); }
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if (q0 + j < nsplit) {
+                        acc[n][0].x += lo[j].x; acc[n][0].y += lo[j].y; acc[n][1].x += lo[j].z; acc[n][1].y += lo[j].w;
+                        acc[n][2].x += hi[j].x; acc[n][2].y += hi[j].y; acc[n][3].x += hi[j].z; acc[n][3].y += hi[j].w;
+                    }
+            }
+        }
+    }
+
     // ---- a5: reaction term and update ------------------------------------------------------------------------
     const float lambda = a.lambda_ptr ? __ldg(a.lambda_ptr) : a.lambda_val;
     const float* __restrict__ f_img = a.f + (size_t)img * a.H * a.W;
@@ -318,19 +378,32 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty)
 
 // ---- host side: tile plan and launch ------------------------------------------------------------------------------
 struct Plan {
-    int ntx, nty, tw, th;
-    long long cost;   // estimated time in thread-rounds per SM (see plan_tiles)
+    int ntx, nty, tw, th, nsplit;
+    double cost;      // estimated time of the launch in (thread-rounds x filters) per SM (see plan_tiles)
     long long work;   // thread-rounds of one CTA (critical path; tie-break)
 };
 
+inline int env_int(const char* name)
+{
+    const char* e = getenv(name);
+    return e ? atoi(e) : 0;
+}
+// TNRD_TILE=<id> / TNRD_SPLIT=<n> (environment, read at every plan) force a kernel configuration / a filter split;
+// tuning and test knobs, not part of the ABI.
+inline int forced_tile() { return env_int("TNRD_TILE"); }
+inline int forced_split() { return env_int("TNRD_SPLIT"); }
+
 // Tile plan for one kernel configuration.  The path is XU-bound, so an SM's time is proportional to the phi work
-// assigned to it: (CTAs per SM) x (rounds of 4x2 blocks per thread, 1..NB) x (threads per CTA).  Try the fewest equal
-// tiles that cover the image and a few more in each direction (a smaller tile can save a whole round), keep the cheapest.
-template <int KS, int RW, int RH, int NT>
+// assigned to it: (CTAs per SM) x (rounds of 4x2 blocks per thread, 1..NB) x (threads per CTA) x (filters per CTA + a
+// constant for the tile gather, the pipeline fill/drain and the epilogue).  Try the fewest equal tiles that cover the
+// image and a few more in each direction (a smaller tile can save a whole round); when the tiles of the whole batch
+// do not fill the GPU (small images), also try splitting the filter bank of a tile over nsplit CTAs -- every split
+// pays the constant again plus the read-back of the partial sums by the last CTA.  Keep the cheapest.
+template <int KS, int RW, int RH, int NT, int MINB>
 Plan plan_tiles(const StageArgs& a, int num_sms)
 {
     constexpr int R = (KS - 1) / 2;
-    Plan best{0, 0, 0, 0, -1, 0};
+    Plan best{0, 0, 0, 0, 1, -1.0, 0};
     const int ntx0 = (a.W + RW - 2 * R - 1) / (RW - 2 * R), nty0 = (a.H + RH - 2 * R - 1) / (RH - 2 * R);
     for (int dx = 0; dx < 3; ++dx)
         for (int dy = 0; dy < 3; ++dy) {
@@ -339,16 +412,29 @@ Plan plan_tiles(const StageArgs& a, int num_sms)
             const int tw = (a.W + ntx - 1) / ntx, th = (a.H + nty - 1) / nty;
             const long long blocks = (long long)((tw + 2 * R + 3) / 4) * ((th + 2 * R + 1) / 2);
             const long long rounds = (blocks + NT - 1) / NT;
-            const long long ctas = (long long)ntx * nty * a.B;
-            const long long cost = ((ctas + num_sms - 1) / num_sms) * rounds * NT;
-            if (best.cost < 0 || cost < best.cost || (cost == best.cost && rounds * NT < best.work))
-                best = Plan{ntx, nty, tw, th, cost, rounds * NT};
+            const long long tiles = (long long)ntx * nty * a.B;
+            int smax = 1;
+            if (tiles < (long long)num_sms * MINB) smax = a.N_k < 32 ? a.N_k : 32;
+            if (tiles > SPLIT_COUNTERS) smax = 1;
+            int slo = 1;
+            if (forced_split() > 0) slo = smax = forced_split() < a.N_k ? forced_split() : a.N_k;
+            for (int sp = slo; sp <= smax; ++sp) {
+                const int nf = (a.N_k + sp - 1) / sp;                      // filters of the largest chunk
+                if (sp > slo && (a.N_k + sp - 2) / (sp - 1) == nf) continue; // same chunk as sp - 1: only more CTAs
+                const long long ctas = tiles * sp;
+                // measured (C3, B200): ~18 us per filter for 1024 thread-rounds, ~20 us per CTA of fixed cost (tile
+                // gather, pipeline fill and drain, epilogue), ~0.5 us per split for the read-back
+                const double per_cta = (double)(rounds * NT) * nf + 1100.0 + (sp > 1 ? 30.0 * sp : 0.0);
+                const double cost = (double)((ctas + num_sms - 1) / num_sms) * per_cta;
+                if (best.cost < 0 || cost < best.cost || (cost == best.cost && rounds * NT < best.work))
+                    best = Plan{ntx, nty, tw, th, sp, cost, rounds * NT};
+            }
         }
     return best;
 }
 
 template <int KS, int RW, int RH, int NT, int MINB, int PHI>
-cudaError_t launch_cfg(const StageArgs& a, const Plan& pl, cudaStream_t st)
+cudaError_t launch_cfg(const StageArgs& a, const FusedPlan& pl, float* split, cudaStream_t st)
 {
     using C = Cfg<KS, RW, RH, NT, MINB>;
     static bool attr_done = false;  // per-process; the attribute is per-function and sticky
@@ -359,41 +445,47 @@ cudaError_t launch_cfg(const StageArgs& a, const Plan& pl, cudaStream_t st)
         attr_done = true;
     }
     const long long grid = (long long)pl.ntx * pl.nty * a.B;
-    if (grid > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    stage_fused_kernel<KS, RW, RH, NT, MINB, PHI><<<(unsigned)grid, NT, C::SMEM, st>>>(a, pl.tw, pl.th, pl.ntx, pl.nty);
+    if (grid > 0x7fffffffLL || pl.nsplit > 65535) return cudaErrorInvalidConfiguration;
+    if (pl.nsplit > 1 && !split) return cudaErrorInvalidValue;
+    stage_fused_kernel<KS, RW, RH, NT, MINB, PHI><<<dim3((unsigned)grid, (unsigned)pl.nsplit), NT, C::SMEM, st>>>(
+        a, pl.tw, pl.th, pl.ntx, pl.nty, pl.nsplit, split);
     return cudaGetLastError();
 }
 
-// TNRD_TILE=<id> (environment, read once) forces a kernel configuration; a tuning knob, not part of the ABI.
-inline int forced_tile()
-{
-    static int v = -1;
-    if (v < 0) {
-        const char* e = getenv("TNRD_TILE");
-        v = e ? atoi(e) : 0;
-    }
-    return v;
-}
-
-template <int KS, int PHI>
-cudaError_t launch_ks(const StageArgs& a, int num_sms, cudaStream_t st)
+template <int KS>
+FusedPlan plan_ks(const StageArgs& a, int num_sms)
 {
     // 1: 128x128 phi region, 512 threads, 1 CTA/SM (least halo); 2: 64x32, 256 threads, 2 CTAs/SM (small images);
     // 3: 64x64, 256 threads, 2 CTAs/SM.  Cheapest estimated plan wins; ties go to the shorter CTA.
-    const Plan p1 = plan_tiles<KS, 128, 128, 512>(a, num_sms);
-    const Plan p2 = plan_tiles<KS, 64, 32, 256>(a, num_sms);
-    const Plan p3 = plan_tiles<KS, 64, 64, 256>(a, num_sms);
+    const Plan p[3] = {plan_tiles<KS, 128, 128, 512, 1>(a, num_sms), plan_tiles<KS, 64, 32, 256, 2>(a, num_sms),
+                       plan_tiles<KS, 64, 64, 256, 2>(a, num_sms)};
+    const size_t per_cta[3] = {Cfg<KS, 128, 128, 512, 1>::NB * 512 * 8, Cfg<KS, 64, 32, 256, 2>::NB * 256 * 8,
+                               Cfg<KS, 64, 64, 256, 2>::NB * 256 * 8};
     int id = forced_tile();
-    if (id == 0) {
+    if (id < 1 || id > 3) {
         id = 1;
-        Plan b = p1;
-        if (p3.cost < b.cost || (p3.cost == b.cost && p3.work < b.work)) { id = 3; b = p3; }
-        if (p2.cost < b.cost || (p2.cost == b.cost && p2.work < b.work)) { id = 2; b = p2; }
+        if (p[2].cost < p[id - 1].cost || (p[2].cost == p[id - 1].cost && p[2].work < p[id - 1].work)) id = 3;
+        if (p[1].cost < p[id - 1].cost || (p[1].cost == p[id - 1].cost && p[1].work < p[id - 1].work)) id = 2;
     }
-    switch (id) {
-        case 1: return launch_cfg<KS, 128, 128, 512, 1, PHI>(a, p1, st);
-        case 2: return launch_cfg<KS, 64, 32, 256, 2, PHI>(a, p2, st);
-        case 3: return launch_cfg<KS, 64, 64, 256, 2, PHI>(a, p3, st);
+    const Plan& b = p[id - 1];
+    if (env_int("TNRD_DEBUG_PLAN"))
+        fprintf(stderr, "tnrd plan: %dx%dx%d ks %d N_k %d -> cfg %d, %d x %d tiles of %d x %d, split %d, cost %.0f\n", a.B,
+                a.H, a.W, KS, a.N_k, id, b.ntx, b.nty, b.tw, b.th, b.nsplit, b.cost);
+    FusedPlan fp{id, b.ntx, b.nty, b.tw, b.th, b.nsplit, 0};
+    if (b.nsplit > 1) {
+        const size_t tiles = (size_t)b.ntx * b.nty * a.B;
+        fp.split_floats = SPLIT_COUNTERS + tiles * b.nsplit * per_cta[id - 1];
+    }
+    return fp;
+}
+
+template <int KS, int PHI>
+cudaError_t launch_ks(const StageArgs& a, const FusedPlan& pl, float* split, cudaStream_t st)
+{
+    switch (pl.cfg) {
+        case 1: return launch_cfg<KS, 128, 128, 512, 1, PHI>(a, pl, split, st);
+        case 2: return launch_cfg<KS, 64, 32, 256, 2, PHI>(a, pl, split, st);
+        case 3: return launch_cfg<KS, 64, 64, 256, 2, PHI>(a, pl, split, st);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -402,29 +494,39 @@ cudaError_t launch_ks(const StageArgs& a, int num_sms, cudaStream_t st)
 
 cudaError_t fused_init() { return cudaSuccess; }
 
-template <int PHI>
-cudaError_t launch_phi(const StageArgs& a, int num_sms, cudaStream_t st)
+FusedPlan plan_stage_fused(const StageArgs& a, int num_sms)
 {
     switch (a.ksize) {
-        case 3: return launch_ks<3, PHI>(a, num_sms, st);
-        case 5: return launch_ks<5, PHI>(a, num_sms, st);
-        case 7: return launch_ks<7, PHI>(a, num_sms, st);
-        case 9: return launch_ks<9, PHI>(a, num_sms, st);
+        case 3: return plan_ks<3>(a, num_sms);
+        case 5: return plan_ks<5>(a, num_sms);
+        case 7: return plan_ks<7>(a, num_sms);
+        default: return plan_ks<9>(a, num_sms);
+    }
+}
+
+template <int PHI>
+cudaError_t launch_phi(const StageArgs& a, const FusedPlan& pl, float* split, cudaStream_t st)
+{
+    switch (a.ksize) {
+        case 3: return launch_ks<3, PHI>(a, pl, split, st);
+        case 5: return launch_ks<5, PHI>(a, pl, split, st);
+        case 7: return launch_ks<7, PHI>(a, pl, split, st);
+        case 9: return launch_ks<9, PHI>(a, pl, split, st);
         default: return cudaErrorInvalidValue;
     }
 }
 
-cudaError_t launch_stage_fused(const StageArgs& a_in, int num_sms, int phi_mode, cudaStream_t st,
+cudaError_t launch_stage_fused(const StageArgs& a_in, const FusedPlan& pl, float* split, int phi_mode, cudaStream_t st,
                                unsigned long long* launches)
 {
     StageArgs a = a_in;
     a.dense_is_fallback = (phi_mode == 1);
     if (phi_mode == 1) {            // windowed evaluator; exits at once when the centres are not equidistant ...
-        cudaError_t e = launch_phi<1>(a, num_sms, st);
+        cudaError_t e = launch_phi<1>(a, pl, split, st);
         ++*launches;
         if (e != cudaSuccess) return e;
     }
-    cudaError_t e = launch_phi<0>(a, num_sms, st);   // ... in which case this dense launch does the work (else it exits)
+    cudaError_t e = launch_phi<0>(a, pl, split, st);   // ... in which case this dense launch does the work (else it exits)
     ++*launches;
     return e;
 }

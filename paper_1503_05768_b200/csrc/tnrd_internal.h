@@ -50,13 +50,27 @@ struct StageArgs {
     int dense_is_fallback;  // set by the launcher: the dense kernel returns at once when the windowed one applies
 };
 
+// Launch plan of the fused stage kernel (tnrd_fused.cu: plan_stage_fused).  nsplit > 1 = the small-image path: the
+// filter bank of one tile is split over nsplit CTAs, whose partial transposed-filter sums meet in `split_floats`
+// floats of scratch (the last CTA of a tile to arrive adds them in fixed order and writes u_t).
+struct FusedPlan {
+    int cfg;                 // kernel configuration 1..3 (tile size / threads)
+    int ntx, nty, tw, th;    // tiles per image and output tile size
+    int nsplit;              // CTAs per tile (each takes a contiguous chunk of the N_k filters)
+    size_t split_floats;     // scratch needed when nsplit > 1: counters (one per tile) + partial sums; else 0
+};
+
 // launchers (each returns the cudaError_t of the launch; *launches += kernels launched)
 cudaError_t launch_prep(const float* filters, const float* rbf_w, const float* rbf_mu, float gamma,
                         int T, int N_k, int ksize, float* prm, cudaStream_t st, unsigned long long* launches);
 cudaError_t launch_stage_ref(const StageArgs& a, float* vbuf, cudaStream_t st, unsigned long long* launches);
 size_t ref_scratch_floats(int B, int H, int W, int N_k, int ksize);
-cudaError_t launch_stage_fused(const StageArgs& a, int num_sms, int phi_mode, cudaStream_t st,
-                               unsigned long long* launches);   // phi_mode: 0 dense, 1 windowed (with dense fallback)
+FusedPlan plan_stage_fused(const StageArgs& a, int num_sms);
+// phi_mode: 0 dense, 1 windowed (with dense fallback).  split = scratch of plan.split_floats floats whose first
+// 4096 words (tile counters) are zero before the first launch (the kernel leaves them zero); may be null when
+// nsplit == 1.
+cudaError_t launch_stage_fused(const StageArgs& a, const FusedPlan& plan, float* split, int phi_mode, cudaStream_t st,
+                               unsigned long long* launches);
 cudaError_t launch_qcs_project(const float* y, const float* lo, const float* hi, float* u, int B, int H, int W,
                                cudaStream_t st, unsigned long long* launches);   // u may alias y
 cudaError_t fused_init();   // opt-in shared memory attributes; idempotent
