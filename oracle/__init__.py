@@ -19,6 +19,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "tnrd_oracle.c")
+_SRCS = [_SRC, os.path.join(_HERE, "tnrd_oracle_bwd.c")]
 _LIB = os.path.join(_HERE, "liboracle_tnrd.so")
 
 SYMMETRIC_2R = 0   # reading A, the default boundary handling
@@ -29,8 +30,8 @@ _lib = None
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc -O2 (no fast-math).  Building the checker is not using it."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp", "-o", _LIB, _SRC, "-lm"]
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(s) for s in _SRCS):
+        cmd = ["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp", "-o", _LIB] + _SRCS + ["-lm"]
         subprocess.run(cmd, check=True, cwd=_HERE)
     return _LIB
 
@@ -232,3 +233,94 @@ def deblock_diffuse(u0, filters, rbf_w, rbf_mu, rbf_gamma: float, qcs_lo, qcs_hi
     if rc != 0:
         raise ValueError(f"oracle_deblock_diffuse failed with {rc}")
     return out if np.ndim(u0) == 3 else out[0]
+
+
+# ---- backward pass of a stage (Supp. Sec. 2: Eq. 7, 10, 19, 21) -- oracle/tnrd_oracle_bwd.c ---------------------
+def _load_bwd():
+    lib = _load()
+    if not getattr(lib, "_bwd_ready", False):
+        dp, ci, cd = ctypes.POINTER(ctypes.c_double), ctypes.c_int, ctypes.c_double
+        lib.oracle_pad_T.argtypes = [dp, ci, ci, ci, dp]
+        lib.oracle_pad_T.restype = None
+        lib.oracle_conv_valid_T.argtypes = [dp, ci, ci, dp, ci, dp]
+        lib.oracle_conv_valid_T.restype = None
+        lib.oracle_corr_valid_T.argtypes = [dp, ci, ci, dp, ci, dp]
+        lib.oracle_corr_valid_T.restype = None
+        lib.oracle_dphi.argtypes = [dp, ctypes.c_size_t, dp, dp, ci, cd, dp]
+        lib.oracle_dphi.restype = None
+        lib.oracle_stage_backward.argtypes = [dp, dp, dp, ci, ci, ci, ci, ci, dp, dp, dp, ci, cd, cd, dp, dp, dp, dp]
+        lib.oracle_stage_backward.restype = ci
+        lib.oracle_diffuse_backward.argtypes = [dp, dp, dp, dp, ci, ci, ci, ci, ci, ci, dp, dp, dp, ci, cd, dp,
+                                                dp, dp, dp, dp, dp]
+        lib.oracle_diffuse_backward.restype = ci
+        lib._bwd_ready = True
+    return lib
+
+
+def pad_T(up, H: int, W: int, p: int):
+    """Adjoint of pad(symmetric): folds a (H+2p) x (W+2p) image back onto H x W."""
+    up = _d(up)
+    assert up.shape == (H + 2 * p, W + 2 * p)
+    out = np.empty((H, W), dtype=np.float64)
+    _load_bwd().oracle_pad_T(_p(up), H, W, int(p), _p(out))
+    return out
+
+
+def conv_valid_T(out_img, k):
+    """Adjoint of conv_valid: (Ho, Wo) -> (Ho + K - 1, Wo + K - 1)."""
+    o, k = _d(out_img), _d(k)
+    K = k.shape[0]
+    res = np.empty((o.shape[0] + K - 1, o.shape[1] + K - 1), dtype=np.float64)
+    _load_bwd().oracle_conv_valid_T(_p(o), res.shape[0], res.shape[1], _p(k), K, _p(res))
+    return res
+
+
+def corr_valid_T(out_img, k):
+    """Adjoint of corr_valid: (Ho, Wo) -> (Ho + K - 1, Wo + K - 1)."""
+    o, k = _d(out_img), _d(k)
+    K = k.shape[0]
+    res = np.empty((o.shape[0] + K - 1, o.shape[1] + K - 1), dtype=np.float64)
+    _load_bwd().oracle_corr_valid_T(_p(o), res.shape[0], res.shape[1], _p(k), K, _p(res))
+    return res
+
+
+def dphi(z, w, mu, gamma: float):
+    """phi'(z), point-wise (derivative of PAPER.md:553)."""
+    z, w, mu = _d(z), _d(w), _d(mu)
+    out = np.empty_like(z)
+    _load_bwd().oracle_dphi(_p(z), z.size, _p(w), _p(mu), mu.size, float(gamma), _p(out))
+    return out
+
+
+def stage_backward(f, u_in, e, filters_t, rbf_w_t, rbf_mu, rbf_gamma: float, lambda_t: float):
+    """Backward pass of one stage; returns dict(g_u [B][H][W], g_k [N_k][K][K], g_w [N_k][M], g_lambda float)."""
+    f3, u3, e3 = _img3(f), _img3(u_in), _img3(e)
+    k, w, mu = _d(filters_t), _d(rbf_w_t), _d(rbf_mu)
+    B, H, W = u3.shape
+    n_k, K = k.shape[0], k.shape[1]
+    assert f3.shape == u3.shape == e3.shape and k.shape == (n_k, K, K) and w.shape == (n_k, mu.size)
+    g_u, g_k, g_w, g_l = np.empty_like(u3), np.empty_like(k), np.empty_like(w), np.zeros(1)
+    rc = _load_bwd().oracle_stage_backward(_p(f3), _p(u3), _p(e3), B, H, W, n_k, K, _p(k), _p(w), _p(mu), mu.size,
+                                           float(rbf_gamma), float(lambda_t), _p(g_u), _p(g_k), _p(g_w), _p(g_l))
+    if rc != 0:
+        raise ValueError(f"oracle_stage_backward failed with {rc}")
+    return {"g_u": g_u if np.ndim(u_in) == 3 else g_u[0], "g_k": g_k, "g_w": g_w, "g_lambda": float(g_l[0])}
+
+
+def diffuse_backward(f, u0, filters, rbf_w, rbf_mu, rbf_gamma: float, lambdas, u_gt=None, e_T=None):
+    """Forward T stages + back-propagation (Supp. Eq. 20-21).  Loss 1/2 ||u_T - u_gt||^2 when u_gt is given, else
+    e_T = dl/du_T is used.  Returns dict(u_T, g_u0, g_k [T][N_k][K][K], g_w [T][N_k][M], g_lambda [T])."""
+    f3, u3 = _img3(f), _img3(u0)
+    k, w, mu, lam = _d(filters), _d(rbf_w), _d(rbf_mu), _d(lambdas)
+    B, H, W = u3.shape
+    T, n_k, K = k.shape[0], k.shape[1], k.shape[2]
+    gt = _img3(u_gt) if u_gt is not None else None
+    eT = _img3(e_T) if e_T is not None else None
+    u_T, g_u0, g_k, g_w, g_l = np.empty_like(u3), np.empty_like(u3), np.empty_like(k), np.empty_like(w), np.zeros(T)
+    rc = _load_bwd().oracle_diffuse_backward(_p(f3), _p(u3), _p(gt) if gt is not None else None,
+                                             _p(eT) if eT is not None else None, B, H, W, T, n_k, K, _p(k), _p(w),
+                                             _p(mu), mu.size, float(rbf_gamma), _p(lam), _p(u_T), _p(g_u0), _p(g_k),
+                                             _p(g_w), _p(g_l))
+    if rc != 0:
+        raise ValueError(f"oracle_diffuse_backward failed with {rc}")
+    return {"u_T": u_T, "g_u0": g_u0, "g_k": g_k, "g_w": g_w, "g_lambda": g_l}
