@@ -114,6 +114,49 @@ int tnrd_qcs_project(const float* y, int B, int H, int W, const float* qcs_lo, c
                      void* stream);
 
 /*
+ * Backward pass of one stage (the step on the other side of inference: training on the same kernels).
+ * For u_t = u_in - ( sum_i kbar_i * phi_i(k_i * u_in) + lambda (u_in - f) ) as tnrd_stage computes it (mirror
+ * extension by 2r, crop built in) and e = dl/du_t, it returns
+ *     grad_u       = (du_t/du_in)^T e = (1 - lambda) e - P^T sum_i K_i^T Lambda_i Kbar_i^T e   (Supp. Eq. 21)
+ *     grad_filters = dl/dk_i = -(P_inv^T V^T + U^T Lambda_i Kbar_i^T) e                         (Supp. Eq. 10)
+ *     grad_w       = dl/dw_i = -G^T Kbar_i^T e                                                  (Supp. Eq. 19)
+ *     grad_lambda  = dl/dlambda = -<u_in - f, e>                                                (Supp. Eq. 7)
+ * Lambda_i = diag(phi_i'(k_i * u_in)) with phi'(z) = -sum_j w_j (z - mu_j)/gamma^2 exp(-(z - mu_j)^2 / (2 gamma^2)), the
+ * derivative of PAPER.md:553 (the printed formula at :568 is garbled); the sign of grad_lambda follows Supp. Eq. 4
+ * (Eq. 6 prints it without the minus).  Parameter gradients are SUMMED over the B images (Supp. Eq. 3), grad_u is per
+ * image.
+ *   f, u_in, e    device, [B][H][W];  filters_t [N_k][ksize][ksize], rbf_w_t [N_k][63], rbf_mu [63] device
+ *   grad_u        device, [B][H][W], or NULL;  must not be u_in, e or f (TNRD_ERR_ALIAS)
+ *   grad_filters  device, [N_k][ksize][ksize], or NULL.  When asked for, the library keeps two maps of
+ *                 B*N_k*(H+2r)*(W+2r) floats in its scratch (Lambda_i Kbar_i^T e and phi_i(z_i), read back by the
+ *                 filter-gradient kernel)
+ *   grad_w        device, [N_k][63], or NULL;   grad_lambda  device, [1], or NULL
+ * All outputs are written (not accumulated); results are deterministic run to run.  Asynchronous on `stream`.
+ */
+int tnrd_stage_backward(const float* f, const float* u_in, const float* e, int B, int H, int W, int N_k, int ksize,
+                        const float* filters_t, const float* rbf_w_t, const float* rbf_mu, float rbf_gamma,
+                        float lambda_t, float* grad_u, float* grad_filters, float* grad_w, float* grad_lambda,
+                        void* stream);
+
+/*
+ * Back-propagation through T stages (joint training, Supp. Eq. 20-21): runs the T forward stages
+ * from u0 keeping every iterate in the library scratch (T planes of B*H*W floats), then the backward recurrence
+ * e_{t-1} = (du_t/du_{t-1})^T e_t with the parameter gradients of every stage.
+ *   Exactly one of u_gt / e_T is non-NULL (device, [B][H][W]): with u_gt the loss is 1/2 ||u_T - u_gt||^2 (Supp. Eq. 3)
+ *   and e_T = u_T - u_gt is formed on the device; otherwise e_T = dl/du_T is taken as given (it cannot depend on this
+ *   call's u_T).
+ *   lambda        device, [T]
+ *   u_T           device, [B][H][W], or NULL: receives the forward result
+ *   grad_u0       device, [B][H][W], or NULL;  grad_filters [T][N_k][ksize][ksize], grad_w [T][N_k][63],
+ *                 grad_lambda [T]: device, each may be NULL
+ * T >= 1.  Asynchronous on `stream`.
+ */
+int tnrd_diffuse_backward(const float* f, const float* u0, const float* u_gt, const float* e_T, int B, int H, int W,
+                          int T, int N_k, int ksize, const float* filters, const float* rbf_w, const float* rbf_mu,
+                          float rbf_gamma, const float* lambda, float* u_T, float* grad_u0, float* grad_filters,
+                          float* grad_w, float* grad_lambda, void* stream);
+
+/*
  * Kernel selection, for tests and profiling.  which = 0: automatic (default); 1: the plain one-thread-per-
  * pixel reference kernel (global memory only); 2: the fused tiled stage kernel.  Returns TNRD_ERR_UNSUPPORTED
  * for other values.  Process-wide.

@@ -55,6 +55,11 @@ def lib() -> ctypes.CDLL:
         L.tnrd_deblock_diffuse.restype = ci
         L.tnrd_qcs_project.argtypes = [vp, ci, ci, ci, vp, vp, vp, vp]
         L.tnrd_qcs_project.restype = ci
+        L.tnrd_stage_backward.argtypes = [vp, vp, vp, ci, ci, ci, ci, ci, vp, vp, vp, cf, cf, vp, vp, vp, vp, vp]
+        L.tnrd_stage_backward.restype = ci
+        L.tnrd_diffuse_backward.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, ci, ci, vp, vp, vp, cf, vp, vp, vp, vp, vp,
+                                            vp, vp]
+        L.tnrd_diffuse_backward.restype = ci
         L.tnrd_set_kernel.argtypes = [ci]
         L.tnrd_set_kernel.restype = ci
         L.tnrd_set_phi_mode.argtypes = [ci]
@@ -138,6 +143,22 @@ def tnrd_qcs_project(y, B, H, W, qcs_lo, qcs_hi, u_out, stream=None):
     """u_out = D^T eta(D y) on device buffers (include/tnrd.h: tnrd_qcs_project)."""
     _check(lib().tnrd_qcs_project(_ptr(y), B, H, W, _ptr(qcs_lo), _ptr(qcs_hi), _ptr(u_out), _stream(stream)))
     return u_out
+
+
+def tnrd_stage_backward(f, u_in, e, B, H, W, N_k, ksize, filters_t, rbf_w_t, rbf_mu, rbf_gamma, lambda_t, grad_u=None,
+                        grad_filters=None, grad_w=None, grad_lambda=None, stream=None):
+    """Backward pass of one stage on device buffers (include/tnrd.h: tnrd_stage_backward)."""
+    _check(lib().tnrd_stage_backward(_ptr(f), _ptr(u_in), _ptr(e), B, H, W, N_k, ksize, _ptr(filters_t), _ptr(rbf_w_t),
+                                     _ptr(rbf_mu), float(rbf_gamma), float(lambda_t), _ptr(grad_u), _ptr(grad_filters),
+                                     _ptr(grad_w), _ptr(grad_lambda), _stream(stream)))
+
+
+def tnrd_diffuse_backward(f, u0, u_gt, e_T, B, H, W, T, N_k, ksize, filters, rbf_w, rbf_mu, rbf_gamma, lam, u_T=None,
+                          grad_u0=None, grad_filters=None, grad_w=None, grad_lambda=None, stream=None):
+    """Forward T stages + back-propagation on device buffers (include/tnrd.h: tnrd_diffuse_backward)."""
+    _check(lib().tnrd_diffuse_backward(_ptr(f), _ptr(u0), _ptr(u_gt), _ptr(e_T), B, H, W, T, N_k, ksize, _ptr(filters),
+                                       _ptr(rbf_w), _ptr(rbf_mu), float(rbf_gamma), _ptr(lam), _ptr(u_T), _ptr(grad_u0),
+                                       _ptr(grad_filters), _ptr(grad_w), _ptr(grad_lambda), _stream(stream)))
 
 
 def tnrd_set_kernel(which: int):

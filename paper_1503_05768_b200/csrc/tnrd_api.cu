@@ -43,6 +43,7 @@ struct Scratch {
     Buf prm, plane[2], refv;          // staged parameters, ping-pong planes, reference-path phi maps
     Buf split;                        // small-image path: tile counters (kept zero between launches) + partial sums
     Buf h_f, h_u, h_out, h_par;       // device staging of the host entry point
+    Buf bw_maps, bw_part, bw_trace, bw_e[2];   // backward pass: P/V maps, per-CTA partial sums, iterates, dl/du planes
 };
 std::vector<Scratch*> g_scratch;
 
@@ -264,6 +265,109 @@ int tnrd_deblock_diffuse(const float* u0, int B, int H, int W, int T, int N_k, i
     return TNRD_OK;
 }
 
+// Backward pass of one stage on staged parameters (shared by tnrd_stage_backward and tnrd_diffuse_backward).
+static int run_stage_backward(Scratch* sc, const float* f, const float* u, const float* e, int B, int H, int W, int N_k,
+                              int ksize, const float* prm, const float* lambda_ptr, float lambda_val, float gamma,
+                              float* g_u, float* g_k, float* g_w, float* g_l, cudaStream_t st)
+{
+    const tnrd::BwdPlan pl = tnrd::plan_stage_bwd(B, H, W, N_k, ksize, sc->num_sms);
+    const int R = (ksize - 1) / 2, KK = ksize * ksize;
+    const bool want_k = g_k != nullptr, want_w = g_w != nullptr || want_k;
+    const size_t n_w = want_w ? (size_t)pl.n_cta * N_k * 64 : 0, n_l = (size_t)pl.n_cta;
+    const size_t n_k = want_k ? (size_t)pl.G * N_k * KK : 0;
+    int rc = grow(sc->bw_part, n_w + n_l + n_k + 4, st);
+    if (rc != TNRD_OK) return rc;
+    const size_t map = want_k ? (size_t)B * N_k * (H + 2 * R) * (W + 2 * R) : 0;
+    if (want_k && (rc = grow(sc->bw_maps, 2 * map, st)) != TNRD_OK) return rc;
+    float* part_w = sc->bw_part.p;
+    float* part_l = part_w + n_w;
+    float* part_k = part_l + n_l;
+    tnrd::BwdArgs a{f, u, e, g_u, prm, lambda_ptr, lambda_val, B, H, W, N_k, ksize,
+                    want_k ? sc->bw_maps.p : nullptr, want_k ? sc->bw_maps.p + map : nullptr,
+                    want_w ? part_w : nullptr, g_l ? part_l : nullptr};
+    TNRD_CUDA(tnrd::launch_stage_bwd(a, pl, part_k, st, &g_launches));
+    if (want_w || g_l) {
+        const float s = sqrtf(1.4426950408889634f / (2.0f * gamma * gamma));
+        TNRD_CUDA(tnrd::launch_reduce_partials(part_w, pl.n_cta, part_k, pl.G, part_l, N_k, ksize, s, g_w, g_k, g_l, st,
+                                               &g_launches));
+    }
+    return TNRD_OK;
+}
+
+int tnrd_stage_backward(const float* f, const float* u_in, const float* e, int B, int H, int W, int N_k, int ksize,
+                        const float* filters_t, const float* rbf_w_t, const float* rbf_mu, float rbf_gamma,
+                        float lambda_t, float* grad_u, float* grad_filters, float* grad_w, float* grad_lambda,
+                        void* stream)
+{
+    if (!f || !u_in || !e || !filters_t || !rbf_w_t || !rbf_mu) return TNRD_ERR_NULL;
+    int rc = check_shape(B, H, W, N_k, ksize);
+    if (rc != TNRD_OK) return rc;
+    if ((rc = check_gamma(rbf_gamma)) != TNRD_OK) return rc;
+    if (grad_u && (grad_u == u_in || grad_u == e || grad_u == f)) return TNRD_ERR_ALIAS;
+    cudaStream_t st = (cudaStream_t)stream;
+    Scratch* sc = nullptr;
+    if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
+    if ((rc = grow(sc->prm, (size_t)N_k * tnrd::prm_stride(ksize), st)) != TNRD_OK) return rc;
+    TNRD_CUDA(tnrd::launch_prep(filters_t, rbf_w_t, rbf_mu, rbf_gamma, 1, N_k, ksize, sc->prm.p, st, &g_launches));
+    return run_stage_backward(sc, f, u_in, e, B, H, W, N_k, ksize, sc->prm.p, nullptr, lambda_t, rbf_gamma, grad_u,
+                              grad_filters, grad_w, grad_lambda, st);
+}
+
+int tnrd_diffuse_backward(const float* f, const float* u0, const float* u_gt, const float* e_T, int B, int H, int W,
+                          int T, int N_k, int ksize, const float* filters, const float* rbf_w, const float* rbf_mu,
+                          float rbf_gamma, const float* lambda, float* u_T, float* grad_u0, float* grad_filters,
+                          float* grad_w, float* grad_lambda, void* stream)
+{
+    if (!f || !u0 || !filters || !rbf_w || !rbf_mu || !lambda) return TNRD_ERR_NULL;
+    if ((u_gt == nullptr) == (e_T == nullptr)) return TNRD_ERR_NULL;       // exactly one of them
+    if (T < 1) return TNRD_ERR_SHAPE;
+    int rc = check_shape(B, H, W, N_k, ksize);
+    if (rc != TNRD_OK) return rc;
+    if ((rc = check_gamma(rbf_gamma)) != TNRD_OK) return rc;
+    if (grad_u0 && (grad_u0 == u0 || grad_u0 == f || grad_u0 == e_T || grad_u0 == u_gt)) return TNRD_ERR_ALIAS;
+    if (u_T && (u_T == u0 || u_T == f)) return TNRD_ERR_ALIAS;
+    cudaStream_t st = (cudaStream_t)stream;
+    Scratch* sc = nullptr;
+    if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
+    const size_t n = (size_t)B * H * W, rec = (size_t)N_k * tnrd::prm_stride(ksize);
+    const int KK = ksize * ksize;
+    if ((rc = grow(sc->prm, (size_t)T * rec, st)) != TNRD_OK) return rc;
+    if ((rc = grow(sc->bw_trace, (size_t)T * n, st)) != TNRD_OK) return rc;     // u_1 .. u_T
+    if ((rc = grow(sc->bw_e[0], n, st)) != TNRD_OK) return rc;
+    if ((rc = grow(sc->bw_e[1], n, st)) != TNRD_OK) return rc;
+    TNRD_CUDA(tnrd::launch_prep(filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, sc->prm.p, st, &g_launches));
+    // forward, keeping every iterate (Supp. Eq. 21 needs u_{t-1} of every stage)
+    const float* src = u0;
+    for (int t = 1; t <= T; ++t) {
+        float* dst = sc->bw_trace.p + (size_t)(t - 1) * n;
+        tnrd::StageArgs a{f, src, dst, sc->prm.p + (size_t)(t - 1) * rec, lambda + (t - 1), 0.0f, B, H, W, N_k, ksize};
+        if ((rc = run_stage(sc, a, st)) != TNRD_OK) return rc;
+        src = dst;
+    }
+    if (u_T) TNRD_CUDA(cudaMemcpyAsync(u_T, src, n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    // e_T = dl/du_T: given, or u_T - u_gt for the loss 1/2 ||u_T - u_gt||^2 (Supp. Eq. 3, 20)
+    const float* e = e_T;
+    if (u_gt) {
+        TNRD_CUDA(tnrd::launch_sub(src, u_gt, sc->bw_e[0].p, n, st, &g_launches));
+        e = sc->bw_e[0].p;
+    }
+    // backward recurrence (Supp. Eq. 21): e_{t-1} = (du_t/du_{t-1})^T e_t; parameter gradients of stage t from (u_{t-1}, e_t)
+    for (int t = T; t >= 1; --t) {
+        const float* u_prev = (t == 1) ? u0 : sc->bw_trace.p + (size_t)(t - 2) * n;
+        float* g_u;
+        if (t == 1) g_u = grad_u0;                                   // may be null: not needed then
+        else g_u = (e == sc->bw_e[0].p) ? sc->bw_e[1].p : sc->bw_e[0].p;
+        rc = run_stage_backward(sc, f, u_prev, e, B, H, W, N_k, ksize, sc->prm.p + (size_t)(t - 1) * rec,
+                                lambda + (t - 1), 0.0f, rbf_gamma, g_u,
+                                grad_filters ? grad_filters + (size_t)(t - 1) * N_k * KK : nullptr,
+                                grad_w ? grad_w + (size_t)(t - 1) * N_k * TNRD_NUM_RBF : nullptr,
+                                grad_lambda ? grad_lambda + (t - 1) : nullptr, st);
+        if (rc != TNRD_OK) return rc;
+        e = g_u;
+    }
+    return TNRD_OK;
+}
+
 int tnrd_set_kernel(int which)
 {
     if (which < 0 || which > 2) return TNRD_ERR_UNSUPPORTED;
@@ -313,7 +417,7 @@ void tnrd_shutdown(void)
     (void)cudaGetDevice(&cur);
     for (Scratch* s : g_scratch) {
         (void)cudaSetDevice(s->dev);
-        Buf* bufs[] = {&s->prm, &s->plane[0], &s->plane[1], &s->refv, &s->split, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
+        Buf* bufs[] = {&s->prm, &s->plane[0], &s->plane[1], &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->refv, &s->split, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
         for (Buf* b : bufs)
             if (b->p) (void)cudaFree(b->p);   // synchronising free: the stream may be gone by now
         delete s;

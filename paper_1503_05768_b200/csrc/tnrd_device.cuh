@@ -1,0 +1,46 @@
+// tnrd_device.cuh -- device helpers shared by the stage kernels (forward: tnrd_fused.cu, backward: tnrd_bwd.cu).
+#pragma once
+#include "tnrd_internal.h"
+
+namespace tnrd {
+
+// 2^{-x}: the negation rides on the MUFU operand
+__device__ __forceinline__ float ex2_neg(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(-x));
+    return y;
+}
+
+template <int N>
+__device__ __forceinline__ void lds_vec(const float* __restrict__ p, float (&d)[N])
+{
+#pragma unroll
+    for (int q = 0; q < N / 4; ++q) {
+        const float4 t = *reinterpret_cast<const float4*>(p + 4 * q);
+        d[4 * q + 0] = t.x; d[4 * q + 1] = t.y; d[4 * q + 2] = t.z; d[4 * q + 3] = t.w;
+    }
+}
+
+// One window row of either filtering for a 4x2 block.  acc[p] holds the two output rows of column p as one pair;
+// trow = row of tap pairs P[rho][b] = (k[rho-1][b], k[rho][b]).  REV = false: forward filter (a2), pair = (row 0,
+// row 1), rho = KS - wr, source column p + 2r - b.  REV = true: transposed filter (a4), pair = (row 1, row 0),
+// rho = wr, source column p + b.
+template <int KS, bool REV>
+__device__ __forceinline__ void rowstep(const float* __restrict__ srow, const float* __restrict__ trow,
+                                        float2 (&acc)[4])
+{
+    constexpr int TS = prm_ts(KS), NV = (4 + KS - 1 + 3) / 4;
+    float row[NV * 4], kp[TS];
+    lds_vec(srow, row);
+    lds_vec(trow, kp);
+#pragma unroll
+    for (int b = 0; b < KS; ++b)
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+            const float x = REV ? row[p + b] : row[p + (KS - 1) - b];
+            acc[p] = __ffma2_rn(make_float2(kp[2 * b], kp[2 * b + 1]), make_float2(x, x), acc[p]);
+        }
+}
+
+}  // namespace tnrd

@@ -60,6 +60,34 @@ struct FusedPlan {
     size_t split_floats;     // scratch needed when nsplit > 1: counters (one per tile) + partial sums; else 0
 };
 
+// ---- backward pass of a stage (tnrd_bwd.cu) ----------------------------------------------------------------
+struct BwdArgs {
+    const float* f;      // [B][H][W]
+    const float* u;      // [B][H][W]  u_{t-1}
+    const float* e;      // [B][H][W]  dl/du_t
+    float* g_u;          // [B][H][W]  dl/du_{t-1}, or null
+    const float* prm;    // staged records of this stage
+    const float* lambda_ptr;
+    float lambda_val;
+    int B, H, W, N_k, ksize;
+    float* pmap;         // [B][N_k][H+2r][W+2r]  Lambda_i Kbar_i^T e / s   (null unless g_k is wanted)
+    float* vmap;         // [B][N_k][H+2r][W+2r]  phi_i(z_i) / s
+    float* part_w;       // [n_cta][N_k][64] per-CTA g_w sums (null unless g_w is wanted)
+    float* part_l;       // [n_cta] per-CTA g_lambda sums (null unless wanted)
+};
+struct BwdPlan {
+    int ntx, nty;        // tiles of the extended output domain per image (stage_bwd_kernel)
+    long long n_cta;     // ntx * nty * B
+    int wtx, wty, G;     // wgrad tiles per image; CTAs per filter
+};
+BwdPlan plan_stage_bwd(int B, int H, int W, int N_k, int ksize, int num_sms);
+cudaError_t launch_stage_bwd(const BwdArgs& a, const BwdPlan& pl, float* part_k /*[G][N_k][ks*ks]*/, cudaStream_t st,
+                             unsigned long long* launches);
+cudaError_t launch_reduce_partials(const float* part_w, long long n_cta, const float* part_k, int G, const float* part_l,
+                                   int N_k, int ksize, float s, float* g_w, float* g_k, float* g_lambda, cudaStream_t st,
+                                   unsigned long long* launches);
+cudaError_t launch_sub(const float* x, const float* y, float* out, size_t n, cudaStream_t st, unsigned long long* launches);
+
 // launchers (each returns the cudaError_t of the launch; *launches += kernels launched)
 cudaError_t launch_prep(const float* filters, const float* rbf_w, const float* rbf_mu, float gamma,
                         int T, int N_k, int ksize, float* prm, cudaStream_t st, unsigned long long* launches);
