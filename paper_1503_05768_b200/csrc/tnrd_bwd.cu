@@ -401,17 +401,7 @@ wgrad_kernel(BwdArgs a, int ntx, int nty, int G, float* __restrict__ part_k)
         const int PX0 = tx * C::TW, PY0 = ty * C::TH;          // phi-region index of the tile origin (= image coord + r)
         const float* __restrict__ u_img = a.u + img * plane;
         const float* __restrict__ e_img = a.e + img * plane;
-        __syncthreads();                                        // the previous tile's source is no longer read
-        // source pixel of phi index (Y, X) and lag (a, b): image coordinate (Y - r) - a + r = Y - a  ->  rows PY0 - (KS-1) ..
-        for (int idx = tid; idx < C::SH * C::SW; idx += NT) {
-            const int sy = idx / C::SW, sx = idx - sy * C::SW;
-            const int y = PY0 - (KS - 1) + sy, x = PX0 - (KS - 1) + sx;             // image coordinates
-            const bool in = y >= 0 && y < a.H && x >= 0 && x < a.W;
-            const bool ext = y >= -2 * R && y < a.H + 2 * R && x >= -2 * R && x < a.W + 2 * R;
-            us[sy * C::SS + sx] = ext ? __ldg(u_img + (size_t)mirror_clamp(y, a.H) * a.W + mirror_clamp(x, a.W)) : 0.f;
-            es[sy * C::SS + sx] = in ? __ldg(e_img + (size_t)y * a.W + x) : 0.f;
-        }
-        // this thread's P and V values (zero outside the phi region)
+        // this thread's P and V values (zero outside the phi region): issued first, consumed after the source fill
         float P[2][4], V[2][4];
         const size_t mb = ((size_t)img * a.N_k + i) * (size_t)Hz * Wz;
 #pragma unroll
@@ -423,6 +413,27 @@ wgrad_kernel(BwdArgs a, int ntx, int nty, int G, float* __restrict__ part_k)
                 P[j][p] = ok ? __ldg(a.pmap + mb + (size_t)Y * Wz + X) : 0.f;
                 V[j][p] = ok ? __ldg(a.vmap + mb + (size_t)Y * Wz + X) : 0.f;
             }
+        // source pixel of phi index (Y, X) and lag (a, b): image coordinate (Y - r) - a + r = Y - a  ->  rows PY0 - (KS-1) ..
+        // all loads of the fill are issued before the first store (a rolled loop would serialise on the load latency)
+        constexpr int NFILL = (C::SH * C::SW + NT - 1) / NT;
+        float fu[NFILL], fe[NFILL];
+#pragma unroll
+        for (int q = 0; q < NFILL; ++q) {
+            const int idx = tid + q * NT;
+            const int sy = idx / C::SW, sx = idx - sy * C::SW;
+            const int y = PY0 - (KS - 1) + sy, x = PX0 - (KS - 1) + sx;             // image coordinates
+            const bool in = idx < C::SH * C::SW && y >= 0 && y < a.H && x >= 0 && x < a.W;
+            const bool ext = idx < C::SH * C::SW && y >= -2 * R && y < a.H + 2 * R && x >= -2 * R && x < a.W + 2 * R;
+            fu[q] = ext ? __ldg(u_img + (size_t)mirror_clamp(y, a.H) * a.W + mirror_clamp(x, a.W)) : 0.f;
+            fe[q] = in ? __ldg(e_img + (size_t)y * a.W + x) : 0.f;
+        }
+        __syncthreads();                                        // the previous tile's source is no longer read
+#pragma unroll
+        for (int q = 0; q < NFILL; ++q) {
+            const int idx = tid + q * NT;
+            const int sy = idx / C::SW, sx = idx - sy * C::SW;
+            if (idx < C::SH * C::SW) { us[sy * C::SS + sx] = fu[q]; es[sy * C::SS + sx] = fe[q]; }
+        }
         __syncthreads();
         // window rows wr = 0..KS: source row sy = by2 + wr serves lag a = j + (KS-1) - wr of block row j
 #pragma unroll
