@@ -147,7 +147,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5", "deblock"],
+    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5", "deblock", "backward"],
                     help="BASELINE.json config; c4 (default) is the headline, the others are for exploration")
     ap.add_argument("--size", type=int, default=4096)
     ap.add_argument("--T", type=int, default=5)
@@ -180,6 +180,11 @@ def main():
     warmup = max(args.warmup, 3)
 
     deblock = args.workload == "deblock"
+    backward = args.workload == "backward"   # joint-training step: T forward stages + back-propagation, all gradients
+    if backward:
+        args.workload, args.no_window = "c4", True
+        if args.size == 4096:
+            args.size = 2048                 # keeps the P/V maps of the filter gradient at 1.6 GB
     if deblock:      # TRD^4_{7x7} JPEG deblocking at 1024^2, the size the paper times it at
         cfg = tnrd_gen.make_deblock(9, 1, 1024, 1024, 4, 48, 7)
         cfg["f"], cfg["lambda"] = cfg["u0"], np.zeros(4, dtype=np.float32)
@@ -201,8 +206,15 @@ def main():
     if deblock:
         qlo, qhi = torch.from_numpy(cfg["qcs_lo"]).to(devs), torch.from_numpy(cfg["qcs_hi"]).to(devs)
 
+    if backward:
+        gt = torch.from_numpy(cfg["clean"]).to(devs) if "clean" in cfg else f * 0.98
+        g_u0, g_k, g_w, g_l = torch.empty_like(f), torch.empty_like(k), torch.empty_like(w), torch.empty_like(lam)
+
     def step():
-        if deblock:
+        if backward:
+            tnrd.tnrd_diffuse_backward(f, f, gt, None, B, H, W, T, N_K, KSIZE, k, w, mu, gamma, lam, out, g_u0, g_k, g_w,
+                                       g_l, stream)
+        elif deblock:
             tnrd.tnrd_deblock_diffuse(f, B, H, W, T, N_K, KSIZE, k, w, mu, gamma, qlo, qhi, out, stream)
         else:
             tnrd.tnrd_diffuse(f, f, B, H, W, T, N_K, KSIZE, k, w, mu, gamma, lam, out, stream)
@@ -238,8 +250,21 @@ def main():
         hq = [torch.from_numpy(cfg["qcs_lo"]).pin_memory(), torch.from_numpy(cfg["qcs_hi"]).pin_memory()]
         dq = [torch.empty_like(f), torch.empty_like(f), torch.empty_like(f), torch.empty_like(f)]
 
+    if backward:
+        hgt = gt.cpu().pin_memory()
+        hg = [torch.empty(g_k.shape).pin_memory(), torch.empty(g_w.shape).pin_memory(), torch.empty(g_l.shape).pin_memory()]
+        dgt = torch.empty_like(f)
+
     def step_host():
-        if deblock:   # no host entry point for this variant: explicit pinned copies around the device call
+        if backward:  # host f, u_gt up; parameter gradients and u_T down
+            dq0 = out  # reuse
+            f.copy_(hf, non_blocking=True); dgt.copy_(hgt, non_blocking=True)
+            tnrd.tnrd_diffuse_backward(f, f, dgt, None, B, H, W, T, N_K, KSIZE, k, w, mu, gamma, lam, dq0, None, g_k, g_w,
+                                       g_l, stream)
+            hout.copy_(dq0, non_blocking=True)
+            hg[0].copy_(g_k, non_blocking=True); hg[1].copy_(g_w, non_blocking=True); hg[2].copy_(g_l, non_blocking=True)
+            stream.synchronize()
+        elif deblock:   # no host entry point for this variant: explicit pinned copies around the device call
             dq[0].copy_(hf, non_blocking=True); dq[1].copy_(hq[0], non_blocking=True); dq[2].copy_(hq[1], non_blocking=True)
             tnrd.tnrd_deblock_diffuse(dq[0], B, H, W, T, N_K, KSIZE, k, w, mu, gamma, dq[1], dq[2], dq[3], stream)
             hout.copy_(dq[3], non_blocking=True)
@@ -258,8 +283,8 @@ def main():
     barrier()
     ms_e2e = max_over_ranks(e2.elapsed_time(e3), devs)
     e2e_value = sum_over_ranks(float(B) * H * W * T * e2e_steps, devs) / (ms_e2e * 1e-3) / 1e6
-    h2d = hf.numel() * 4 * (3 if deblock else 1) + (0 if deblock else sum(int(a.nbytes) for a in hp))
-    d2h = hout.numel() * 4
+    h2d = hf.numel() * 4 * (3 if deblock else 2 if backward else 1) + (0 if deblock or backward else sum(int(a.nbytes) for a in hp))
+    d2h = hout.numel() * 4 + (sum(x.numel() * 4 for x in hg) if backward else 0)
     same = bool(torch.equal(hout.to(devs), out))
 
     # ---- extra: the windowed phi evaluator (tnrd_set_phi_mode(1)), same workload, same timing protocol ----------
@@ -304,6 +329,9 @@ def main():
         "warmup": warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": (f"JPEG deblocking TRD^4_7x7 {B}x{H}x{W} (PAPER.md:287), synthetic QCS" if deblock else
+                                f"joint-training step (T={T} forward stages + back-propagation, Supp. Eq. 21; dl/du0, dl/dk, "
+                                f"dl/dw, dl/dlambda) {B}x{H}x{W} N_k={N_K} {KSIZE}x{KSIZE}; value counts B*H*W*T per step; "
+                                f"roofline fields count the forward exponentials only" if backward else
                                 f"C{args.workload[1]} {B}x{H}x{W} T={T} N_k={N_K} {KSIZE}x{KSIZE} M=63 "
                                 f"(BASELINE.json configs[{int(args.workload[1]) - 1}]), one such batch per GPU"),
                    "global_batch": world * B, "parallelism": f"dp{world} (independent images, no collective)",
