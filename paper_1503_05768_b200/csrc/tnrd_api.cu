@@ -41,7 +41,7 @@ struct Scratch {
     cudaStream_t st = nullptr;
     int num_sms = 0;
     Buf prm, plane[2], refv;          // staged parameters, ping-pong planes, reference-path phi maps
-    Buf split;                        // small-image path: tile counters (kept zero between launches) + partial sums
+    Buf split;                        // partial transposed-filter sums of the fused kernel's CTAs
     Buf h_f, h_u, h_out, h_par;       // device staging of the host entry point
     Buf bw_maps, bw_part, bw_trace, bw_e[2];   // backward pass: P/V maps, per-CTA partial sums, iterates, dl/du planes
 };
@@ -96,11 +96,8 @@ int run_stage(Scratch* sc, const tnrd::StageArgs& a, cudaStream_t st)
         TNRD_CUDA(tnrd::launch_stage_ref(a, sc->refv.p, st, &g_launches));
     } else {
         const tnrd::FusedPlan pl = tnrd::plan_stage_fused(a, sc->num_sms);
-        if (pl.split_floats > sc->split.cap) {
-            int rc = grow(sc->split, pl.split_floats, st);
-            if (rc != TNRD_OK) return rc;
-            TNRD_CUDA(cudaMemsetAsync(sc->split.p, 0, sc->split.cap * sizeof(float), st));
-        }
+        int rc = grow(sc->split, pl.part_floats, st);
+        if (rc != TNRD_OK) return rc;
         TNRD_CUDA(tnrd::launch_stage_fused(a, pl, sc->split.p, g_phi_mode, st, &g_launches));
     }
     return TNRD_OK;

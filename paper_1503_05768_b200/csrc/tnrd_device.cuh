@@ -26,11 +26,12 @@ __device__ __forceinline__ void lds_vec(const float* __restrict__ p, float (&d)[
 // trow = row of tap pairs P[rho][b] = (k[rho-1][b], k[rho][b]).  REV = false: forward filter (a2), pair = (row 0,
 // row 1), rho = KS - wr, source column p + 2r - b.  REV = true: transposed filter (a4), pair = (row 1, row 0),
 // rho = wr, source column p + b.
-template <int KS, bool REV>
+// SHIFT: extra column offset of the source window (the source row is read from a 16-byte aligned address).
+template <int KS, bool REV, int SHIFT = 0>
 __device__ __forceinline__ void rowstep(const float* __restrict__ srow, const float* __restrict__ trow,
                                         float2 (&acc)[4])
 {
-    constexpr int TS = prm_ts(KS), NV = (4 + KS - 1 + 3) / 4;
+    constexpr int TS = prm_ts(KS), NV = (4 + KS - 1 + SHIFT + 3) / 4;
     float row[NV * 4], kp[TS];
     lds_vec(srow, row);
     lds_vec(trow, kp);
@@ -38,7 +39,7 @@ __device__ __forceinline__ void rowstep(const float* __restrict__ srow, const fl
     for (int b = 0; b < KS; ++b)
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
-            const float x = REV ? row[p + b] : row[p + (KS - 1) - b];
+            const float x = REV ? row[p + b + SHIFT] : row[p + (KS - 1) - b + SHIFT];
             acc[p] = __ffma2_rn(make_float2(kp[2 * b], kp[2 * b + 1]), make_float2(x, x), acc[p]);
         }
 }

@@ -32,17 +32,26 @@ namespace tnrd {
 
 namespace {
 
-// small-image path: the scratch starts with this many tile counters (a fixed area, so that launches with different
-// tile counts never see each other's partial sums as counters), followed by the partial sums
-constexpr int SPLIT_COUNTERS = 4096;
-
+// Geometry of one CTA (all in "phi coordinates": index 0 = image coordinate -r; the phi region is (H+2r) x (W+2r)).
+// The CTA owns a tile of tw x th phi pixels at (X0, Y0) -- tiles PARTITION the phi region, nothing is computed twice --
+// and produces the partial transposed-filter sums of those pixels on the output area
+//   columns [X0 - 4, X0 + tw + r)  (only X0 - r .. are needed; starting 4 to the left keeps every vector access aligned)
+//   rows    [Y0 - r, Y0 + th + r),
+// at most RW x RH pixels, i.e. tw <= RW - 4 - r, th <= RH - 2r.  Shared memory:
+//   us   u tile, origin (Y0 - r, X0 - r) in phi coordinates = (Y0 - 2r, X0 - 2r) in image coordinates
+//   vs   two influence maps, origin (Y0 - 2r, X0 - 8): the tile's own values surrounded by a ring of zeros, so that
+//        the transposed filter can run over the whole output area (window row oy + a, column ox + b + 4 - r)
 template <int KS, int RW, int RH, int NT, int MINB = 1>
 struct Cfg {
     static constexpr int R = (KS - 1) / 2;
+    static constexpr int TWMAX = RW - 4 - R, THMAX = RH - 2 * R;   // largest tile
     static constexpr int US = RW + 8;                   // u tile row stride (floats)
-    static constexpr int UH = RH + 2 * R;               // u tile rows
-    static constexpr int VS = RW;                       // phi map row stride
-    static constexpr int VPLANE = RH * RW + 16;         // one phi map (+ overrun pad for masked pixels)
+    static constexpr int UH = RH + 2;                   // u tile rows (th + 2r + 1 window rows)
+    static constexpr int VS = RW + 8;                   // phi map row stride
+    static constexpr int VH = RH + 2 * R;               // phi map rows
+    static constexpr int VPLANE = VH * VS;              // one phi map
+    static constexpr int SHIFT = 4 - R;                 // column shift of the transposed-filter window (see above)
+    static constexpr int CTA_FLOATS = (RW / 4) * (RH / 2) * 8;      // partial sums of one CTA (block-major)
     static constexpr int TS = prm_ts(KS);               // floats per row of tap pairs
     static constexpr int PRM = prm_stride(KS);          // floats per staged record
     static constexpr int NB = ((RW / 4) * (RH / 2) + NT - 1) / NT;  // 4x2 work blocks per thread (max)
@@ -106,13 +115,13 @@ __device__ __forceinline__ void phi_win_step(unsigned wsec, const int (&wofs)[4]
 
 template <int KS, int RW, int RH, int NT, int MINB, int PHI>
 __global__ void __launch_bounds__(NT, MINB)
-stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty, int nsplit, float* __restrict__ split)
+stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int nsplit, float* __restrict__ part)
 {
     using C = Cfg<KS, RW, RH, NT, MINB>;
     constexpr int R = C::R, TS = C::TS, KKP = prm_kkp(KS);
     extern __shared__ __align__(16) float smem[];
-    float* us = smem;                              // [UH][US]   u tile with 2r halo
-    float* vs = us + C::UH * C::US;                // [2][VPLANE] influence maps of filters i and i-1
+    float* us = smem;                              // [UH][US]   u tile with r halo
+    float* vs = us + C::UH * C::US;                // [2][VPLANE] influence maps of filters i and i-1 (zero ring)
     float* ps = vs + 2 * C::VPLANE;                // [4][PRM]   staged records of filters i-1 .. i+2
 
     const int tid = threadIdx.x;
@@ -120,7 +129,8 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty, int nsplit, fl
     const int tx = t % ntx; t /= ntx;
     const int ty = t % nty; t /= nty;
     const int img = t;
-    const int X0 = tx * tw, Y0 = ty * th;          // image coordinates of the output tile origin
+    const int X0 = tx * tw_nom, Y0 = ty * th_nom;  // phi coordinates of the tile origin
+    const int tw = min(tw_nom, a.W + 2 * R - X0), th = min(th_nom, a.H + 2 * R - Y0);   // ragged last tiles
     const float* __restrict__ u_img = a.u_in + (size_t)img * a.H * a.W;
     const int f0 = (int)(blockIdx.y * a.N_k / nsplit);
     const int N_k = (int)((blockIdx.y + 1) * a.N_k / nsplit) - f0;          // filters f0 .. f0 + N_k - 1
@@ -137,14 +147,16 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty, int nsplit, fl
     }
 
     // ---- work decomposition: 4x2 pixel blocks, NB per thread ----------------------------------------------
-    const int nbx = (tw + 2 * R + 3) >> 2, nby = (th + 2 * R + 1) >> 1;   // phi region
-    const int nbxo = (tw + 3) >> 2, nbyo = (th + 1) >> 1;                  // output tile
-    const int nrounds = (nbx * nby + NT - 1) / NT;   // rounds of blocks this tile needs (<= NB): the software pipeline
+    const int nbx = (tw + 3) >> 2, nby = (th + 1) >> 1;                         // phi blocks: the tile itself
+    const int nbxo = (tw + 4 + R + 3) >> 2, nbyo = (th + 2 * R + 1) >> 1;       // output blocks: tile + ring
+    const int nrounds = (nbxo * nbyo + NT - 1) / NT; // rounds of blocks this tile needs (<= NB): the software pipeline
                                                      // wraps from the last USED round to block 0 of the next filter
 
     // ---- a1: gather the u tile through the mirror map (only the rows / columns some block will read) -----
     {
         const int nr = min(C::UH, 2 * nby + 2 * R), nc = min(C::US, 4 * nbx + 2 * R + 4);
+        for (int idx = tid; idx < 2 * C::VPLANE / 4; idx += NT)               // zero ring of both maps
+            reinterpret_cast<float4*>(vs)[idx] = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll 2
         for (int uy = tid >> 5; uy < nr; uy += NT / 32) {
             const float* __restrict__ grow = u_img + (size_t)mirror_clamp(Y0 - 2 * R + uy, a.H) * a.W;
@@ -159,12 +171,18 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty, int nsplit, fl
         if (idx < N_k * C::PRM) ps[idx] = __ldg(a.prm + (size_t)f0 * C::PRM + idx);   // records 0 and 1
 
     int uoff[C::NB], voff[C::NB], coff[C::NB];   // block origins in us / a phi map (phi side) / a phi map (output side)
+    unsigned own = 0;                            // bit 8 n + 4 j + p: pixel (row j, column p) of phi block n is in the tile
 #pragma unroll
     for (int n = 0; n < C::NB; ++n) {
         const int blk = tid + n * NT;
         const int by = blk / nbx, bx = blk - by * nbx;
         uoff[n] = (by < nby) ? (2 * by) * C::US + 4 * bx : -1;
-        voff[n] = (2 * by) * C::VS + 4 * bx;
+        voff[n] = (2 * by + 2 * R) * C::VS + 4 * bx + 8;
+#pragma unroll
+        for (int j = 0; j < 2; ++j)
+#pragma unroll
+            for (int p = 0; p < 4; ++p)
+                if (2 * by + j < th && 4 * bx + p < tw) own |= 1u << (8 * n + 4 * j + p);
         const int cy = blk / nbxo, cx = blk - cy * nbxo;
         coff[n] = (cy < nbyo) ? (2 * cy) * C::VS + 4 * cx : -1;
     }
@@ -227,12 +245,12 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty, int nsplit, fl
                 }
                 if (g <= KS) {
                     if (hasN) rowstep<KS, false>(uwn + g * C::US, tapsN + (KS - g) * TS, zn);
-                    if (hasC) rowstep<KS, true>(vw + g * C::VS, recp + g * TS, acc[n]);
+                    if (hasC) rowstep<KS, true, C::SHIFT>(vw + g * C::VS, recp + g * TS, acc[n]);
                 }
                 if (KS + 1 > C::NG && g + C::NG <= KS) {      // ksize 9: ten row-steps in eight phi steps
                     const int g2 = g + C::NG;
                     if (hasN) rowstep<KS, false>(uwn + g2 * C::US, tapsN + (KS - g2) * TS, zn);
-                    if (hasC) rowstep<KS, true>(vw + g2 * C::VS, recp + g2 * TS, acc[n]);
+                    if (hasC) rowstep<KS, true, C::SHIFT>(vw + g2 * C::VS, recp + g2 * TS, acc[n]);
                 }
             }
             {   // last step: the remaining 63 - 56 = 7 terms (dense) / window centres 14, 15
@@ -243,12 +261,15 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty, int nsplit, fl
                 }
                 if (g <= KS) {
                     if (hasN) rowstep<KS, false>(uwn + g * C::US, tapsN + (KS - g) * TS, zn);
-                    if (hasC) rowstep<KS, true>(vw + g * C::VS, recp + g * TS, acc[n]);
+                    if (hasC) rowstep<KS, true, C::SHIFT>(vw + g * C::VS, recp + g * TS, acc[n]);
                 }
             }
-            if (hasB) {
-                *reinterpret_cast<float4*>(vcur + voff[n]) = make_float4(v[0].x, v[1].x, v[2].x, v[3].x);
-                *reinterpret_cast<float4*>(vcur + voff[n] + C::VS) = make_float4(v[0].y, v[1].y, v[2].y, v[3].y);
+            if (hasB) {     // pixels of a ragged block that lie outside the tile belong to the neighbour: keep the ring zero
+                const unsigned m = own >> (8 * n);
+                *reinterpret_cast<float4*>(vcur + voff[n]) = make_float4(
+                    m & 1 ? v[0].x : 0.f, m & 2 ? v[1].x : 0.f, m & 4 ? v[2].x : 0.f, m & 8 ? v[3].x : 0.f);
+                *reinterpret_cast<float4*>(vcur + voff[n] + C::VS) = make_float4(
+                    m & 16 ? v[0].y : 0.f, m & 32 ? v[1].y : 0.f, m & 64 ? v[2].y : 0.f, m & 128 ? v[3].y : 0.f);
             }
 #pragma unroll
             for (int p = 0; p < 4; ++p) zc[p] = zn[p];
@@ -264,85 +285,59 @@ stage_fused_kernel(StageArgs a, int tw, int th, int ntx, int nty, int nsplit, fl
         for (int n = 0; n < C::NB; ++n) {
             if (coff[n] < 0) continue;
 #pragma unroll
-            for (int wr = 0; wr <= KS; ++wr) rowstep<KS, true>(vprev + coff[n] + wr * C::VS, recp + wr * TS, acc[n]);
+            for (int wr = 0; wr <= KS; ++wr)
+                rowstep<KS, true, C::SHIFT>(vprev + coff[n] + wr * C::VS, recp + wr * TS, acc[n]);
         }
     }
 
-    // ---- small-image path: the nsplit CTAs of a tile meet in scratch; the last one to arrive adds the partial
-    // sums in fixed order (deterministic) and goes on to a5, the others are done ---------------------------------
-    if (nsplit > 1) {
-        __shared__ int s_last;
-        unsigned* counters = reinterpret_cast<unsigned*>(split);
-        const int tile = blockIdx.x, part = blockIdx.y;
-        float* part0 = split + SPLIT_COUNTERS + (size_t)tile * nsplit * (C::NB * NT * 8);
-        float* mine = part0 + (size_t)part * (C::NB * NT * 8);
-#pragma unroll
-        for (int n = 0; n < C::NB; ++n) {
-            if (coff[n] < 0) continue;
-            float4* d = reinterpret_cast<float4*>(mine + ((size_t)n * NT + tid) * 8);
-            __stcg(d, make_float4(acc[n][0].x, acc[n][0].y, acc[n][1].x, acc[n][1].y));
-            __stcg(d + 1, make_float4(acc[n][2].x, acc[n][2].y, acc[n][3].x, acc[n][3].y));
-        }
-        __threadfence();
-        __syncthreads();
-        if (tid == 0) {
-            const unsigned prev = atomicAdd(counters + tile, 1u);
-            s_last = (prev == (unsigned)nsplit - 1);
-            if (s_last) counters[tile] = 0;                    // ready for the next launch
-        }
-        __syncthreads();
-        if (!s_last) return;
-        __threadfence();
-#pragma unroll
-        for (int n = 0; n < C::NB; ++n) {
-            if (coff[n] < 0) continue;
-#pragma unroll
-            for (int p = 0; p < 4; ++p) acc[n][p] = make_float2(0.f, 0.f);
-            const float4* sp = reinterpret_cast<const float4*>(part0 + ((size_t)n * NT + tid) * 8);
-            constexpr size_t QS = (size_t)C::NB * NT * 2;            // float4s between the partial sums of two CTAs
-            for (int q0 = 0; q0 < nsplit; q0 += 4) {                 // loads in batches of 4 CTAs, adds in CTA order
-                float4 lo[4], hi[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    if (q0 + j < nsplit) { lo[j] = __ldcg(sp + (q0 + j) * QS); hi[j] = __ldcg(sp + (q0 + j) * QS + 1); }
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    if (q0 + j < nsplit) {
-                        acc[n][0].x += lo[j].x; acc[n][0].y += lo[j].y; acc[n][1].x += lo[j].z; acc[n][1].y += lo[j].w;
-                        acc[n][2].x += hi[j].x; acc[n][2].y += hi[j].y; acc[n][3].x += hi[j].z; acc[n][3].y += hi[j].w;
-                    }
-            }
-        }
-    }
-
-    // ---- a5: reaction term and update ------------------------------------------------------------------------
-    const float lambda = a.lambda_ptr ? __ldg(a.lambda_ptr) : a.lambda_val;
-    const float* __restrict__ f_img = a.f + (size_t)img * a.H * a.W;
-    float* __restrict__ o_img = a.u_out + (size_t)img * a.H * a.W;
+    // ---- the partial sums of this CTA (its tile, its chunk of the filter bank) go to scratch, block-major: pixel
+    // (oy, ox) of the output area at  8 * ((oy >> 1) * nbxo + (ox >> 2)) + 4 * (oy & 1) + (ox & 3).  stage_update_kernel
+    // adds the partial sums of every CTA that reaches a pixel in fixed order and applies the reaction term (a5).
+    float* mine = part + ((size_t)blockIdx.x * nsplit + blockIdx.y) * C::CTA_FLOATS;
 #pragma unroll
     for (int n = 0; n < C::NB; ++n) {
         if (coff[n] < 0) continue;
-        const int oy = coff[n] / C::VS, ox = coff[n] - oy * C::VS;
-#pragma unroll
-        for (int j = 0; j < 2; ++j)
-#pragma unroll
-            for (int p = 0; p < 4; ++p) {
-                const int ly = oy + j, lx = ox + p, gy = Y0 + ly, gx = X0 + lx;
-                if (ly < th && lx < tw && gy < a.H && gx < a.W) {
-                    const float uu = us[(ly + 2 * R) * C::US + lx + 2 * R];
-                    const float s = j ? acc[n][p].x : acc[n][p].y;
-                    const size_t g = (size_t)gy * a.W + gx;
-                    o_img[g] = uu - (s + lambda * (uu - __ldg(f_img + g)));
-                }
-            }
+        float4* d = reinterpret_cast<float4*>(mine + ((size_t)n * NT + tid) * 8);
+        __stcg(d, make_float4(acc[n][0].y, acc[n][1].y, acc[n][2].y, acc[n][3].y));
+        __stcg(d + 1, make_float4(acc[n][0].x, acc[n][1].x, acc[n][2].x, acc[n][3].x));
     }
+}
+
+// a5: u_t = u - (s + lambda (u - f)), s = sum of the partial sums of the (at most 2 x 2) tiles whose output
+// area holds the pixel, times the nsplit chunks of the filter bank, added in a fixed order (deterministic).
+// grid (ceil(W / 128), rows of the batch over y and z), 128 threads: one pixel per thread.
+__global__ void __launch_bounds__(128)
+stage_update_kernel(StageArgs a, const float* __restrict__ part, int tw, int th, int ntx, int nty, int nsplit,
+                    int cta_floats, int R)
+{
+    const long long row = (long long)blockIdx.z * 65535 + blockIdx.y;            // row of the whole batch
+    const int x = blockIdx.x * 128 + threadIdx.x;
+    if (x >= a.W || row >= (long long)a.B * a.H) return;
+    const int img = (int)(row / a.H), y = (int)(row - (long long)img * a.H);
+    const size_t idx = ((size_t)img * a.H + y) * a.W + x;
+    const float uu = __ldg(a.u_in + idx), ff = __ldg(a.f + idx);
+    const int xp = x + R, yp = y + R, Wz = a.W + 2 * R;                         // phi coordinates
+    const int txlo = x / tw, txhi = min(ntx - 1, (xp + R) / tw), tylo = y / th, tyhi = min(nty - 1, (yp + R) / th);
+    float s = 0.f;
+    for (int ty = tylo; ty <= tyhi; ++ty) {
+        const int oy = yp - (ty * th - R);
+        for (int tx = txlo; tx <= txhi; ++tx) {
+            const int X0 = tx * tw, twa = min(tw, Wz - X0), ox = xp - (X0 - 4);
+            const int nbxo = (twa + 4 + R + 3) >> 2;
+            const float* p = part + ((size_t)(img * nty + ty) * ntx + tx) * nsplit * cta_floats
+                           + 8 * ((oy >> 1) * nbxo + (ox >> 2)) + 4 * (oy & 1) + (ox & 3);
+            for (int q = 0; q < nsplit; ++q) s += __ldcg(p + (size_t)q * cta_floats);
+        }
+    }
+    const float lambda = a.lambda_ptr ? __ldg(a.lambda_ptr) : a.lambda_val;
+    a.u_out[idx] = uu - (s + lambda * (uu - ff));
 }
 
 // ---- host side: tile plan and launch ------------------------------------------------------------------------------
 struct Plan {
     int ntx, nty, tw, th, nsplit;
     double cost;      // estimated time of the launch in (thread-rounds x filters) per SM (see plan_tiles)
-    long long work;   // thread-rounds of one CTA (critical path; tie-break)
+    long long work;   // phi blocks of one CTA (critical path; tie-break)
 };
 
 inline int env_int(const char* name)
@@ -356,47 +351,49 @@ inline int forced_tile() { return env_int("TNRD_TILE"); }
 inline int forced_split() { return env_int("TNRD_SPLIT"); }
 
 // Tile plan for one kernel configuration.  The path is XU-bound, so an SM's time is proportional to the phi work
-// assigned to it: (CTAs per SM) x (rounds of 4x2 blocks per thread, 1..NB) x (threads per CTA) x (filters per CTA + a
-// constant for the tile gather, the pipeline fill/drain and the epilogue).  Try the fewest equal tiles that cover the
-// image and a few more in each direction (a smaller tile can save a whole round); when the tiles of the whole batch
-// do not fill the GPU (small images), also try splitting the filter bank of a tile over nsplit CTAs -- every split
-// pays the constant again plus the read-back of the partial sums by the last CTA.  Keep the cheapest.
+// assigned to it: (CTAs per SM) x (4x2 phi blocks of a tile; idle threads of a partly filled round cost no XU time, but
+// the transposed filter runs over the whole output area on the FMA pipe) x (filters per CTA) + a constant for the tile
+// gather, the pipeline fill/drain and the store of the partial sums.  Try the fewest equal tiles that cover the phi
+// region and a few more in each direction; when the tiles of the whole batch do not fill the GPU (small images), also
+// try splitting the filter bank of a tile over nsplit CTAs -- every split pays the constant again.  Keep the cheapest.
 template <int KS, int RW, int RH, int NT, int MINB>
 Plan plan_tiles(const StageArgs& a, int num_sms)
 {
+    using C = Cfg<KS, RW, RH, NT, MINB>;
     constexpr int R = (KS - 1) / 2;
+    const int Wz = a.W + 2 * R, Hz = a.H + 2 * R;
     Plan best{0, 0, 0, 0, 1, -1.0, 0};
-    const int ntx0 = (a.W + RW - 2 * R - 1) / (RW - 2 * R), nty0 = (a.H + RH - 2 * R - 1) / (RH - 2 * R);
+    const int ntx0 = (Wz + C::TWMAX - 1) / C::TWMAX, nty0 = (Hz + C::THMAX - 1) / C::THMAX;
     for (int dx = 0; dx < 3; ++dx)
         for (int dy = 0; dy < 3; ++dy) {
             const int ntx = ntx0 + dx, nty = nty0 + dy;
-            if (ntx > a.W || nty > a.H) continue;
-            const int tw = (a.W + ntx - 1) / ntx, th = (a.H + nty - 1) / nty;
-            const long long blocks = (long long)((tw + 2 * R + 3) / 4) * ((th + 2 * R + 1) / 2);
-            const long long rounds = (blocks + NT - 1) / NT;
+            if (ntx > Wz || nty > Hz) continue;
+            const int tw = (Wz + ntx - 1) / ntx, th = (Hz + nty - 1) / nty;
+            if ((long long)(ntx - 1) * tw >= Wz || (long long)(nty - 1) * th >= Hz) continue;   // an empty last tile
+            const long long bphi = (long long)((tw + 3) / 4) * ((th + 1) / 2);
+            const long long bout = (long long)((tw + 4 + R + 3) / 4) * ((th + 2 * R + 1) / 2);
+            const double work = bphi > 0.55 * bout ? (double)bphi : 0.55 * bout;
             const long long tiles = (long long)ntx * nty * a.B;
             int smax = 1;
             if (tiles < (long long)num_sms * MINB) smax = a.N_k < 32 ? a.N_k : 32;
-            if (tiles > SPLIT_COUNTERS) smax = 1;
             int slo = 1;
             if (forced_split() > 0) slo = smax = forced_split() < a.N_k ? forced_split() : a.N_k;
             for (int sp = slo; sp <= smax; ++sp) {
                 const int nf = (a.N_k + sp - 1) / sp;                      // filters of the largest chunk
                 if (sp > slo && (a.N_k + sp - 2) / (sp - 1) == nf) continue; // same chunk as sp - 1: only more CTAs
                 const long long ctas = tiles * sp;
-                // measured (C3, B200): ~18 us per filter for 1024 thread-rounds, ~20 us per CTA of fixed cost (tile
-                // gather, pipeline fill and drain, epilogue), ~0.5 us per split for the read-back
-                const double per_cta = (double)(rounds * NT) * nf + 1100.0 + (sp > 1 ? 30.0 * sp : 0.0);
+                // measured (C3, B200): ~18 us per filter for 1024 thread-rounds, ~20 us per CTA of fixed cost
+                const double per_cta = work * nf + 1100.0;
                 const double cost = (double)((ctas + num_sms - 1) / num_sms) * per_cta;
-                if (best.cost < 0 || cost < best.cost || (cost == best.cost && rounds * NT < best.work))
-                    best = Plan{ntx, nty, tw, th, sp, cost, rounds * NT};
+                if (best.cost < 0 || cost < best.cost || (cost == best.cost && bphi < best.work))
+                    best = Plan{ntx, nty, tw, th, sp, cost, bphi};
             }
         }
     return best;
 }
 
 template <int KS, int RW, int RH, int NT, int MINB, int PHI>
-cudaError_t launch_cfg(const StageArgs& a, const FusedPlan& pl, float* split, cudaStream_t st)
+cudaError_t launch_cfg(const StageArgs& a, const FusedPlan& pl, float* part, cudaStream_t st)
 {
     using C = Cfg<KS, RW, RH, NT, MINB>;
     static bool attr_done = false;  // per-process; the attribute is per-function and sticky
@@ -407,22 +404,21 @@ cudaError_t launch_cfg(const StageArgs& a, const FusedPlan& pl, float* split, cu
         attr_done = true;
     }
     const long long grid = (long long)pl.ntx * pl.nty * a.B;
-    if (grid > 0x7fffffffLL || pl.nsplit > 65535) return cudaErrorInvalidConfiguration;
-    if (pl.nsplit > 1 && !split) return cudaErrorInvalidValue;
+    if (grid > 0x7fffffffLL || pl.nsplit > 65535 || !part) return cudaErrorInvalidConfiguration;
     stage_fused_kernel<KS, RW, RH, NT, MINB, PHI><<<dim3((unsigned)grid, (unsigned)pl.nsplit), NT, C::SMEM, st>>>(
-        a, pl.tw, pl.th, pl.ntx, pl.nty, pl.nsplit, split);
+        a, pl.tw, pl.th, pl.ntx, pl.nty, pl.nsplit, part);
     return cudaGetLastError();
 }
 
 template <int KS>
 FusedPlan plan_ks(const StageArgs& a, int num_sms)
 {
-    // 1: 128x128 phi region, 512 threads, 1 CTA/SM (least halo); 2: 64x32, 256 threads, 2 CTAs/SM (small images);
+    // 1: 128x128 output area, 512 threads, 1 CTA/SM; 2: 64x32, 256 threads, 2 CTAs/SM (small images);
     // 3: 64x64, 256 threads, 2 CTAs/SM.  Cheapest estimated plan wins; ties go to the shorter CTA.
     const Plan p[3] = {plan_tiles<KS, 128, 128, 512, 1>(a, num_sms), plan_tiles<KS, 64, 32, 256, 2>(a, num_sms),
                        plan_tiles<KS, 64, 64, 256, 2>(a, num_sms)};
-    const size_t per_cta[3] = {Cfg<KS, 128, 128, 512, 1>::NB * 512 * 8, Cfg<KS, 64, 32, 256, 2>::NB * 256 * 8,
-                               Cfg<KS, 64, 64, 256, 2>::NB * 256 * 8};
+    const int per_cta[3] = {Cfg<KS, 128, 128, 512, 1>::CTA_FLOATS, Cfg<KS, 64, 32, 256, 2>::CTA_FLOATS,
+                            Cfg<KS, 64, 64, 256, 2>::CTA_FLOATS};
     int id = forced_tile();
     if (id < 1 || id > 3) {
         id = 1;
@@ -433,21 +429,18 @@ FusedPlan plan_ks(const StageArgs& a, int num_sms)
     if (env_int("TNRD_DEBUG_PLAN"))
         fprintf(stderr, "tnrd plan: %dx%dx%d ks %d N_k %d -> cfg %d, %d x %d tiles of %d x %d, split %d, cost %.0f\n", a.B,
                 a.H, a.W, KS, a.N_k, id, b.ntx, b.nty, b.tw, b.th, b.nsplit, b.cost);
-    FusedPlan fp{id, b.ntx, b.nty, b.tw, b.th, b.nsplit, 0};
-    if (b.nsplit > 1) {
-        const size_t tiles = (size_t)b.ntx * b.nty * a.B;
-        fp.split_floats = SPLIT_COUNTERS + tiles * b.nsplit * per_cta[id - 1];
-    }
+    FusedPlan fp{id, b.ntx, b.nty, b.tw, b.th, b.nsplit, per_cta[id - 1], 0};
+    fp.part_floats = (size_t)b.ntx * b.nty * a.B * b.nsplit * per_cta[id - 1];
     return fp;
 }
 
 template <int KS, int PHI>
-cudaError_t launch_ks(const StageArgs& a, const FusedPlan& pl, float* split, cudaStream_t st)
+cudaError_t launch_ks(const StageArgs& a, const FusedPlan& pl, float* part, cudaStream_t st)
 {
     switch (pl.cfg) {
-        case 1: return launch_cfg<KS, 128, 128, 512, 1, PHI>(a, pl, split, st);
-        case 2: return launch_cfg<KS, 64, 32, 256, 2, PHI>(a, pl, split, st);
-        case 3: return launch_cfg<KS, 64, 64, 256, 2, PHI>(a, pl, split, st);
+        case 1: return launch_cfg<KS, 128, 128, 512, 1, PHI>(a, pl, part, st);
+        case 2: return launch_cfg<KS, 64, 32, 256, 2, PHI>(a, pl, part, st);
+        case 3: return launch_cfg<KS, 64, 64, 256, 2, PHI>(a, pl, part, st);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -467,30 +460,36 @@ FusedPlan plan_stage_fused(const StageArgs& a, int num_sms)
 }
 
 template <int PHI>
-cudaError_t launch_phi(const StageArgs& a, const FusedPlan& pl, float* split, cudaStream_t st)
+cudaError_t launch_phi(const StageArgs& a, const FusedPlan& pl, float* part, cudaStream_t st)
 {
     switch (a.ksize) {
-        case 3: return launch_ks<3, PHI>(a, pl, split, st);
-        case 5: return launch_ks<5, PHI>(a, pl, split, st);
-        case 7: return launch_ks<7, PHI>(a, pl, split, st);
-        case 9: return launch_ks<9, PHI>(a, pl, split, st);
+        case 3: return launch_ks<3, PHI>(a, pl, part, st);
+        case 5: return launch_ks<5, PHI>(a, pl, part, st);
+        case 7: return launch_ks<7, PHI>(a, pl, part, st);
+        case 9: return launch_ks<9, PHI>(a, pl, part, st);
         default: return cudaErrorInvalidValue;
     }
 }
 
-cudaError_t launch_stage_fused(const StageArgs& a_in, const FusedPlan& pl, float* split, int phi_mode, cudaStream_t st,
+cudaError_t launch_stage_fused(const StageArgs& a_in, const FusedPlan& pl, float* part, int phi_mode, cudaStream_t st,
                                unsigned long long* launches)
 {
     StageArgs a = a_in;
     a.dense_is_fallback = (phi_mode == 1);
     if (phi_mode == 1) {            // windowed evaluator; exits at once when the centres are not equidistant ...
-        cudaError_t e = launch_phi<1>(a, pl, split, st);
+        cudaError_t e = launch_phi<1>(a, pl, part, st);
         ++*launches;
         if (e != cudaSuccess) return e;
     }
-    cudaError_t e = launch_phi<0>(a, pl, split, st);   // ... in which case this dense launch does the work (else it exits)
+    cudaError_t e = launch_phi<0>(a, pl, part, st);   // ... in which case this dense launch does the work (else it exits)
     ++*launches;
-    return e;
+    if (e != cudaSuccess) return e;
+    const long long rows = (long long)a.B * a.H;
+    stage_update_kernel<<<dim3((unsigned)((a.W + 127) / 128), (unsigned)(rows < 65535 ? rows : 65535),
+                               (unsigned)((rows + 65534) / 65535)), 128, 0, st>>>(
+        a, part, pl.tw, pl.th, pl.ntx, pl.nty, pl.nsplit, pl.cta_floats, (a.ksize - 1) / 2);
+    ++*launches;
+    return cudaGetLastError();
 }
 
 }  // namespace tnrd

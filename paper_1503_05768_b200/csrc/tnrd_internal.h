@@ -50,14 +50,15 @@ struct StageArgs {
     int dense_is_fallback;  // set by the launcher: the dense kernel returns at once when the windowed one applies
 };
 
-// Launch plan of the fused stage kernel (tnrd_fused.cu: plan_stage_fused).  nsplit > 1 = the small-image path: the
-// filter bank of one tile is split over nsplit CTAs, whose partial transposed-filter sums meet in `split_floats`
-// floats of scratch (the last CTA of a tile to arrive adds them in fixed order and writes u_t).
+// Launch plan of the fused stage kernel (tnrd_fused.cu: plan_stage_fused).  Tiles partition the phi region
+// (H + 2r) x (W + 2r); nsplit > 1 = the small-image path: the filter bank of a tile is split over nsplit CTAs.  Every CTA
+// stores its partial transposed-filter sums in `part_floats` floats of scratch; stage_update_kernel adds them up.
 struct FusedPlan {
-    int cfg;                 // kernel configuration 1..3 (tile size / threads)
-    int ntx, nty, tw, th;    // tiles per image and output tile size
+    int cfg;                 // kernel configuration 1..3 (output area / threads)
+    int ntx, nty, tw, th;    // tiles per image and nominal tile size (the last tile of a row / column may be smaller)
     int nsplit;              // CTAs per tile (each takes a contiguous chunk of the N_k filters)
-    size_t split_floats;     // scratch needed when nsplit > 1: counters (one per tile) + partial sums; else 0
+    int cta_floats;          // partial sums of one CTA
+    size_t part_floats;      // scratch needed: ntx * nty * B * nsplit * cta_floats
 };
 
 // ---- backward pass of a stage (tnrd_bwd.cu) ----------------------------------------------------------------
@@ -94,10 +95,8 @@ cudaError_t launch_prep(const float* filters, const float* rbf_w, const float* r
 cudaError_t launch_stage_ref(const StageArgs& a, float* vbuf, cudaStream_t st, unsigned long long* launches);
 size_t ref_scratch_floats(int B, int H, int W, int N_k, int ksize);
 FusedPlan plan_stage_fused(const StageArgs& a, int num_sms);
-// phi_mode: 0 dense, 1 windowed (with dense fallback).  split = scratch of plan.split_floats floats whose first
-// 4096 words (tile counters) are zero before the first launch (the kernel leaves them zero); may be null when
-// nsplit == 1.
-cudaError_t launch_stage_fused(const StageArgs& a, const FusedPlan& plan, float* split, int phi_mode, cudaStream_t st,
+// phi_mode: 0 dense, 1 windowed (with dense fallback).  part = scratch of plan.part_floats floats.
+cudaError_t launch_stage_fused(const StageArgs& a, const FusedPlan& plan, float* part, int phi_mode, cudaStream_t st,
                                unsigned long long* launches);
 cudaError_t launch_qcs_project(const float* y, const float* lo, const float* hi, float* u, int B, int H, int W,
                                cudaStream_t st, unsigned long long* launches);   // u may alias y
