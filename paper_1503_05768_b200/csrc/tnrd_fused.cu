@@ -351,11 +351,10 @@ inline int forced_tile() { return env_int("TNRD_TILE"); }
 inline int forced_split() { return env_int("TNRD_SPLIT"); }
 
 // Tile plan for one kernel configuration.  The path is XU-bound, so an SM's time is proportional to the phi work
-// assigned to it: (CTAs per SM) x (4x2 phi blocks of a tile; idle threads of a partly filled round cost no XU time, but
-// the transposed filter runs over the whole output area on the FMA pipe) x (filters per CTA) + a constant for the tile
-// gather, the pipeline fill/drain and the store of the partial sums.  Try the fewest equal tiles that cover the phi
-// region and a few more in each direction; when the tiles of the whole batch do not fill the GPU (small images), also
-// try splitting the filter bank of a tile over nsplit CTAs -- every split pays the constant again.  Keep the cheapest.
+// assigned to it: (CTAs per SM) x (filters per CTA) x (time of one filter, see below; constants fitted on B200 at 4096^2
+// and on C3).  Try the fewest equal tiles that cover the phi region and a few more in each direction; when the tiles of
+// the whole batch do not fill the GPU (small images), also try splitting the filter bank of a tile over nsplit CTAs --
+// every split pays the per-CTA constant again.  Keep the cheapest.
 template <int KS, int RW, int RH, int NT, int MINB>
 Plan plan_tiles(const StageArgs& a, int num_sms)
 {
@@ -364,15 +363,29 @@ Plan plan_tiles(const StageArgs& a, int num_sms)
     const int Wz = a.W + 2 * R, Hz = a.H + 2 * R;
     Plan best{0, 0, 0, 0, 1, -1.0, 0};
     const int ntx0 = (Wz + C::TWMAX - 1) / C::TWMAX, nty0 = (Hz + C::THMAX - 1) / C::THMAX;
+    const int fx = env_int("TNRD_NTX"), fy = env_int("TNRD_NTY");       // tuning knobs: force the tile counts
     for (int dx = 0; dx < 3; ++dx)
         for (int dy = 0; dy < 3; ++dy) {
-            const int ntx = ntx0 + dx, nty = nty0 + dy;
+            int ntx = ntx0 + dx, nty = nty0 + dy;
+            if (fx >= ntx0 && fy >= nty0) { ntx = fx; nty = fy; }
             if (ntx > Wz || nty > Hz) continue;
             const int tw = (Wz + ntx - 1) / ntx, th = (Hz + nty - 1) / nty;
             if ((long long)(ntx - 1) * tw >= Wz || (long long)(nty - 1) * th >= Hz) continue;   // an empty last tile
             const long long bphi = (long long)((tw + 3) / 4) * ((th + 1) / 2);
             const long long bout = (long long)((tw + 4 + R + 3) / 4) * ((th + 2 * R + 1) / 2);
-            const double work = bphi > 0.55 * bout ? (double)bphi : 0.55 * bout;
+            // time of one filter on one CTA in units of one warp-block on the XU pipe of an SM sub-partition (~2 us:
+            // 8 px x 63 ex2 x 32 lanes at 4 lanes per clock): rounds of NT blocks, a round with w warps of phi work
+            // takes k = ceil(w / 4) units when k >= 4 warps share a sub-partition; fewer warps feed the pipe worse (3.3, 2.5,
+            // 1.6 units for k = 3, 2, 1); plus ~2 units per filter that do not overlap (barrier, pipeline restart) and
+            // ~6 per CTA (tile gather, fill / drain, stores)
+            double per_filter = 2.0;
+            for (long long done = 0; done < bout; done += NT) {
+                const long long inr = bphi - done < 0 ? 0 : (bphi - done > NT ? NT : bphi - done);
+                const long long wr = (inr + 31) / 32;
+                const int kw = (int)((wr + 3) / 4);                       // warps per SM sub-partition in this round
+                if (wr > 0) per_filter += kw >= 4 ? (double)kw : kw == 3 ? 3.3 : kw == 2 ? 2.5 : 1.6;
+                else per_filter += 0.3;                                    // transposed filter only
+            }
             const long long tiles = (long long)ntx * nty * a.B;
             int smax = 1;
             if (tiles < (long long)num_sms * MINB) smax = a.N_k < 32 ? a.N_k : 32;
@@ -382,9 +395,7 @@ Plan plan_tiles(const StageArgs& a, int num_sms)
                 const int nf = (a.N_k + sp - 1) / sp;                      // filters of the largest chunk
                 if (sp > slo && (a.N_k + sp - 2) / (sp - 1) == nf) continue; // same chunk as sp - 1: only more CTAs
                 const long long ctas = tiles * sp;
-                // measured (C3, B200): ~18 us per filter for 1024 thread-rounds, ~20 us per CTA of fixed cost
-                const double per_cta = work * nf + 1100.0;
-                const double cost = (double)((ctas + num_sms - 1) / num_sms) * per_cta;
+                const double cost = (double)((ctas + num_sms - 1) / num_sms) * (per_filter * nf + 6.0);
                 if (best.cost < 0 || cost < best.cost || (cost == best.cost && bphi < best.work))
                     best = Plan{ntx, nty, tw, th, sp, cost, bphi};
             }
