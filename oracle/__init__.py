@@ -55,6 +55,9 @@ def _load():
         lib.oracle_corr_valid.restype = None
         lib.oracle_phi.argtypes = [dp, ctypes.c_size_t, dp, dp, ci, cd, dp]
         lib.oracle_phi.restype = None
+        lib.oracle_set_basis.argtypes = [ci]
+        lib.oracle_set_basis.restype = None
+        lib.oracle_get_basis.restype = ci
         lib.oracle_stage.argtypes = [dp, dp, ci, ci, ci, ci, ci, dp, dp, dp, ci, cd, cd, dp, ci]
         lib.oracle_stage.restype = ci
         lib.oracle_diffuse.argtypes = [dp, dp, ci, ci, ci, ci, ci, ci, dp, dp, dp, ci, cd, dp, dp, ci]
@@ -69,6 +72,24 @@ def _d(a):
 
 def _p(a):
     return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+GAUSSIAN, TRIANGLE = 0, 1   # radial basis of phi
+
+
+class basis:
+    """Context manager: evaluate phi with the given radial basis inside the block (the oracle's switch is restored)."""
+
+    def __init__(self, which: int):
+        self.which = int(which)
+
+    def __enter__(self):
+        self.old = int(_load().oracle_get_basis())
+        _load().oracle_set_basis(self.which)
+        return self
+
+    def __exit__(self, *exc):
+        _load().oracle_set_basis(self.old)
 
 
 def num_threads() -> int:

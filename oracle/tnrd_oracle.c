@@ -23,7 +23,8 @@
  * zero padding, P5 finite-difference of the FoE energy (erf closed form), P6 linear-phi
  * special case against scipy.signal, P7 dense-matrix brute force on 8x8, P8 literal
  * pad-omega/crop procedure for several omega, P9 flip/transpose equivariance, P12 degenerate
- * parameters, P13 interior shift-equivariance.  Absolute end-to-end values for the
+ * parameters, P13 interior shift-equivariance; PT1-PT3 (tests/test_oracle_triangle.py) the triangular basis against
+ * numpy.interp, its partition of unity and closed forms.  Absolute end-to-end values for the
  * BASELINE.json configs are "parity unpinned by the paper" (no printed example, no weights).
  *
  * Layouts: images row-major [B][H][W] (x fastest); filters [N_k][K][K] with k[a][b],
@@ -127,14 +128,27 @@ void oracle_corr_valid(const double *in, int Hin, int Win, const double *k, int 
     }
 }
 
-/* O3 influence function, Gaussian RBF mixture (PAPER.md:113-117 Eq. 6; :553 phi_g):
- *   phi(z) = sum_{j=1..M} w_j exp( -(z - mu_j)^2 / (2 gamma^2) )                        */
+/* Radial basis of the influence functions: 0 = Gaussian phi_g (the paper's results, default),
+ * 1 = triangular-shaped phi_t.  A process-wide switch of the ORACLE (tests set it around a call and restore it); it
+ * selects which of the two printed formulas oracle_phi1 evaluates, nothing else. */
+static int g_basis = 0;
+void oracle_set_basis(int basis) { g_basis = basis ? 1 : 0; }
+int oracle_get_basis(void) { return g_basis; }
+
+/* O3 influence function, RBF mixture (Eq. 6):  phi(z) = sum_{j=1..M} w_j varphi(|z - mu_j| / gamma)
+ *   Gaussian   (:553)  varphi_g = exp( -(z - mu_j)^2 / (2 gamma^2) )
+ *   triangular (:557)  varphi_t = 1 - |z - mu_j| / gamma  if |z - mu_j| <= gamma,  0 otherwise                        */
 double oracle_phi1(double z, const double *w, const double *mu, int M, double gamma)
 {
     double acc = 0.0;
     for (int j = 0; j < M; ++j) {
         const double d = z - mu[j];
-        acc += w[j] * exp(-(d * d) / (2.0 * gamma * gamma));
+        if (g_basis == 0) {
+            acc += w[j] * exp(-(d * d) / (2.0 * gamma * gamma));
+        } else {
+            const double ad = fabs(d);
+            if (ad <= gamma) acc += w[j] * (1.0 - ad / gamma);
+        }
     }
     return acc;
 }
