@@ -303,6 +303,22 @@ def main():
         tnrd.tnrd_set_phi_mode(0)
         ms_w = max_over_ranks(e4.elapsed_time(e5), devs)
         win = px_stages_all / (ms_w * 1e-3) / 1e6
+        # ... and the lookup-table evaluator (tnrd_set_phi_mode(2): the authors' own approximation)
+        tnrd.tnrd_set_phi_mode(2)
+        for _ in range(warmup):
+            step()
+        barrier()
+        lut_out = out.clone()
+        e6, e7 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e6.record(stream)
+        for _ in range(args.steps):
+            step()
+        e7.record(stream)
+        barrier()
+        tnrd.tnrd_set_phi_mode(0)
+        lut = px_stages_all / (max_over_ranks(e6.elapsed_time(e7), devs) * 1e-3) / 1e6
+        step(); barrier()
+        lut_dist = float((lut_out - out).abs().max())
 
     if rank != 0:
         if world > 1:
@@ -352,6 +368,10 @@ def main():
                                          / (ms_w * 1e-3) / 1e12 / peak_nominal,
             "x_dense_roofline": win / (peak_nominal * 1e12 / EX2_PER_PX_STAGE / 1e6),
             "note": "tnrd_set_phi_mode(1): 16 of 63 Gaussians per response, dropped terms < 6.7e-10 w each"}
+        line["lut_phi"] = {
+            "value": lut, "unit": "Mpixel-stages/s", "x_dense_roofline": lut / (peak_nominal * 1e12 / EX2_PER_PX_STAGE / 1e6),
+            "max_abs_from_dense": lut_dist,
+            "note": "tnrd_set_phi_mode(2): 4096-node table + linear interpolation per filter (PAPER.md:572), an approximation"}
     if not args.no_cpu_baseline and world == 1:
         v, cores, sample, _ = oracle_sample(cfg, target_s=args.ref_seconds)
         line["cpu_baseline"] = {"value": v, "unit": "Mpixel-stages/s", "cores": cores, "kind": "oracle",

@@ -171,11 +171,30 @@ int tnrd_set_kernel(int which);
  *       contain every centre within 6.5 gamma; the dropped terms are each below e^{-21.1} = 6.7e-10 of their weight, i.e.
  *       below fp32 rounding of the sum ("equidistant centers").  When the check
  *       fails the dense evaluator runs instead -- decided on the device, two launches per stage, no host synchronisation.
+ *   TNRD_PHI_LUT (2): the authors' own speed-up: phi_i is tabulated at 4096 equidistant nodes from 6 gamma
+ *       below the lowest centre to 6 gamma above the highest (every node the full 63-term sum, rebuilt on the device at
+ *       every call) and evaluated by linear interpolation -- one gather and one FMA per response.  An APPROXIMATION of
+ *       Main Eq. 6: per response |error| <= h^2/8 max|phi''| with node spacing h (0.18 for the configs' centres); the
+ *       end-to-end distance from the oracle stays inside the library's tolerance.
  * Returns TNRD_ERR_UNSUPPORTED for other values.
  */
 #define TNRD_PHI_DENSE 0
 #define TNRD_PHI_WINDOW 1
+#define TNRD_PHI_LUT 2
 int tnrd_set_phi_mode(int mode);
+
+/*
+ * Radial basis of the influence functions.  Process-wide.
+ *   TNRD_RBF_GAUSSIAN (0, default): phi_i(z) = sum_j w_ij exp(-(z - mu_j)^2 / (2 gamma^2))            (the paper's results)
+ *   TNRD_RBF_TRIANGLE (1): phi_i(z) = sum_j w_ij max(0, 1 - |z - mu_j| / gamma)
+ *       evaluated through the table evaluator whatever tnrd_set_phi_mode says: EXACTLY (the linear interpolant of the
+ *       weights, two basis functions per z) when rbf_mu is equidistant and rbf_gamma equals the spacing;
+ *       otherwise on the 4096-node grid of TNRD_PHI_LUT (approximate).  tnrd_stage_backward / tnrd_diffuse_backward and
+ *       the reference kernel (tnrd_set_kernel(1)) return TNRD_ERR_UNSUPPORTED with this basis.
+ */
+#define TNRD_RBF_GAUSSIAN 0
+#define TNRD_RBF_TRIANGLE 1
+int tnrd_set_rbf_basis(int basis);
 
 /* Number of kernels this library has launched since load (or since the last tnrd_reset_launch_count). */
 unsigned long long tnrd_launch_count(void);

@@ -64,6 +64,8 @@ def lib() -> ctypes.CDLL:
         L.tnrd_set_kernel.restype = ci
         L.tnrd_set_phi_mode.argtypes = [ci]
         L.tnrd_set_phi_mode.restype = ci
+        L.tnrd_set_rbf_basis.argtypes = [ci]
+        L.tnrd_set_rbf_basis.restype = ci
         L.tnrd_launch_count.restype = ctypes.c_ulonglong
         L.tnrd_reset_launch_count.restype = None
         L.tnrd_microbench.argtypes = [ci, ctypes.POINTER(ctypes.c_double), vp]
@@ -166,8 +168,14 @@ def tnrd_set_kernel(which: int):
 
 
 def tnrd_set_phi_mode(mode: int):
-    """0 = dense 63-term phi (default), 1 = windowed evaluator (include/tnrd.h: tnrd_set_phi_mode)."""
+    """0 = dense 63-term phi (default), 1 = windowed evaluator, 2 = lookup table + linear interpolation
+    (include/tnrd.h: tnrd_set_phi_mode)."""
     _check(lib().tnrd_set_phi_mode(int(mode)))
+
+
+def tnrd_set_rbf_basis(basis: int):
+    """0 = Gaussian radial basis (default), 1 = triangular-shaped (include/tnrd.h: tnrd_set_rbf_basis)."""
+    _check(lib().tnrd_set_rbf_basis(int(basis)))
 
 
 def tnrd_launch_count() -> int:

@@ -15,7 +15,8 @@ namespace {
 thread_local char g_cuda_err[512] = "";
 unsigned long long g_launches = 0;
 int g_kernel = 0;  // 0 auto, 1 reference, 2 fused
-int g_phi_mode = 0;  // 0 dense 63-term phi, 1 windowed evaluator (dense fallback decided on the device)
+int g_phi_mode = 0;  // 0 dense 63-term phi, 1 windowed evaluator (dense fallback decided on the device), 2 table
+int g_basis = 0;     // 0 Gaussian radial basis, 1 triangular-shaped (table evaluator)
 std::mutex g_mu;
 
 int cuda_fail(cudaError_t e, const char* what)
@@ -42,6 +43,7 @@ struct Scratch {
     int num_sms = 0;
     Buf prm, plane[2], refv;          // staged parameters, ping-pong planes, reference-path phi maps
     Buf split;                        // partial transposed-filter sums of the fused kernel's CTAs
+    Buf tab;                          // piecewise-linear phi tables [T][N_k][4096] float2 + 4 header floats
     Buf h_f, h_u, h_out, h_par;       // device staging of the host entry point
     Buf bw_maps, bw_part, bw_trace, bw_e[2];   // backward pass: P/V maps, per-CTA partial sums, iterates, dl/du planes
 };
@@ -87,10 +89,35 @@ int check_shape(int B, int H, int W, int N_k, int ksize)
 
 int check_gamma(float g) { return (std::isfinite(g) && g > 0.0f) ? TNRD_OK : TNRD_ERR_PARAM; }
 
-int run_stage(Scratch* sc, const tnrd::StageArgs& a, cudaStream_t st)
+// evaluator of the fused kernel for the current settings: the triangular basis always goes through the table
+int effective_phi() { return (g_basis == 1 || g_phi_mode == 2) ? 2 : g_phi_mode; }
+
+// Stages the parameters of T stages; with the table evaluator also builds the phi tables.
+int stage_params(Scratch* sc, const float* filters, const float* rbf_w, const float* rbf_mu, float gamma, int T, int N_k,
+                 int ksize, int phi, cudaStream_t st)
+{
+    int rc = grow(sc->prm, (size_t)T * N_k * tnrd::prm_stride(ksize), st);
+    if (rc != TNRD_OK) return rc;
+    TNRD_CUDA(tnrd::launch_prep(filters, rbf_w, rbf_mu, gamma, T, N_k, ksize, sc->prm.p, st, &g_launches));
+    if (phi == 2) {
+        const size_t n = (size_t)T * N_k * TNRD_TAB_NODES * 2;
+        if ((rc = grow(sc->tab, n + 4, st)) != TNRD_OK) return rc;
+        TNRD_CUDA(tnrd::launch_build_table(rbf_w, rbf_mu, gamma, T * N_k, g_basis, sc->tab.p + 4, sc->tab.p, st,
+                                           &g_launches));
+    }
+    return TNRD_OK;
+}
+
+// phi: evaluator (0, 1, 2); t = stage index inside the staged parameters (selects the table)
+int run_stage(Scratch* sc, tnrd::StageArgs a, int phi, int t, cudaStream_t st)
 {
     const bool use_ref = (g_kernel == 1);
+    if (phi == 2) {
+        a.tabhdr = sc->tab.p;
+        a.tab = sc->tab.p + 4 + (size_t)t * a.N_k * TNRD_TAB_NODES * 2;
+    }
     if (use_ref) {
+        if (g_basis == 1) return TNRD_ERR_UNSUPPORTED;     // the reference kernel knows the Gaussian basis only
         int rc = grow(sc->refv, tnrd::ref_scratch_floats(a.B, a.H, a.W, a.N_k, a.ksize), st);
         if (rc != TNRD_OK) return rc;
         TNRD_CUDA(tnrd::launch_stage_ref(a, sc->refv.p, st, &g_launches));
@@ -98,7 +125,7 @@ int run_stage(Scratch* sc, const tnrd::StageArgs& a, cudaStream_t st)
         const tnrd::FusedPlan pl = tnrd::plan_stage_fused(a, sc->num_sms);
         int rc = grow(sc->split, pl.part_floats, st);
         if (rc != TNRD_OK) return rc;
-        TNRD_CUDA(tnrd::launch_stage_fused(a, pl, sc->split.p, g_phi_mode, st, &g_launches));
+        TNRD_CUDA(tnrd::launch_stage_fused(a, pl, sc->split.p, phi, st, &g_launches));
     }
     return TNRD_OK;
 }
@@ -119,10 +146,10 @@ int tnrd_stage(const float* f, const float* u_in, int B, int H, int W, int N_k, 
     cudaStream_t st = (cudaStream_t)stream;
     Scratch* sc = nullptr;
     if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
-    if ((rc = grow(sc->prm, (size_t)N_k * tnrd::prm_stride(ksize), st)) != TNRD_OK) return rc;
-    TNRD_CUDA(tnrd::launch_prep(filters_t, rbf_w_t, rbf_mu, rbf_gamma, 1, N_k, ksize, sc->prm.p, st, &g_launches));
+    const int phi = effective_phi();
+    if ((rc = stage_params(sc, filters_t, rbf_w_t, rbf_mu, rbf_gamma, 1, N_k, ksize, phi, st)) != TNRD_OK) return rc;
     tnrd::StageArgs a{f, u_in, u_out, sc->prm.p, nullptr, lambda_t, B, H, W, N_k, ksize};
-    return run_stage(sc, a, st);
+    return run_stage(sc, a, phi, 0, st);
 }
 
 int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, int N_k, int ksize,
@@ -145,20 +172,20 @@ int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, in
     Scratch* sc = nullptr;
     if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
     const size_t rec = (size_t)N_k * tnrd::prm_stride(ksize);
-    if ((rc = grow(sc->prm, (size_t)T * rec, st)) != TNRD_OK) return rc;
+    const int phi = effective_phi();
     // Destinations d_1..d_T: alternate scratch / out so that d_T = out and no stage writes what it reads.
     // In place (out == u0) with odd T the first stage may not write out: it goes to a second plane.
     const bool inplace_odd = (out == u0) && (T & 1);
     if (T > 1 && (rc = grow(sc->plane[0], n, st)) != TNRD_OK) return rc;
     if (inplace_odd && (rc = grow(sc->plane[1], n, st)) != TNRD_OK) return rc;
-    TNRD_CUDA(tnrd::launch_prep(filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, sc->prm.p, st, &g_launches));
+    if ((rc = stage_params(sc, filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, phi, st)) != TNRD_OK) return rc;
     const float* src = u0;
     for (int t = 1; t <= T; ++t) {
         float* dst;
         if (t == 1 && inplace_odd) dst = sc->plane[1].p;
         else dst = ((T - t) & 1) ? sc->plane[0].p : out;
         tnrd::StageArgs a{f, src, dst, sc->prm.p + (size_t)(t - 1) * rec, lambda + (t - 1), 0.0f, B, H, W, N_k, ksize};
-        if ((rc = run_stage(sc, a, st)) != TNRD_OK) return rc;
+        if ((rc = run_stage(sc, a, phi, t - 1, st)) != TNRD_OK) return rc;
         src = dst;
     }
     if (src != out)  // T == 1 in place: the single stage went to the second plane
@@ -240,11 +267,11 @@ int tnrd_deblock_diffuse(const float* u0, int B, int H, int W, int T, int N_k, i
     Scratch* sc = nullptr;
     if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
     const size_t rec = (size_t)N_k * tnrd::prm_stride(ksize);
-    if ((rc = grow(sc->prm, (size_t)T * rec, st)) != TNRD_OK) return rc;
+    const int phi = effective_phi();
     const bool inplace_odd = (out == u0) && (T & 1);
     if (T > 1 && (rc = grow(sc->plane[0], n, st)) != TNRD_OK) return rc;
     if (inplace_odd && (rc = grow(sc->plane[1], n, st)) != TNRD_OK) return rc;
-    TNRD_CUDA(tnrd::launch_prep(filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, sc->prm.p, st, &g_launches));
+    if ((rc = stage_params(sc, filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, phi, st)) != TNRD_OK) return rc;
     // Same ping-pong as tnrd_diffuse.  Per stage (Supp. Eq. 29): the fused kernel with lambda = 0 writes
     // y = u - sum_i kbar_i * phi_i(k_i * u) to the destination plane (f is then irrelevant: u itself is passed),
     // the projection kernel turns it into u_t = D^T eta(D y) in place.
@@ -254,7 +281,7 @@ int tnrd_deblock_diffuse(const float* u0, int B, int H, int W, int T, int N_k, i
         if (t == 1 && inplace_odd) dst = sc->plane[1].p;
         else dst = ((T - t) & 1) ? sc->plane[0].p : out;
         tnrd::StageArgs a{src, src, dst, sc->prm.p + (size_t)(t - 1) * rec, nullptr, 0.0f, B, H, W, N_k, ksize};
-        if ((rc = run_stage(sc, a, st)) != TNRD_OK) return rc;
+        if ((rc = run_stage(sc, a, phi, t - 1, st)) != TNRD_OK) return rc;
         TNRD_CUDA(tnrd::launch_qcs_project(dst, qcs_lo, qcs_hi, dst, B, H, W, st, &g_launches));
         src = dst;
     }
@@ -301,6 +328,7 @@ int tnrd_stage_backward(const float* f, const float* u_in, const float* e, int B
     if (rc != TNRD_OK) return rc;
     if ((rc = check_gamma(rbf_gamma)) != TNRD_OK) return rc;
     if (grad_u && (grad_u == u_in || grad_u == e || grad_u == f)) return TNRD_ERR_ALIAS;
+    if (g_basis == 1) return TNRD_ERR_UNSUPPORTED;          // gradients exist for the Gaussian basis only
     cudaStream_t st = (cudaStream_t)stream;
     Scratch* sc = nullptr;
     if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
@@ -323,6 +351,7 @@ int tnrd_diffuse_backward(const float* f, const float* u0, const float* u_gt, co
     if ((rc = check_gamma(rbf_gamma)) != TNRD_OK) return rc;
     if (grad_u0 && (grad_u0 == u0 || grad_u0 == f || grad_u0 == e_T || grad_u0 == u_gt)) return TNRD_ERR_ALIAS;
     if (u_T && (u_T == u0 || u_T == f)) return TNRD_ERR_ALIAS;
+    if (g_basis == 1) return TNRD_ERR_UNSUPPORTED;          // gradients exist for the Gaussian basis only
     cudaStream_t st = (cudaStream_t)stream;
     Scratch* sc = nullptr;
     if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
@@ -338,7 +367,8 @@ int tnrd_diffuse_backward(const float* f, const float* u0, const float* u_gt, co
     for (int t = 1; t <= T; ++t) {
         float* dst = sc->bw_trace.p + (size_t)(t - 1) * n;
         tnrd::StageArgs a{f, src, dst, sc->prm.p + (size_t)(t - 1) * rec, lambda + (t - 1), 0.0f, B, H, W, N_k, ksize};
-        if ((rc = run_stage(sc, a, st)) != TNRD_OK) return rc;
+        // the forward pass of a gradient is the exact evaluator (dense, or windowed if selected), never the table
+        if ((rc = run_stage(sc, a, g_phi_mode == 1 ? 1 : 0, t - 1, st)) != TNRD_OK) return rc;
         src = dst;
     }
     if (u_T) TNRD_CUDA(cudaMemcpyAsync(u_T, src, n * sizeof(float), cudaMemcpyDeviceToDevice, st));
@@ -374,8 +404,15 @@ int tnrd_set_kernel(int which)
 
 int tnrd_set_phi_mode(int mode)
 {
-    if (mode < 0 || mode > 1) return TNRD_ERR_UNSUPPORTED;
+    if (mode < 0 || mode > 2) return TNRD_ERR_UNSUPPORTED;
     g_phi_mode = mode;
+    return TNRD_OK;
+}
+
+int tnrd_set_rbf_basis(int basis)
+{
+    if (basis < 0 || basis > 1) return TNRD_ERR_UNSUPPORTED;
+    g_basis = basis;
     return TNRD_OK;
 }
 
@@ -414,7 +451,7 @@ void tnrd_shutdown(void)
     (void)cudaGetDevice(&cur);
     for (Scratch* s : g_scratch) {
         (void)cudaSetDevice(s->dev);
-        Buf* bufs[] = {&s->prm, &s->plane[0], &s->plane[1], &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->refv, &s->split, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
+        Buf* bufs[] = {&s->prm, &s->plane[0], &s->plane[1], &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->refv, &s->split, &s->tab, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
         for (Buf* b : bufs)
             if (b->p) (void)cudaFree(b->p);   // synchronising free: the stream may be gone by now
         delete s;

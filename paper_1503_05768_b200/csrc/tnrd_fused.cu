@@ -142,9 +142,12 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int ns
         w_inv_delta = __ldg(a.prm + prm_hdr(KS) + 0);
         w_mu0 = __ldg(a.prm + prm_hdr(KS) + 1);
         w_delta = __ldg(a.prm + prm_hdr(KS) + 2);
-    } else if (a.dense_is_fallback) {
+    } else if (PHI == 0 && a.dense_is_fallback) {
         if (__ldg(a.prm + prm_hdr(KS) + 3) != 0.0f) return;
     }
+    // piecewise-linear table evaluator (PHI = 2; tnrd_table.cu): t = a z' + b in node units
+    float t_a = 0.f, t_b = 0.f, t_max = 0.f;
+    if (PHI == 2) { t_a = __ldg(a.tabhdr); t_b = __ldg(a.tabhdr + 1); t_max = __ldg(a.tabhdr + 2); }
 
     // ---- work decomposition: 4x2 pixel blocks, NB per thread ----------------------------------------------
     const int nbx = (tw + 3) >> 2, nby = (th + 1) >> 1;                         // phi blocks: the tile itself
@@ -229,6 +232,20 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int ns
             float2 dd[4];
             int wofs[4][2];
             unsigned wsec = 0;
+            float2 te[4][2];                       // PHI = 2: table entries (value, slope) of the 8 responses ...
+            float2 tf[4];                          // ... and the positions inside their table cells
+            if (PHI == 2 && hasB) {                // the gathers are issued here and used after the row-steps below
+                const float2* __restrict__ tabi = reinterpret_cast<const float2*>(a.tab) + (size_t)(f0 + i) * TNRD_TAB_NODES;
+#pragma unroll
+                for (int p = 0; p < 4; ++p) {
+                    const float tx_ = fminf(fmaxf(fmaf(zc[p].x, t_a, t_b), 0.0f), t_max);
+                    const float ty_ = fminf(fmaxf(fmaf(zc[p].y, t_a, t_b), 0.0f), t_max);
+                    const int jx = min((int)tx_, (int)t_max - 1), jy = min((int)ty_, (int)t_max - 1);
+                    tf[p] = make_float2(tx_ - (float)jx, ty_ - (float)jy);
+                    te[p][0] = __ldg(tabi + jx);
+                    te[p][1] = __ldg(tabi + jy);
+                }
+            }
             if (PHI == 1) {
 #pragma unroll
                 for (int p = 0; p < 4; ++p) {
@@ -241,7 +258,7 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int ns
             for (int g = 0; g < C::NG - 1; ++g) {
                 if (hasB) {
                     if (PHI == 1) phi_win_step(wsec + 8 * g, wofs, w_delta, dd, v);
-                    else phi_step<8>(rec + KKP + 16 * g, zc, v);
+                    else if (PHI == 0) phi_step<8>(rec + KKP + 16 * g, zc, v);
                 }
                 if (g <= KS) {
                     if (hasN) rowstep<KS, false>(uwn + g * C::US, tapsN + (KS - g) * TS, zn);
@@ -257,12 +274,17 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int ns
                 constexpr int g = C::NG - 1;
                 if (hasB) {
                     if (PHI == 1) phi_win_step(wsec + 8 * g, wofs, w_delta, dd, v);
-                    else phi_step<TNRD_M - 8 * g>(rec + KKP + 16 * g, zc, v);
+                    else if (PHI == 0) phi_step<TNRD_M - 8 * g>(rec + KKP + 16 * g, zc, v);
                 }
                 if (g <= KS) {
                     if (hasN) rowstep<KS, false>(uwn + g * C::US, tapsN + (KS - g) * TS, zn);
                     if (hasC) rowstep<KS, true, C::SHIFT>(vw + g * C::VS, recp + g * TS, acc[n]);
                 }
+            }
+            if (PHI == 2 && hasB) {
+#pragma unroll
+                for (int p = 0; p < 4; ++p)
+                    v[p] = make_float2(fmaf(tf[p].x, te[p][0].y, te[p][0].x), fmaf(tf[p].y, te[p][1].y, te[p][1].x));
             }
             if (hasB) {     // pixels of a ragged block that lie outside the tile belong to the neighbour: keep the ring zero
                 const unsigned m = own >> (8 * n);
@@ -487,13 +509,20 @@ cudaError_t launch_stage_fused(const StageArgs& a_in, const FusedPlan& pl, float
 {
     StageArgs a = a_in;
     a.dense_is_fallback = (phi_mode == 1);
-    if (phi_mode == 1) {            // windowed evaluator; exits at once when the centres are not equidistant ...
-        cudaError_t e = launch_phi<1>(a, pl, part, st);
+    cudaError_t e;
+    if (phi_mode == 2) {            // piecewise-linear table evaluator (always applicable)
+        if (!a.tab || !a.tabhdr) return cudaErrorInvalidValue;
+        e = launch_phi<2>(a, pl, part, st);
         ++*launches;
-        if (e != cudaSuccess) return e;
+    } else {
+        if (phi_mode == 1) {        // windowed evaluator; exits at once when the centres are not equidistant ...
+            e = launch_phi<1>(a, pl, part, st);
+            ++*launches;
+            if (e != cudaSuccess) return e;
+        }
+        e = launch_phi<0>(a, pl, part, st);   // ... in which case this dense launch does the work (else it exits)
+        ++*launches;
     }
-    cudaError_t e = launch_phi<0>(a, pl, part, st);   // ... in which case this dense launch does the work (else it exits)
-    ++*launches;
     if (e != cudaSuccess) return e;
     const long long rows = (long long)a.B * a.H;
     stage_update_kernel<<<dim3((unsigned)((a.W + 127) / 128), (unsigned)(rows < 65535 ? rows : 65535),

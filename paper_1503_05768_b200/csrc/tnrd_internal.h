@@ -5,6 +5,7 @@
 
 #define TNRD_M 63          // RBF terms per influence function
 #define TNRD_MP 64         // padded to 64 (term 63 has weight 0)
+#define TNRD_TAB_NODES 4096  // nodes of a piecewise-linear phi table (tnrd_table.cu)
 
 namespace tnrd {
 
@@ -48,6 +49,8 @@ struct StageArgs {
     float lambda_val;
     int B, H, W, N_k, ksize;
     int dense_is_fallback;  // set by the launcher: the dense kernel returns at once when the windowed one applies
+    const float* tab;       // piecewise-linear phi tables of this stage [N_k][TNRD_TAB_NODES] float2 (phi evaluator 2)
+    const float* tabhdr;    // their header (tnrd_table.cu), device
 };
 
 // Launch plan of the fused stage kernel (tnrd_fused.cu: plan_stage_fused).  Tiles partition the phi region
@@ -95,11 +98,15 @@ cudaError_t launch_prep(const float* filters, const float* rbf_w, const float* r
 cudaError_t launch_stage_ref(const StageArgs& a, float* vbuf, cudaStream_t st, unsigned long long* launches);
 size_t ref_scratch_floats(int B, int H, int W, int N_k, int ksize);
 FusedPlan plan_stage_fused(const StageArgs& a, int num_sms);
-// phi_mode: 0 dense, 1 windowed (with dense fallback).  part = scratch of plan.part_floats floats.
+// phi_mode: 0 dense, 1 windowed (with dense fallback), 2 piecewise-linear table (a.tab).  part = scratch of
+// plan.part_floats floats.
 cudaError_t launch_stage_fused(const StageArgs& a, const FusedPlan& plan, float* part, int phi_mode, cudaStream_t st,
                                unsigned long long* launches);
 cudaError_t launch_qcs_project(const float* y, const float* lo, const float* hi, float* u, int B, int H, int W,
                                cudaStream_t st, unsigned long long* launches);   // u may alias y
+// phi tables: [TN][TNRD_TAB_NODES] float2 + 4 header floats; basis 0 Gaussian, 1 triangular
+cudaError_t launch_build_table(const float* rbf_w, const float* rbf_mu, float gamma, int TN, int basis, float* tab,
+                               float* hdr, cudaStream_t st, unsigned long long* launches);
 cudaError_t fused_init();   // opt-in shared memory attributes; idempotent
 cudaError_t run_microbench(int which, double* rate, cudaStream_t st, unsigned long long* launches);
 

@@ -304,3 +304,75 @@ def test_filter_split_auto_plan_on_single_paper_image(tnrd):
     c = tnrd_gen.make_config(3)
     want = run_oracle(c, T=2)
     check(run_gpu(tnrd, c, T=2), want, "C3 auto plan")
+
+
+# --- piecewise-linear table evaluator: lookup table of the Gaussian phi and the triangular basis ------
+def run_gpu_mode(tnrd, c, phi_mode=0, basis=0, **kw):
+    tnrd.tnrd_set_phi_mode(phi_mode)
+    tnrd.tnrd_set_rbf_basis(basis)
+    try:
+        return run_gpu(tnrd, c, **kw)
+    finally:
+        tnrd.tnrd_set_phi_mode(0)
+        tnrd.tnrd_set_rbf_basis(0)
+
+
+@pytest.mark.parametrize("case", [SMALL[1], SMALL[3], SMALL[5], SMALL[7], SMALL[8]], ids=lambda c: f"s{c[0]}")
+def test_lut_phi_small_cases_within_tolerance(tnrd, case):
+    """TNRD_PHI_LUT approximates Main Eq. 6 (4096 nodes, linear interpolation): same tolerance against the SAME oracle."""
+    seed, B, H, W, T, n_k, K = case
+    c = tnrd_gen.make_small(seed, B, H, W, T, n_k, K)
+    check(run_gpu_mode(tnrd, c, phi_mode=2), run_oracle(c), f"lut {case}")
+
+
+def test_lut_phi_config3_and_distance_from_dense(tnrd):
+    c = tnrd_gen.make_config(3)
+    want = run_oracle(c)
+    lut = run_gpu_mode(tnrd, c, phi_mode=2)
+    mx, rms = check(lut, want, "lut C3")
+    d = np.max(np.abs(lut - run_gpu(tnrd, c)))
+    print(f"C3 lookup-table phi: max-abs {mx:.3e} rms {rms:.3e} vs oracle; {d:.3e} from the dense GPU result")
+    assert d <= 5e-3
+
+
+def run_oracle_triangle(c, T=None):
+    with oracle.basis(oracle.TRIANGLE):
+        return run_oracle(c, T)
+
+
+@pytest.mark.parametrize("case", [SMALL[0], SMALL[1], SMALL[3], SMALL[5], SMALL[7], SMALL[8], SMALL[11]],
+                         ids=lambda c: f"s{c[0]}")
+def test_triangular_basis_exact_table(tnrd, case):
+    """gamma = spacing of the centres: phi_t is the linear interpolant of the weights, 65-node table."""
+    seed, B, H, W, T, n_k, K = case
+    c = tnrd_gen.make_small(seed, B, H, W, T, n_k, K)
+    assert c["rbf_gamma"] == float(c["rbf_mu"][1] - c["rbf_mu"][0])
+    check(run_gpu_mode(tnrd, c, basis=1), run_oracle_triangle(c), f"triangle {case}")
+
+
+def test_triangular_basis_config3_and_other_gamma(tnrd):
+    c = tnrd_gen.make_config(3)
+    mx, rms = check(run_gpu_mode(tnrd, c, basis=1), run_oracle_triangle(c), "triangle C3")
+    print(f"C3 triangular basis: max-abs {mx:.3e} rms {rms:.3e}")
+    # gamma != spacing: tabulated on the fine grid (kinks between nodes: approximate, still inside the tolerance)
+    d = dict(tnrd_gen.make_small(61, 1, 60, 70, 2, 6, 5), rbf_gamma=7.0)
+    check(run_gpu_mode(tnrd, d, basis=1), run_oracle_triangle(d), "triangle gamma 7")
+    # the Gaussian default is restored afterwards
+    check(run_gpu(tnrd, d), run_oracle(d), "gaussian after triangle")
+
+
+def test_triangular_basis_unsupported_paths(tnrd):
+    c = tnrd_gen.make_small(62, 1, 20, 20, 1, 3, 3)
+    with pytest.raises(tnrd.TnrdError) as ei:
+        run_gpu_mode(tnrd, c, basis=1, kernel=1)
+    assert ei.value.status == tnrd.ERR_UNSUPPORTED
+    tnrd.tnrd_set_rbf_basis(1)
+    try:
+        f = dev(c["f"])
+        with pytest.raises(tnrd.TnrdError) as ei:
+            tnrd.tnrd_stage_backward(f, f, f, 1, 20, 20, 3, 3, dev(c["filters"][0]), dev(c["rbf_w"][0]), dev(c["rbf_mu"]),
+                                     10.0, 0.1, grad_w=torch.empty((3, 63), device="cuda"))
+        assert ei.value.status == tnrd.ERR_UNSUPPORTED
+    finally:
+        tnrd.tnrd_set_rbf_basis(0)
+        tnrd.tnrd_set_kernel(0)
