@@ -376,3 +376,19 @@ def test_triangular_basis_unsupported_paths(tnrd):
     finally:
         tnrd.tnrd_set_rbf_basis(0)
         tnrd.tnrd_set_kernel(0)
+
+
+# --- extreme aspect ratios: more than 65535 rows in the batch (the update kernel folds rows over grid.y and grid.z) -----
+def test_many_rows_tall_image_and_large_batch(tnrd):
+    tall = tnrd_gen.make_small(71, 1, 70000, 8, 1, 3, 3)
+    got = run_gpu(tnrd, tall)[0]
+    assert np.all(np.isfinite(got))
+    for y0 in (0, 33000, 65530, 70000 - 24):
+        want = oracle.diffuse_window(tall["f"][0], tall["u0"][0], tall["filters"], tall["rbf_w"], tall["rbf_mu"],
+                                     tall["rbf_gamma"], tall["lambda"], y0, 0, 24, 8)
+        check(got[y0:y0 + 24, :], want, f"tall image rows {y0}")
+    many = tnrd_gen.make_small(72, 1200, 60, 9, 1, 2, 5)           # 72000 rows in the batch
+    gotb = run_gpu(tnrd, many)
+    for b in (0, 1091, 1092, 1199):                                 # around row 65535 and the last image
+        one = dict(many, B=1, f=many["f"][b:b + 1], u0=many["u0"][b:b + 1])
+        check(gotb[b:b + 1], run_oracle(one), f"batch image {b}")
