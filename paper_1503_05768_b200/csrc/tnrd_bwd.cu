@@ -106,7 +106,7 @@ __device__ __forceinline__ float warp_reduce8(const float (&S)[8], int lane)
 __device__ __forceinline__ int tile_origin(int t, int n, int len, int R) { return (int)((long long)t * (len + 4 * R) / n) - 2 * R; }
 
 template <int KS, bool WANT_W, bool WANT_K>
-__global__ void __launch_bounds__(BCfg<KS>::NT, 1)
+__global__ void __launch_bounds__(BCfg<KS>::NT, 2)
 stage_bwd_kernel(BwdArgs a, int ntx, int nty)
 {
     using C = BCfg<KS>;
