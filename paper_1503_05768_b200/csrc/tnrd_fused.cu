@@ -51,7 +51,7 @@ struct Cfg {
     static constexpr int VH = RH + 2 * R;               // phi map rows
     static constexpr int VPLANE = VH * VS;              // one phi map
     static constexpr int SHIFT = 4 - R;                 // column shift of the transposed-filter window (see above)
-    static constexpr int CTA_FLOATS = (RW / 4) * (RH / 2) * 8;      // partial sums of one CTA (block-major)
+    static constexpr int CTA_FLOATS = RW * RH;          // partial sums of one CTA (row-major over the output area)
     static constexpr int TS = prm_ts(KS);               // floats per row of tap pairs
     static constexpr int PRM = prm_stride(KS);          // floats per staged record
     static constexpr int NB = ((RW / 4) * (RH / 2) + NT - 1) / NT;  // 4x2 work blocks per thread (max)
@@ -312,47 +312,61 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int ns
         }
     }
 
-    // ---- the partial sums of this CTA (its tile, its chunk of the filter bank) go to scratch, block-major: pixel
-    // (oy, ox) of the output area at  8 * ((oy >> 1) * nbxo + (ox >> 2)) + 4 * (oy & 1) + (ox & 3).  stage_update_kernel
-    // adds the partial sums of every CTA that reaches a pixel in fixed order and applies the reaction term (a5).
+    // ---- the partial sums of this CTA (its tile, its chunk of the filter bank) go to scratch, row-major over the
+    // output area: pixel (oy, ox) at oy * RW + ox.  stage_update_kernel adds the partial sums of every CTA that reaches a
+    // pixel in fixed order and applies the reaction term (a5).
     float* mine = part + ((size_t)blockIdx.x * nsplit + blockIdx.y) * C::CTA_FLOATS;
 #pragma unroll
     for (int n = 0; n < C::NB; ++n) {
         if (coff[n] < 0) continue;
-        float4* d = reinterpret_cast<float4*>(mine + ((size_t)n * NT + tid) * 8);
-        __stcg(d, make_float4(acc[n][0].y, acc[n][1].y, acc[n][2].y, acc[n][3].y));
-        __stcg(d + 1, make_float4(acc[n][0].x, acc[n][1].x, acc[n][2].x, acc[n][3].x));
+        const int oy = coff[n] / C::VS, ox = coff[n] - oy * C::VS;
+        float* d = mine + oy * RW + ox;
+        __stcg(reinterpret_cast<float4*>(d), make_float4(acc[n][0].y, acc[n][1].y, acc[n][2].y, acc[n][3].y));
+        __stcg(reinterpret_cast<float4*>(d + RW), make_float4(acc[n][0].x, acc[n][1].x, acc[n][2].x, acc[n][3].x));
     }
 }
 
 // a5: u_t = u - (s + lambda (u - f)), s = sum of the partial sums of the (at most 2 x 2) tiles whose output
 // area holds the pixel, times the nsplit chunks of the filter bank, added in a fixed order (deterministic).
-// grid (ceil(W / 128), rows of the batch over y and z), 128 threads: one pixel per thread.
+// grid (ceil(W / 512), rows of the batch over y and z), 128 threads, 4 consecutive pixels per thread: all loads of the
+// four pixels are issued before the first use (the kernel is bound by the latency of its scattered 4-byte reads).
 __global__ void __launch_bounds__(128)
 stage_update_kernel(StageArgs a, const float* __restrict__ part, int tw, int th, int ntx, int nty, int nsplit,
-                    int cta_floats, int R)
+                    int cta_floats, int rw, int R)
 {
     const long long row = (long long)blockIdx.z * 65535 + blockIdx.y;            // row of the whole batch
-    const int x = blockIdx.x * 128 + threadIdx.x;
-    if (x >= a.W || row >= (long long)a.B * a.H) return;
+    const int x0 = (blockIdx.x * 128 + threadIdx.x) * 4;
+    if (x0 >= a.W || row >= (long long)a.B * a.H) return;
     const int img = (int)(row / a.H), y = (int)(row - (long long)img * a.H);
-    const size_t idx = ((size_t)img * a.H + y) * a.W + x;
-    const float uu = __ldg(a.u_in + idx), ff = __ldg(a.f + idx);
-    const int xp = x + R, yp = y + R, Wz = a.W + 2 * R;                         // phi coordinates
-    const int txlo = x / tw, txhi = min(ntx - 1, (xp + R) / tw), tylo = y / th, tyhi = min(nty - 1, (yp + R) / th);
-    float s = 0.f;
+    const size_t idx0 = (size_t)row * a.W + x0;
+    const int yp = y + R;                                                        // phi coordinates
+    const int tylo = y / th, tyhi = min(nty - 1, (yp + R) / th);
+    float uu[4], ff[4], s[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const bool ok = x0 + q < a.W;
+        uu[q] = ok ? __ldg(a.u_in + idx0 + q) : 0.f;
+        ff[q] = ok ? __ldg(a.f + idx0 + q) : 0.f;
+        s[q] = 0.f;
+    }
     for (int ty = tylo; ty <= tyhi; ++ty) {
         const int oy = yp - (ty * th - R);
-        for (int tx = txlo; tx <= txhi; ++tx) {
-            const int X0 = tx * tw, twa = min(tw, Wz - X0), ox = xp - (X0 - 4);
-            const int nbxo = (twa + 4 + R + 3) >> 2;
-            const float* p = part + ((size_t)(img * nty + ty) * ntx + tx) * nsplit * cta_floats
-                           + 8 * ((oy >> 1) * nbxo + (ox >> 2)) + 4 * (oy & 1) + (ox & 3);
-            for (int q = 0; q < nsplit; ++q) s += __ldcg(p + (size_t)q * cta_floats);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int x = x0 + q, xp = x + R;
+            if (x >= a.W) continue;
+            const int txlo = x / tw, txhi = min(ntx - 1, (xp + R) / tw);
+            for (int tx = txlo; tx <= txhi; ++tx) {
+                const int ox = xp - (tx * tw - 4);
+                const float* p = part + ((size_t)(img * nty + ty) * ntx + tx) * nsplit * cta_floats + oy * rw + ox;
+                for (int c = 0; c < nsplit; ++c) s[q] += __ldcg(p + (size_t)c * cta_floats);
+            }
         }
     }
     const float lambda = a.lambda_ptr ? __ldg(a.lambda_ptr) : a.lambda_val;
-    a.u_out[idx] = uu - (s + lambda * (uu - ff));
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+        if (x0 + q < a.W) a.u_out[idx0 + q] = uu[q] - (s[q] + lambda * (uu[q] - ff[q]));
 }
 
 // ---- host side: tile plan and launch ------------------------------------------------------------------------------
@@ -525,9 +539,9 @@ cudaError_t launch_stage_fused(const StageArgs& a_in, const FusedPlan& pl, float
     }
     if (e != cudaSuccess) return e;
     const long long rows = (long long)a.B * a.H;
-    stage_update_kernel<<<dim3((unsigned)((a.W + 127) / 128), (unsigned)(rows < 65535 ? rows : 65535),
+    stage_update_kernel<<<dim3((unsigned)((a.W + 511) / 512), (unsigned)(rows < 65535 ? rows : 65535),
                                (unsigned)((rows + 65534) / 65535)), 128, 0, st>>>(
-        a, part, pl.tw, pl.th, pl.ntx, pl.nty, pl.nsplit, pl.cta_floats, (a.ksize - 1) / 2);
+        a, part, pl.tw, pl.th, pl.ntx, pl.nty, pl.nsplit, pl.cta_floats, pl.cfg == 1 ? 128 : 64, (a.ksize - 1) / 2);
     ++*launches;
     return cudaGetLastError();
 }
