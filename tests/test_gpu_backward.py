@@ -147,3 +147,26 @@ def test_diffuse_backward_matches_oracle(tnrd, case):
                                None)
     torch.cuda.synchronize()
     close(g_w2.cpu().numpy(), want["g_w"], "dl/dw from e_T")
+
+
+def _random_bwd_cases(n):
+    r = np.random.default_rng([150305768, 98])
+    out = []
+    for i in range(n):
+        K = int(r.choice([3, 5, 7, 9]))
+        out.append((200 + i, int(r.integers(1, 3)), int(r.integers(K - 1, 140)), int(r.integers(K - 1, 200)),
+                    int(r.integers(1, 7)), K))
+    return out
+
+
+@pytest.mark.parametrize("case", _random_bwd_cases(10), ids=lambda c: f"r{c[0]}-{c[1]}x{c[2]}x{c[3]}-k{c[5]}")
+def test_stage_backward_random_shapes(tnrd, case):
+    seed, B, H, W, n_k, K = case
+    c, e, _ = problem(seed, B, H, W, 1, n_k, K)
+    want = oracle.stage_backward(c["f"], c["u0"], e, c["filters"][0], c["rbf_w"][0], c["rbf_mu"], c["rbf_gamma"],
+                                 float(c["lambda"][0]))
+    got = gpu_stage_backward(tnrd, c, e)
+    close(got["g_u"], want["g_u"], f"{case} dl/du")
+    close(got["g_w"], want["g_w"], f"{case} dl/dw")
+    close(got["g_k"], want["g_k"], f"{case} dl/dk")
+    close(got["g_l"], np.array([want["g_lambda"]]), f"{case} dl/dlambda")

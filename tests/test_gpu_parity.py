@@ -392,3 +392,26 @@ def test_many_rows_tall_image_and_large_batch(tnrd):
     for b in (0, 1091, 1092, 1199):                                 # around row 65535 and the last image
         one = dict(many, B=1, f=many["f"][b:b + 1], u0=many["u0"][b:b + 1])
         check(gotb[b:b + 1], run_oracle(one), f"batch image {b}")
+
+
+# --- seeded random shapes, every evaluator: ragged tiles, images smaller than a tile, images of a few tiles ------------
+def _random_cases(n):
+    r = np.random.default_rng([150305768, 99])
+    out = []
+    for i in range(n):
+        K = int(r.choice([3, 5, 7, 9]))
+        lo = K - 1
+        H, W = int(r.integers(lo, 160)), int(r.integers(lo, 260))
+        out.append((100 + i, int(r.integers(1, 4)), H, W, int(r.integers(1, 4)), int(r.integers(1, 11)), K))
+    return out
+
+
+@pytest.mark.parametrize("case", _random_cases(18), ids=lambda c: f"r{c[0]}-{c[1]}x{c[2]}x{c[3]}-k{c[6]}")
+def test_random_shapes_all_evaluators(tnrd, case):
+    seed, B, H, W, T, n_k, K = case
+    c = tnrd_gen.make_small(seed, B, H, W, T, n_k, K)
+    want = run_oracle(c)
+    check(run_gpu(tnrd, c), want, f"dense {case}")
+    check(run_gpu_mode(tnrd, c, phi_mode=1), want, f"window {case}")
+    check(run_gpu_mode(tnrd, c, phi_mode=2), want, f"lut {case}")
+    check(run_gpu_mode(tnrd, c, basis=1), run_oracle_triangle(c), f"triangle {case}")
