@@ -44,8 +44,9 @@ __global__ void prep_params_kernel(const float* __restrict__ filters, const floa
             else if (h == 2) val = s * delta;
             else {
                 bool ok = delta > 0.0f && gamma <= delta * 1.000001f;
-                for (int j = 0; j < TNRD_M && ok; ++j)
-                    ok = fabsf(rbf_mu[j] - (mu0 + (float)j * delta)) <= 1e-4f * delta;
+#pragma unroll 9
+                for (int j = 0; j < TNRD_M; ++j)       // no early exit: the 63 loads are independent and overlap
+                    ok &= fabsf(__ldg(rbf_mu + j) - (mu0 + (float)j * delta)) <= 1e-4f * delta;
                 val = ok ? 1.0f : 0.0f;
             }
         }
