@@ -154,6 +154,9 @@ def main():
     ap.add_argument("--ref-seconds", type=float, default=10.0, help="CPU seconds per oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-window", action="store_true", help="skip the extra windowed-phi measurement")
+    ap.add_argument("--shard", default="images", choices=["images", "slab"],
+                    help="N > 1: 'images' = one image per GPU (weak scaling, default); 'slab' = ONE image split into row "
+                         "slabs with a 2rT overlap, no exchange (strong scaling; c4 only)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -192,6 +195,13 @@ def main():
     else:
         cfg = (tnrd_gen.make_config(4, size=args.size, T=args.T) if args.workload == "c4"
                else tnrd_gen.make_config(int(args.workload[1])))
+    own_rows = cfg["H"]
+    slab = args.shard == "slab" and world > 1 and args.workload == "c4" and not deblock and not backward
+    if slab:    # this rank's rows of the one image, with the 2 r T margin it needs (paper_1503_05768_b200/shard.py)
+        from paper_1503_05768_b200.shard import slab_bounds
+        lo, hi, s0, s1 = slab_bounds(cfg["H"], rank, world, cfg["T"], cfg["ksize"])
+        cfg = dict(cfg, H=s1 - s0, f=np.ascontiguousarray(cfg["f"][:, s0:s1]), u0=np.ascontiguousarray(cfg["u0"][:, s0:s1]))
+        own_rows = hi - lo
     B, H, W, T = cfg["B"], cfg["H"], cfg["W"], cfg["T"]
     N_K, KSIZE = cfg["N_k"], cfg["ksize"]
     EX2_PER_PX_STAGE, FMA_PER_PX_STAGE = N_K * M, 2 * N_K * KSIZE * KSIZE
@@ -238,7 +248,7 @@ def main():
         barrier()
     launches = tnrd.tnrd_launch_count()
     ms = max_over_ranks(e0.elapsed_time(e1), devs)
-    px_stages_all = sum_over_ranks(float(B) * H * W * T * args.steps, devs)
+    px_stages_all = sum_over_ranks(float(B) * own_rows * W * T * args.steps, devs)     # output pixels only
     value = px_stages_all / (ms * 1e-3) / 1e6
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region -------------
@@ -282,7 +292,7 @@ def main():
     e3.record(stream)
     barrier()
     ms_e2e = max_over_ranks(e2.elapsed_time(e3), devs)
-    e2e_value = sum_over_ranks(float(B) * H * W * T * e2e_steps, devs) / (ms_e2e * 1e-3) / 1e6
+    e2e_value = sum_over_ranks(float(B) * own_rows * W * T * e2e_steps, devs) / (ms_e2e * 1e-3) / 1e6
     h2d = hf.numel() * 4 * (3 if deblock else 2 if backward else 1) + (0 if deblock or backward else sum(int(a.nbytes) for a in hp))
     d2h = hout.numel() * 4 + (sum(x.numel() * 4 for x in hg) if backward else 0)
     same = bool(torch.equal(hout.to(devs), out))
@@ -342,7 +352,7 @@ def main():
     }
     line = {
         "metric": METRIC, "value": value, "unit": "Mpixel-stages/s", "n_gpus": world, "steps": args.steps,
-        "warmup": warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "warmup": warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if slab else "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": (f"JPEG deblocking TRD^4_7x7 {B}x{H}x{W} (PAPER.md:287), synthetic QCS" if deblock else
                                 f"joint-training step (T={T} forward stages + back-propagation, Supp. Eq. 21; dl/du0, dl/dk, "
@@ -350,7 +360,9 @@ def main():
                                 f"roofline fields count the forward exponentials only" if backward else
                                 f"C{args.workload[1]} {B}x{H}x{W} T={T} N_k={N_K} {KSIZE}x{KSIZE} M=63 "
                                 f"(BASELINE.json configs[{int(args.workload[1]) - 1}]), one such batch per GPU"),
-                   "global_batch": world * B, "parallelism": f"dp{world} (independent images, no collective)",
+                   "global_batch": B if slab else world * B,
+                   "parallelism": (f"{world} row slabs of one image, 2rT overlap, no collective" if slab else
+                                   f"dp{world} (independent images, no collective)"),
                    "l2": ("inputs larger than L2 (3 planes x %d MB)" % (B * H * W * 4 // 2 ** 20)) if 3 * B * H * W * 4 > 126e6
                    else "working set fits L2 (exploration workload)"},
         "roofline": roofline, "clocks": clocks.summary(),

@@ -36,3 +36,16 @@ def sum_over_ranks(value: float, device=None) -> float:
     t = torch.tensor([float(value)], dtype=torch.float64, device=device or "cpu")
     dist.all_reduce(t, op=dist.ReduceOp.SUM)
     return float(t.item())
+
+
+def slab_bounds(H: int, rank: int, world: int, T: int, ksize: int) -> tuple[int, int, int, int]:
+    """Row slab of ONE large image for `rank`: returns (lo, hi, src_lo, src_hi).
+
+    Rows [lo, hi) are the rank's share of the output; rows [src_lo, src_hi) of f and u0 are what it must process to get
+    them right.  Every stage reaches 2r rows (r = (ksize - 1) / 2: k_i * u, then kbar_i * phi), so u_T on [lo, hi)
+    depends on rows within 2 r T of it; the margin is cut off only at the true image border, where the
+    slab's own mirror extension IS the image's.  No exchange between ranks: a 2 r T overlap instead (every
+    operation is local)."""
+    lo, hi = shard_range(H, rank, world)
+    m = (ksize - 1) * T
+    return lo, hi, max(0, lo - m), min(H, hi + m)

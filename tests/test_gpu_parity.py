@@ -415,3 +415,21 @@ def test_random_shapes_all_evaluators(tnrd, case):
     check(run_gpu_mode(tnrd, c, phi_mode=1), want, f"window {case}")
     check(run_gpu_mode(tnrd, c, phi_mode=2), want, f"lut {case}")
     check(run_gpu_mode(tnrd, c, basis=1), run_oracle_triangle(c), f"triangle {case}")
+
+
+# --- one image as row slabs with a 2 r T overlap (multi-GPU strong-scaling mode of bench.py, run here on one GPU) ------
+def test_row_slabs_with_overlap_match_the_full_image(tnrd):
+    from paper_1503_05768_b200.shard import slab_bounds
+    c = tnrd_gen.make_config(4, size=1024, T=5)
+    full = run_gpu(tnrd, c)[0]
+    stitched = np.empty_like(full)
+    for rank in range(3):
+        lo, hi, s0, s1 = slab_bounds(1024, rank, 3, c["T"], c["ksize"])
+        part = run_gpu(tnrd, dict(c, H=s1 - s0, f=np.ascontiguousarray(c["f"][:, s0:s1]),
+                                  u0=np.ascontiguousarray(c["u0"][:, s0:s1])))[0]
+        stitched[lo:hi] = part[lo - s0:hi - s0]
+    assert np.max(np.abs(stitched - full)) <= 2e-4          # other tiles, other partial-sum boundaries: fp32 rounding
+    y0 = slab_bounds(1024, 1, 3, c["T"], c["ksize"])[0] - 12  # a window across the first slab seam against the oracle
+    want = oracle.diffuse_window(c["f"][0], c["u0"][0], c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"], c["lambda"],
+                                 y0, 500, 24, 24)
+    check(stitched[y0:y0 + 24, 500:524], want, "slab seam")
