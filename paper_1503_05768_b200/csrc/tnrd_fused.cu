@@ -328,22 +328,24 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int ns
 
 // a5: u_t = u - (s + lambda (u - f)), s = sum of the partial sums of the (at most 2 x 2) tiles whose output
 // area holds the pixel, times the nsplit chunks of the filter bank, added in a fixed order (deterministic).
-// grid (ceil(W / 512), rows of the batch over y and z), 128 threads, 4 consecutive pixels per thread: all loads of the
-// four pixels are issued before the first use (the kernel is bound by the latency of its scattered 4-byte reads).
+// grid (ceil(W / (128 PX)), rows of the batch over y and z), 128 threads, PX consecutive pixels per thread: the kernel is
+// bound by the latency of its 4-byte reads, so large images take PX = 4 (more loads in flight per thread) and small ones
+// PX = 1 (more threads).
+template <int PX>
 __global__ void __launch_bounds__(128)
 stage_update_kernel(StageArgs a, const float* __restrict__ part, int tw, int th, int ntx, int nty, int nsplit,
                     int cta_floats, int rw, int R)
 {
     const long long row = (long long)blockIdx.z * 65535 + blockIdx.y;            // row of the whole batch
-    const int x0 = (blockIdx.x * 128 + threadIdx.x) * 4;
+    const int x0 = (blockIdx.x * 128 + threadIdx.x) * PX;
     if (x0 >= a.W || row >= (long long)a.B * a.H) return;
     const int img = (int)(row / a.H), y = (int)(row - (long long)img * a.H);
     const size_t idx0 = (size_t)row * a.W + x0;
     const int yp = y + R;                                                        // phi coordinates
     const int tylo = y / th, tyhi = min(nty - 1, (yp + R) / th);
-    float uu[4], ff[4], s[4];
+    float uu[PX], ff[PX], s[PX];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
+    for (int q = 0; q < PX; ++q) {
         const bool ok = x0 + q < a.W;
         uu[q] = ok ? __ldg(a.u_in + idx0 + q) : 0.f;
         ff[q] = ok ? __ldg(a.f + idx0 + q) : 0.f;
@@ -352,20 +354,21 @@ stage_update_kernel(StageArgs a, const float* __restrict__ part, int tw, int th,
     for (int ty = tylo; ty <= tyhi; ++ty) {
         const int oy = yp - (ty * th - R);
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
+        for (int q = 0; q < PX; ++q) {
             const int x = x0 + q, xp = x + R;
             if (x >= a.W) continue;
             const int txlo = x / tw, txhi = min(ntx - 1, (xp + R) / tw);
             for (int tx = txlo; tx <= txhi; ++tx) {
                 const int ox = xp - (tx * tw - 4);
                 const float* p = part + ((size_t)(img * nty + ty) * ntx + tx) * nsplit * cta_floats + oy * rw + ox;
+#pragma unroll 4
                 for (int c = 0; c < nsplit; ++c) s[q] += __ldcg(p + (size_t)c * cta_floats);
             }
         }
     }
     const float lambda = a.lambda_ptr ? __ldg(a.lambda_ptr) : a.lambda_val;
 #pragma unroll
-    for (int q = 0; q < 4; ++q)
+    for (int q = 0; q < PX; ++q)
         if (x0 + q < a.W) a.u_out[idx0 + q] = uu[q] - (s[q] + lambda * (uu[q] - ff[q]));
 }
 
@@ -539,9 +542,14 @@ cudaError_t launch_stage_fused(const StageArgs& a_in, const FusedPlan& pl, float
     }
     if (e != cudaSuccess) return e;
     const long long rows = (long long)a.B * a.H;
-    stage_update_kernel<<<dim3((unsigned)((a.W + 511) / 512), (unsigned)(rows < 65535 ? rows : 65535),
-                               (unsigned)((rows + 65534) / 65535)), 128, 0, st>>>(
-        a, part, pl.tw, pl.th, pl.ntx, pl.nty, pl.nsplit, pl.cta_floats, pl.cfg == 1 ? 128 : 64, (a.ksize - 1) / 2);
+    const int rw = pl.cfg == 1 ? 128 : 64, R = (a.ksize - 1) / 2;
+    const dim3 gy((unsigned)(rows < 65535 ? rows : 65535), (unsigned)((rows + 65534) / 65535));
+    if (rows * a.W >= (1LL << 22))
+        stage_update_kernel<4><<<dim3((unsigned)((a.W + 511) / 512), gy.x, gy.y), 128, 0, st>>>(
+            a, part, pl.tw, pl.th, pl.ntx, pl.nty, pl.nsplit, pl.cta_floats, rw, R);
+    else
+        stage_update_kernel<1><<<dim3((unsigned)((a.W + 127) / 128), gy.x, gy.y), 128, 0, st>>>(
+            a, part, pl.tw, pl.th, pl.ntx, pl.nty, pl.nsplit, pl.cta_floats, rw, R);
     ++*launches;
     return cudaGetLastError();
 }
