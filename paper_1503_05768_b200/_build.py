@@ -59,7 +59,8 @@ def build(verbose: bool = False, force: bool = False) -> str:
             sys.stderr.write(log)
     if any(rc != 0 for _, rc, _ in results):
         raise RuntimeError("nvcc failed building libtnrd.so")
-    res = subprocess.run([nvcc, "-shared", "-o", OUT] + [o for o, _, _ in results], capture_output=True, text=True)
+    res = subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", OUT]
+                         + [o for o, _, _ in results], capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
     if res.returncode != 0:
