@@ -115,7 +115,8 @@ __device__ __forceinline__ void phi_win_step(unsigned wsec, const int (&wofs)[4]
 
 template <int KS, int RW, int RH, int NT, int MINB, int PHI>
 __global__ void __launch_bounds__(NT, MINB)
-stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int nsplit, float* __restrict__ part)
+stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_full, int nsplit,
+                   float* __restrict__ part)
 {
     using C = Cfg<KS, RW, RH, NT, MINB>;
     constexpr int R = C::R, TS = C::TS, KKP = prm_kkp(KS);
@@ -125,15 +126,19 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int ns
     float* ps = vs + 2 * C::VPLANE;                // [4][PRM]   staged records of filters i-1 .. i+2
 
     const int tid = threadIdx.x;
-    int t = blockIdx.x;                            // tile; blockIdx.y = this CTA's chunk of the filter bank
+    // CTAs 0 .. n_full-1 take a whole tile each; the tiles after that are split over nsplit CTAs, each with a contiguous
+    // chunk of the filter bank (small images: n_full = 0; large ones: only the tiles of the last, partly filled wave)
+    const int split_r = (int)blockIdx.x - n_full;
+    const int parts = split_r < 0 ? 1 : nsplit, chunk = split_r < 0 ? 0 : split_r % nsplit;
+    int t = split_r < 0 ? (int)blockIdx.x : n_full + split_r / nsplit;   // tile
     const int tx = t % ntx; t /= ntx;
     const int ty = t % nty; t /= nty;
     const int img = t;
     const int X0 = tx * tw_nom, Y0 = ty * th_nom;  // phi coordinates of the tile origin
     const int tw = min(tw_nom, a.W + 2 * R - X0), th = min(th_nom, a.H + 2 * R - Y0);   // ragged last tiles
     const float* __restrict__ u_img = a.u_in + (size_t)img * a.H * a.W;
-    const int f0 = (int)(blockIdx.y * a.N_k / nsplit);
-    const int N_k = (int)((blockIdx.y + 1) * a.N_k / nsplit) - f0;          // filters f0 .. f0 + N_k - 1
+    const int f0 = chunk * a.N_k / parts;
+    const int N_k = (chunk + 1) * a.N_k / parts - f0;                       // filters f0 .. f0 + N_k - 1
     // The windowed evaluator runs only if the staging kernel found the centres equidistant; when it is selected both
     // kernels are launched and the one that does not apply returns at once (no host synchronisation needed).
     float w_inv_delta = 0.f, w_mu0 = 0.f, w_delta = 0.f;
@@ -207,7 +212,7 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int ns
     // ---- filter loop ------------------------------------------------------------------------------------------
     for (int i = 0; i < N_k; ++i) {
         if (i + 2 < N_k) {                                    // stage record i+2 (read from iteration i+1 on)
-            const float* src = a.prm + (size_t)((int)(blockIdx.y * a.N_k / nsplit) + i + 2) * C::PRM;
+            const float* src = a.prm + (size_t)(f0 + i + 2) * C::PRM;
             float* dst = ps + ((i + 2) & 3) * C::PRM;
             for (int idx = tid; idx < C::PRM; idx += NT) dst[idx] = __ldg(src + idx);
         }
@@ -315,7 +320,7 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int ns
     // ---- the partial sums of this CTA (its tile, its chunk of the filter bank) go to scratch, row-major over the
     // output area: pixel (oy, ox) at oy * RW + ox.  stage_update_kernel adds the partial sums of every CTA that reaches a
     // pixel in fixed order and applies the reaction term (a5).
-    float* mine = part + ((size_t)blockIdx.x * nsplit + blockIdx.y) * C::CTA_FLOATS;
+    float* mine = part + (size_t)blockIdx.x * C::CTA_FLOATS;            // slot = CTA index
 #pragma unroll
     for (int n = 0; n < C::NB; ++n) {
         if (coff[n] < 0) continue;
@@ -333,7 +338,7 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int ns
 // PX = 1 (more threads).
 template <int PX>
 __global__ void __launch_bounds__(128)
-stage_update_kernel(StageArgs a, const float* __restrict__ part, int tw, int th, int ntx, int nty, int nsplit,
+stage_update_kernel(StageArgs a, const float* __restrict__ part, int tw, int th, int ntx, int nty, int n_full, int nsplit,
                     int cta_floats, int rw, int R)
 {
     const long long row = (long long)blockIdx.z * 65535 + blockIdx.y;            // row of the whole batch
@@ -360,9 +365,12 @@ stage_update_kernel(StageArgs a, const float* __restrict__ part, int tw, int th,
             const int txlo = x / tw, txhi = min(ntx - 1, (xp + R) / tw);
             for (int tx = txlo; tx <= txhi; ++tx) {
                 const int ox = xp - (tx * tw - 4);
-                const float* p = part + ((size_t)(img * nty + ty) * ntx + tx) * nsplit * cta_floats + oy * rw + ox;
+                const long long tile = ((long long)img * nty + ty) * ntx + tx;       // slots are in CTA order
+                const long long slot = tile < n_full ? tile : n_full + (tile - n_full) * nsplit;
+                const int cnt = tile < n_full ? 1 : nsplit;
+                const float* p = part + (size_t)slot * cta_floats + oy * rw + ox;
 #pragma unroll 4
-                for (int c = 0; c < nsplit; ++c) s[q] += __ldcg(p + (size_t)c * cta_floats);
+                for (int c = 0; c < cnt; ++c) s[q] += __ldcg(p + (size_t)c * cta_floats);
             }
         }
     }
@@ -375,6 +383,7 @@ stage_update_kernel(StageArgs a, const float* __restrict__ part, int tw, int th,
 // ---- host side: tile plan and launch ------------------------------------------------------------------------------
 struct Plan {
     int ntx, nty, tw, th, nsplit;
+    long long n_full; // tiles taken by one CTA each (the rest are split over nsplit CTAs)
     double cost;      // estimated time of the launch in (thread-rounds x filters) per SM (see plan_tiles)
     long long work;   // phi blocks of one CTA (critical path; tie-break)
 };
@@ -400,7 +409,7 @@ Plan plan_tiles(const StageArgs& a, int num_sms)
     using C = Cfg<KS, RW, RH, NT, MINB>;
     constexpr int R = (KS - 1) / 2;
     const int Wz = a.W + 2 * R, Hz = a.H + 2 * R;
-    Plan best{0, 0, 0, 0, 1, -1.0, 0};
+    Plan best{0, 0, 0, 0, 1, 0, -1.0, 0};
     const int ntx0 = (Wz + C::TWMAX - 1) / C::TWMAX, nty0 = (Hz + C::THMAX - 1) / C::THMAX;
     const int fx = env_int("TNRD_NTX"), fy = env_int("TNRD_NTY");       // tuning knobs: force the tile counts
     for (int dx = 0; dx < 3; ++dx)
@@ -436,7 +445,18 @@ Plan plan_tiles(const StageArgs& a, int num_sms)
                 const long long ctas = tiles * sp;
                 const double cost = (double)((ctas + num_sms - 1) / num_sms) * (per_filter * nf + 6.0);
                 if (best.cost < 0 || cost < best.cost || (cost == best.cost && bphi < best.work))
-                    best = Plan{ntx, nty, tw, th, sp, cost, bphi};
+                    best = Plan{ntx, nty, tw, th, sp, 0, cost, bphi};
+            }
+            // large images: whole waves of one CTA per tile, and the tiles of the last, partly filled wave split over
+            // sp CTAs each so that the tail costs a fraction of a wave (MINB = 1 only: one CTA per SM at a time)
+            if (MINB == 1 && smax == 1 && forced_split() <= 0 && tiles > num_sms && tiles % num_sms != 0) {
+                const long long full = tiles / num_sms * num_sms, rem = tiles - full;
+                for (int sp = 2; sp <= (a.N_k < 16 ? a.N_k : 16); ++sp) {
+                    const int nf = (a.N_k + sp - 1) / sp;
+                    const double tail = (double)((rem * sp + num_sms - 1) / num_sms) * (per_filter * nf + 6.0);
+                    const double cost = (double)(full / num_sms) * (per_filter * a.N_k + 6.0) + tail;
+                    if (cost < best.cost) best = Plan{ntx, nty, tw, th, sp, full, cost, bphi};
+                }
             }
         }
     return best;
@@ -453,10 +473,11 @@ cudaError_t launch_cfg(const StageArgs& a, const FusedPlan& pl, float* part, cud
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    const long long grid = (long long)pl.ntx * pl.nty * a.B;
-    if (grid > 0x7fffffffLL || pl.nsplit > 65535 || !part) return cudaErrorInvalidConfiguration;
-    stage_fused_kernel<KS, RW, RH, NT, MINB, PHI><<<dim3((unsigned)grid, (unsigned)pl.nsplit), NT, C::SMEM, st>>>(
-        a, pl.tw, pl.th, pl.ntx, pl.nty, pl.nsplit, part);
+    const long long tiles = (long long)pl.ntx * pl.nty * a.B;
+    const long long grid = pl.n_full + (tiles - pl.n_full) * pl.nsplit;
+    if (grid > 0x7fffffffLL || pl.n_full > tiles || !part) return cudaErrorInvalidConfiguration;
+    stage_fused_kernel<KS, RW, RH, NT, MINB, PHI><<<(unsigned)grid, NT, C::SMEM, st>>>(
+        a, pl.tw, pl.th, pl.ntx, pl.nty, (int)pl.n_full, pl.nsplit, part);
     return cudaGetLastError();
 }
 
@@ -477,10 +498,11 @@ FusedPlan plan_ks(const StageArgs& a, int num_sms)
     }
     const Plan& b = p[id - 1];
     if (env_int("TNRD_DEBUG_PLAN"))
-        fprintf(stderr, "tnrd plan: %dx%dx%d ks %d N_k %d -> cfg %d, %d x %d tiles of %d x %d, split %d, cost %.0f\n", a.B,
-                a.H, a.W, KS, a.N_k, id, b.ntx, b.nty, b.tw, b.th, b.nsplit, b.cost);
-    FusedPlan fp{id, b.ntx, b.nty, b.tw, b.th, b.nsplit, per_cta[id - 1], 0};
-    fp.part_floats = (size_t)b.ntx * b.nty * a.B * b.nsplit * per_cta[id - 1];
+        fprintf(stderr, "tnrd plan: %dx%dx%d ks %d N_k %d -> cfg %d, %d x %d tiles of %d x %d, %lld whole + split %d, cost %.0f\n",
+                a.B, a.H, a.W, KS, a.N_k, id, b.ntx, b.nty, b.tw, b.th, b.n_full, b.nsplit, b.cost);
+    FusedPlan fp{id, b.ntx, b.nty, b.tw, b.th, b.nsplit, b.n_full, per_cta[id - 1], 0};
+    const long long tiles = (long long)b.ntx * b.nty * a.B;
+    fp.part_floats = (size_t)(b.n_full + (tiles - b.n_full) * b.nsplit) * per_cta[id - 1];
     return fp;
 }
 
@@ -546,10 +568,10 @@ cudaError_t launch_stage_fused(const StageArgs& a_in, const FusedPlan& pl, float
     const dim3 gy((unsigned)(rows < 65535 ? rows : 65535), (unsigned)((rows + 65534) / 65535));
     if (rows * a.W >= (1LL << 22))
         stage_update_kernel<4><<<dim3((unsigned)((a.W + 511) / 512), gy.x, gy.y), 128, 0, st>>>(
-            a, part, pl.tw, pl.th, pl.ntx, pl.nty, pl.nsplit, pl.cta_floats, rw, R);
+            a, part, pl.tw, pl.th, pl.ntx, pl.nty, (int)pl.n_full, pl.nsplit, pl.cta_floats, rw, R);
     else
         stage_update_kernel<1><<<dim3((unsigned)((a.W + 127) / 128), gy.x, gy.y), 128, 0, st>>>(
-            a, part, pl.tw, pl.th, pl.ntx, pl.nty, pl.nsplit, pl.cta_floats, rw, R);
+            a, part, pl.tw, pl.th, pl.ntx, pl.nty, (int)pl.n_full, pl.nsplit, pl.cta_floats, rw, R);
     ++*launches;
     return cudaGetLastError();
 }

@@ -59,9 +59,10 @@ struct StageArgs {
 struct FusedPlan {
     int cfg;                 // kernel configuration 1..3 (output area / threads)
     int ntx, nty, tw, th;    // tiles per image and nominal tile size (the last tile of a row / column may be smaller)
-    int nsplit;              // CTAs per tile (each takes a contiguous chunk of the N_k filters)
+    int nsplit;              // CTAs per split tile (each takes a contiguous chunk of the N_k filters)
+    long long n_full;        // the first n_full tiles are taken by one CTA each, the others by nsplit CTAs
     int cta_floats;          // partial sums of one CTA
-    size_t part_floats;      // scratch needed: ntx * nty * B * nsplit * cta_floats
+    size_t part_floats;      // scratch needed: (n_full + (tiles - n_full) * nsplit) * cta_floats
 };
 
 // ---- backward pass of a stage (tnrd_bwd.cu) ----------------------------------------------------------------
