@@ -35,22 +35,23 @@ namespace {
 // Geometry of one CTA (all in "phi coordinates": index 0 = image coordinate -r; the phi region is (H+2r) x (W+2r)).
 // The CTA owns a tile of tw x th phi pixels at (X0, Y0) -- tiles PARTITION the phi region, nothing is computed twice --
 // and produces the partial transposed-filter sums of those pixels on the output area
-//   columns [X0 - 4, X0 + tw + r)  (only X0 - r .. are needed; starting 4 to the left keeps every vector access aligned)
+//   columns [X0 - r, X0 + tw + r)
 //   rows    [Y0 - r, Y0 + th + r),
-// at most RW x RH pixels, i.e. tw <= RW - 4 - r, th <= RH - 2r.  Shared memory:
+// at most RW x RH pixels, i.e. tw <= RW - 2r, th <= RH - 2r.  Shared memory:
 //   us   u tile, origin (Y0 - r, X0 - r) in phi coordinates = (Y0 - 2r, X0 - 2r) in image coordinates
 //   vs   two influence maps, origin (Y0 - 2r, X0 - 8): the tile's own values surrounded by a ring of zeros, so that
-//        the transposed filter can run over the whole output area (window row oy + a, column ox + b + 4 - r)
+//        the transposed filter can run over the whole output area (window row oy + a, column ox + b + 8 - 2r: the row
+//        is read from the 16-byte aligned column of the output block and the window starts SHIFT = 8 - 2r into it)
 template <int KS, int RW, int RH, int NT, int MINB = 1>
 struct Cfg {
     static constexpr int R = (KS - 1) / 2;
-    static constexpr int TWMAX = RW - 4 - R, THMAX = RH - 2 * R;   // largest tile
+    static constexpr int TWMAX = RW - 2 * R, THMAX = RH - 2 * R;   // largest tile
     static constexpr int US = RW + 8;                   // u tile row stride (floats)
     static constexpr int UH = RH + 2;                   // u tile rows (th + 2r + 1 window rows)
     static constexpr int VS = RW + 8;                   // phi map row stride
     static constexpr int VH = RH + 2 * R;               // phi map rows
     static constexpr int VPLANE = VH * VS;              // one phi map
-    static constexpr int SHIFT = 4 - R;                 // column shift of the transposed-filter window (see above)
+    static constexpr int SHIFT = 8 - 2 * R;             // column shift of the transposed-filter window (see above)
     static constexpr int CTA_FLOATS = RW * RH;          // partial sums of one CTA (row-major over the output area)
     static constexpr int TS = prm_ts(KS);               // floats per row of tap pairs
     static constexpr int PRM = prm_stride(KS);          // floats per staged record
@@ -156,7 +157,7 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_
 
     // ---- work decomposition: 4x2 pixel blocks, NB per thread ----------------------------------------------
     const int nbx = (tw + 3) >> 2, nby = (th + 1) >> 1;                         // phi blocks: the tile itself
-    const int nbxo = (tw + 4 + R + 3) >> 2, nbyo = (th + 2 * R + 1) >> 1;       // output blocks: tile + ring
+    const int nbxo = (tw + 2 * R + 3) >> 2, nbyo = (th + 2 * R + 1) >> 1;       // output blocks: tile + ring
     const int nrounds = (nbxo * nbyo + NT - 1) / NT; // rounds of blocks this tile needs (<= NB): the software pipeline
                                                      // wraps from the last USED round to block 0 of the next filter
 
@@ -364,7 +365,7 @@ stage_update_kernel(StageArgs a, const float* __restrict__ part, int tw, int th,
             if (x >= a.W) continue;
             const int txlo = x / tw, txhi = min(ntx - 1, (xp + R) / tw);
             for (int tx = txlo; tx <= txhi; ++tx) {
-                const int ox = xp - (tx * tw - 4);
+                const int ox = xp - (tx * tw - R);
                 const long long tile = ((long long)img * nty + ty) * ntx + tx;       // slots are in CTA order
                 const long long slot = tile < n_full ? tile : n_full + (tile - n_full) * nsplit;
                 const int cnt = tile < n_full ? 1 : nsplit;
@@ -420,7 +421,7 @@ Plan plan_tiles(const StageArgs& a, int num_sms)
             const int tw = (Wz + ntx - 1) / ntx, th = (Hz + nty - 1) / nty;
             if ((long long)(ntx - 1) * tw >= Wz || (long long)(nty - 1) * th >= Hz) continue;   // an empty last tile
             const long long bphi = (long long)((tw + 3) / 4) * ((th + 1) / 2);
-            const long long bout = (long long)((tw + 4 + R + 3) / 4) * ((th + 2 * R + 1) / 2);
+            const long long bout = (long long)((tw + 2 * R + 3) / 4) * ((th + 2 * R + 1) / 2);
             // time of one filter on one CTA in units of one warp-block on the XU pipe of an SM sub-partition (~2 us:
             // 8 px x 63 ex2 x 32 lanes at 4 lanes per clock): rounds of NT blocks, a round with w warps of phi work
             // takes k = ceil(w / 4) units when k >= 4 warps share a sub-partition; fewer warps feed the pipe worse (3.3, 2.5,
