@@ -433,3 +433,23 @@ def test_row_slabs_with_overlap_match_the_full_image(tnrd):
     want = oracle.diffuse_window(c["f"][0], c["u0"][0], c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"], c["lambda"],
                                  y0, 500, 24, 24)
     check(stitched[y0:y0 + 24, 500:524], want, "slab seam")
+
+
+# --- a large single image: 16384 x 16384 (2^28 pixels, 1 GiB per plane; the API limit is B*H*W < 2^31) --------------------
+def test_large_image_16384_sampled_windows(tnrd):
+    c = tnrd_gen.make_config(4, size=4096, T=5)
+    T, n = 2, 16384
+    f = np.tile(c["f"][0], (4, 4))
+    f += np.random.default_rng(5).standard_normal(f.shape, dtype=np.float32)      # break the periodicity
+    df = torch.from_numpy(f).cuda()
+    out = torch.empty_like(df)
+    tnrd.tnrd_diffuse(df, df, 1, n, n, T, c["N_k"], c["ksize"], dev(c["filters"][:T]), dev(c["rbf_w"][:T]), dev(c["rbf_mu"]),
+                      c["rbf_gamma"], dev(c["lambda"][:T]), out)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(out).all())
+    for (y0, x0) in [(0, 0), (n - 24, n - 24), (n // 2, n // 2), (n - 24, 0), (12345, n - 24), (n - 3000, 7777)]:
+        want = oracle.diffuse_window(f, f, c["filters"][:T], c["rbf_w"][:T], c["rbf_mu"], c["rbf_gamma"], c["lambda"][:T],
+                                     y0, x0, 24, 24)
+        check(out[y0:y0 + 24, x0:x0 + 24].cpu().numpy().astype(np.float64), want, f"16384^2 window {(y0, x0)}")
+    del df, out
+    torch.cuda.empty_cache()
