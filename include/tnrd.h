@@ -24,8 +24,9 @@
  *   - "device pointer": memory of the CURRENT CUDA device (cudaMalloc / torch allocator), 4-byte aligned.
  *     "host pointer": ordinary or pinned host memory.
  *   - Ownership: the caller owns every buffer and keeps device buffers alive until the work queued on
- *     `stream` has completed.  The library owns only an internal per-device scratch (one ping-pong plane of
- *     B*H*W floats plus a parameter staging block), grown on demand and released by tnrd_shutdown().
+ *     `stream` has completed.  The library owns only an internal per-(device, stream) scratch (the staged parameters
+ *     and the partial sums of the tile kernel, about 4.5 bytes per pixel), grown on demand and released by
+ *     tnrd_shutdown().
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device entry points
  *     are asynchronous on `stream` and never synchronise the device.
  *   - Every function returning int returns TNRD_OK (0) or a negative tnrd_status.  Nothing throws.
@@ -63,8 +64,8 @@ typedef enum {
  *   rbf_mu      device, [63]                     mu_j (any values; equidistant in the paper, :117)
  *   rbf_gamma   by value, > 0 and finite         shared width gamma (:117 "unified scaling", :553)
  *   lambda_t    by value                          reaction weight lambda^t
- *   u_out       device, [B][H][W]   u_t; must not be u_in or f (halo reads) -> TNRD_ERR_ALIAS on pointer
- *               equality; partial overlap is undefined behaviour.
+ *   u_out       device, [B][H][W]   u_t; may equal u_in (in place: every halo read is done before the first write);
+ *               must not be f -> TNRD_ERR_ALIAS on pointer equality; partial overlap is undefined behaviour.
  */
 int tnrd_stage(const float* f, const float* u_in, int B, int H, int W, int N_k, int ksize,
                const float* filters_t, const float* rbf_w_t, const float* rbf_mu, float rbf_gamma,
@@ -77,7 +78,7 @@ int tnrd_stage(const float* f, const float* u_in, int B, int H, int W, int N_k, 
  *   lambda      device, [T]  (device so that the call needs no host sync and can be graph-captured)
  *   out         device, [B][H][W]; receives u_T.  out may equal u0 (in place); out must not equal f.
  *   T = 0 copies u0 to out.
- * Stages ping-pong between `out` and the internal scratch so that the last stage writes `out`.
+ * Every stage writes `out`, from the second one on in place; no image-sized scratch is needed.
  */
 int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, int N_k, int ksize,
                  const float* filters, const float* rbf_w, const float* rbf_mu, float rbf_gamma,

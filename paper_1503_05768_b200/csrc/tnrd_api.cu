@@ -41,7 +41,7 @@ struct Scratch {
     int dev = -1;
     cudaStream_t st = nullptr;
     int num_sms = 0;
-    Buf prm, plane[2], refv;          // staged parameters, ping-pong planes, reference-path phi maps
+    Buf prm, refv;                    // staged parameters, reference-path phi maps
     Buf split;                        // partial transposed-filter sums of the fused kernel's CTAs
     Buf tab;                          // piecewise-linear phi tables [T][N_k][4096] float2 + 4 header floats
     Buf h_f, h_u, h_out, h_par;       // device staging of the host entry point
@@ -142,7 +142,7 @@ int tnrd_stage(const float* f, const float* u_in, int B, int H, int W, int N_k, 
     int rc = check_shape(B, H, W, N_k, ksize);
     if (rc != TNRD_OK) return rc;
     if ((rc = check_gamma(rbf_gamma)) != TNRD_OK) return rc;
-    if (u_out == u_in || u_out == f) return TNRD_ERR_ALIAS;
+    if (u_out == f) return TNRD_ERR_ALIAS;
     cudaStream_t st = (cudaStream_t)stream;
     Scratch* sc = nullptr;
     if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
@@ -173,23 +173,15 @@ int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, in
     if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
     const size_t rec = (size_t)N_k * tnrd::prm_stride(ksize);
     const int phi = effective_phi();
-    // Destinations d_1..d_T: alternate scratch / out so that d_T = out and no stage writes what it reads.
-    // In place (out == u0) with odd T the first stage may not write out: it goes to a second plane.
-    const bool inplace_odd = (out == u0) && (T & 1);
-    if (T > 1 && (rc = grow(sc->plane[0], n, st)) != TNRD_OK) return rc;
-    if (inplace_odd && (rc = grow(sc->plane[1], n, st)) != TNRD_OK) return rc;
     if ((rc = stage_params(sc, filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, phi, st)) != TNRD_OK) return rc;
+    // Every stage writes `out`, from the second one on in place: the tile kernel only READS u_{t-1} (all halo reads
+    // happen there) and stores partial sums in scratch; the update kernel that follows it on the stream is point-wise.
     const float* src = u0;
     for (int t = 1; t <= T; ++t) {
-        float* dst;
-        if (t == 1 && inplace_odd) dst = sc->plane[1].p;
-        else dst = ((T - t) & 1) ? sc->plane[0].p : out;
-        tnrd::StageArgs a{f, src, dst, sc->prm.p + (size_t)(t - 1) * rec, lambda + (t - 1), 0.0f, B, H, W, N_k, ksize};
+        tnrd::StageArgs a{f, src, out, sc->prm.p + (size_t)(t - 1) * rec, lambda + (t - 1), 0.0f, B, H, W, N_k, ksize};
         if ((rc = run_stage(sc, a, phi, t - 1, st)) != TNRD_OK) return rc;
-        src = dst;
+        src = out;
     }
-    if (src != out)  // T == 1 in place: the single stage went to the second plane
-        TNRD_CUDA(cudaMemcpyAsync(out, src, n * sizeof(float), cudaMemcpyDeviceToDevice, st));
     return TNRD_OK;
 }
 
@@ -268,24 +260,17 @@ int tnrd_deblock_diffuse(const float* u0, int B, int H, int W, int T, int N_k, i
     if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
     const size_t rec = (size_t)N_k * tnrd::prm_stride(ksize);
     const int phi = effective_phi();
-    const bool inplace_odd = (out == u0) && (T & 1);
-    if (T > 1 && (rc = grow(sc->plane[0], n, st)) != TNRD_OK) return rc;
-    if (inplace_odd && (rc = grow(sc->plane[1], n, st)) != TNRD_OK) return rc;
     if ((rc = stage_params(sc, filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, phi, st)) != TNRD_OK) return rc;
-    // Same ping-pong as tnrd_diffuse.  Per stage (Supp. Eq. 29): the fused kernel with lambda = 0 writes
-    // y = u - sum_i kbar_i * phi_i(k_i * u) to the destination plane (f is then irrelevant: u itself is passed),
-    // the projection kernel turns it into u_t = D^T eta(D y) in place.
+    // Per stage (Supp. Eq. 29): the stage kernels with lambda = 0 write y = u - sum_i kbar_i * phi_i(k_i * u) to `out`
+    // (f is then irrelevant: u itself is passed; in place from the second stage on, as in tnrd_diffuse), the projection
+    // kernel turns it into u_t = D^T eta(D y) in place.
     const float* src = u0;
     for (int t = 1; t <= T; ++t) {
-        float* dst;
-        if (t == 1 && inplace_odd) dst = sc->plane[1].p;
-        else dst = ((T - t) & 1) ? sc->plane[0].p : out;
-        tnrd::StageArgs a{src, src, dst, sc->prm.p + (size_t)(t - 1) * rec, nullptr, 0.0f, B, H, W, N_k, ksize};
+        tnrd::StageArgs a{src, src, out, sc->prm.p + (size_t)(t - 1) * rec, nullptr, 0.0f, B, H, W, N_k, ksize};
         if ((rc = run_stage(sc, a, phi, t - 1, st)) != TNRD_OK) return rc;
-        TNRD_CUDA(tnrd::launch_qcs_project(dst, qcs_lo, qcs_hi, dst, B, H, W, st, &g_launches));
-        src = dst;
+        TNRD_CUDA(tnrd::launch_qcs_project(out, qcs_lo, qcs_hi, out, B, H, W, st, &g_launches));
+        src = out;
     }
-    if (src != out) TNRD_CUDA(cudaMemcpyAsync(out, src, n * sizeof(float), cudaMemcpyDeviceToDevice, st));
     return TNRD_OK;
 }
 
@@ -451,7 +436,7 @@ void tnrd_shutdown(void)
     (void)cudaGetDevice(&cur);
     for (Scratch* s : g_scratch) {
         (void)cudaSetDevice(s->dev);
-        Buf* bufs[] = {&s->prm, &s->plane[0], &s->plane[1], &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->refv, &s->split, &s->tab, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
+        Buf* bufs[] = {&s->prm, &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->refv, &s->split, &s->tab, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
         for (Buf* b : bufs)
             if (b->p) (void)cudaFree(b->p);   // synchronising free: the stream may be gone by now
         delete s;

@@ -189,6 +189,13 @@ def test_diffuse_equals_repeated_stage_and_inplace(tnrd, kernel):
         assert np.array_equal(u.cpu().numpy().astype(np.float64), ref), f"T={T}: diffuse != T x stage"
         u0 = dev(c["u0"])                                   # in place: out == u0
         assert np.array_equal(run_gpu(tnrd, c, kernel=kernel, out=u0, u0=u0), ref), f"T={T}: in-place differs"
+        tnrd.tnrd_set_kernel(kernel)                        # tnrd_stage in place: u_out == u_in
+        v = dev(c["u0"])
+        for t in range(T):
+            tnrd.tnrd_stage(f, v, 2, 33, 47, 5, 5, k[t], w[t], mu, c["rbf_gamma"], float(c["lambda"][t]), v)
+        torch.cuda.synchronize()
+        tnrd.tnrd_set_kernel(0)
+        assert np.array_equal(v.cpu().numpy().astype(np.float64), ref), f"T={T}: in-place stage differs"
 
 
 def test_host_entry_point_and_determinism(tnrd):
