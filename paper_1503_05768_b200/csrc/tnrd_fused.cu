@@ -260,7 +260,7 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_
                 }
                 wsec = (unsigned)__cvta_generic_to_shared(rec + prm_wplain(KS));
             }
-#pragma unroll 1
+#pragma unroll (PHI == 0 ? 1 : 2)
             for (int g = 0; g < C::NG - 1; ++g) {
                 if (hasB) {
                     if (PHI == 1) phi_win_step(wsec + 8 * g, wofs, w_delta, dd, v);
