@@ -1,18 +1,21 @@
-// tnrd_fused.cu -- the fused per-stage kernel (rows a1-a5 of the hot path in ONE pass; kernel variant 2).
+// tnrd_fused.cu -- the fused stage kernel (rows a1-a4 of the hot path in one pass) and the update kernel (a5).
 //
 //   u_t = u - ( sum_i kbar_i * phi_i(k_i * u~) + lambda (u - f) )          Main Eq. 7
 //
-// One CTA owns one output tile of tw x th pixels of one image:
-//   a1  the u tile with its 2r halo is gathered through the mirror index map into shared
+// stage_fused_kernel: one CTA owns one tile of tw x th pixels of the phi region (the image plus its r ring) of one
+// image; tiles PARTITION that region, so no influence value is computed twice:
+//   a1  the u tile with its r halo is gathered through the mirror index map into shared
 //       memory -- the padded image is never materialised;
 //   then, one filter i at a time (streamed, so that only two influence maps live on chip):
-//   a2  z' = k'_i * u~ on the (tw+2r) x (th+2r) "phi region", in registers, 4x2 pixels per unit of work,
-//   a3  v = sum_j w'_ij 2^{-(z' - mu'_j)^2}, all 63 terms, one MUFU.EX2 each (ex2.approx.ftz), in registers,
-//       written once to a double-buffered shared-memory map,
-//   a4  the rot180 taps of filter i-1 are applied to the map finished in the previous iteration and summed into
-//       per-thread output accumulators that live across the whole filter loop,
-//   a5  epilogue: u_t = u - (s + lambda (u - f)) straight from the shared u tile to global memory.
-// One __syncthreads() per filter.  HBM traffic is the algorithmic 12 B per pixel-stage plus the halo re-read.
+//   a2  z' = k'_i * u~ on the tile, in registers, 4x2 pixels per unit of work,
+//   a3  v = phi_i(z'): all 63 Gaussians, one MUFU.EX2 each (ex2.approx.ftz) -- or the windowed / table evaluator --
+//       in registers, written once to a double-buffered shared-memory map whose ring outside the tile is zero,
+//   a4  the rot180 taps of filter i-1 are applied to the map finished in the previous iteration, over the tile AND its
+//       r ring (the pixels this tile's values reach), and summed into per-thread accumulators that live across the
+//       whole filter loop; at the end the CTA stores these partial sums (64 KB).
+// One __syncthreads() per filter.  stage_update_kernel (a5): u_t = u - (sum of the partial sums of the <= 2 x 2 tiles
+// -- times the chunks of a split filter bank -- that reach the pixel + lambda (u - f)), point-wise, fixed order.
+// HBM traffic: 4 B read + ~4.5 B written per pixel-stage by the tile kernel, ~16.5 B by the update kernel.
 //
 // The path is bound by the XU (MUFU) pipe: 3024 ex2 per pixel-stage for the 48 x 7x7 model against 4704 FFMA of
 // filtering; tensor cores are not used.  Two things keep the XU pipe fed
