@@ -460,3 +460,23 @@ def test_large_image_16384_sampled_windows(tnrd):
         check(out[y0:y0 + 24, x0:x0 + 24].cpu().numpy().astype(np.float64), want, f"16384^2 window {(y0, x0)}")
     del df, out
     torch.cuda.empty_cache()
+
+
+# --- run-to-run determinism at a size with many tiles, a split wave tail and every evaluator (no float atomics anywhere;
+# compute-sanitizer is not available on this pool, so a shared-memory race would have to show up here) -----------------
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_bitwise_determinism_2048(tnrd, mode):
+    c = tnrd_gen.make_config(4, size=2048, T=5)
+    f = dev(c["f"])
+    k, w, mu, lam = dev(c["filters"]), dev(c["rbf_w"]), dev(c["rbf_mu"]), dev(c["lambda"])
+    outs = []
+    tnrd.tnrd_set_phi_mode(mode)
+    try:
+        for _ in range(4):
+            out = torch.empty_like(f)
+            tnrd.tnrd_diffuse(f, f, 1, 2048, 2048, 5, c["N_k"], c["ksize"], k, w, mu, c["rbf_gamma"], lam, out)
+            outs.append(out)
+        torch.cuda.synchronize()
+    finally:
+        tnrd.tnrd_set_phi_mode(0)
+    assert all(torch.equal(outs[0], o) for o in outs[1:])
