@@ -168,7 +168,7 @@ int tnrd_set_kernel(int which);
  * Influence-function evaluator of the fused kernel.  Process-wide.
  *   TNRD_PHI_DENSE  (0, default): every one of the 63 Gaussians of Main Eq. 6 is evaluated (one ex2 per term).
  *   TNRD_PHI_WINDOW (1): when rbf_mu is equidistant (|mu_j - mu_0 - j delta| <= 1e-4 delta, checked on the device by the
- *       staging kernel) and rbf_gamma <= delta, each response evaluates only the 16 consecutive centres around it that
+ *       staging kernel) and rbf_gamma <= delta, each response evaluates only the 14 consecutive centres around it that
  *       contain every centre within 6.5 gamma; the dropped terms are each below e^{-21.1} = 6.7e-10 of their weight, i.e.
  *       below fp32 rounding of the sum ("equidistant centers").  When the check
  *       fails the dense evaluator runs instead -- decided on the device, two launches per stage, no host synchronisation.

@@ -84,14 +84,14 @@ __device__ __forceinline__ void phi_step(const float* __restrict__ mw, const flo
 // ---- windowed phi evaluator (PHI = 1) -------------------------------------------------------------------------------
 // With equidistant centres (spacing delta' in scaled units) and gamma <= delta, every centre farther than 6.5 gamma from
 // a response z contributes less than e^{-21.1} = 6.7e-10 of its weight -- below fp32 rounding of the sum.  Each response
-// therefore evaluates only the 16 consecutive centres j0 .. j0+15 (j0 a multiple of 4) that contain [jc-6, jc+6], jc =
-// nearest centre: 16 MUFU.EX2 instead of 63, weights gathered per lane from the plain w' row of the staged record.
+// therefore evaluates only the 14 consecutive centres j0 .. j0+13 (j0 even) that contain [jc-6, jc+6], jc = nearest
+// centre: 14 MUFU.EX2 instead of 63, weights gathered per lane (8-byte loads) from the plain w' row of the staged record.
 // win_setup: per response the offset d = z' - mu'_{j0} and the byte offset of w'_{j0} inside the record.
 __device__ __forceinline__ void win_setup1(float z, float inv_delta, float mu0, float delta, float& d, int& wofs)
 {
     const float tq = (z - mu0) * inv_delta;
     int jc = __float2int_rn(fminf(fmaxf(tq, 0.0f), 62.0f));
-    int j0 = min(max(jc - 6, 0) & ~3, 48);
+    int j0 = min(max(jc - 6, 0) & ~1, 50);
     d = (z - mu0) - (float)j0 * delta;
     wofs = j0 * 4;
 }
@@ -279,11 +279,10 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_
                     if (hasC) rowstep<KS, true, C::SHIFT>(vw + g2 * C::VS, recp + g2 * TS, acc[n]);
                 }
             }
-            {   // last step: the remaining 63 - 56 = 7 terms (dense) / window centres 14, 15
+            {   // last step: the remaining 63 - 56 = 7 terms (dense); the window's 14 centres are done after 7 steps
                 constexpr int g = C::NG - 1;
                 if (hasB) {
-                    if (PHI == 1) phi_win_step(wsec + 8 * g, wofs, w_delta, dd, v);
-                    else if (PHI == 0) phi_step<TNRD_M - 8 * g>(rec + KKP + 16 * g, zc, v);
+                    if (PHI == 0) phi_step<TNRD_M - 8 * g>(rec + KKP + 16 * g, zc, v);
                 }
                 if (g <= KS) {
                     if (hasN) rowstep<KS, false>(uwn + g * C::US, tapsN + (KS - g) * TS, zn);

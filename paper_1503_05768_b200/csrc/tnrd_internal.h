@@ -19,7 +19,7 @@ namespace tnrd {
 //   pairs    at offset prm_kkp: 64 pairs (-mu'_j, w'_ij) = (-s * mu_j, w_ij / s), pair 63 = (0, 0)
 //   wplain   at offset prm_wplain: w'_ij, j = 0..63 (w'_i63 = 0), for the windowed phi evaluator's per-lane gathers
 //   hdr      at offset prm_hdr: (1/delta', mu'_0, delta', ok) -- centre spacing in scaled units and ok = 1.0f when the
-//            centres are equidistant (|mu_j - mu_0 - j delta| <= 1e-4 delta) and gamma <= delta (window of 16 centres
+//            centres are equidistant (|mu_j - mu_0 - j delta| <= 1e-4 delta) and gamma <= delta (window of 14 centres
 //            then holds every centre within 6.5 gamma of any z); the same four floats in every record
 // so that phi_i(k_i * u) = sum_j w_ij 2^{-(z' - mu'_j)^2} with z' = k'_i * u, and the transposed bank
 // sum_i kbar_i * v_i = sum_i kbar'_i * (v_i / s) re-uses the same scaled taps.

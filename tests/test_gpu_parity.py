@@ -272,7 +272,7 @@ def test_window_phi_falls_back_to_dense(tnrd):
         d = dict(c)
         if change == "jitter":                      # centres not equidistant
             mu = c["rbf_mu"].copy(); mu[10] += 2.0; d["rbf_mu"] = mu
-        else:                                       # gamma > delta: 16 centres no longer cover 6.5 gamma
+        else:                                       # gamma > delta: 14 centres no longer cover 6.5 gamma
             d["rbf_gamma"] = 14.0
         dense = run_gpu(tnrd, d)
         tnrd.tnrd_reset_launch_count()
