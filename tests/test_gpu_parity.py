@@ -480,3 +480,19 @@ def test_bitwise_determinism_2048(tnrd, mode):
     finally:
         tnrd.tnrd_set_phi_mode(0)
     assert all(torch.equal(outs[0], o) for o in outs[1:])
+
+
+# --- the opt-in evaluators at the size bench.py times (4096^2, T = 5): sampled windows against the oracle --------------
+@pytest.mark.parametrize("mode,basis", [(1, 0), (2, 0), (0, 1)], ids=["window", "lut", "triangle"])
+def test_evaluators_4096_sampled_windows(tnrd, mode, basis):
+    c = tnrd_gen.make_config(4, size=4096, T=5)
+    got = run_gpu_mode(tnrd, c, phi_mode=mode, basis=basis)[0]
+    assert np.all(np.isfinite(got))
+    worst = 0.0
+    for (y0, x0) in _windows(4096, 4096, 24, 2, 11)[::2] + [(121 * 17 - 12, 121 * 5 - 12)]:
+        with oracle.basis(oracle.TRIANGLE if basis else oracle.GAUSSIAN):
+            want = oracle.diffuse_window(c["f"][0], c["u0"][0], c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"],
+                                         c["lambda"], y0, x0, 24, 24)
+        mx, _ = check(got[y0:y0 + 24, x0:x0 + 24], want, f"4096^2 mode {mode} basis {basis} window {(y0, x0)}")
+        worst = max(worst, mx)
+    print(f"4096^2 phi mode {mode} basis {basis}: worst window max-abs {worst:.3e}")
