@@ -12,6 +12,19 @@ __device__ __forceinline__ float ex2_neg(float x)
     return y;
 }
 
+// asynchronous global -> shared copies (LDGSTS): no register staging, every copy of a loop is in flight at once
+__device__ __forceinline__ void cp_async4(float* smem_dst, const float* gmem_src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::
+                 "r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async16(float* smem_dst, const float* gmem_src)      // both 16-byte aligned
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::
+                 "r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 template <int N>
 __device__ __forceinline__ void lds_vec(const float* __restrict__ p, float (&d)[N])
 {

@@ -173,14 +173,14 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_
         for (int uy = tid >> 5; uy < nr; uy += NT / 32) {
             const float* __restrict__ grow = u_img + (size_t)mirror_clamp(Y0 - 2 * R + uy, a.H) * a.W;
 #pragma unroll
-            for (int q = 0; q < (C::US + 31) / 32; ++q) {          // all loads of a row issued before the first store
+            for (int q = 0; q < (C::US + 31) / 32; ++q) {          // asynchronous copies: every row of the tile is in flight at once
                 const int ux = (tid & 31) + 32 * q;
-                if (ux < nc) us[uy * C::US + ux] = __ldg(grow + mirror_clamp(X0 - 2 * R + ux, a.W));
+                if (ux < nc) cp_async4(us + uy * C::US + ux, grow + mirror_clamp(X0 - 2 * R + ux, a.W));
             }
         }
     }
-    for (int idx = tid; idx < 2 * C::PRM; idx += NT)
-        if (idx < N_k * C::PRM) ps[idx] = __ldg(a.prm + (size_t)f0 * C::PRM + idx);   // records 0 and 1
+    for (int idx = tid; idx < 2 * C::PRM / 4; idx += NT)                                // records 0 and 1
+        if (4 * idx < N_k * C::PRM) cp_async16(ps + 4 * idx, a.prm + (size_t)f0 * C::PRM + 4 * idx);
 
     int uoff[C::NB], voff[C::NB], coff[C::NB];   // block origins in us / a phi map (phi side) / a phi map (output side)
     unsigned own = 0;                            // bit 8 n + 4 j + p: pixel (row j, column p) of phi block n is in the tile
@@ -204,6 +204,7 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_
 #pragma unroll
         for (int p = 0; p < 4; ++p) acc[n][p] = make_float2(0.f, 0.f);
 
+    cp_async_wait_all();                           // the u tile and the first records have landed
     __syncthreads();
 
     // prologue: responses of filter 0 on this thread's first block
@@ -218,7 +219,7 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_
         if (i + 2 < N_k) {                                    // stage record i+2 (read from iteration i+1 on)
             const float* src = a.prm + (size_t)(f0 + i + 2) * C::PRM;
             float* dst = ps + ((i + 2) & 3) * C::PRM;
-            for (int idx = tid; idx < C::PRM; idx += NT) dst[idx] = __ldg(src + idx);
+            for (int idx = tid; idx < C::PRM / 4; idx += NT) cp_async16(dst + 4 * idx, src + 4 * idx);
         }
         const float* rec = ps + (i & 3) * C::PRM;             // filter i: phi pairs, a2 of blocks 1..NB-1
         const float* recn = ps + ((i + 1) & 3) * C::PRM;      // filter i+1: a2 of block 0
@@ -304,6 +305,7 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_
 #pragma unroll
             for (int p = 0; p < 4; ++p) zc[p] = zn[p];
         }
+        cp_async_wait_all();                                  // record i+2 has landed
         __syncthreads();
     }
 
