@@ -147,8 +147,9 @@ stage_bwd_kernel(BwdArgs a, int ntx, int nty)
                 const int ux = lane + 32 * q;
                 if (ux < nc) {
                     const int X = OX0 - 2 * R + ux;
-                    us[uy * C::US + ux] = __ldg(u_img + ro + mirror_clamp(X, a.W));
-                    es[uy * C::US + ux] = (yin && X >= 0 && X < a.W) ? __ldg(e_img + ro + X) : 0.0f;
+                    cp_async4(us + uy * C::US + ux, u_img + ro + mirror_clamp(X, a.W));     // asynchronous copies
+                    if (yin && X >= 0 && X < a.W) cp_async4(es + uy * C::US + ux, e_img + ro + X);
+                    else es[uy * C::US + ux] = 0.0f;
                 }
             }
         }
@@ -183,6 +184,7 @@ stage_bwd_kernel(BwdArgs a, int ntx, int nty)
 #pragma unroll
         for (int p = 0; p < 4; ++p) acc[n][p] = make_float2(0.f, 0.f);
 
+    cp_async_wait_all();
     __syncthreads();
 
     // prologue: z' and q' of filter 0 on this thread's first block
