@@ -197,6 +197,16 @@ int tnrd_set_phi_mode(int mode);
 #define TNRD_RBF_TRIANGLE 1
 int tnrd_set_rbf_basis(int basis);
 
+/*
+ * Launch plan the library would use for one stage of this shape on a device with `num_sms` multiprocessors (pure host
+ * logic, no device needed; for tests and tuning).  plan[0..9] = kernel configuration (1: 128 x 128 output area, 512 threads;
+ * 2: 64 x 32, 256 threads; 3: 64 x 64, 256 threads), tiles per image in x, in y, nominal tile width, height (pixels of
+ * the (H + 2r) x (W + 2r) phi region), number of leading tiles taken by one CTA each, CTAs per remaining tile (filter
+ * split), total CTAs, floats of partial sums per CTA, floats of scratch.  Honours the TNRD_TILE / TNRD_SPLIT / TNRD_NTX /
+ * TNRD_NTY environment knobs.
+ */
+int tnrd_plan_query(int B, int H, int W, int N_k, int ksize, int num_sms, long long* plan);
+
 /* Number of kernels this library has launched since load (or since the last tnrd_reset_launch_count). */
 unsigned long long tnrd_launch_count(void);
 void tnrd_reset_launch_count(void);

@@ -66,6 +66,8 @@ def lib() -> ctypes.CDLL:
         L.tnrd_set_phi_mode.restype = ci
         L.tnrd_set_rbf_basis.argtypes = [ci]
         L.tnrd_set_rbf_basis.restype = ci
+        L.tnrd_plan_query.argtypes = [ci, ci, ci, ci, ci, ci, ctypes.POINTER(ctypes.c_longlong)]
+        L.tnrd_plan_query.restype = ci
         L.tnrd_launch_count.restype = ctypes.c_ulonglong
         L.tnrd_reset_launch_count.restype = None
         L.tnrd_microbench.argtypes = [ci, ctypes.POINTER(ctypes.c_double), vp]
@@ -176,6 +178,14 @@ def tnrd_set_phi_mode(mode: int):
 def tnrd_set_rbf_basis(basis: int):
     """0 = Gaussian radial basis (default), 1 = triangular-shaped (include/tnrd.h: tnrd_set_rbf_basis)."""
     _check(lib().tnrd_set_rbf_basis(int(basis)))
+
+
+def tnrd_plan_query(B, H, W, N_k, ksize, num_sms=148) -> dict:
+    """Launch plan of one stage (include/tnrd.h: tnrd_plan_query); host logic only, works without a GPU."""
+    buf = (ctypes.c_longlong * 10)()
+    _check(lib().tnrd_plan_query(B, H, W, N_k, ksize, num_sms, buf))
+    keys = ("cfg", "ntx", "nty", "tw", "th", "n_full", "nsplit", "ctas", "cta_floats", "part_floats")
+    return dict(zip(keys, (int(v) for v in buf)))
 
 
 def tnrd_launch_count() -> int:

@@ -380,6 +380,21 @@ int tnrd_diffuse_backward(const float* f, const float* u0, const float* u_gt, co
     return TNRD_OK;
 }
 
+int tnrd_plan_query(int B, int H, int W, int N_k, int ksize, int num_sms, long long* plan)
+{
+    if (!plan) return TNRD_ERR_NULL;
+    int rc = check_shape(B, H, W, N_k, ksize);
+    if (rc != TNRD_OK) return rc;
+    if (num_sms < 1) return TNRD_ERR_SHAPE;
+    tnrd::StageArgs a{nullptr, nullptr, nullptr, nullptr, nullptr, 0.0f, B, H, W, N_k, ksize};
+    const tnrd::FusedPlan pl = tnrd::plan_stage_fused(a, num_sms);
+    const long long tiles = (long long)pl.ntx * pl.nty * B;
+    plan[0] = pl.cfg; plan[1] = pl.ntx; plan[2] = pl.nty; plan[3] = pl.tw; plan[4] = pl.th; plan[5] = pl.n_full;
+    plan[6] = pl.nsplit; plan[7] = pl.n_full + (tiles - pl.n_full) * pl.nsplit; plan[8] = pl.cta_floats;
+    plan[9] = (long long)pl.part_floats;
+    return TNRD_OK;
+}
+
 int tnrd_set_kernel(int which)
 {
     if (which < 0 || which > 2) return TNRD_ERR_UNSUPPORTED;
