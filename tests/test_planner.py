@@ -47,8 +47,8 @@ def test_plans_cover_every_shape(lib):
 
 
 def test_known_plans(lib):
-    p = tnrd.tnrd_plan_query(1, 4096, 4096, 48, 7)          # headline: 34 x 34 tiles, 7 whole waves + a split tail
-    assert (p["cfg"], p["ntx"], p["nty"], p["tw"], p["th"]) == (1, 34, 34, 121, 121)
+    p = tnrd.tnrd_plan_query(1, 4096, 4096, 48, 7)          # headline: 34 x 34 tiles (33 of the largest size 122 and a
+    assert (p["cfg"], p["ntx"], p["nty"], p["tw"], p["th"]) == (1, 34, 34, 122, 122)   # ragged one), 7 waves + a split tail
     assert p["n_full"] == 7 * 148 and p["nsplit"] > 1
     p = tnrd.tnrd_plan_query(128, 321, 481, 48, 7)          # C5: a 481-wide image needs 4 tile columns (487 <= 4 x 122)
     assert (p["ntx"], p["nty"]) == (4, 3)
