@@ -37,7 +37,7 @@ FMA_PER_PX_STAGE = 2 * N_K * KSIZE * KSIZE       # 4704 FFMA of filtering
 FLOP_PER_PX_STAGE = 2 * FMA_PER_PX_STAGE + 5 * EX2_PER_PX_STAGE   # per RBF term: sub, mul, ex2, fma(2) -> 24528
 NOMINAL_SM_MHZ, NOMINAL_SMS, MUFU_PER_CLK_SM = 1965.0, 148, 16
 # dram__bytes_read.sum + dram__bytes_write.sum per fused-stage launch at 4096^2 (profiles/r01_fused_stage_ncu.md)
-TRAFFIC_BYTES_PER_LAUNCH = {4096: 122.6e6}
+TRAFFIC_BYTES_PER_LAUNCH = {4096: 119.0e6}
 
 
 def read_peaks():
