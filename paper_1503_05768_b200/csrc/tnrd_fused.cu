@@ -417,21 +417,25 @@ Plan plan_tiles(const StageArgs& a, int num_sms)
     Plan best{0, 0, 0, 0, 1, 0, -1.0, 0};
     // time of one filter on one CTA with a tw x th tile, in units of one warp-block on the XU pipe of an SM sub-partition
     // (~2 us: 8 px x 63 ex2 x 32 lanes at 4 lanes per clock): rounds of NT blocks, a round with w warps of phi work takes
-    // k = ceil(w / 4) units when k >= 4 warps share a sub-partition; fewer warps feed the pipe worse (3.3, 2.5, 1.6 units
-    // for k = 3, 2, 1); plus ~2 units per filter that do not overlap (barrier, pipeline restart).  A CTA costs
-    // filters x this + ~6 units (tile gather, fill / drain, stores).
+    // k = ceil(w / 4) units when k >= 4 warps share a sub-partition; fewer warps feed the pipe worse (3.3, 2.1, 1.4 units
+    // for k = 3, 2, 1); plus 1.2 + 0.3 per round that do not overlap (barrier, pipeline restart).  A CTA costs
+    // filters x this + 4 to 10 units (tile gather, fill / drain, stores: cta_const).  Constants fitted on one-wave
+    // launches of 12 x 12 tiles of 44 .. 122 pixels (B200, 48 and 24 filters 7x7).
     auto per_filter = [&](int tw, int th) {
         const long long bphi = (long long)((tw + 3) / 4) * ((th + 1) / 2);
         const long long bout = (long long)((tw + 2 * R + 3) / 4) * ((th + 2 * R + 1) / 2);
-        double pf = 2.0;
+        double pf = 1.2;
         for (long long done = 0; done < bout; done += NT) {
             const long long inr = bphi - done < 0 ? 0 : (bphi - done > NT ? NT : bphi - done);
             const long long wr = (inr + 31) / 32;
             const int kw = (int)((wr + 3) / 4);                       // warps per SM sub-partition in this round
-            if (wr > 0) pf += kw >= 4 ? (double)kw : kw == 3 ? 3.3 : kw == 2 ? 2.5 : 1.6;
+            if (wr > 0) pf += 0.3 + (kw >= 4 ? (double)kw : kw == 3 ? 3.3 : kw == 2 ? 2.1 : 1.4);
             else pf += 0.3;                                            // transposed filter only
         }
         return pf;
+    };
+    auto cta_const = [&](int tw, int th) {
+        return 4.0 + (double)((tw + 2 * R + 3) / 4) * ((th + 2 * R + 1) / 2) / 350.0;
     };
     const int ntx0 = (Wz + C::TWMAX - 1) / C::TWMAX, nty0 = (Hz + C::THMAX - 1) / C::THMAX;
     const int fx = env_int("TNRD_NTX"), fy = env_int("TNRD_NTY");       // tuning knobs: force the tile counts
@@ -443,7 +447,7 @@ Plan plan_tiles(const StageArgs& a, int num_sms)
             const int tw = (Wz + ntx - 1) / ntx, th = (Hz + nty - 1) / nty;
             if ((long long)(ntx - 1) * tw >= Wz || (long long)(nty - 1) * th >= Hz) continue;   // an empty last tile
             const long long bphi = (long long)((tw + 3) / 4) * ((th + 1) / 2);
-            const double pf = per_filter(tw, th);
+            const double pf = per_filter(tw, th), cc = cta_const(tw, th);
             const long long tiles = (long long)ntx * nty * a.B;
             int smax = 1;
             if (tiles < (long long)num_sms * MINB) smax = a.N_k < 32 ? a.N_k : 32;
@@ -453,7 +457,7 @@ Plan plan_tiles(const StageArgs& a, int num_sms)
                 const int nf = (a.N_k + sp - 1) / sp;                      // filters of the largest chunk
                 if (sp > slo && (a.N_k + sp - 2) / (sp - 1) == nf) continue; // same chunk as sp - 1: only more CTAs
                 const long long ctas = tiles * sp;
-                const double cost = (double)((ctas + num_sms - 1) / num_sms) * (pf * nf + 6.0);
+                const double cost = (double)((ctas + num_sms - 1) / num_sms) * (pf * nf + cc);
                 if (best.cost < 0 || cost < best.cost || (cost == best.cost && bphi < best.work))
                     best = Plan{ntx, nty, tw, th, sp, 0, cost, bphi};
             }
@@ -462,16 +466,16 @@ Plan plan_tiles(const StageArgs& a, int num_sms)
             // sp CTAs each so that the tail costs a fraction of a wave (MINB = 1 only: one CTA per SM at a time)
             const long long full = tiles / num_sms * num_sms, rem = tiles - full;
             auto tail_of = [&](double pf_tile, int& sp_best) {
-                double t = rem ? pf_tile * a.N_k + 6.0 : 0.0;
+                double t = rem ? pf_tile * a.N_k + cc : 0.0;
                 sp_best = 1;
                 for (int sp = 2; rem && sp <= (a.N_k < 16 ? a.N_k : 16); ++sp) {
-                    const double c = (double)((rem * sp + num_sms - 1) / num_sms) * (pf_tile * ((a.N_k + sp - 1) / sp) + 6.0);
+                    const double c = (double)((rem * sp + num_sms - 1) / num_sms) * (pf_tile * ((a.N_k + sp - 1) / sp) + cc);
                     if (c < t) { t = c; sp_best = sp; }
                 }
                 return t;
             };
             int sp_eq = 1;
-            const double cost_eq = (double)(full / num_sms) * (pf * a.N_k + 6.0) + tail_of(pf, sp_eq);
+            const double cost_eq = (double)(full / num_sms) * (pf * a.N_k + cc) + tail_of(pf, sp_eq);
             if (sp_eq > 1 && cost_eq < best.cost) best = Plan{ntx, nty, tw, th, sp_eq, full, cost_eq, bphi};
             // many waves: tiles of the LARGEST size with a ragged last row / column do the same phi work per CTA on more
             // pixels (a 122 x 122 tile costs what a 121 x 121 one does); CTAs then differ in length, which only many
@@ -481,8 +485,10 @@ Plan plan_tiles(const StageArgs& a, int num_sms)
                 const int nx = (Wz + twm - 1) / twm, ny = (Hz + thm - 1) / thm;
                 if (nx == ntx && ny == nty && (twm != tw || thm != th)) {
                     const int twr = Wz - (nx - 1) * twm, thr = Hz - (ny - 1) * thm;
-                    const double c_ff = per_filter(twm, thm) * a.N_k + 6.0, c_rf = per_filter(twr, thm) * a.N_k + 6.0,
-                                 c_fr = per_filter(twm, thr) * a.N_k + 6.0, c_rr = per_filter(twr, thr) * a.N_k + 6.0;
+                    const double c_ff = per_filter(twm, thm) * a.N_k + cta_const(twm, thm),
+                                 c_rf = per_filter(twr, thm) * a.N_k + cta_const(twr, thm),
+                                 c_fr = per_filter(twm, thr) * a.N_k + cta_const(twm, thr),
+                                 c_rr = per_filter(twr, thr) * a.N_k + cta_const(twr, thr);
                     const double total = a.B * ((double)(nx - 1) * (ny - 1) * c_ff + (double)(ny - 1) * c_rf
                                                 + (double)(nx - 1) * c_fr + c_rr);
                     int sp_rg = 1;
