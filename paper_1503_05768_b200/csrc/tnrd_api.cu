@@ -404,7 +404,7 @@ int tnrd_set_kernel(int which)
 
 int tnrd_set_phi_mode(int mode)
 {
-    if (mode < 0 || mode > 2) return TNRD_ERR_UNSUPPORTED;
+    if (mode < 0 || mode > 3) return TNRD_ERR_UNSUPPORTED;
     g_phi_mode = mode;
     return TNRD_OK;
 }

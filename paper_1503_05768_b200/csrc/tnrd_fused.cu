@@ -117,6 +117,62 @@ __device__ __forceinline__ void phi_win_step(unsigned wsec, const int (&wofs)[4]
     }
 }
 
+// ---- factorised phi evaluator (PHI = 3) -----------------------------------------------------------------------------
+// All 63 Gaussians, but 3 ex2 per GROUP of 2S+1 = 13 neighbouring centres instead of one per centre (tnrd_internal.h,
+// "fact"): with d = z' - mu'_a (a = the group's middle centre), g = 2^{-d^2}, rho = 2^{kappa d},
+//   sum_{j=-S..S} w'_{a+j} 2^{-(d - j delta')^2} = g * ( sum_{j>=0} c_j rho^j + sum_{j<0} c_j rho^j ),
+// the two sums by Horner's rule in rho and 1/rho.  Per response and group: FADD, 2 FMNMX (clamp), 2 FMUL, 3 MUFU.EX2,
+// 2S + 1 FFMA -- 15 ex2 and 80 FMA-pipe operations per response where the direct form needs 63 and 189.
+// fact_pairs: pairs P0, P0+1 of the block (two packed responses each) for one group record.
+__device__ __forceinline__ float fclamp_nan(float x, float lim)          // NaN stays NaN (as in the direct evaluator)
+{
+    float y;
+    asm("min.NaN.f32 %0, %1, %2;" : "=f"(y) : "f"(x), "f"(lim));
+    asm("max.NaN.f32 %0, %0, %1;" : "+f"(y) : "f"(-lim));
+    return y;
+}
+__device__ __forceinline__ float ex2_pos(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+template <int P0>
+__device__ __forceinline__ void fact_pairs(const float* __restrict__ grec, float kappa, float dmax,
+                                           const float2 (&z)[4], float2 (&v)[4])
+{
+    constexpr int S = TNRD_FS;
+    float c[TNRD_FSTRIDE];
+    lds_vec(grec, c);
+    float2 g[2], rho[2], rhoi[2], h[2], hl[2];
+#pragma unroll
+    for (int p = 0; p < 2; ++p) {
+        float2 d = __fadd2_rn(z[P0 + p], make_float2(c[0], c[1]));
+        d = make_float2(fclamp_nan(d.x, dmax), fclamp_nan(d.y, dmax));
+        const float2 t = __fmul2_rn(d, d);
+        const float2 e = __fmul2_rn(d, make_float2(kappa, kappa));
+        g[p] = make_float2(ex2_neg(t.x), ex2_neg(t.y));
+        rho[p] = make_float2(ex2_pos(e.x), ex2_pos(e.y));
+        rhoi[p] = make_float2(ex2_neg(e.x), ex2_neg(e.y));
+        h[p] = make_float2(c[2], c[3]);                                      // c_S
+        hl[p] = make_float2(c[2 * (S + 2)], c[2 * (S + 2) + 1]);             // c_{-S}
+    }
+#pragma unroll
+    for (int q = 1; q <= S; ++q)                                             // c_{S-1} .. c_0
+#pragma unroll
+        for (int p = 0; p < 2; ++p) h[p] = __ffma2_rn(h[p], rho[p], make_float2(c[2 * (1 + q)], c[2 * (1 + q) + 1]));
+#pragma unroll
+    for (int q = 1; q < S; ++q)                                              // c_{-S+1} .. c_{-1}
+#pragma unroll
+        for (int p = 0; p < 2; ++p)
+            hl[p] = __ffma2_rn(hl[p], rhoi[p], make_float2(c[2 * (S + 2 + q)], c[2 * (S + 2 + q) + 1]));
+#pragma unroll
+    for (int p = 0; p < 2; ++p) {
+        h[p] = __ffma2_rn(hl[p], rhoi[p], h[p]);
+        v[P0 + p] = __ffma2_rn(g[p], h[p], v[P0 + p]);
+    }
+}
+
 template <int KS, int RW, int RH, int NT, int MINB, int PHI>
 __global__ void __launch_bounds__(NT, MINB)
 stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_full, int nsplit,
@@ -153,6 +209,15 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_
         w_delta = __ldg(a.prm + prm_hdr(KS) + 2);
     } else if (PHI == 0 && a.dense_is_fallback) {
         if (__ldg(a.prm + prm_hdr(KS) + 3) != 0.0f) return;
+    }
+    // factorised evaluator: applies when the staging kernel said so, else this kernel evaluates the direct form
+    constexpr bool DIRECT = PHI == 0 || PHI == 3;
+    float f_kappa = 0.f, f_dmax = 0.f;
+    bool fact = false;
+    if (PHI == 3) {
+        f_kappa = __ldg(a.prm + prm_hdr(KS) + 4);
+        f_dmax = __ldg(a.prm + prm_hdr(KS) + 5);
+        fact = __ldg(a.prm + prm_hdr(KS) + 6) != 0.0f;
     }
     // piecewise-linear table evaluator (PHI = 2; tnrd_table.cu): t = a z' + b in node units
     float t_a = 0.f, t_b = 0.f, t_max = 0.f;
@@ -264,11 +329,29 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_
                 }
                 wsec = (unsigned)__cvta_generic_to_shared(rec + prm_wplain(KS));
             }
-#pragma unroll (PHI == 0 ? 1 : 2)
+            if (PHI == 3 && fact) {
+                // TNRD_FG groups, two pairs of responses at a time; row-steps 2g and 2g+1 of both filterings ride along
+                static_assert(2 * TNRD_FG >= KS + 1, "not enough phi steps for the row-steps");
+#pragma unroll 1
+                for (int g = 0; g < TNRD_FG; ++g) {
+                    const float* grec = rec + prm_fact(KS) + g * TNRD_FSTRIDE;
+                    if (hasB) fact_pairs<0>(grec, f_kappa, f_dmax, zc, v);
+                    if (2 * g <= KS) {
+                        if (hasN) rowstep<KS, false>(uwn + (2 * g) * C::US, tapsN + (KS - 2 * g) * TS, zn);
+                        if (hasC) rowstep<KS, true, C::SHIFT>(vw + (2 * g) * C::VS, recp + (2 * g) * TS, acc[n]);
+                    }
+                    if (hasB) fact_pairs<2>(grec, f_kappa, f_dmax, zc, v);
+                    if (2 * g + 1 <= KS) {
+                        if (hasN) rowstep<KS, false>(uwn + (2 * g + 1) * C::US, tapsN + (KS - 2 * g - 1) * TS, zn);
+                        if (hasC) rowstep<KS, true, C::SHIFT>(vw + (2 * g + 1) * C::VS, recp + (2 * g + 1) * TS, acc[n]);
+                    }
+                }
+            } else {
+#pragma unroll (DIRECT ? 1 : 2)
             for (int g = 0; g < C::NG - 1; ++g) {
                 if (hasB) {
                     if (PHI == 1) phi_win_step(wsec + 8 * g, wofs, w_delta, dd, v);
-                    else if (PHI == 0) phi_step<8>(rec + KKP + 16 * g, zc, v);
+                    else if (DIRECT) phi_step<8>(rec + KKP + 16 * g, zc, v);
                 }
                 if (g <= KS) {
                     if (hasN) rowstep<KS, false>(uwn + g * C::US, tapsN + (KS - g) * TS, zn);
@@ -283,12 +366,13 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_
             {   // last step: the remaining 63 - 56 = 7 terms (dense); the window's 14 centres are done after 7 steps
                 constexpr int g = C::NG - 1;
                 if (hasB) {
-                    if (PHI == 0) phi_step<TNRD_M - 8 * g>(rec + KKP + 16 * g, zc, v);
+                    if (DIRECT) phi_step<TNRD_M - 8 * g>(rec + KKP + 16 * g, zc, v);
                 }
                 if (g <= KS) {
                     if (hasN) rowstep<KS, false>(uwn + g * C::US, tapsN + (KS - g) * TS, zn);
                     if (hasC) rowstep<KS, true, C::SHIFT>(vw + g * C::VS, recp + g * TS, acc[n]);
                 }
+            }
             }
             if (PHI == 2 && hasB) {
 #pragma unroll
@@ -589,7 +673,10 @@ cudaError_t launch_stage_fused(const StageArgs& a_in, const FusedPlan& pl, float
     StageArgs a = a_in;
     a.dense_is_fallback = (phi_mode == 1);
     cudaError_t e;
-    if (phi_mode == 2) {            // piecewise-linear table evaluator (always applicable)
+    if (phi_mode == 3) {            // factorised dense evaluator (the kernel falls back to the direct form by itself)
+        e = launch_phi<3>(a, pl, part, st);
+        ++*launches;
+    } else if (phi_mode == 2) {            // piecewise-linear table evaluator (always applicable)
         if (!a.tab || !a.tabhdr) return cudaErrorInvalidValue;
         e = launch_phi<2>(a, pl, part, st);
         ++*launches;

@@ -6,6 +6,11 @@
 #define TNRD_M 63          // RBF terms per influence function
 #define TNRD_MP 64         // padded to 64 (term 63 has weight 0)
 #define TNRD_TAB_NODES 4096  // nodes of a piecewise-linear phi table (tnrd_table.cu)
+#define TNRD_FS 6          // factorised phi evaluator: a group = one anchor centre and its TNRD_FS neighbours on each side
+#define TNRD_FM (2 * TNRD_FS + 1)                        // centres per group
+#define TNRD_FG ((TNRD_M + TNRD_FM - 1) / TNRD_FM)       // groups
+#define TNRD_FSTRIDE (((2 * (TNRD_FM + 1)) + 3) / 4 * 4) // floats per group record
+#define TNRD_FCLAMP 11.3f  // |d| clamp in scaled units: 2^{-d^2} is flushed to zero beyond sqrt(126) = 11.22
 
 namespace tnrd {
 
@@ -18,9 +23,20 @@ namespace tnrd {
 //            at window row wr uses row rho = wr.
 //   pairs    at offset prm_kkp: 64 pairs (-mu'_j, w'_ij) = (-s * mu_j, w_ij / s), pair 63 = (0, 0)
 //   wplain   at offset prm_wplain: w'_ij, j = 0..63 (w'_i63 = 0), for the windowed phi evaluator's per-lane gathers
-//   hdr      at offset prm_hdr: (1/delta', mu'_0, delta', ok) -- centre spacing in scaled units and ok = 1.0f when the
-//            centres are equidistant (|mu_j - mu_0 - j delta| <= 1e-4 delta) and gamma <= delta (window of 14 centres
-//            then holds every centre within 6.5 gamma of any z); the same four floats in every record
+//   hdr      at offset prm_hdr, 8 floats, the same in every record: (1/delta', mu'_0, delta', ok_w, kappa, D, ok_f, 0) --
+//            centre spacing in scaled units; ok_w = 1.0f when the centres are equidistant (|mu_j - mu_0 - j delta| <=
+//            1e-4 delta) and gamma <= delta (window of 14 centres then holds every centre within 6.5 gamma of any z);
+//            kappa = 2 delta', D and ok_f belong to the factorised evaluator (next item)
+//   fact     at offset prm_fact: TNRD_FG groups of TNRD_FSTRIDE floats for the factorised phi evaluator.  Group g has its
+//            anchor at centre a = g (2 S + 1) + S (S = TNRD_FS) and holds, every value twice (both halves of a packed
+//            operand):  -mu'_a,  c_S, c_{S-1}, .., c_0,  c_{-S}, c_{-S+1}, .., c_{-1}   with
+//            c_j = w'_{i,a+j} 2^{-(j delta')^2} (0 where a + j is not a centre).  With d = z' - mu'_a and equidistant
+//            centres,  2^{-(d - j delta')^2} = 2^{-d^2} (2^{kappa d})^j 2^{-(j delta')^2},  so the 2S+1 terms of a group
+//            are  2^{-d^2} * (polynomial in rho = 2^{kappa d} for j >= 0, in 1/rho for j < 0): 3 ex2 instead of 2S+1.
+//            d is clamped to [-D, D], D = 11.3: there 2^{-d^2} has flushed to zero, so the clamp changes nothing, and
+//            rho^S stays finite.  ok_f = 1.0f when the centres are equidistant, the dropped terms are negligible
+//            ((D - S delta')^2 >= 30, i.e. below 2^-30 of their weight) and max_j (j kappa D - (j delta')^2) <= 92
+//            (the polynomial cannot overflow for |w'| < 2^31); gamma = delta gives 38.4 and 89.2.
 // so that phi_i(k_i * u) = sum_j w_ij 2^{-(z' - mu'_j)^2} with z' = k'_i * u, and the transposed bank
 // sum_i kbar_i * v_i = sum_i kbar'_i * (v_i / s) re-uses the same scaled taps.
 __host__ __device__ constexpr int prm_ts(int ksize) { return ((2 * ksize + 3) / 4) * 4; }
@@ -28,7 +44,8 @@ __host__ __device__ constexpr int prm_tap(int ksize, int a, int b) { return (a +
 __host__ __device__ constexpr int prm_kkp(int ksize) { return (ksize + 1) * prm_ts(ksize); }
 __host__ __device__ constexpr int prm_wplain(int ksize) { return prm_kkp(ksize) + 2 * TNRD_MP; }
 __host__ __device__ constexpr int prm_hdr(int ksize) { return prm_wplain(ksize) + TNRD_MP; }
-__host__ __device__ constexpr int prm_stride(int ksize) { return prm_hdr(ksize) + 4; }
+__host__ __device__ constexpr int prm_fact(int ksize) { return prm_hdr(ksize) + 8; }
+__host__ __device__ constexpr int prm_stride(int ksize) { return prm_fact(ksize) + TNRD_FG * TNRD_FSTRIDE; }
 
 // Half-sample symmetric mirror map, edge pixel repeated, then clamped so that
 // coordinates beyond the 2r halo (ragged tiles) still address memory inside the image.
@@ -99,7 +116,8 @@ cudaError_t launch_prep(const float* filters, const float* rbf_w, const float* r
 cudaError_t launch_stage_ref(const StageArgs& a, float* vbuf, cudaStream_t st, unsigned long long* launches);
 size_t ref_scratch_floats(int B, int H, int W, int N_k, int ksize);
 FusedPlan plan_stage_fused(const StageArgs& a, int num_sms);
-// phi_mode: 0 dense, 1 windowed (with dense fallback), 2 piecewise-linear table (a.tab).  part = scratch of
+// phi_mode: 0 dense, direct (one ex2 per Gaussian), 1 windowed (with dense fallback), 2 piecewise-linear table (a.tab),
+// 3 dense, factorised (direct inside the same kernel when the staged flag says it does not apply).  part = scratch of
 // plan.part_floats floats.
 cudaError_t launch_stage_fused(const StageArgs& a, const FusedPlan& plan, float* part, int phi_mode, cudaStream_t st,
                                unsigned long long* launches);

@@ -35,19 +35,42 @@ __global__ void prep_params_kernel(const float* __restrict__ filters, const floa
         } else if (e < KKP + 3 * TNRD_MP) {
             const int j = e - KKP - 2 * TNRD_MP;
             if (j < TNRD_M) val = rbf_w[(size_t)rec * TNRD_M + j] / s;
-        } else {
-            // header: spacing of the centres in scaled units and the "windowed evaluator is valid" flag
+        } else if (e < prm_fact(ksize)) {
+            // header: spacing of the centres in scaled units and the "windowed / factorised evaluator is valid" flags
             const float mu0 = rbf_mu[0], delta = (rbf_mu[TNRD_M - 1] - mu0) / (float)(TNRD_M - 1);
-            const int h = e - KKP - 3 * TNRD_MP;
-            if (h == 0) val = 1.0f / (s * delta);
+            const float ds = s * delta;
+            const int h = e - prm_hdr(ksize);
+            if (h == 0) val = 1.0f / ds;
             else if (h == 1) val = s * mu0;
-            else if (h == 2) val = s * delta;
-            else {
-                bool ok = delta > 0.0f && gamma <= delta * 1.000001f;
+            else if (h == 2) val = ds;
+            else if (h == 4) val = 2.0f * ds;
+            else if (h == 5) val = TNRD_FCLAMP;
+            else if (h == 3 || h == 6) {
+                bool ok = delta > 0.0f;
 #pragma unroll 9
                 for (int j = 0; j < TNRD_M; ++j)       // no early exit: the 63 loads are independent and overlap
                     ok &= fabsf(__ldg(rbf_mu + j) - (mu0 + (float)j * delta)) <= 1e-4f * delta;
+                if (h == 3) ok &= gamma <= delta * 1.000001f;
+                else {
+                    const float reach = TNRD_FCLAMP - (float)TNRD_FS * ds;
+                    float emax = 0.0f;
+                    for (int j = 1; j <= TNRD_FS; ++j)
+                        emax = fmaxf(emax, (float)j * 2.0f * ds * TNRD_FCLAMP - (float)(j * j) * ds * ds);
+                    ok &= reach > 0.0f && reach * reach >= 30.0f && emax <= 92.0f;
+                }
                 val = ok ? 1.0f : 0.0f;
+            }
+        } else {
+            // factorised evaluator: group g, anchor a = g (2S+1) + S; (-mu'_a, c_S .. c_0, c_-S .. c_-1), each twice
+            const int q = e - prm_fact(ksize), g = q / TNRD_FSTRIDE, o = (q - g * TNRD_FSTRIDE) >> 1;
+            const int anchor = g * TNRD_FM + TNRD_FS;
+            const float mu0 = rbf_mu[0], delta = (rbf_mu[TNRD_M - 1] - mu0) / (float)(TNRD_M - 1);
+            const float ds = s * delta;
+            if (o == 0) val = -s * (mu0 + (float)anchor * delta);
+            else if (o <= TNRD_FM) {
+                const int j = o <= TNRD_FS + 1 ? TNRD_FS + 1 - o : o - 2 * TNRD_FS - 2;   // S .. 0, then -S .. -1
+                const int c = anchor + j;
+                if (c >= 0 && c < TNRD_M) val = rbf_w[(size_t)rec * TNRD_M + c] / s * exp2f(-(float)(j * j) * ds * ds);
             }
         }
         prm[idx] = val;
