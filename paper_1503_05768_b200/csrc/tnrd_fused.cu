@@ -138,34 +138,34 @@ __device__ __forceinline__ float ex2_pos(float x)
     return y;
 }
 template <int P0>
-__device__ __forceinline__ void fact_pairs(const float* __restrict__ grec, float kappa, float dmax,
+__device__ __forceinline__ void fact_pairs(const float (&c)[TNRD_FSTRIDE], float kappa, float dmax,
                                            const float2 (&z)[4], float2 (&v)[4])
 {
     constexpr int S = TNRD_FS;
-    float c[TNRD_FSTRIDE];
-    lds_vec(grec, c);
     float2 g[2], rho[2], rhoi[2], h[2], hl[2];
 #pragma unroll
     for (int p = 0; p < 2; ++p) {
-        float2 d = __fadd2_rn(z[P0 + p], make_float2(c[0], c[1]));
+        float2 d = __fadd2_rn(z[P0 + p], make_float2(c[0], c[0]));
         d = make_float2(fclamp_nan(d.x, dmax), fclamp_nan(d.y, dmax));
         const float2 t = __fmul2_rn(d, d);
         const float2 e = __fmul2_rn(d, make_float2(kappa, kappa));
         g[p] = make_float2(ex2_neg(t.x), ex2_neg(t.y));
         rho[p] = make_float2(ex2_pos(e.x), ex2_pos(e.y));
         rhoi[p] = make_float2(ex2_neg(e.x), ex2_neg(e.y));
-        h[p] = make_float2(c[2], c[3]);                                      // c_S
-        hl[p] = make_float2(c[2 * (S + 2)], c[2 * (S + 2) + 1]);             // c_{-S}
     }
 #pragma unroll
-    for (int q = 1; q <= S; ++q)                                             // c_{S-1} .. c_0
+    for (int p = 0; p < 2; ++p) {
+        h[p] = __ffma2_rn(make_float2(c[1], c[1]), rho[p], make_float2(c[2], c[2]));               // c_S rho + c_{S-1}
+        hl[p] = __ffma2_rn(make_float2(c[S + 2], c[S + 2]), rhoi[p], make_float2(c[S + 3], c[S + 3]));
+    }
 #pragma unroll
-        for (int p = 0; p < 2; ++p) h[p] = __ffma2_rn(h[p], rho[p], make_float2(c[2 * (1 + q)], c[2 * (1 + q) + 1]));
+    for (int q = 2; q <= S; ++q)                                             // c_{S-2} .. c_0
 #pragma unroll
-    for (int q = 1; q < S; ++q)                                              // c_{-S+1} .. c_{-1}
+        for (int p = 0; p < 2; ++p) h[p] = __ffma2_rn(h[p], rho[p], make_float2(c[1 + q], c[1 + q]));
 #pragma unroll
-        for (int p = 0; p < 2; ++p)
-            hl[p] = __ffma2_rn(hl[p], rhoi[p], make_float2(c[2 * (S + 2 + q)], c[2 * (S + 2 + q) + 1]));
+    for (int q = 2; q < S; ++q)                                              // c_{-S+2} .. c_{-1}
+#pragma unroll
+        for (int p = 0; p < 2; ++p) hl[p] = __ffma2_rn(hl[p], rhoi[p], make_float2(c[S + 2 + q], c[S + 2 + q]));
 #pragma unroll
     for (int p = 0; p < 2; ++p) {
         h[p] = __ffma2_rn(hl[p], rhoi[p], h[p]);
@@ -332,15 +332,17 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_
             if (PHI == 3 && fact) {
                 // TNRD_FG groups, two pairs of responses at a time; row-steps 2g and 2g+1 of both filterings ride along
                 static_assert(2 * TNRD_FG >= KS + 1, "not enough phi steps for the row-steps");
+                float fc[TNRD_FSTRIDE];
+                lds_vec(rec + prm_fact(KS), fc);
 #pragma unroll 1
                 for (int g = 0; g < TNRD_FG; ++g) {
-                    const float* grec = rec + prm_fact(KS) + g * TNRD_FSTRIDE;
-                    if (hasB) fact_pairs<0>(grec, f_kappa, f_dmax, zc, v);
+                    if (hasB) fact_pairs<0>(fc, f_kappa, f_dmax, zc, v);
                     if (2 * g <= KS) {
                         if (hasN) rowstep<KS, false>(uwn + (2 * g) * C::US, tapsN + (KS - 2 * g) * TS, zn);
                         if (hasC) rowstep<KS, true, C::SHIFT>(vw + (2 * g) * C::VS, recp + (2 * g) * TS, acc[n]);
                     }
-                    if (hasB) fact_pairs<2>(grec, f_kappa, f_dmax, zc, v);
+                    if (hasB) fact_pairs<2>(fc, f_kappa, f_dmax, zc, v);
+                    lds_vec(rec + prm_fact(KS) + (g + 1 < TNRD_FG ? g + 1 : g) * TNRD_FSTRIDE, fc);     // next group
                     if (2 * g + 1 <= KS) {
                         if (hasN) rowstep<KS, false>(uwn + (2 * g + 1) * C::US, tapsN + (KS - 2 * g - 1) * TS, zn);
                         if (hasC) rowstep<KS, true, C::SHIFT>(vw + (2 * g + 1) * C::VS, recp + (2 * g + 1) * TS, acc[n]);

@@ -9,7 +9,7 @@
 #define TNRD_FS 6          // factorised phi evaluator: a group = one anchor centre and its TNRD_FS neighbours on each side
 #define TNRD_FM (2 * TNRD_FS + 1)                        // centres per group
 #define TNRD_FG ((TNRD_M + TNRD_FM - 1) / TNRD_FM)       // groups
-#define TNRD_FSTRIDE (((2 * (TNRD_FM + 1)) + 3) / 4 * 4) // floats per group record
+#define TNRD_FSTRIDE ((TNRD_FM + 1 + 3) / 4 * 4)        // floats per group record
 #define TNRD_FCLAMP 11.3f  // |d| clamp in scaled units: 2^{-d^2} is flushed to zero beyond sqrt(126) = 11.22
 
 namespace tnrd {
@@ -28,8 +28,8 @@ namespace tnrd {
 //            1e-4 delta) and gamma <= delta (window of 14 centres then holds every centre within 6.5 gamma of any z);
 //            kappa = 2 delta', D and ok_f belong to the factorised evaluator (next item)
 //   fact     at offset prm_fact: TNRD_FG groups of TNRD_FSTRIDE floats for the factorised phi evaluator.  Group g has its
-//            anchor at centre a = g (2 S + 1) + S (S = TNRD_FS) and holds, every value twice (both halves of a packed
-//            operand):  -mu'_a,  c_S, c_{S-1}, .., c_0,  c_{-S}, c_{-S+1}, .., c_{-1}   with
+//            anchor at centre a = g (2 S + 1) + S (S = TNRD_FS) and holds
+//            -mu'_a,  c_S, c_{S-1}, .., c_0,  c_{-S}, c_{-S+1}, .., c_{-1}  (then zeros up to TNRD_FSTRIDE)  with
 //            c_j = w'_{i,a+j} 2^{-(j delta')^2} (0 where a + j is not a centre).  With d = z' - mu'_a and equidistant
 //            centres,  2^{-(d - j delta')^2} = 2^{-d^2} (2^{kappa d})^j 2^{-(j delta')^2},  so the 2S+1 terms of a group
 //            are  2^{-d^2} * (polynomial in rho = 2^{kappa d} for j >= 0, in 1/rho for j < 0): 3 ex2 instead of 2S+1.

@@ -61,8 +61,8 @@ __global__ void prep_params_kernel(const float* __restrict__ filters, const floa
                 val = ok ? 1.0f : 0.0f;
             }
         } else {
-            // factorised evaluator: group g, anchor a = g (2S+1) + S; (-mu'_a, c_S .. c_0, c_-S .. c_-1), each twice
-            const int q = e - prm_fact(ksize), g = q / TNRD_FSTRIDE, o = (q - g * TNRD_FSTRIDE) >> 1;
+            // factorised evaluator: group g, anchor a = g (2S+1) + S; (-mu'_a, c_S .. c_0, c_-S .. c_-1)
+            const int q = e - prm_fact(ksize), g = q / TNRD_FSTRIDE, o = q - g * TNRD_FSTRIDE;
             const int anchor = g * TNRD_FM + TNRD_FS;
             const float mu0 = rbf_mu[0], delta = (rbf_mu[TNRD_M - 1] - mu0) / (float)(TNRD_M - 1);
             const float ds = s * delta;
