@@ -166,7 +166,17 @@ int tnrd_set_kernel(int which);
 
 /*
  * Influence-function evaluator of the fused kernel.  Process-wide.
- *   TNRD_PHI_DENSE  (0, default): every one of the 63 Gaussians of Main Eq. 6 is evaluated (one ex2 per term).
+ *   TNRD_PHI_FACTORED (3, default): every one of the 63 Gaussians of Main Eq. 6 is evaluated, the exponentials of 13
+ *       neighbouring centres from three ex2: with equidistant centres (spacing delta) and d = z - mu_a,
+ *         exp(-(d - j delta)^2 / 2 gamma^2) = exp(-d^2 / 2 gamma^2) * rho^j * exp(-(j delta)^2 / 2 gamma^2),
+ *         rho = exp(delta d / gamma^2),
+ *       so a group of centres a-6 .. a+6 costs exp(-d^2/2gamma^2), rho, 1/rho and two polynomials (Horner's rule) whose
+ *       coefficients w_{a+j} exp(-(j delta)^2 / 2 gamma^2) are staged on the device at every call.  An identity, not an
+ *       approximation: the result differs from TNRD_PHI_DENSE by fp32 rounding only.  When
+ *       rbf_mu is not equidistant (same device-side check as TNRD_PHI_WINDOW) or rbf_gamma < 0.96 delta (the powers of
+ *       rho would leave the fp32 range) the same kernel evaluates the direct form -- decided on the device, one launch.
+ *       Weights with |w| * rbf_gamma beyond about 1e9 overflow in this form (the direct form holds up to ~1e38).
+ *   TNRD_PHI_DENSE  (0): the direct form, one ex2 per Gaussian.
  *   TNRD_PHI_WINDOW (1): when rbf_mu is equidistant (|mu_j - mu_0 - j delta| <= 1e-4 delta, checked on the device by the
  *       staging kernel) and rbf_gamma <= delta, each response evaluates only the 14 consecutive centres around it that
  *       contain every centre within 6.5 gamma; the dropped terms are each below e^{-21.1} = 6.7e-10 of their weight, i.e.
@@ -182,6 +192,7 @@ int tnrd_set_kernel(int which);
 #define TNRD_PHI_DENSE 0
 #define TNRD_PHI_WINDOW 1
 #define TNRD_PHI_LUT 2
+#define TNRD_PHI_FACTORED 3
 int tnrd_set_phi_mode(int mode);
 
 /*

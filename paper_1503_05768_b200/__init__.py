@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libtnrd.so")
 NUM_RBF = 63
 
 OK, ERR_NULL, ERR_SHAPE, ERR_UNSUPPORTED, ERR_ALIAS, ERR_CUDA, ERR_PARAM = 0, -1, -2, -3, -4, -5, -6
+PHI_DENSE, PHI_WINDOW, PHI_LUT, PHI_FACTORED = 0, 1, 2, 3          # tnrd_set_phi_mode (include/tnrd.h)
 
 _lib = None
 
@@ -170,8 +171,8 @@ def tnrd_set_kernel(which: int):
 
 
 def tnrd_set_phi_mode(mode: int):
-    """0 = dense 63-term phi (default), 1 = windowed evaluator, 2 = lookup table + linear interpolation
-    (include/tnrd.h: tnrd_set_phi_mode)."""
+    """3 = factorised 63-term phi (default), 0 = direct 63-term phi, 1 = windowed evaluator, 2 = lookup table + linear
+    interpolation (include/tnrd.h: tnrd_set_phi_mode)."""
     _check(lib().tnrd_set_phi_mode(int(mode)))
 
 

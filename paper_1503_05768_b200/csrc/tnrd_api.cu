@@ -15,7 +15,8 @@ namespace {
 thread_local char g_cuda_err[512] = "";
 unsigned long long g_launches = 0;
 int g_kernel = 0;  // 0 auto, 1 reference, 2 fused
-int g_phi_mode = 0;  // 0 dense 63-term phi, 1 windowed evaluator (dense fallback decided on the device), 2 table
+int g_phi_mode = 3;  // 0 direct 63-term phi, 1 windowed evaluator (dense fallback decided on the device), 2 table,
+                     // 3 factorised 63-term phi (direct fallback inside the kernel)
 int g_basis = 0;     // 0 Gaussian radial basis, 1 triangular-shaped (table evaluator)
 std::mutex g_mu;
 
@@ -352,8 +353,8 @@ int tnrd_diffuse_backward(const float* f, const float* u0, const float* u_gt, co
     for (int t = 1; t <= T; ++t) {
         float* dst = sc->bw_trace.p + (size_t)(t - 1) * n;
         tnrd::StageArgs a{f, src, dst, sc->prm.p + (size_t)(t - 1) * rec, lambda + (t - 1), 0.0f, B, H, W, N_k, ksize};
-        // the forward pass of a gradient is the exact evaluator (dense, or windowed if selected), never the table
-        if ((rc = run_stage(sc, a, g_phi_mode == 1 ? 1 : 0, t - 1, st)) != TNRD_OK) return rc;
+        // the forward pass of a gradient is an exact evaluator (factorised, direct, or windowed if selected), never the table
+        if ((rc = run_stage(sc, a, g_phi_mode == 2 ? 3 : g_phi_mode, t - 1, st)) != TNRD_OK) return rc;
         src = dst;
     }
     if (u_T) TNRD_CUDA(cudaMemcpyAsync(u_T, src, n * sizeof(float), cudaMemcpyDeviceToDevice, st));

@@ -137,40 +137,95 @@ __device__ __forceinline__ float ex2_pos(float x)
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+struct FactState { float2 g[2], rho[2], rhoi[2]; };   // of two pairs of responses: 2^{-d^2}, 2^{kappa d}, 2^{-kappa d}
+
+// first half of a group for pairs P0, P0+1: the clamped distances to the anchor and the three exponentials of each response
 template <int P0>
-__device__ __forceinline__ void fact_pairs(const float (&c)[TNRD_FSTRIDE], float kappa, float dmax,
-                                           const float2 (&z)[4], float2 (&v)[4])
+__device__ __forceinline__ void fact_exp(const float (&c)[TNRD_FSTRIDE], float kappa, float dmax, const float2 (&z)[4],
+                                         FactState& s)
 {
-    constexpr int S = TNRD_FS;
-    float2 g[2], rho[2], rhoi[2], h[2], hl[2];
 #pragma unroll
     for (int p = 0; p < 2; ++p) {
         float2 d = __fadd2_rn(z[P0 + p], make_float2(c[0], c[0]));
         d = make_float2(fclamp_nan(d.x, dmax), fclamp_nan(d.y, dmax));
         const float2 t = __fmul2_rn(d, d);
         const float2 e = __fmul2_rn(d, make_float2(kappa, kappa));
-        g[p] = make_float2(ex2_neg(t.x), ex2_neg(t.y));
-        rho[p] = make_float2(ex2_pos(e.x), ex2_pos(e.y));
-        rhoi[p] = make_float2(ex2_neg(e.x), ex2_neg(e.y));
+        s.g[p] = make_float2(ex2_neg(t.x), ex2_neg(t.y));
+        s.rho[p] = make_float2(ex2_pos(e.x), ex2_pos(e.y));
+        s.rhoi[p] = make_float2(ex2_neg(e.x), ex2_neg(e.y));
     }
+}
+// second half: the two Horner polynomials and the sum into v
+template <int P0>
+__device__ __forceinline__ void fact_poly(const float (&c)[TNRD_FSTRIDE], const FactState& s, float2 (&v)[4])
+{
+    constexpr int S = TNRD_FS;
+    float2 h[2], hl[2];
 #pragma unroll
     for (int p = 0; p < 2; ++p) {
-        h[p] = __ffma2_rn(make_float2(c[1], c[1]), rho[p], make_float2(c[2], c[2]));               // c_S rho + c_{S-1}
-        hl[p] = __ffma2_rn(make_float2(c[S + 2], c[S + 2]), rhoi[p], make_float2(c[S + 3], c[S + 3]));
+        h[p] = __ffma2_rn(make_float2(c[1], c[1]), s.rho[p], make_float2(c[2], c[2]));               // c_S rho + c_{S-1}
+        hl[p] = __ffma2_rn(make_float2(c[S + 2], c[S + 2]), s.rhoi[p], make_float2(c[S + 3], c[S + 3]));
     }
 #pragma unroll
     for (int q = 2; q <= S; ++q)                                             // c_{S-2} .. c_0
 #pragma unroll
-        for (int p = 0; p < 2; ++p) h[p] = __ffma2_rn(h[p], rho[p], make_float2(c[1 + q], c[1 + q]));
+        for (int p = 0; p < 2; ++p) h[p] = __ffma2_rn(h[p], s.rho[p], make_float2(c[1 + q], c[1 + q]));
 #pragma unroll
     for (int q = 2; q < S; ++q)                                              // c_{-S+2} .. c_{-1}
 #pragma unroll
-        for (int p = 0; p < 2; ++p) hl[p] = __ffma2_rn(hl[p], rhoi[p], make_float2(c[S + 2 + q], c[S + 2 + q]));
+        for (int p = 0; p < 2; ++p) hl[p] = __ffma2_rn(hl[p], s.rhoi[p], make_float2(c[S + 2 + q], c[S + 2 + q]));
 #pragma unroll
     for (int p = 0; p < 2; ++p) {
-        h[p] = __ffma2_rn(hl[p], rhoi[p], h[p]);
-        v[P0 + p] = __ffma2_rn(g[p], h[p], v[P0 + p]);
+        h[p] = __ffma2_rn(hl[p], s.rhoi[p], h[p]);
+        v[P0 + p] = __ffma2_rn(s.g[p], h[p], v[P0 + p]);
     }
+}
+
+// One block of the software pipeline with the factorised evaluator: phi of the block's 8 responses (TNRD_FG groups, two
+// pairs of responses at a time) with the KS + 1 window rows of both filterings riding along -- rows 1 .. KS-1 two per
+// group in the first (KS-1)/2 groups, the one-sided rows 0 and KS (rowstep_half) in the last group.  A window row of the
+// forward filter sits between the exponentials of a pair and their polynomials: its FMAs cover the MUFU latency.
+template <int KS, class C>
+__device__ __forceinline__ void fact_block(const float* __restrict__ frec, float kappa, float dmax, const float2 (&zc)[4],
+                                           float2 (&v)[4], const float* __restrict__ uwn, const float* __restrict__ tapsN,
+                                           float2 (&zn)[4], const float* __restrict__ vw, const float* __restrict__ recp,
+                                           float2 (&acc)[4], bool hasB, bool hasN, bool hasC)
+{
+    constexpr int TS = C::TS, NGR = (KS - 1) / 2;
+    static_assert(NGR <= TNRD_FG - 1, "not enough phi groups for the window rows");
+    float fc[TNRD_FSTRIDE];
+    FactState st;
+    lds_vec(frec, fc);
+#pragma unroll 1
+    for (int g = 0; g < NGR; ++g) {
+        if (hasB) fact_exp<0>(fc, kappa, dmax, zc, st);
+        if (hasN) rowstep<KS, false>(uwn + (2 * g + 1) * C::US, tapsN + (KS - 2 * g - 1) * TS, zn);
+        if (hasB) fact_poly<0>(fc, st, v);
+        if (hasC) rowstep<KS, true, C::SHIFT>(vw + (2 * g + 1) * C::VS, recp + (2 * g + 1) * TS, acc);
+        if (hasB) fact_exp<2>(fc, kappa, dmax, zc, st);
+        if (hasN) rowstep<KS, false>(uwn + (2 * g + 2) * C::US, tapsN + (KS - 2 * g - 2) * TS, zn);
+        if (hasB) fact_poly<2>(fc, st, v);
+        if (hasC) rowstep<KS, true, C::SHIFT>(vw + (2 * g + 2) * C::VS, recp + (2 * g + 2) * TS, acc);
+        lds_vec(frec + (g + 1) * TNRD_FSTRIDE, fc);
+    }
+#pragma unroll 1
+    for (int g = NGR; g < TNRD_FG - 1; ++g) {
+        if (hasB) {
+            fact_exp<0>(fc, kappa, dmax, zc, st);
+            fact_poly<0>(fc, st, v);
+            fact_exp<2>(fc, kappa, dmax, zc, st);
+            fact_poly<2>(fc, st, v);
+        }
+        lds_vec(frec + (g + 1) * TNRD_FSTRIDE, fc);
+    }
+    if (hasB) fact_exp<0>(fc, kappa, dmax, zc, st);
+    if (hasN) rowstep_half<KS, false, 0, 0>(uwn, tapsN + KS * TS, zn);                            // window row 0
+    if (hasB) fact_poly<0>(fc, st, v);
+    if (hasC) rowstep_half<KS, true, C::SHIFT, 1>(vw, recp, acc);
+    if (hasB) fact_exp<2>(fc, kappa, dmax, zc, st);
+    if (hasN) rowstep_half<KS, false, 0, 1>(uwn + KS * C::US, tapsN, zn);                         // window row KS
+    if (hasB) fact_poly<2>(fc, st, v);
+    if (hasC) rowstep_half<KS, true, C::SHIFT, 0>(vw + KS * C::VS, recp + KS * TS, acc);
 }
 
 template <int KS, int RW, int RH, int NT, int MINB, int PHI>
@@ -330,24 +385,8 @@ stage_fused_kernel(StageArgs a, int tw_nom, int th_nom, int ntx, int nty, int n_
                 wsec = (unsigned)__cvta_generic_to_shared(rec + prm_wplain(KS));
             }
             if (PHI == 3 && fact) {
-                // TNRD_FG groups, two pairs of responses at a time; row-steps 2g and 2g+1 of both filterings ride along
-                static_assert(2 * TNRD_FG >= KS + 1, "not enough phi steps for the row-steps");
-                float fc[TNRD_FSTRIDE];
-                lds_vec(rec + prm_fact(KS), fc);
-#pragma unroll 1
-                for (int g = 0; g < TNRD_FG; ++g) {
-                    if (hasB) fact_pairs<0>(fc, f_kappa, f_dmax, zc, v);
-                    if (2 * g <= KS) {
-                        if (hasN) rowstep<KS, false>(uwn + (2 * g) * C::US, tapsN + (KS - 2 * g) * TS, zn);
-                        if (hasC) rowstep<KS, true, C::SHIFT>(vw + (2 * g) * C::VS, recp + (2 * g) * TS, acc[n]);
-                    }
-                    if (hasB) fact_pairs<2>(fc, f_kappa, f_dmax, zc, v);
-                    lds_vec(rec + prm_fact(KS) + (g + 1 < TNRD_FG ? g + 1 : g) * TNRD_FSTRIDE, fc);     // next group
-                    if (2 * g + 1 <= KS) {
-                        if (hasN) rowstep<KS, false>(uwn + (2 * g + 1) * C::US, tapsN + (KS - 2 * g - 1) * TS, zn);
-                        if (hasC) rowstep<KS, true, C::SHIFT>(vw + (2 * g + 1) * C::VS, recp + (2 * g + 1) * TS, acc[n]);
-                    }
-                }
+                const float* frec = rec + prm_fact(KS);
+                    fact_block<KS, C>(frec, f_kappa, f_dmax, zc, v, uwn, tapsN, zn, vw, recp, acc[n], hasB, hasN, hasC);
             } else {
 #pragma unroll (DIRECT ? 1 : 2)
             for (int g = 0; g < C::NG - 1; ++g) {

@@ -80,7 +80,8 @@ def test_argument_validation_without_gpu(L):
     assert L.tnrd_deblock_diffuse(p, 1, 16, 16, 1, 4, 3, p, p, p, 10.0, p, p + 64, p + 64, st) == tnrd.ERR_ALIAS
     assert L.tnrd_qcs_project(p, 1, 16, 20, p, p, p + 64, st) == tnrd.ERR_SHAPE
     assert L.tnrd_qcs_project(p, 1, 16, 16, p + 64, p, p + 64, st) == tnrd.ERR_ALIAS
-    assert L.tnrd_set_phi_mode(3) == tnrd.ERR_UNSUPPORTED and L.tnrd_set_phi_mode(0) == tnrd.OK
+    assert L.tnrd_set_phi_mode(4) == tnrd.ERR_UNSUPPORTED and L.tnrd_set_phi_mode(0) == tnrd.OK
+    assert L.tnrd_set_phi_mode(tnrd.PHI_FACTORED) == tnrd.OK
     # options
     assert L.tnrd_set_kernel(7) == tnrd.ERR_UNSUPPORTED
     assert L.tnrd_set_kernel(0) == tnrd.OK

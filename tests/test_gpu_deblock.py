@@ -19,7 +19,7 @@ def tnrd():
     t.build()
     t.lib()
     t.tnrd_set_kernel(0)
-    t.tnrd_set_phi_mode(0)
+    t.tnrd_set_phi_mode(t.PHI_FACTORED)
     return t
 
 

@@ -21,6 +21,7 @@ def tnrd():
     t.build()                    # compiles libtnrd.so with nvcc if it is stale or absent (not a fallback)
     t.lib()                      # fails loudly if libtnrd.so is missing: no fallback
     t.tnrd_set_kernel(0)
+    t.tnrd_set_phi_mode(t.PHI_FACTORED)     # the default evaluator (include/tnrd.h)
     return t
 
 
@@ -238,7 +239,7 @@ def run_gpu_window(tnrd, c, **kw):
     try:
         return run_gpu(tnrd, c, **kw)
     finally:
-        tnrd.tnrd_set_phi_mode(0)
+        tnrd.tnrd_set_phi_mode(tnrd.PHI_FACTORED)
 
 
 @pytest.mark.parametrize("case", SMALL, ids=[f"s{c[0]}" for c in SMALL])
@@ -274,7 +275,7 @@ def test_window_phi_falls_back_to_dense(tnrd):
             mu = c["rbf_mu"].copy(); mu[10] += 2.0; d["rbf_mu"] = mu
         else:                                       # gamma > delta: 14 centres no longer cover 6.5 gamma
             d["rbf_gamma"] = 14.0
-        dense = run_gpu(tnrd, d)
+        dense = run_gpu_mode(tnrd, d, phi_mode=0)
         tnrd.tnrd_reset_launch_count()
         got = run_gpu_window(tnrd, d)
         assert tnrd.tnrd_launch_count() == 1 + 3 * d["T"]      # both fused kernels launched (one returns at once) + update
@@ -289,6 +290,84 @@ def test_window_phi_full_size_windows(tnrd):
         want = oracle.diffuse_window(c["f"][0], c["u0"][0], c["filters"], c["rbf_w"], c["rbf_mu"],
                                      c["rbf_gamma"], c["lambda"], y0, x0, 24, 24)
         check(got[y0:y0 + 24, x0:x0 + 24], want, f"window C4-2048 {(y0, x0)}")
+
+
+# --- the two exact evaluators: TNRD_PHI_FACTORED (default; every test above ran it) and TNRD_PHI_DENSE (direct) -----------
+@pytest.mark.parametrize("case", SMALL, ids=[f"s{c[0]}" for c in SMALL])
+def test_direct_phi_small_cases(tnrd, case):
+    seed, B, H, W, T, n_k, K = case
+    c = tnrd_gen.make_small(seed, B, H, W, T, n_k, K)
+    check(run_gpu_mode(tnrd, c, phi_mode=0), run_oracle(c), f"direct case {case}")
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_direct_and_factorised_phi_configs(tnrd, cfg):
+    """Both exact evaluators against the oracle on BASELINE.json's configs, and against each other: the factorisation is an
+    identity, the two differ by fp32 rounding only."""
+    c = tnrd_gen.make_config(cfg)
+    want = run_oracle(c)
+    direct, fact = run_gpu_mode(tnrd, c, phi_mode=0), run_gpu_mode(tnrd, c, phi_mode=3)
+    md, _ = check(direct, want, f"direct config {cfg}")
+    mf, _ = check(fact, want, f"factorised config {cfg}")
+    d = float(np.max(np.abs(direct - fact)))
+    print(f"config {cfg}: direct {md:.3e}, factorised {mf:.3e} from the oracle; {d:.3e} from each other")
+    assert d <= 2e-4 and mf <= 2.0 * md + 1e-4
+
+
+def test_factorised_phi_extreme_responses(tnrd):
+    """Responses far outside the centres (the clamp of the distance to a group's anchor is active for every group), large
+    weights on the outermost centres, and a response exactly on a centre."""
+    c = tnrd_gen.make_small(50, 1, 40, 44, 1, 6, 5)
+    c["f"] = (c["f"] * 6.0 - 400.0).astype(np.float32); c["u0"] = c["f"].copy()     # z up to ~ +-1000
+    w = c["rbf_w"].copy(); w[..., :3] = 0.5; w[..., -3:] = -0.5; c["rbf_w"] = w
+    check(run_gpu_mode(tnrd, c, phi_mode=3), run_oracle(c), "factorised extreme")
+    c = tnrd_gen.make_small(52, 1, 33, 35, 1, 4, 3)
+    c["f"] = np.full_like(c["f"], 40.0); c["u0"] = c["f"].copy()                    # constant image
+    k = np.zeros_like(c["filters"]); k[:, :, 1, 1] = np.array([1.0, -2.0, 0.25, 7.75])[None, :]   # z = 40, -80, 10, 310
+    c["filters"] = k
+    check(run_gpu_mode(tnrd, c, phi_mode=3), run_oracle(c), "factorised on-centre responses")
+
+
+def test_factorised_phi_large_weights(tnrd):
+    # weights 1e4 times the configs' (|w| ~ 2e3): the polynomials stay far inside the fp32 range
+    c = tnrd_gen.make_small(53, 1, 48, 52, 1, 5, 7)
+    c["rbf_w"] = (c["rbf_w"] * 1e4).astype(np.float32)
+    want = run_oracle(c)
+    got = run_gpu_mode(tnrd, c, phi_mode=3)
+    assert np.all(np.isfinite(got))
+    scale = float(np.max(np.abs(want - c["f"].astype(np.float64))))
+    assert np.max(np.abs(got - want)) <= 2e-5 * scale, "relative to the size of the update"
+
+
+@pytest.mark.parametrize("change", ["jitter", "narrow", "wide", "wider"])
+def test_factorised_phi_other_centres_and_widths(tnrd, change):
+    """jitter: centres not equidistant -> the kernel evaluates the direct form (same launch); narrow: gamma = 0.8 delta ->
+    direct form as well (the powers of rho would overflow); wide / wider: gamma = 1.4 / 3 delta -> factorised."""
+    c = tnrd_gen.make_small(51, 2, 50, 61, 2, 5, 7)
+    d = dict(c)
+    if change == "jitter":
+        mu = c["rbf_mu"].copy(); mu[10] += 2.0; d["rbf_mu"] = mu
+    else:
+        d["rbf_gamma"] = {"narrow": 8.0, "wide": 14.0, "wider": 30.0}[change]
+    want = run_oracle(d)
+    tnrd.tnrd_reset_launch_count()
+    got = run_gpu_mode(tnrd, d, phi_mode=3)
+    assert tnrd.tnrd_launch_count() == 1 + 2 * d["T"]
+    check(got, want, f"factorised {change}")
+    direct = run_gpu_mode(tnrd, d, phi_mode=0)
+    if change in ("jitter", "narrow"):
+        assert np.array_equal(got, direct), "the direct form inside the factorised kernel is the direct kernel's"
+    else:
+        assert np.max(np.abs(got - direct)) <= 2e-4
+
+
+def test_nan_input_propagates_in_both_exact_evaluators(tnrd):
+    c = tnrd_gen.make_small(54, 1, 40, 40, 1, 3, 5)
+    c["f"][0, 20, 20] = np.nan; c["u0"] = c["f"].copy()
+    for mode in (0, 3):
+        got = run_gpu_mode(tnrd, c, phi_mode=mode)[0]
+        assert np.isnan(got[20, 20]) and np.isnan(got[18:23, 18:23]).all(), mode     # inside the 5x5 footprint
+        assert np.isfinite(got[:10, :10]).all(), mode
 
 
 # --- small-image path: the filter bank of a tile split over several CTAs (tnrd_fused.cu, nsplit > 1) ------------
@@ -314,13 +393,13 @@ def test_filter_split_auto_plan_on_single_paper_image(tnrd):
 
 
 # --- piecewise-linear table evaluator: lookup table of the Gaussian phi and the triangular basis ------
-def run_gpu_mode(tnrd, c, phi_mode=0, basis=0, **kw):
+def run_gpu_mode(tnrd, c, phi_mode=3, basis=0, **kw):
     tnrd.tnrd_set_phi_mode(phi_mode)
     tnrd.tnrd_set_rbf_basis(basis)
     try:
         return run_gpu(tnrd, c, **kw)
     finally:
-        tnrd.tnrd_set_phi_mode(0)
+        tnrd.tnrd_set_phi_mode(tnrd.PHI_FACTORED)
         tnrd.tnrd_set_rbf_basis(0)
 
 
@@ -464,7 +543,7 @@ def test_large_image_16384_sampled_windows(tnrd):
 
 # --- run-to-run determinism at a size with many tiles, a split wave tail and every evaluator (no float atomics anywhere;
 # compute-sanitizer is not available on this pool, so a shared-memory race would have to show up here) -----------------
-@pytest.mark.parametrize("mode", [0, 1, 2])
+@pytest.mark.parametrize("mode", [0, 1, 2, 3])
 def test_bitwise_determinism_2048(tnrd, mode):
     c = tnrd_gen.make_config(4, size=2048, T=5)
     f = dev(c["f"])
@@ -478,12 +557,12 @@ def test_bitwise_determinism_2048(tnrd, mode):
             outs.append(out)
         torch.cuda.synchronize()
     finally:
-        tnrd.tnrd_set_phi_mode(0)
+        tnrd.tnrd_set_phi_mode(tnrd.PHI_FACTORED)
     assert all(torch.equal(outs[0], o) for o in outs[1:])
 
 
 # --- the opt-in evaluators at the size bench.py times (4096^2, T = 5): sampled windows against the oracle --------------
-@pytest.mark.parametrize("mode,basis", [(1, 0), (2, 0), (0, 1)], ids=["window", "lut", "triangle"])
+@pytest.mark.parametrize("mode,basis", [(0, 0), (1, 0), (2, 0), (0, 1)], ids=["direct", "window", "lut", "triangle"])
 def test_evaluators_4096_sampled_windows(tnrd, mode, basis):
     c = tnrd_gen.make_config(4, size=4096, T=5)
     got = run_gpu_mode(tnrd, c, phi_mode=mode, basis=basis)[0]
