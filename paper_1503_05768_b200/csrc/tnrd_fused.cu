@@ -31,6 +31,10 @@
 #include "tnrd_internal.h"
 #include "tnrd_device.cuh"
 
+#ifndef TNRD_FACT_NP
+#define TNRD_FACT_NP 2   // pairs of responses per factorised-phi step (2 or 4)
+#endif
+
 namespace tnrd {
 
 namespace {
@@ -137,15 +141,17 @@ __device__ __forceinline__ float ex2_pos(float x)
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-struct FactState { float2 g[2], rho[2], rhoi[2]; };   // of two pairs of responses: 2^{-d^2}, 2^{kappa d}, 2^{-kappa d}
+template <int NP> struct FactStateN { float2 g[NP], rho[NP], rhoi[NP]; };
+using FactState = FactStateN<TNRD_FACT_NP>;   // of two pairs of responses: 2^{-d^2}, 2^{kappa d}, 2^{-kappa d}
 
 // first half of a group for pairs P0, P0+1: the clamped distances to the anchor and the three exponentials of each response
 template <int P0>
 __device__ __forceinline__ void fact_exp(const float (&c)[TNRD_FSTRIDE], float kappa, float dmax, const float2 (&z)[4],
                                          FactState& s)
 {
+    constexpr int NP = TNRD_FACT_NP;
 #pragma unroll
-    for (int p = 0; p < 2; ++p) {
+    for (int p = 0; p < NP; ++p) {
         float2 d = __fadd2_rn(z[P0 + p], make_float2(c[0], c[0]));
         d = make_float2(fclamp_nan(d.x, dmax), fclamp_nan(d.y, dmax));
         const float2 t = __fmul2_rn(d, d);
@@ -159,23 +165,23 @@ __device__ __forceinline__ void fact_exp(const float (&c)[TNRD_FSTRIDE], float k
 template <int P0>
 __device__ __forceinline__ void fact_poly(const float (&c)[TNRD_FSTRIDE], const FactState& s, float2 (&v)[4])
 {
-    constexpr int S = TNRD_FS;
-    float2 h[2], hl[2];
+    constexpr int S = TNRD_FS, NP = TNRD_FACT_NP;
+    float2 h[NP], hl[NP];
 #pragma unroll
-    for (int p = 0; p < 2; ++p) {
+    for (int p = 0; p < NP; ++p) {
         h[p] = __ffma2_rn(make_float2(c[1], c[1]), s.rho[p], make_float2(c[2], c[2]));               // c_S rho + c_{S-1}
         hl[p] = __ffma2_rn(make_float2(c[S + 2], c[S + 2]), s.rhoi[p], make_float2(c[S + 3], c[S + 3]));
     }
 #pragma unroll
     for (int q = 2; q <= S; ++q)                                             // c_{S-2} .. c_0
 #pragma unroll
-        for (int p = 0; p < 2; ++p) h[p] = __ffma2_rn(h[p], s.rho[p], make_float2(c[1 + q], c[1 + q]));
+        for (int p = 0; p < NP; ++p) h[p] = __ffma2_rn(h[p], s.rho[p], make_float2(c[1 + q], c[1 + q]));
 #pragma unroll
     for (int q = 2; q < S; ++q)                                              // c_{-S+2} .. c_{-1}
 #pragma unroll
-        for (int p = 0; p < 2; ++p) hl[p] = __ffma2_rn(hl[p], s.rhoi[p], make_float2(c[S + 2 + q], c[S + 2 + q]));
+        for (int p = 0; p < NP; ++p) hl[p] = __ffma2_rn(hl[p], s.rhoi[p], make_float2(c[S + 2 + q], c[S + 2 + q]));
 #pragma unroll
-    for (int p = 0; p < 2; ++p) {
+    for (int p = 0; p < NP; ++p) {
         h[p] = __ffma2_rn(hl[p], s.rhoi[p], h[p]);
         v[P0 + p] = __ffma2_rn(s.g[p], h[p], v[P0 + p]);
     }
@@ -196,6 +202,32 @@ __device__ __forceinline__ void fact_block(const float* __restrict__ frec, float
     float fc[TNRD_FSTRIDE];
     FactState st;
     lds_vec(frec, fc);
+#if TNRD_FACT_NP == 4
+#pragma unroll 1
+    for (int g = 0; g < NGR; ++g) {
+        if (hasB) fact_exp<0>(fc, kappa, dmax, zc, st);
+        if (hasN) rowstep<KS, false>(uwn + (2 * g + 1) * C::US, tapsN + (KS - 2 * g - 1) * TS, zn);
+        if (hasC) rowstep<KS, true, C::SHIFT>(vw + (2 * g + 1) * C::VS, recp + (2 * g + 1) * TS, acc);
+        if (hasB) fact_poly<0>(fc, st, v);
+        if (hasN) rowstep<KS, false>(uwn + (2 * g + 2) * C::US, tapsN + (KS - 2 * g - 2) * TS, zn);
+        if (hasC) rowstep<KS, true, C::SHIFT>(vw + (2 * g + 2) * C::VS, recp + (2 * g + 2) * TS, acc);
+        lds_vec(frec + (g + 1) * TNRD_FSTRIDE, fc);
+    }
+#pragma unroll 1
+    for (int g = NGR; g < TNRD_FG - 1; ++g) {
+        if (hasB) {
+            fact_exp<0>(fc, kappa, dmax, zc, st);
+            fact_poly<0>(fc, st, v);
+        }
+        lds_vec(frec + (g + 1) * TNRD_FSTRIDE, fc);
+    }
+    if (hasB) fact_exp<0>(fc, kappa, dmax, zc, st);
+    if (hasN) rowstep_half<KS, false, 0, 0>(uwn, tapsN + KS * TS, zn);                            // window row 0
+    if (hasC) rowstep_half<KS, true, C::SHIFT, 1>(vw, recp, acc);
+    if (hasB) fact_poly<0>(fc, st, v);
+    if (hasN) rowstep_half<KS, false, 0, 1>(uwn + KS * C::US, tapsN, zn);                         // window row KS
+    if (hasC) rowstep_half<KS, true, C::SHIFT, 0>(vw + KS * C::VS, recp + KS * TS, acc);
+#else
 #pragma unroll 1
     for (int g = 0; g < NGR; ++g) {
         if (hasB) fact_exp<0>(fc, kappa, dmax, zc, st);
@@ -226,6 +258,7 @@ __device__ __forceinline__ void fact_block(const float* __restrict__ frec, float
     if (hasN) rowstep_half<KS, false, 0, 1>(uwn + KS * C::US, tapsN, zn);                         // window row KS
     if (hasB) fact_poly<2>(fc, st, v);
     if (hasC) rowstep_half<KS, true, C::SHIFT, 0>(vw + KS * C::VS, recp + KS * TS, acc);
+#endif
 }
 
 template <int KS, int RW, int RH, int NT, int MINB, int PHI>
@@ -528,9 +561,8 @@ inline int env_int(const char* name)
 inline int forced_tile() { return env_int("TNRD_TILE"); }
 inline int forced_split() { return env_int("TNRD_SPLIT"); }
 
-// Tile plan for one kernel configuration.  The path is XU-bound, so an SM's time is proportional to the phi work
-// assigned to it: (CTAs per SM) x (filters per CTA) x (time of one filter, see below; constants fitted on B200 at 4096^2
-// and on C3).  Try the fewest equal tiles that cover the phi region and a few more in each direction; when the tiles of
+// Tile plan for one kernel configuration.  An SM's time is (CTAs per SM) x (filters per CTA x time of one filter + a
+// per-CTA constant), both from a model fitted on B200 (see below).  Try the fewest equal tiles that cover the phi region and a few more in each direction; when the tiles of
 // the whole batch do not fill the GPU (small images), also try splitting the filter bank of a tile over nsplit CTAs --
 // every split pays the per-CTA constant again.  Keep the cheapest.
 template <int KS, int RW, int RH, int NT, int MINB>
@@ -540,27 +572,28 @@ Plan plan_tiles(const StageArgs& a, int num_sms)
     constexpr int R = (KS - 1) / 2;
     const int Wz = a.W + 2 * R, Hz = a.H + 2 * R;
     Plan best{0, 0, 0, 0, 1, 0, -1.0, 0};
-    // time of one filter on one CTA with a tw x th tile, in units of one warp-block on the XU pipe of an SM sub-partition
-    // (~2 us: 8 px x 63 ex2 x 32 lanes at 4 lanes per clock): rounds of NT blocks, a round with w warps of phi work takes
-    // k = ceil(w / 4) units when k >= 4 warps share a sub-partition; fewer warps feed the pipe worse (3.3, 2.1, 1.4 units
-    // for k = 3, 2, 1); plus 1.2 + 0.3 per round that do not overlap (barrier, pipeline restart).  A CTA costs
-    // filters x this + 4 to 10 units (tile gather, fill / drain, stores: cta_const).  Constants fitted on one-wave
-    // launches of 12 x 12 tiles of 44 .. 122 pixels (B200, 48 and 24 filters 7x7).
+    // Time of one filter on one CTA with a tw x th tile, in microseconds, for the default (factorised) evaluator.  The CTA
+    // works in rounds of NT blocks; a round in which w warps have phi work takes 2.85 + 0.105 w us (the instruction stream
+    // of one block, ~1200 mostly dependent instructions, sets the floor; more warps only fill its gaps), a round with
+    // transposed-filter work only 1.5 us, plus 1.0 us per filter that does not overlap (barrier, pipeline restart); a tile
+    // of a single round runs 2.8 + 0.18 w.  A CTA costs filters x this + 6 to 17 us (tile gather, fill / drain, stores:
+    // cta_const).  Fitted on one-wave launches of 12 x 12 tiles of 28 .. 122 pixels (B200, 48 and 24 filters 7x7); two
+    // co-resident CTAs of 256 threads share the sub-partitions, hence the factor on w.
     auto per_filter = [&](int tw, int th) {
         const long long bphi = (long long)((tw + 3) / 4) * ((th + 1) / 2);
         const long long bout = (long long)((tw + 2 * R + 3) / 4) * ((th + 2 * R + 1) / 2);
-        double pf = 1.2;
+        const double share = MINB * NT / 512.0;
+        if (bout <= NT) return 2.8 + 0.18 * share * (double)((bphi + 31) / 32);
+        double pf = 1.0;
         for (long long done = 0; done < bout; done += NT) {
             const long long inr = bphi - done < 0 ? 0 : (bphi - done > NT ? NT : bphi - done);
-            const long long wr = (inr + 31) / 32;
-            const int kw = (int)((wr + 3) / 4);                       // warps per SM sub-partition in this round
-            if (wr > 0) pf += 0.3 + (kw >= 4 ? (double)kw : kw == 3 ? 3.3 : kw == 2 ? 2.1 : 1.4);
-            else pf += 0.3;                                            // transposed filter only
+            const long long wr = (inr + 31) / 32;                      // warps with phi work in this round
+            pf += wr > 0 ? 2.85 + 0.105 * share * (double)wr : 1.5;
         }
         return pf;
     };
     auto cta_const = [&](int tw, int th) {
-        return 4.0 + (double)((tw + 2 * R + 3) / 4) * ((th + 2 * R + 1) / 2) / 350.0;
+        return 6.2 + (double)((tw + 2 * R + 3) / 4) * ((th + 2 * R + 1) / 2) / 190.0;
     };
     const int ntx0 = (Wz + C::TWMAX - 1) / C::TWMAX, nty0 = (Hz + C::THMAX - 1) / C::THMAX;
     const int fx = env_int("TNRD_NTX"), fy = env_int("TNRD_NTY");       // tuning knobs: force the tile counts
