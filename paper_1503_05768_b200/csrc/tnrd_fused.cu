@@ -228,7 +228,7 @@ __device__ __forceinline__ void fact_block(const float* __restrict__ frec, float
     if (hasN) rowstep_half<KS, false, 0, 1>(uwn + KS * C::US, tapsN, zn);                         // window row KS
     if (hasC) rowstep_half<KS, true, C::SHIFT, 0>(vw + KS * C::VS, recp + KS * TS, acc);
 #else
-#pragma unroll 1
+#pragma unroll
     for (int g = 0; g < NGR; ++g) {
         if (hasB) fact_exp<0>(fc, kappa, dmax, zc, st);
         if (hasN) rowstep<KS, false>(uwn + (2 * g + 1) * C::US, tapsN + (KS - 2 * g - 1) * TS, zn);
