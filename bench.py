@@ -40,7 +40,7 @@ NOMINAL_SM_MHZ, NOMINAL_SMS, MUFU_PER_CLK_SM, FMA_PER_CLK_SM = 1965.0, 148, 16, 
 # 3 ex2 and 16 FMA-pipe operations (add, 2 mul, 12 Horner FMAs, 1 FMA into the sum)
 FACT_GROUPS, FACT_EX2_PER_GROUP, FACT_FMA_PER_GROUP = 5, 3, 16
 # dram__bytes_read.sum + dram__bytes_write.sum per fused-stage launch at 4096^2 (profiles/r01_fused_stage_ncu.md)
-TRAFFIC_BYTES_PER_LAUNCH = {4096: 121.8e6}
+TRAFFIC_BYTES_PER_LAUNCH = {4096: 119.5e6}
 
 
 def read_peaks():
