@@ -228,6 +228,10 @@ void tnrd_reset_launch_count(void);
  *   which = 0: FP32 FFMA rate      -> *rate = FMA lane-operations per second (x2 = FLOP/s)
  *   which = 1: MUFU.EX2 rate       -> *rate = ex2 evaluations per second
  *   which = 2: the phi inner loop (FADD, FMUL, MUFU.EX2, FFMA per term) -> RBF terms per second
+ *   which = 3: warp-level tensor path, mma.sync m16n8k8 TF32, fp32 accumulation -> multiply-adds per second (x2 = FLOP/s)
+ *   which = 4: the same with m16n8k16 BF16
+ * (3 and 4 are not used by any kernel of this library yet: they size the filterings as an implicit GEMM.)
+ * Any other value: TNRD_ERR_UNSUPPORTED.
  */
 int tnrd_microbench(int which, double* rate, void* stream);
 

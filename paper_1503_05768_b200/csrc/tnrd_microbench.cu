@@ -1,6 +1,7 @@
 // tnrd_microbench.cu -- register-only micro-kernels that measure the roofline denominators of the TNRD path on
-// the current device: FP32 FFMA rate, MUFU.EX2 rate and the rate of the phi inner loop (FADD, FMUL, MUFU.EX2,
-// FFMA per RBF term; Main Eq. 6).  Timed with CUDA events on the caller's stream.
+// the current device: FP32 FFMA rate, MUFU.EX2 rate, the rate of the phi inner loop (FADD, FMUL, MUFU.EX2,
+// FFMA per RBF term; Main Eq. 6) and the warp-level tensor path (mma.sync TF32 / BF16).  Timed with
+// CUDA events on the caller's stream.
 #include "tnrd_internal.h"
 
 namespace tnrd {
@@ -79,6 +80,38 @@ __global__ void __launch_bounds__(MB_THREADS, 1) mb_phi(float* out, int iters)
     if (s == 123.456f) out[0] = s;
 }
 
+// legacy warp-level tensor path (mma.sync -> HMMA), register-only: TF32 m16n8k8 (BF16 = false) or BF16 m16n8k16, fp32
+// accumulation.  The denominator for the filterings as an implicit GEMM.
+template <bool BF16>
+__global__ void __launch_bounds__(MB_THREADS, 1) mb_mma(float* out, int iters)
+{
+    float c[MB_ILP][4];
+    const unsigned a0 = threadIdx.x, a1 = 3u * threadIdx.x, a2 = 7u, a3 = 9u, b0 = blockIdx.x, b1 = 5u;
+#pragma unroll
+    for (int k = 0; k < MB_ILP; ++k)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) c[k][q] = 0.f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < MB_ILP; ++k) {
+            if (BF16)
+                asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                             : "+f"(c[k][0]), "+f"(c[k][1]), "+f"(c[k][2]), "+f"(c[k][3])
+                             : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+            else
+                asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                             : "+f"(c[k][0]), "+f"(c[k][1]), "+f"(c[k][2]), "+f"(c[k][3])
+                             : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+        }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < MB_ILP; ++k)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) s += c[k][q];
+    if (s == 123.456f) out[0] = s;
+}
+
 }  // namespace
 
 cudaError_t run_microbench(int which, double* rate, cudaStream_t st, unsigned long long* launches)
@@ -107,10 +140,18 @@ cudaError_t run_microbench(int which, double* rate, cudaStream_t st, unsigned lo
             const int iters = 1024;
             mb_mufu<<<grid, MB_THREADS, 0, st>>>(d_out, iters);
             ops_per_thread = (double)iters * 16 * MB_ILP;
-        } else {
+        } else if (which == 2) {
             const int iters = 256;
             mb_phi<<<grid, MB_THREADS, 0, st>>>(d_out, iters);
             ops_per_thread = (double)iters * TNRD_MP * MB_ILP;
+        } else if (which == 3) {
+            const int iters = 4096;
+            mb_mma<false><<<grid, MB_THREADS, 0, st>>>(d_out, iters);
+            ops_per_thread = (double)iters * MB_ILP * (16 * 8 * 8) / 32.0;      // multiply-adds per thread
+        } else {
+            const int iters = 4096;
+            mb_mma<true><<<grid, MB_THREADS, 0, st>>>(d_out, iters);
+            ops_per_thread = (double)iters * MB_ILP * (16 * 8 * 16) / 32.0;
         }
         ++*launches;
         cudaEventRecord(e1, st);

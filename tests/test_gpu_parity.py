@@ -231,6 +231,9 @@ def test_microbench_rates_are_sane(tnrd):
     ffma, mufu, phi = (tnrd.tnrd_microbench(i) for i in range(3))
     print(f"FFMA {ffma / 1e12:.2f} T/s  MUFU.EX2 {mufu / 1e12:.2f} T/s  phi terms {phi / 1e12:.2f} T/s")
     assert 5e12 < ffma < 60e12 and 1e12 < mufu < 12e12 and 0.5e12 < phi <= mufu * 1.05
+    tf32, bf16 = tnrd.tnrd_microbench(3), tnrd.tnrd_microbench(4)     # mma.sync multiply-adds per second
+    print(f"mma.sync TF32 {2 * tf32 / 1e12:.0f} TFLOP/s  BF16 {2 * bf16 / 1e12:.0f} TFLOP/s")
+    assert ffma < tf32 < bf16 < 2e15
 
 
 # --- windowed phi evaluator (tnrd_set_phi_mode(1)): same oracle, same tolerance ------------------------------------
