@@ -230,7 +230,11 @@ void tnrd_reset_launch_count(void);
  *   which = 2: the phi inner loop (FADD, FMUL, MUFU.EX2, FFMA per term) -> RBF terms per second
  *   which = 3: warp-level tensor path, mma.sync m16n8k8 TF32, fp32 accumulation -> multiply-adds per second (x2 = FLOP/s)
  *   which = 4: the same with m16n8k16 BF16
- * (3 and 4 are not used by any kernel of this library yet: they size the filterings as an implicit GEMM.)
+ *   which = 5: prototype of the forward filter bank (48 filters 7x7) as an implicit GEMM on that path: A fragments gathered tap
+ *              by tap from a 128 x 128 tile in shared memory, operands split into BF16 halves, three products, fp32
+ *              accumulation -> pixels (48 responses each) per second; checks itself against plain fp32 FMAs on the device
+ *              and fails with TNRD_ERR_CUDA if the two differ by more than 0.05 (|z| ~ 75)
+ * (3 .. 5 are not used by the product path: they size the filterings as an implicit GEMM.)
  * Any other value: TNRD_ERR_UNSUPPORTED.
  */
 int tnrd_microbench(int which, double* rate, void* stream);

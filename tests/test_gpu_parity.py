@@ -234,6 +234,11 @@ def test_microbench_rates_are_sane(tnrd):
     tf32, bf16 = tnrd.tnrd_microbench(3), tnrd.tnrd_microbench(4)     # mma.sync multiply-adds per second
     print(f"mma.sync TF32 {2 * tf32 / 1e12:.0f} TFLOP/s  BF16 {2 * bf16 / 1e12:.0f} TFLOP/s")
     assert ffma < tf32 < bf16 < 2e15
+    # prototype of the forward bank on that path (BF16 x3 split, A fragments gathered tap by tap); the call fails if its
+    # device-side comparison with plain fp32 FMAs does
+    fwd = tnrd.tnrd_microbench(5)
+    print(f"forward bank 48 x 7x7 by mma.sync BF16 x3: {fwd / 1e9:.1f} Gpixel/s (FFMA pipe alone: {ffma / 2352 / 1e9:.1f})")
+    assert 2e9 < fwd < bf16 / (48 * 64 * 3)
 
 
 # --- windowed phi evaluator (tnrd_set_phi_mode(1)): same oracle, same tolerance ------------------------------------
