@@ -234,7 +234,9 @@ void tnrd_reset_launch_count(void);
  *              by tap from a 128 x 128 tile in shared memory, operands split into BF16 halves, three products, fp32
  *              accumulation -> pixels (48 responses each) per second; checks itself against plain fp32 FMAs on the device
  *              and fails with TNRD_ERR_CUDA if the two differ by more than 0.05 (|z| ~ 75)
- * (3 .. 5 are not used by the product path: they size the filterings as an implicit GEMM.)
+ *   which = 6: the same followed by the factorised phi evaluated on the accumulator fragments (two adjacent filters of a
+ *              pixel per register pair, packed coefficient pairs from shared memory; synthetic coefficients) -> pixels per second
+ * (3 .. 6 are not used by the product path: they size the filterings as an implicit GEMM.)
  * Any other value: TNRD_ERR_UNSUPPORTED.
  */
 int tnrd_microbench(int which, double* rate, void* stream);

@@ -121,7 +121,9 @@ __global__ void __launch_bounds__(MB_THREADS, 1) mb_mma(float* out, int iters)
 // is gathered tap by tap from the fp32 tile (the im2col matrix never exists) and split in registers into BF16 halves
 // x = x_hi + x_lo; the filters are split once on the device; three products (hi hi, hi lo, lo hi) accumulate in fp32.
 constexpr int FB_NK = 48, FB_TW = 128, FB_TH = 128, FB_UH = FB_TH + 8, FB_US = 148, FB_MT = 2, FB_NKS = 4, FB_NNT = FB_NK / 8;
-constexpr int FB_SMEM = FB_UH * FB_US * 4 + FB_NKS * FB_NNT * 32 * 16;
+constexpr int FB_FG = 5, FB_FST = 16;                 // phi groups, coefficient slots per group (which = 6)
+constexpr int FB_CSTRIDE = FB_FG * FB_FST + 1;        // float2 per filter pair: odd, so that the four pairs a warp reads hit different banks
+constexpr int FB_SMEM = FB_UH * FB_US * 4 + FB_NKS * FB_NNT * 32 * 16 + FB_NK / 2 * FB_CSTRIDE * 8;
 
 __device__ __forceinline__ float fb_hash(unsigned i)      // [0, 1)
 {
@@ -172,7 +174,60 @@ __global__ void __launch_bounds__(512) fb_init(float* U, float* kf, uint4* bfrag
     }
 }
 
-template <bool CHECK>
+// which = 6: the factorised phi on the accumulator layout -- a register pair holds two ADJACENT FILTERS of one
+// pixel, so the Horner coefficients are packed pairs (LDS.64, one per FFMA2 of each of the NZ responses) instead of broadcast
+// scalars.  Synthetic coefficients: the instruction stream does not depend on the values.
+template <int NZ>
+__device__ __forceinline__ void fb_phi_pairs(float2 (&z)[NZ], const float2* __restrict__ cf)
+{
+    float2 v[NZ];
+#pragma unroll
+    for (int i = 0; i < NZ; ++i) v[i] = make_float2(0.f, 0.f);
+#pragma unroll 1
+    for (int gr = 0; gr < FB_FG; ++gr) {
+        const float2* c = cf + gr * FB_FST;
+        float2 g[NZ], rho[NZ], rhoi[NZ], h[NZ], hl[NZ];
+        const float2 c0 = c[0];
+#pragma unroll
+        for (int i = 0; i < NZ; ++i) {
+            float2 d = __ffma2_rn(z[i], make_float2(0.0849f, 0.0849f), c0);
+            asm("min.NaN.f32 %0, %0, %1;" : "+f"(d.x) : "f"(11.3f));
+            asm("max.NaN.f32 %0, %0, %1;" : "+f"(d.x) : "f"(-11.3f));
+            asm("min.NaN.f32 %0, %0, %1;" : "+f"(d.y) : "f"(11.3f));
+            asm("max.NaN.f32 %0, %0, %1;" : "+f"(d.y) : "f"(-11.3f));
+            const float2 t = __fmul2_rn(d, d), e = __fmul2_rn(d, make_float2(1.698f, 1.698f));
+            g[i] = make_float2(ex2_approx(-t.x), ex2_approx(-t.y));
+            rho[i] = make_float2(ex2_approx(e.x), ex2_approx(e.y));
+            rhoi[i] = make_float2(ex2_approx(-e.x), ex2_approx(-e.y));
+        }
+        {
+            const float2 a = c[1], b = c[2], a2 = c[8], b2 = c[9];
+#pragma unroll
+            for (int i = 0; i < NZ; ++i) { h[i] = __ffma2_rn(a, rho[i], b); hl[i] = __ffma2_rn(a2, rhoi[i], b2); }
+        }
+#pragma unroll
+        for (int q = 3; q <= 7; ++q) {
+            const float2 a = c[q];
+#pragma unroll
+            for (int i = 0; i < NZ; ++i) h[i] = __ffma2_rn(h[i], rho[i], a);
+        }
+#pragma unroll
+        for (int q = 10; q <= 13; ++q) {
+            const float2 a = c[q];
+#pragma unroll
+            for (int i = 0; i < NZ; ++i) hl[i] = __ffma2_rn(hl[i], rhoi[i], a);
+        }
+#pragma unroll
+        for (int i = 0; i < NZ; ++i) {
+            h[i] = __ffma2_rn(hl[i], rhoi[i], h[i]);
+            v[i] = __ffma2_rn(g[i], h[i], v[i]);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < NZ; ++i) z[i] = v[i];
+}
+
+template <bool CHECK, bool PHI>
 __global__ void __launch_bounds__(MB_THREADS, 1) fb_fwd(const float* __restrict__ U, const float* __restrict__ kf,
                                                         const uint4* __restrict__ bfrag, float* __restrict__ sink,
                                                         unsigned* __restrict__ maxdiff, int reps)
@@ -181,7 +236,10 @@ __global__ void __launch_bounds__(MB_THREADS, 1) fb_fwd(const float* __restrict_
     float* us = fb_sm;                                               // [FB_UH][FB_US]
     uint4* bs = reinterpret_cast<uint4*>(us + FB_UH * FB_US);       // [FB_NKS][FB_NNT][32]
     for (int i = threadIdx.x; i < FB_UH * FB_US; i += MB_THREADS) us[i] = U[i];
+    float2* cfs = reinterpret_cast<float2*>(bs + FB_NKS * FB_NNT * 32);   // [FB_NK / 2][FB_CSTRIDE]
     for (int i = threadIdx.x; i < FB_NKS * FB_NNT * 32; i += MB_THREADS) bs[i] = bfrag[i];
+    for (int i = threadIdx.x; i < FB_NK / 2 * FB_CSTRIDE; i += MB_THREADS)
+        cfs[i] = make_float2(0.01f * (float)(i % 13) - 0.05f, 0.02f * (float)(i % 7) - 0.06f);
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, c = lane & 3;
     float total = 0.f;
@@ -240,6 +298,23 @@ __global__ void __launch_bounds__(MB_THREADS, 1) fb_fwd(const float* __restrict_
                         }
                 atomicMax(maxdiff, __float_as_uint(worst));
             }
+            if (PHI) {
+#pragma unroll
+                for (int n = 0; n < FB_NNT; ++n) {
+                    float2 zz[2 * FB_MT];
+#pragma unroll
+                    for (int m = 0; m < FB_MT; ++m) {
+                        zz[2 * m] = make_float2(acc[m][n][0], acc[m][n][1]);
+                        zz[2 * m + 1] = make_float2(acc[m][n][2], acc[m][n][3]);
+                    }
+                    fb_phi_pairs<2 * FB_MT>(zz, cfs + (4 * n + c) * FB_CSTRIDE);
+#pragma unroll
+                    for (int m = 0; m < FB_MT; ++m) {
+                        acc[m][n][0] = zz[2 * m].x; acc[m][n][1] = zz[2 * m].y;
+                        acc[m][n][2] = zz[2 * m + 1].x; acc[m][n][3] = zz[2 * m + 1].y;
+                    }
+                }
+            }
 #pragma unroll
             for (int m = 0; m < FB_MT; ++m)
 #pragma unroll
@@ -249,7 +324,7 @@ __global__ void __launch_bounds__(MB_THREADS, 1) fb_fwd(const float* __restrict_
     if (total == 123.456f) sink[0] = total;
 }
 
-cudaError_t run_fwd_bank_probe(double* rate, cudaStream_t st, unsigned long long* launches, int sms)
+cudaError_t run_fwd_bank_probe(bool with_phi, double* rate, cudaStream_t st, unsigned long long* launches, int sms)
 {
     float *U = nullptr, *kf = nullptr, *sink = nullptr;
     uint4* bfrag = nullptr;
@@ -259,8 +334,9 @@ cudaError_t run_fwd_bank_probe(double* rate, cudaStream_t st, unsigned long long
     if (e == cudaSuccess) e = cudaMalloc(&sink, 4);
     if (e == cudaSuccess) e = cudaMalloc(&bfrag, (size_t)FB_NKS * FB_NNT * 32 * 16);
     if (e == cudaSuccess) e = cudaMalloc(&maxdiff, 4);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fb_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, FB_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fb_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, FB_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fb_fwd<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, FB_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fb_fwd<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, FB_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fb_fwd<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, FB_SMEM);
     float best_ms = 1e30f;
     unsigned diff_bits = 0;
     if (e == cudaSuccess) {
@@ -269,12 +345,13 @@ cudaError_t run_fwd_bank_probe(double* rate, cudaStream_t st, unsigned long long
         cudaEventCreate(&e1);
         cudaMemsetAsync(maxdiff, 0, 4, st);
         fb_init<<<1, 512, 0, st>>>(U, kf, bfrag);
-        fb_fwd<true><<<1, MB_THREADS, FB_SMEM, st>>>(U, kf, bfrag, sink, maxdiff, 1);
+        fb_fwd<true, false><<<1, MB_THREADS, FB_SMEM, st>>>(U, kf, bfrag, sink, maxdiff, 1);
         *launches += 2;
         const int reps = 16;
         for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {   // rep 0 = warm-up
             cudaEventRecord(e0, st);
-            fb_fwd<false><<<sms, MB_THREADS, FB_SMEM, st>>>(U, kf, bfrag, sink, maxdiff, reps);
+            if (with_phi) fb_fwd<false, true><<<sms, MB_THREADS, FB_SMEM, st>>>(U, kf, bfrag, sink, maxdiff, reps);
+            else fb_fwd<false, false><<<sms, MB_THREADS, FB_SMEM, st>>>(U, kf, bfrag, sink, maxdiff, reps);
             ++*launches;
             cudaEventRecord(e1, st);
             e = cudaEventSynchronize(e1);
@@ -306,7 +383,7 @@ cudaError_t run_microbench(int which, double* rate, cudaStream_t st, unsigned lo
     if (e != cudaSuccess) return e;
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) return e;
-    if (which == 5) return run_fwd_bank_probe(rate, st, launches, sms);
+    if (which >= 5) return run_fwd_bank_probe(which == 6, rate, st, launches, sms);
     float* d_out = nullptr;
     e = cudaMalloc(&d_out, sizeof(float));
     if (e != cudaSuccess) return e;

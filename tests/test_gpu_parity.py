@@ -239,6 +239,9 @@ def test_microbench_rates_are_sane(tnrd):
     fwd = tnrd.tnrd_microbench(5)
     print(f"forward bank 48 x 7x7 by mma.sync BF16 x3: {fwd / 1e9:.1f} Gpixel/s (FFMA pipe alone: {ffma / 2352 / 1e9:.1f})")
     assert 2e9 < fwd < bf16 / (48 * 64 * 3)
+    fwd_phi = tnrd.tnrd_microbench(6)      # ... followed by the factorised phi on the accumulator fragments
+    print(f"forward bank + factorised phi on the accumulators: {fwd_phi / 1e9:.2f} Gpixel/s (XU roofline {mufu / 720 / 1e9:.2f})")
+    assert 1e9 < fwd_phi < min(fwd, mufu / 720)
 
 
 # --- windowed phi evaluator (tnrd_set_phi_mode(1)): same oracle, same tolerance ------------------------------------
