@@ -363,7 +363,8 @@ def main():
     xu_peak = NOMINAL_SMS * MUFU_PER_CLK_SM * NOMINAL_SM_MHZ * 1e6 / 1e12
     mb = {n: tnrd.tnrd_microbench(i) / 1e12 for i, n in enumerate(["ffma_T_per_s", "ex2_T_per_s", "phi_terms_T_per_s",
                                                                    "mma_sync_tf32_Tmac_per_s", "mma_sync_bf16_Tmac_per_s",
-                                                                   "fwd_bank_mma_bf16x3_Tpx_per_s", "fwd_bank_mma_plus_phi_Tpx_per_s"])}
+                                                                   "fwd_bank_mma_bf16x3_Tpx_per_s", "fwd_bank_mma_plus_phi_Tpx_per_s",
+                                                                   "fwd_phi_scatter_mma_no_fold_Tpx_per_s"])}
     roofline = {
         "bound": "alu", "pipe": "fma (FFMA2/FFMA/FMUL2/FADD2)", "achieved": achieved, "peak": peak_nominal, "unit": "Tfma/s",
         "frac": achieved / peak_nominal, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(H if (H == W and args.workload == "c4") else -1),

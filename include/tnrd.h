@@ -236,7 +236,11 @@ void tnrd_reset_launch_count(void);
  *              and fails with TNRD_ERR_CUDA if the two differ by more than 0.05 (|z| ~ 75)
  *   which = 6: the same followed by the factorised phi evaluated on the accumulator fragments (two adjacent filters of a
  *              pixel per register pair, packed coefficient pairs from shared memory; synthetic coefficients) -> pixels per second
- * (3 .. 6 are not used by the product path: they size the filterings as an implicit GEMM.)
+ *   which = 7: 6 followed by the transposed bank as a scatter table S[pixel][tap] = sum_f v_f K_f[tap] on the same path (the phi
+ *              accumulators are the A fragments; BF16 halves, three products); the fold s(p) = sum_tap S[p + tap - r][tap]
+ *              is NOT included -> pixels per second.  5 .. 7 all check the forward responses and the scatter table of one
+ *              tile against plain fp32 sums on the device.
+ * (3 .. 7 are not used by the product path: they size the filterings as an implicit GEMM.)
  * Any other value: TNRD_ERR_UNSUPPORTED.
  */
 int tnrd_microbench(int which, double* rate, void* stream);

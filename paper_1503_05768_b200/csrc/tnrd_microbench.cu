@@ -123,7 +123,9 @@ __global__ void __launch_bounds__(MB_THREADS, 1) mb_mma(float* out, int iters)
 constexpr int FB_NK = 48, FB_TW = 128, FB_TH = 128, FB_UH = FB_TH + 8, FB_US = 148, FB_MT = 2, FB_NKS = 4, FB_NNT = FB_NK / 8;
 constexpr int FB_FG = 5, FB_FST = 16;                 // phi groups, coefficient slots per group (which = 6)
 constexpr int FB_CSTRIDE = FB_FG * FB_FST + 1;        // float2 per filter pair: odd, so that the four pairs a warp reads hit different banks
-constexpr int FB_SMEM = FB_UH * FB_US * 4 + FB_NKS * FB_NNT * 32 * 16 + FB_NK / 2 * FB_CSTRIDE * 8;
+constexpr int FB_SNT = 7;                              // n-tiles of the scatter table: 49 taps padded to 56 (which = 7)
+constexpr int FB_SMEM = FB_UH * FB_US * 4 + FB_NKS * FB_NNT * 32 * 16 + FB_NK / 2 * FB_CSTRIDE * 8 + 3 * FB_SNT * 32 * 16;
+static_assert((FB_NK / 2 * FB_CSTRIDE * 8) % 16 == 0, "the scatter-table fragments must stay 16-byte aligned");
 
 __device__ __forceinline__ float fb_hash(unsigned i)      // [0, 1)
 {
@@ -154,7 +156,7 @@ __device__ __forceinline__ float fb_tap(const float* kf, int slot, int n)   // B
 }
 
 // one CTA: a pseudo-random tile on the 0..255 scale, 48 zero-mean unit-norm filters, and their B fragments
-__global__ void __launch_bounds__(512) fb_init(float* U, float* kf, uint4* bfrag)
+__global__ void __launch_bounds__(512) fb_init(float* U, float* kf, uint4* bfrag, uint4* b2frag)
 {
     for (int i = threadIdx.x; i < FB_UH * FB_US; i += 512) U[i] = 255.0f * fb_hash(i);
     if (threadIdx.x < FB_NK) {
@@ -172,6 +174,30 @@ __global__ void __launch_bounds__(512) fb_init(float* U, float* kf, uint4* bfrag
             fb_split2(fb_tap(kf, 16 * ks + 2 * c + 8 * q, n), fb_tap(kf, 16 * ks + 2 * c + 8 * q + 1, n), h[q], l[q]);
         bfrag[i] = make_uint4(h[0], h[1], l[0], l[1]);
     }
+    // transposed bank as a scatter table S[px][tap] = sum_f v_f(px) K_f[tap]: B[k = filter 16 s + ..][n = tap 8 nt + g]
+    for (int i = threadIdx.x; i < 3 * FB_SNT * 32; i += 512) {
+        const int lane = i & 31, nt = (i >> 5) % FB_SNT, s3 = (i >> 5) / FB_SNT, tap = 8 * nt + (lane >> 2), c = lane & 3;
+        unsigned h[2], l[2];
+        for (int q = 0; q < 2; ++q) {
+            const int f = 16 * s3 + 2 * c + 8 * q;
+            fb_split2(tap < 49 ? kf[f * 49 + tap] : 0.f, tap < 49 ? kf[(f + 1) * 49 + tap] : 0.f, h[q], l[q]);
+        }
+        b2frag[i] = make_uint4(h[0], h[1], l[0], l[1]);
+    }
+}
+
+// check of the scatter table of one CTA's tile against plain fp32 sums (v and S as the check launch wrote them)
+__global__ void fb_check_s(const float* __restrict__ v, const float* __restrict__ S, const float* __restrict__ kf, unsigned* maxdiff)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= FB_TH * FB_TW) return;
+    float worst = 0.f;
+    for (int tap = 0; tap < 49; ++tap) {
+        float r = 0.f;
+        for (int f = 0; f < FB_NK; ++f) r = fmaf(v[(size_t)p * FB_NK + f], kf[f * 49 + tap], r);
+        worst = fmaxf(worst, 1000.0f * fabsf(r - S[(size_t)p * 56 + tap]));     // |S| ~ 1: same 0.05 threshold as z after x 1000
+    }
+    atomicMax(maxdiff, __float_as_uint(worst));
 }
 
 // which = 6: the factorised phi on the accumulator layout -- a register pair holds two ADJACENT FILTERS of one
@@ -227,10 +253,11 @@ __device__ __forceinline__ void fb_phi_pairs(float2 (&z)[NZ], const float2* __re
     for (int i = 0; i < NZ; ++i) z[i] = v[i];
 }
 
-template <bool CHECK, bool PHI>
+template <bool CHECK, bool PHI, bool SCATTER>
 __global__ void __launch_bounds__(MB_THREADS, 1) fb_fwd(const float* __restrict__ U, const float* __restrict__ kf,
-                                                        const uint4* __restrict__ bfrag, float* __restrict__ sink,
-                                                        unsigned* __restrict__ maxdiff, int reps)
+                                                        const uint4* __restrict__ bfrag, const uint4* __restrict__ b2frag,
+                                                        float* __restrict__ vout, float* __restrict__ sout,
+                                                        float* __restrict__ sink, unsigned* __restrict__ maxdiff, int reps)
 {
     extern __shared__ __align__(16) float fb_sm[];
     float* us = fb_sm;                                               // [FB_UH][FB_US]
@@ -238,6 +265,8 @@ __global__ void __launch_bounds__(MB_THREADS, 1) fb_fwd(const float* __restrict_
     for (int i = threadIdx.x; i < FB_UH * FB_US; i += MB_THREADS) us[i] = U[i];
     float2* cfs = reinterpret_cast<float2*>(bs + FB_NKS * FB_NNT * 32);   // [FB_NK / 2][FB_CSTRIDE]
     for (int i = threadIdx.x; i < FB_NKS * FB_NNT * 32; i += MB_THREADS) bs[i] = bfrag[i];
+    uint4* b2s = reinterpret_cast<uint4*>(cfs + FB_NK / 2 * FB_CSTRIDE);   // [3][FB_SNT][32]
+    for (int i = threadIdx.x; i < 3 * FB_SNT * 32; i += MB_THREADS) b2s[i] = b2frag[i];
     for (int i = threadIdx.x; i < FB_NK / 2 * FB_CSTRIDE; i += MB_THREADS)
         cfs[i] = make_float2(0.01f * (float)(i % 13) - 0.05f, 0.02f * (float)(i % 7) - 0.06f);
     __syncthreads();
@@ -315,6 +344,52 @@ __global__ void __launch_bounds__(MB_THREADS, 1) fb_fwd(const float* __restrict_
                     }
                 }
             }
+            if (SCATTER) {   // S[px][tap] = sum_f v_f(px) K_f[tap]: two n-tiles of accumulators ARE the A fragment of one k-step
+#pragma unroll
+                for (int m = 0; m < FB_MT; ++m) {
+                    if (!PHI) {
+#pragma unroll
+                        for (int n = 0; n < FB_NNT; ++n)
+#pragma unroll
+                            for (int q = 0; q < 4; ++q) acc[m][n][q] *= 0.004f;       // stand-in for v on its scale
+                    }
+                    float S[FB_SNT][4];
+#pragma unroll
+                    for (int n = 0; n < FB_SNT; ++n)
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) S[n][q] = 0.f;
+#pragma unroll
+                    for (int s3 = 0; s3 < 3; ++s3) {
+                        unsigned vh[4], vl[4];
+                        fb_split2(acc[m][2 * s3][0], acc[m][2 * s3][1], vh[0], vl[0]);
+                        fb_split2(acc[m][2 * s3][2], acc[m][2 * s3][3], vh[1], vl[1]);
+                        fb_split2(acc[m][2 * s3 + 1][0], acc[m][2 * s3 + 1][1], vh[2], vl[2]);
+                        fb_split2(acc[m][2 * s3 + 1][2], acc[m][2 * s3 + 1][3], vh[3], vl[3]);
+#pragma unroll
+                        for (int n = 0; n < FB_SNT; ++n) {
+                            const uint4 b = b2s[(s3 * FB_SNT + n) * 32 + lane];
+                            fb_mma(S[n], vh, b.x, b.y);
+                            fb_mma(S[n], vh, b.z, b.w);
+                            fb_mma(S[n], vl, b.x, b.y);
+                        }
+                    }
+                    if (CHECK) {
+                        const int mt = mt0 + m, y = mt / (FB_TW / 16), x0 = (mt % (FB_TW / 16)) * 16;
+#pragma unroll
+                        for (int n = 0; n < FB_NNT; ++n)
+#pragma unroll
+                            for (int q = 0; q < 4; ++q)
+                                vout[(size_t)(y * FB_TW + x0 + g + 8 * (q >> 1)) * FB_NK + 8 * n + 2 * c + (q & 1)] = acc[m][n][q];
+#pragma unroll
+                        for (int n = 0; n < FB_SNT; ++n)
+#pragma unroll
+                            for (int q = 0; q < 4; ++q)
+                                sout[(size_t)(y * FB_TW + x0 + g + 8 * (q >> 1)) * 56 + 8 * n + 2 * c + (q & 1)] = S[n][q];
+                    }
+#pragma unroll
+                    for (int n = 0; n < FB_SNT; ++n) total += (S[n][0] + S[n][1]) + (S[n][2] + S[n][3]);
+                }
+            }
 #pragma unroll
             for (int m = 0; m < FB_MT; ++m)
 #pragma unroll
@@ -324,19 +399,24 @@ __global__ void __launch_bounds__(MB_THREADS, 1) fb_fwd(const float* __restrict_
     if (total == 123.456f) sink[0] = total;
 }
 
-cudaError_t run_fwd_bank_probe(bool with_phi, double* rate, cudaStream_t st, unsigned long long* launches, int sms)
+cudaError_t run_fwd_bank_probe(int which, double* rate, cudaStream_t st, unsigned long long* launches, int sms)
 {
     float *U = nullptr, *kf = nullptr, *sink = nullptr;
-    uint4* bfrag = nullptr;
+    uint4 *bfrag = nullptr, *b2frag = nullptr;
+    float *vbuf = nullptr, *sbuf = nullptr;
     unsigned* maxdiff = nullptr;
     cudaError_t e = cudaMalloc(&U, (size_t)FB_UH * FB_US * 4);
     if (e == cudaSuccess) e = cudaMalloc(&kf, FB_NK * 49 * 4);
     if (e == cudaSuccess) e = cudaMalloc(&sink, 4);
     if (e == cudaSuccess) e = cudaMalloc(&bfrag, (size_t)FB_NKS * FB_NNT * 32 * 16);
     if (e == cudaSuccess) e = cudaMalloc(&maxdiff, 4);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fb_fwd<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, FB_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fb_fwd<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, FB_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(fb_fwd<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, FB_SMEM);
+    if (e == cudaSuccess) e = cudaMalloc(&b2frag, (size_t)3 * FB_SNT * 32 * 16);
+    if (e == cudaSuccess) e = cudaMalloc(&vbuf, (size_t)FB_TH * FB_TW * FB_NK * 4);
+    if (e == cudaSuccess) e = cudaMalloc(&sbuf, (size_t)FB_TH * FB_TW * 56 * 4);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fb_fwd<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, FB_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fb_fwd<false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, FB_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fb_fwd<false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, FB_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fb_fwd<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, FB_SMEM);
     float best_ms = 1e30f;
     unsigned diff_bits = 0;
     if (e == cudaSuccess) {
@@ -344,14 +424,16 @@ cudaError_t run_fwd_bank_probe(bool with_phi, double* rate, cudaStream_t st, uns
         cudaEventCreate(&e0);
         cudaEventCreate(&e1);
         cudaMemsetAsync(maxdiff, 0, 4, st);
-        fb_init<<<1, 512, 0, st>>>(U, kf, bfrag);
-        fb_fwd<true, false><<<1, MB_THREADS, FB_SMEM, st>>>(U, kf, bfrag, sink, maxdiff, 1);
-        *launches += 2;
+        fb_init<<<1, 512, 0, st>>>(U, kf, bfrag, b2frag);
+        fb_fwd<true, false, true><<<1, MB_THREADS, FB_SMEM, st>>>(U, kf, bfrag, b2frag, vbuf, sbuf, sink, maxdiff, 1);
+        fb_check_s<<<(FB_TH * FB_TW + 255) / 256, 256, 0, st>>>(vbuf, sbuf, kf, maxdiff);
+        *launches += 3;
         const int reps = 16;
         for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {   // rep 0 = warm-up
             cudaEventRecord(e0, st);
-            if (with_phi) fb_fwd<false, true><<<sms, MB_THREADS, FB_SMEM, st>>>(U, kf, bfrag, sink, maxdiff, reps);
-            else fb_fwd<false, false><<<sms, MB_THREADS, FB_SMEM, st>>>(U, kf, bfrag, sink, maxdiff, reps);
+            if (which == 7) fb_fwd<false, true, true><<<sms, MB_THREADS, FB_SMEM, st>>>(U, kf, bfrag, b2frag, vbuf, sbuf, sink, maxdiff, reps);
+            else if (which == 6) fb_fwd<false, true, false><<<sms, MB_THREADS, FB_SMEM, st>>>(U, kf, bfrag, b2frag, vbuf, sbuf, sink, maxdiff, reps);
+            else fb_fwd<false, false, false><<<sms, MB_THREADS, FB_SMEM, st>>>(U, kf, bfrag, b2frag, vbuf, sbuf, sink, maxdiff, reps);
             ++*launches;
             cudaEventRecord(e1, st);
             e = cudaEventSynchronize(e1);
@@ -366,7 +448,7 @@ cudaError_t run_fwd_bank_probe(bool with_phi, double* rate, cudaStream_t st, uns
         if (e == cudaSuccess) e = cudaGetLastError();
         *rate = (double)sms * reps * FB_TH * FB_TW / ((double)best_ms * 1e-3);      // pixels (48 responses each) per second
     }
-    cudaFree(U); cudaFree(kf); cudaFree(sink); cudaFree(bfrag); cudaFree(maxdiff);
+    cudaFree(U); cudaFree(kf); cudaFree(sink); cudaFree(bfrag); cudaFree(maxdiff); cudaFree(b2frag); cudaFree(vbuf); cudaFree(sbuf);
     if (e != cudaSuccess) return e;
     float diff;
     memcpy(&diff, &diff_bits, 4);
@@ -383,7 +465,7 @@ cudaError_t run_microbench(int which, double* rate, cudaStream_t st, unsigned lo
     if (e != cudaSuccess) return e;
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) return e;
-    if (which >= 5) return run_fwd_bank_probe(which == 6, rate, st, launches, sms);
+    if (which >= 5) return run_fwd_bank_probe(which, rate, st, launches, sms);
     float* d_out = nullptr;
     e = cudaMalloc(&d_out, sizeof(float));
     if (e != cudaSuccess) return e;

@@ -242,6 +242,9 @@ def test_microbench_rates_are_sane(tnrd):
     fwd_phi = tnrd.tnrd_microbench(6)      # ... followed by the factorised phi on the accumulator fragments
     print(f"forward bank + factorised phi on the accumulators: {fwd_phi / 1e9:.2f} Gpixel/s (XU roofline {mufu / 720 / 1e9:.2f})")
     assert 1e9 < fwd_phi < min(fwd, mufu / 720)
+    no_fold = tnrd.tnrd_microbench(7)      # ... followed by the transposed bank as a scatter table (fold not included)
+    print(f"forward bank + phi + scatter table (no fold): {no_fold / 1e9:.2f} Gpixel/s")
+    assert 1e9 < no_fold < fwd_phi
 
 
 # --- windowed phi evaluator (tnrd_set_phi_mode(1)): same oracle, same tolerance ------------------------------------
