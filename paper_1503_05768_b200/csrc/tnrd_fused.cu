@@ -31,6 +31,9 @@
 #include "tnrd_internal.h"
 #include "tnrd_device.cuh"
 
+#ifndef TNRD_SKIP_DEAD
+#define TNRD_SKIP_DEAD 0   // experiment: skip a phi group that is dead (Gaussian factor flushed to zero) for the whole warp
+#endif
 #ifndef TNRD_FACT_NP
 #define TNRD_FACT_NP 2   // pairs of responses per factorised-phi step (2 or 4)
 #endif
@@ -141,6 +144,14 @@ __device__ __forceinline__ float ex2_pos(float x)
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+// true if some response of some lane of the warp lies inside the clamp of the group anchored at -c0 (NaNs count as live)
+__device__ __forceinline__ bool fact_group_live(const float2 (&z)[4], float c0, float dmax, bool hasB)
+{
+    bool l = false;
+#pragma unroll
+    for (int p = 0; p < 4; ++p) l = l || !(fabsf(z[p].x + c0) >= dmax) || !(fabsf(z[p].y + c0) >= dmax);
+    return __any_sync(0xffffffffu, hasB && l);
+}
 template <int NP> struct FactStateN { float2 g[NP], rho[NP], rhoi[NP]; };
 using FactState = FactStateN<TNRD_FACT_NP>;   // of two pairs of responses: 2^{-d^2}, 2^{kappa d}, 2^{-kappa d}
 
@@ -195,7 +206,7 @@ template <int KS, class C>
 __device__ __forceinline__ void fact_block(const float* __restrict__ frec, float kappa, float dmax, const float2 (&zc)[4],
                                            float2 (&v)[4], const float* __restrict__ uwn, const float* __restrict__ tapsN,
                                            float2 (&zn)[4], const float* __restrict__ vw, const float* __restrict__ recp,
-                                           float2 (&acc)[4], bool hasB, bool hasN, bool hasC)
+                                           float2 (&acc)[4], bool hasB_, bool hasN, bool hasC)
 {
     constexpr int TS = C::TS, NGR = (KS - 1) / 2;
     static_assert(NGR <= TNRD_FG - 1, "not enough phi groups for the window rows");
@@ -203,6 +214,7 @@ __device__ __forceinline__ void fact_block(const float* __restrict__ frec, float
     FactState st;
     lds_vec(frec, fc);
 #if TNRD_FACT_NP == 4
+    const bool hasB = hasB_;
 #pragma unroll 1
     for (int g = 0; g < NGR; ++g) {
         if (hasB) fact_exp<0>(fc, kappa, dmax, zc, st);
@@ -230,6 +242,7 @@ __device__ __forceinline__ void fact_block(const float* __restrict__ frec, float
 #else
 #pragma unroll
     for (int g = 0; g < NGR; ++g) {
+        const bool hasB = TNRD_SKIP_DEAD ? fact_group_live(zc, fc[0], dmax, hasB_) : hasB_;
         if (hasB) fact_exp<0>(fc, kappa, dmax, zc, st);
         if (hasN) rowstep<KS, false>(uwn + (2 * g + 1) * C::US, tapsN + (KS - 2 * g - 1) * TS, zn);
         if (hasB) fact_poly<0>(fc, st, v);
@@ -242,6 +255,7 @@ __device__ __forceinline__ void fact_block(const float* __restrict__ frec, float
     }
 #pragma unroll 1
     for (int g = NGR; g < TNRD_FG - 1; ++g) {
+        const bool hasB = TNRD_SKIP_DEAD ? fact_group_live(zc, fc[0], dmax, hasB_) : hasB_;
         if (hasB) {
             fact_exp<0>(fc, kappa, dmax, zc, st);
             fact_poly<0>(fc, st, v);
@@ -250,6 +264,7 @@ __device__ __forceinline__ void fact_block(const float* __restrict__ frec, float
         }
         lds_vec(frec + (g + 1) * TNRD_FSTRIDE, fc);
     }
+    const bool hasB = TNRD_SKIP_DEAD ? fact_group_live(zc, fc[0], dmax, hasB_) : hasB_;
     if (hasB) fact_exp<0>(fc, kappa, dmax, zc, st);
     if (hasN) rowstep_half<KS, false, 0, 0>(uwn, tapsN + KS * TS, zn);                            // window row 0
     if (hasB) fact_poly<0>(fc, st, v);
