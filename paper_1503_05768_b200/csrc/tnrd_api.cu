@@ -1,6 +1,7 @@
 // tnrd_api.cu -- host side of libtnrd: the C ABI declared in include/tnrd.h.
 // Validation, per-(device, stream) scratch, parameter staging and the stage loop (row a6: PAPER.md:74, :184).
 // Every step of the path runs in this library's kernels; there is no CPU fallback.
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -13,12 +14,26 @@
 namespace {
 
 thread_local char g_cuda_err[512] = "";
-unsigned long long g_launches = 0;
-int g_kernel = 0;  // 0 auto, 1 reference, 2 fused
-int g_phi_mode = 3;  // 0 direct 63-term phi, 1 windowed evaluator (dense fallback decided on the device), 2 table,
-                     // 3 factorised 63-term phi (direct fallback inside the kernel)
-int g_basis = 0;     // 0 Gaussian radial basis, 1 triangular-shaped (table evaluator)
+// Process-wide options and counters: atomics, read ONCE at the entry of every call (Opts), so that a thread that toggles
+// a mode while another thread is inside a call cannot change that call half-way.
+std::atomic<unsigned long long> g_launches{0};
+std::atomic<int> g_kernel{0};    // 0 auto, 1 reference, 2 fused tile kernel (FMA pipe), 3 tensor-core stage kernel
+std::atomic<int> g_phi_mode{3};  // 0 direct 63-term phi, 1 windowed evaluator (dense fallback decided on the device), 2 table,
+                                 // 3 factorised 63-term phi (direct fallback inside the kernel)
+std::atomic<int> g_basis{0};     // 0 Gaussian radial basis, 1 triangular-shaped (table evaluator)
 std::mutex g_mu;
+
+struct Opts {
+    int kernel, phi_mode, basis;
+    Opts() : kernel(g_kernel.load()), phi_mode(g_phi_mode.load()), basis(g_basis.load()) {}
+    // evaluator of the fused kernel: the triangular basis always goes through the table
+    int phi() const { return (basis == 1 || phi_mode == 2) ? 2 : phi_mode; }
+};
+// kernels launched by one call; added to the process-wide counter when the call returns
+struct LaunchCount {
+    unsigned long long n = 0;
+    ~LaunchCount() { g_launches.fetch_add(n); }
+};
 
 int cuda_fail(cudaError_t e, const char* what)
 {
@@ -44,6 +59,8 @@ struct Scratch {
     int num_sms = 0;
     Buf prm, refv;                    // staged parameters, reference-path phi maps
     Buf split;                        // partial transposed-filter sums of the fused kernel's CTAs
+    Buf pp;                           // ping-pong image plane of the tensor-core kernel (it cannot run in place)
+    Buf tcws;                         // its Toeplitz operands, T stages
     Buf tab;                          // piecewise-linear phi tables [T][N_k][4096] float2 + 4 header floats
     Buf h_f, h_u, h_out, h_par;       // device staging of the host entry point
     Buf bw_maps, bw_part, bw_trace, bw_e[2];   // backward pass: P/V maps, per-CTA partial sums, iterates, dl/du planes
@@ -53,6 +70,11 @@ std::vector<Scratch*> g_scratch;
 int grow(Buf& b, size_t floats, cudaStream_t st)
 {
     if (floats <= b.cap) return TNRD_OK;
+    // An allocation made inside a stream capture would become a graph memory node whose pointer this cache then hands
+    // to later calls outside the graph: refuse, the caller warms the shape up before capturing (include/tnrd.h).
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone)
+        return cuda_fail(cudaErrorStreamCaptureUnsupported, "scratch growth during stream capture (run the shape once before capturing)");
     if (b.p) TNRD_CUDA(cudaFreeAsync(b.p, st));
     b.p = nullptr;
     b.cap = 0;
@@ -90,45 +112,103 @@ int check_shape(int B, int H, int W, int N_k, int ksize)
 
 int check_gamma(float g) { return (std::isfinite(g) && g > 0.0f) ? TNRD_OK : TNRD_ERR_PARAM; }
 
-// evaluator of the fused kernel for the current settings: the triangular basis always goes through the table
-int effective_phi() { return (g_basis == 1 || g_phi_mode == 2) ? 2 : g_phi_mode; }
+// Everything one call needs: the options as they were at its entry, its launch counter, scratch and stream.
+struct Call {
+    Opts o;
+    LaunchCount lc;
+    Scratch* sc = nullptr;
+    cudaStream_t st = nullptr;
+    bool tc = false;   // this call runs the tensor-core stage kernel
+};
 
-// Stages the parameters of T stages; with the table evaluator also builds the phi tables.
-int stage_params(Scratch* sc, const float* filters, const float* rbf_w, const float* rbf_mu, float gamma, int T, int N_k,
-                 int ksize, int phi, cudaStream_t st)
+// Which stage kernel a call uses.  kernel 3 forces the tensor-core kernel (TNRD_ERR_UNSUPPORTED where it does not apply),
+// 0 picks it when it applies and the image keeps its 128-lane strips busy: it needs the Gaussian basis with the
+// factorised evaluator, ksize 5 or 7 and N_k <= 48 (tnrd_tc.cu).
+int pick_kernel(Call& c, int B, int H, int W, int N_k, int ksize, int phi)
 {
-    int rc = grow(sc->prm, (size_t)T * N_k * tnrd::prm_stride(ksize), st);
-    if (rc != TNRD_OK) return rc;
-    TNRD_CUDA(tnrd::launch_prep(filters, rbf_w, rbf_mu, gamma, T, N_k, ksize, sc->prm.p, st, &g_launches));
-    if (phi == 2) {
-        const size_t n = (size_t)T * N_k * TNRD_TAB_NODES * 2;
-        if ((rc = grow(sc->tab, n + 4, st)) != TNRD_OK) return rc;
-        TNRD_CUDA(tnrd::launch_build_table(rbf_w, rbf_mu, gamma, T * N_k, g_basis, sc->tab.p + 4, sc->tab.p, st,
-                                           &g_launches));
+    const bool can = tnrd::tc_supported(N_k, ksize) && phi == 3 && c.o.basis == 0;
+    if (c.o.kernel == 3) {
+        if (!can) return TNRD_ERR_UNSUPPORTED;
+        c.tc = true;
+    } else if (c.o.kernel == 0 && can) {
+        // strips are 256 - 2r columns wide and every CTA recomputes 2r phi rows: worth it once the units fill the GPU
+        const tnrd::TcPlan pl = tnrd::plan_stage_tc(B, H, W, ksize, c.sc->num_sms);
+        c.tc = pl.units >= c.sc->num_sms && pl.seg_rows >= 24 && W >= 192;
     }
     return TNRD_OK;
 }
 
-// phi: evaluator (0, 1, 2); t = stage index inside the staged parameters (selects the table)
-int run_stage(Scratch* sc, tnrd::StageArgs a, int phi, int t, cudaStream_t st)
+// Stages the parameters of T stages; with the table evaluator also builds the phi tables, with the tensor-core kernel
+// the Toeplitz operands.
+int stage_params(Call& c, const float* filters, const float* rbf_w, const float* rbf_mu, float gamma, int T, int N_k,
+                 int ksize, int phi)
 {
-    const bool use_ref = (g_kernel == 1);
+    Scratch* sc = c.sc;
+    int rc = grow(sc->prm, (size_t)T * N_k * tnrd::prm_stride(ksize), c.st);
+    if (rc != TNRD_OK) return rc;
+    TNRD_CUDA(tnrd::launch_prep(filters, rbf_w, rbf_mu, gamma, T, N_k, ksize, sc->prm.p, c.st, &c.lc.n));
+    if (phi == 2) {
+        const size_t n = (size_t)T * N_k * TNRD_TAB_NODES * 2;
+        if ((rc = grow(sc->tab, n + 4, c.st)) != TNRD_OK) return rc;
+        TNRD_CUDA(tnrd::launch_build_table(rbf_w, rbf_mu, gamma, T * N_k, c.o.basis, sc->tab.p + 4, sc->tab.p, c.st,
+                                           &c.lc.n));
+    }
+    if (c.tc) {
+        if ((rc = grow(sc->tcws, (tnrd::tc_workspace_bytes(T, N_k, ksize) + 3) / 4, c.st)) != TNRD_OK) return rc;
+        TNRD_CUDA(tnrd::launch_tc_prep(sc->prm.p, T, N_k, ksize, reinterpret_cast<unsigned char*>(sc->tcws.p), c.st,
+                                       &c.lc.n));
+    }
+    return TNRD_OK;
+}
+
+// phi: evaluator (0 .. 3); t = stage index inside the staged parameters (selects the table / the operands)
+int run_stage(Call& c, tnrd::StageArgs a, int phi, int t)
+{
+    Scratch* sc = c.sc;
     if (phi == 2) {
         a.tabhdr = sc->tab.p;
         a.tab = sc->tab.p + 4 + (size_t)t * a.N_k * TNRD_TAB_NODES * 2;
     }
-    if (use_ref) {
-        if (g_basis == 1) return TNRD_ERR_UNSUPPORTED;     // the reference kernel knows the Gaussian basis only
-        int rc = grow(sc->refv, tnrd::ref_scratch_floats(a.B, a.H, a.W, a.N_k, a.ksize), st);
+    if (c.tc) {
+        if (a.u_out == a.u_in) return TNRD_ERR_ALIAS;        // callers ping-pong (run_stages)
+        const tnrd::TcPlan pl = tnrd::plan_stage_tc(a.B, a.H, a.W, a.ksize, sc->num_sms);
+        const unsigned char* ws = reinterpret_cast<const unsigned char*>(sc->tcws.p) +
+                                  (size_t)t * tnrd::tc_ws_stage_stride(a.N_k, a.ksize);
+        TNRD_CUDA(tnrd::launch_stage_tc(a, pl, ws, c.st, &c.lc.n));
+    } else if (c.o.kernel == 1) {
+        if (c.o.basis == 1) return TNRD_ERR_UNSUPPORTED;     // the reference kernel knows the Gaussian basis only
+        int rc = grow(sc->refv, tnrd::ref_scratch_floats(a.B, a.H, a.W, a.N_k, a.ksize), c.st);
         if (rc != TNRD_OK) return rc;
-        TNRD_CUDA(tnrd::launch_stage_ref(a, sc->refv.p, st, &g_launches));
+        TNRD_CUDA(tnrd::launch_stage_ref(a, sc->refv.p, c.st, &c.lc.n));
     } else {
         const tnrd::FusedPlan pl = tnrd::plan_stage_fused(a, sc->num_sms);
-        int rc = grow(sc->split, pl.part_floats, st);
+        int rc = grow(sc->split, pl.part_floats, c.st);
         if (rc != TNRD_OK) return rc;
-        TNRD_CUDA(tnrd::launch_stage_fused(a, pl, sc->split.p, phi, st, &g_launches));
+        TNRD_CUDA(tnrd::launch_stage_fused(a, pl, sc->split.p, phi, c.st, &c.lc.n));
     }
     return TNRD_OK;
+}
+
+// One stage from `src` to `dst` for the entry points that allow dst == src: the tile kernel runs in place (it only reads
+// u_{t-1} and stores partial sums; the point-wise update kernel follows it on the stream), the tensor-core kernel writes
+// u_t itself while other CTAs still read halos of u_{t-1}, so it goes through the ping-pong plane and is copied back.
+int run_stage_maybe_inplace(Call& c, tnrd::StageArgs a, int phi, int t)
+{
+    if (!c.tc || a.u_out != a.u_in) return run_stage(c, a, phi, t);
+    const size_t n = (size_t)a.B * a.H * a.W;
+    int rc = grow(c.sc->pp, n, c.st);
+    if (rc != TNRD_OK) return rc;
+    float* dst = a.u_out;
+    a.u_out = c.sc->pp.p;
+    if ((rc = run_stage(c, a, phi, t)) != TNRD_OK) return rc;
+    TNRD_CUDA(cudaMemcpyAsync(dst, c.sc->pp.p, n * sizeof(float), cudaMemcpyDeviceToDevice, c.st));
+    return TNRD_OK;
+}
+
+int open_call(Call& c, void* stream)
+{
+    c.st = (cudaStream_t)stream;
+    return get_scratch(c.st, &c.sc);
 }
 
 }  // namespace
@@ -144,13 +224,13 @@ int tnrd_stage(const float* f, const float* u_in, int B, int H, int W, int N_k, 
     if (rc != TNRD_OK) return rc;
     if ((rc = check_gamma(rbf_gamma)) != TNRD_OK) return rc;
     if (u_out == f) return TNRD_ERR_ALIAS;
-    cudaStream_t st = (cudaStream_t)stream;
-    Scratch* sc = nullptr;
-    if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
-    const int phi = effective_phi();
-    if ((rc = stage_params(sc, filters_t, rbf_w_t, rbf_mu, rbf_gamma, 1, N_k, ksize, phi, st)) != TNRD_OK) return rc;
-    tnrd::StageArgs a{f, u_in, u_out, sc->prm.p, nullptr, lambda_t, B, H, W, N_k, ksize};
-    return run_stage(sc, a, phi, 0, st);
+    Call c;
+    if ((rc = open_call(c, stream)) != TNRD_OK) return rc;
+    const int phi = c.o.phi();
+    if ((rc = pick_kernel(c, B, H, W, N_k, ksize, phi)) != TNRD_OK) return rc;
+    if ((rc = stage_params(c, filters_t, rbf_w_t, rbf_mu, rbf_gamma, 1, N_k, ksize, phi)) != TNRD_OK) return rc;
+    tnrd::StageArgs a{f, u_in, u_out, c.sc->prm.p, nullptr, lambda_t, B, H, W, N_k, ksize};
+    return run_stage_maybe_inplace(c, a, phi, 0);
 }
 
 int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, int N_k, int ksize,
@@ -170,18 +250,38 @@ int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, in
         if (out != u0) TNRD_CUDA(cudaMemcpyAsync(out, u0, n * sizeof(float), cudaMemcpyDeviceToDevice, st));
         return TNRD_OK;
     }
-    Scratch* sc = nullptr;
-    if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
+    Call c;
+    if ((rc = open_call(c, stream)) != TNRD_OK) return rc;
     const size_t rec = (size_t)N_k * tnrd::prm_stride(ksize);
-    const int phi = effective_phi();
-    if ((rc = stage_params(sc, filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, phi, st)) != TNRD_OK) return rc;
-    // Every stage writes `out`, from the second one on in place: the tile kernel only READS u_{t-1} (all halo reads
-    // happen there) and stores partial sums in scratch; the update kernel that follows it on the stream is point-wise.
+    const int phi = c.o.phi();
+    if ((rc = pick_kernel(c, B, H, W, N_k, ksize, phi)) != TNRD_OK) return rc;
+    if ((rc = stage_params(c, filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, phi)) != TNRD_OK) return rc;
     const float* src = u0;
+    if (!c.tc) {
+        // Tile kernel: every stage writes `out`, from the second one on in place: the tile kernel only READS u_{t-1} (all
+        // halo reads happen there) and stores partial sums in scratch; the update kernel that follows it is point-wise.
+        for (int t = 1; t <= T; ++t) {
+            tnrd::StageArgs a{f, src, out, c.sc->prm.p + (size_t)(t - 1) * rec, lambda + (t - 1), 0.0f, B, H, W, N_k, ksize};
+            if ((rc = run_stage(c, a, phi, t - 1)) != TNRD_OK) return rc;
+            src = out;
+        }
+        return TNRD_OK;
+    }
+    // Tensor-core kernel: u_t is written by the stage kernel itself, so stages alternate between `out` and one ping-pong
+    // plane such that stage T lands in `out`; when that would make stage 1 write the plane it reads (out == u0 and T odd)
+    // u0 is copied to the plane first.
+    if (T > 1 || out == u0)
+        if ((rc = grow(c.sc->pp, n, st)) != TNRD_OK) return rc;
+    float* pp = c.sc->pp.p;
+    if (out == u0 && (T & 1)) {
+        TNRD_CUDA(cudaMemcpyAsync(pp, u0, n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        src = pp;
+    }
     for (int t = 1; t <= T; ++t) {
-        tnrd::StageArgs a{f, src, out, sc->prm.p + (size_t)(t - 1) * rec, lambda + (t - 1), 0.0f, B, H, W, N_k, ksize};
-        if ((rc = run_stage(sc, a, phi, t - 1, st)) != TNRD_OK) return rc;
-        src = out;
+        float* dst = ((T - t) & 1) ? pp : out;
+        tnrd::StageArgs a{f, src, dst, c.sc->prm.p + (size_t)(t - 1) * rec, lambda + (t - 1), 0.0f, B, H, W, N_k, ksize};
+        if ((rc = run_stage(c, a, phi, t - 1)) != TNRD_OK) return rc;
+        src = dst;
     }
     return TNRD_OK;
 }
@@ -235,7 +335,8 @@ int tnrd_qcs_project(const float* y, int B, int H, int W, const float* qcs_lo, c
     if (!y || !qcs_lo || !qcs_hi || !u_out) return TNRD_ERR_NULL;
     if (B < 1 || H < 8 || W < 8 || (H % 8) || (W % 8) || (long long)B * H * W >= (1LL << 31)) return TNRD_ERR_SHAPE;
     if (u_out == qcs_lo || u_out == qcs_hi) return TNRD_ERR_ALIAS;
-    TNRD_CUDA(tnrd::launch_qcs_project(y, qcs_lo, qcs_hi, u_out, B, H, W, (cudaStream_t)stream, &g_launches));
+    LaunchCount lc;
+    TNRD_CUDA(tnrd::launch_qcs_project(y, qcs_lo, qcs_hi, u_out, B, H, W, (cudaStream_t)stream, &lc.n));
     return TNRD_OK;
 }
 
@@ -257,29 +358,43 @@ int tnrd_deblock_diffuse(const float* u0, int B, int H, int W, int T, int N_k, i
         if (out != u0) TNRD_CUDA(cudaMemcpyAsync(out, u0, n * sizeof(float), cudaMemcpyDeviceToDevice, st));
         return TNRD_OK;
     }
-    Scratch* sc = nullptr;
-    if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
+    Call c;
+    if ((rc = open_call(c, stream)) != TNRD_OK) return rc;
     const size_t rec = (size_t)N_k * tnrd::prm_stride(ksize);
-    const int phi = effective_phi();
-    if ((rc = stage_params(sc, filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, phi, st)) != TNRD_OK) return rc;
-    // Per stage (Supp. Eq. 29): the stage kernels with lambda = 0 write y = u - sum_i kbar_i * phi_i(k_i * u) to `out`
-    // (f is then irrelevant: u itself is passed; in place from the second stage on, as in tnrd_diffuse), the projection
-    // kernel turns it into u_t = D^T eta(D y) in place.
+    const int phi = c.o.phi();
+    if ((rc = pick_kernel(c, B, H, W, N_k, ksize, phi)) != TNRD_OK) return rc;
+    if ((rc = stage_params(c, filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, phi)) != TNRD_OK) return rc;
+    // Per stage (Supp. Eq. 29): the stage kernels with lambda = 0 write y = u - sum_i kbar_i * phi_i(k_i * u) (f is then
+    // irrelevant: u itself is passed), the projection kernel turns it into u_t = D^T eta(D y) in place.  Buffers as in
+    // tnrd_diffuse: in place with the tile kernel, alternating between `out` and the ping-pong plane with the
+    // tensor-core kernel.
+    float* pp = nullptr;
     const float* src = u0;
+    if (c.tc && (T > 1 || out == u0)) {
+        if ((rc = grow(c.sc->pp, n, st)) != TNRD_OK) return rc;
+        pp = c.sc->pp.p;
+        if (out == u0 && (T & 1)) {
+            TNRD_CUDA(cudaMemcpyAsync(pp, u0, n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+            src = pp;
+        }
+    }
     for (int t = 1; t <= T; ++t) {
-        tnrd::StageArgs a{src, src, out, sc->prm.p + (size_t)(t - 1) * rec, nullptr, 0.0f, B, H, W, N_k, ksize};
-        if ((rc = run_stage(sc, a, phi, t - 1, st)) != TNRD_OK) return rc;
-        TNRD_CUDA(tnrd::launch_qcs_project(out, qcs_lo, qcs_hi, out, B, H, W, st, &g_launches));
-        src = out;
+        float* dst = (c.tc && ((T - t) & 1)) ? pp : out;
+        tnrd::StageArgs a{src, src, dst, c.sc->prm.p + (size_t)(t - 1) * rec, nullptr, 0.0f, B, H, W, N_k, ksize};
+        if ((rc = run_stage(c, a, phi, t - 1)) != TNRD_OK) return rc;
+        TNRD_CUDA(tnrd::launch_qcs_project(dst, qcs_lo, qcs_hi, dst, B, H, W, st, &c.lc.n));
+        src = dst;
     }
     return TNRD_OK;
 }
 
 // Backward pass of one stage on staged parameters (shared by tnrd_stage_backward and tnrd_diffuse_backward).
-static int run_stage_backward(Scratch* sc, const float* f, const float* u, const float* e, int B, int H, int W, int N_k,
+static int run_stage_backward(Call& c, const float* f, const float* u, const float* e, int B, int H, int W, int N_k,
                               int ksize, const float* prm, const float* lambda_ptr, float lambda_val, float gamma,
-                              float* g_u, float* g_k, float* g_w, float* g_l, cudaStream_t st)
+                              float* g_u, float* g_k, float* g_w, float* g_l)
 {
+    Scratch* sc = c.sc;
+    cudaStream_t st = c.st;
     const tnrd::BwdPlan pl = tnrd::plan_stage_bwd(B, H, W, N_k, ksize, sc->num_sms);
     const int R = (ksize - 1) / 2, KK = ksize * ksize;
     const bool want_k = g_k != nullptr, want_w = g_w != nullptr || want_k;
@@ -295,11 +410,11 @@ static int run_stage_backward(Scratch* sc, const float* f, const float* u, const
     tnrd::BwdArgs a{f, u, e, g_u, prm, lambda_ptr, lambda_val, B, H, W, N_k, ksize,
                     want_k ? sc->bw_maps.p : nullptr, want_k ? sc->bw_maps.p + map : nullptr,
                     want_w ? part_w : nullptr, g_l ? part_l : nullptr};
-    TNRD_CUDA(tnrd::launch_stage_bwd(a, pl, part_k, st, &g_launches));
+    TNRD_CUDA(tnrd::launch_stage_bwd(a, pl, part_k, st, &c.lc.n));
     if (want_w || g_l) {
         const float s = sqrtf(1.4426950408889634f / (2.0f * gamma * gamma));
         TNRD_CUDA(tnrd::launch_reduce_partials(part_w, pl.n_cta, part_k, pl.G, part_l, N_k, ksize, s, g_w, g_k, g_l, st,
-                                               &g_launches));
+                                               &c.lc.n));
     }
     return TNRD_OK;
 }
@@ -314,14 +429,13 @@ int tnrd_stage_backward(const float* f, const float* u_in, const float* e, int B
     if (rc != TNRD_OK) return rc;
     if ((rc = check_gamma(rbf_gamma)) != TNRD_OK) return rc;
     if (grad_u && (grad_u == u_in || grad_u == e || grad_u == f)) return TNRD_ERR_ALIAS;
-    if (g_basis == 1) return TNRD_ERR_UNSUPPORTED;          // gradients exist for the Gaussian basis only
-    cudaStream_t st = (cudaStream_t)stream;
-    Scratch* sc = nullptr;
-    if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
-    if ((rc = grow(sc->prm, (size_t)N_k * tnrd::prm_stride(ksize), st)) != TNRD_OK) return rc;
-    TNRD_CUDA(tnrd::launch_prep(filters_t, rbf_w_t, rbf_mu, rbf_gamma, 1, N_k, ksize, sc->prm.p, st, &g_launches));
-    return run_stage_backward(sc, f, u_in, e, B, H, W, N_k, ksize, sc->prm.p, nullptr, lambda_t, rbf_gamma, grad_u,
-                              grad_filters, grad_w, grad_lambda, st);
+    Call c;
+    if (c.o.basis == 1) return TNRD_ERR_UNSUPPORTED;          // gradients exist for the Gaussian basis only
+    if ((rc = open_call(c, stream)) != TNRD_OK) return rc;
+    if ((rc = grow(c.sc->prm, (size_t)N_k * tnrd::prm_stride(ksize), c.st)) != TNRD_OK) return rc;
+    TNRD_CUDA(tnrd::launch_prep(filters_t, rbf_w_t, rbf_mu, rbf_gamma, 1, N_k, ksize, c.sc->prm.p, c.st, &c.lc.n));
+    return run_stage_backward(c, f, u_in, e, B, H, W, N_k, ksize, c.sc->prm.p, nullptr, lambda_t, rbf_gamma, grad_u,
+                              grad_filters, grad_w, grad_lambda);
 }
 
 int tnrd_diffuse_backward(const float* f, const float* u0, const float* u_gt, const float* e_T, int B, int H, int W,
@@ -336,32 +450,41 @@ int tnrd_diffuse_backward(const float* f, const float* u0, const float* u_gt, co
     if (rc != TNRD_OK) return rc;
     if ((rc = check_gamma(rbf_gamma)) != TNRD_OK) return rc;
     if (grad_u0 && (grad_u0 == u0 || grad_u0 == f || grad_u0 == e_T || grad_u0 == u_gt)) return TNRD_ERR_ALIAS;
-    if (u_T && (u_T == u0 || u_T == f)) return TNRD_ERR_ALIAS;
-    if (g_basis == 1) return TNRD_ERR_UNSUPPORTED;          // gradients exist for the Gaussian basis only
-    cudaStream_t st = (cudaStream_t)stream;
-    Scratch* sc = nullptr;
-    if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
+    // u_T is written before u_gt / e_T are read and before grad_u0 is formed
+    if (u_T && (u_T == u0 || u_T == f || u_T == u_gt || u_T == e_T || u_T == grad_u0)) return TNRD_ERR_ALIAS;
+    Call c;
+    if (c.o.basis == 1) return TNRD_ERR_UNSUPPORTED;          // gradients exist for the Gaussian basis only
+    if ((rc = open_call(c, stream)) != TNRD_OK) return rc;
+    Scratch* sc = c.sc;
+    cudaStream_t st = c.st;
     const size_t n = (size_t)B * H * W, rec = (size_t)N_k * tnrd::prm_stride(ksize);
     const int KK = ksize * ksize;
-    if ((rc = grow(sc->prm, (size_t)T * rec, st)) != TNRD_OK) return rc;
+    // the forward pass of a gradient is an exact evaluator (factorised, direct, or windowed if selected), never the table
+    const int phi = c.o.phi_mode == 2 ? 3 : c.o.phi_mode;
+    if ((rc = pick_kernel(c, B, H, W, N_k, ksize, phi)) != TNRD_OK) return rc;
     if ((rc = grow(sc->bw_trace, (size_t)T * n, st)) != TNRD_OK) return rc;     // u_1 .. u_T
     if ((rc = grow(sc->bw_e[0], n, st)) != TNRD_OK) return rc;
     if ((rc = grow(sc->bw_e[1], n, st)) != TNRD_OK) return rc;
-    TNRD_CUDA(tnrd::launch_prep(filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, sc->prm.p, st, &g_launches));
+    {
+        Opts keep = c.o;
+        c.o.basis = 0;                                          // stage_params builds no table: phi != 2 here
+        rc = stage_params(c, filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, phi);
+        c.o = keep;
+        if (rc != TNRD_OK) return rc;
+    }
     // forward, keeping every iterate (Supp. Eq. 21 needs u_{t-1} of every stage)
     const float* src = u0;
     for (int t = 1; t <= T; ++t) {
         float* dst = sc->bw_trace.p + (size_t)(t - 1) * n;
         tnrd::StageArgs a{f, src, dst, sc->prm.p + (size_t)(t - 1) * rec, lambda + (t - 1), 0.0f, B, H, W, N_k, ksize};
-        // the forward pass of a gradient is an exact evaluator (factorised, direct, or windowed if selected), never the table
-        if ((rc = run_stage(sc, a, g_phi_mode == 2 ? 3 : g_phi_mode, t - 1, st)) != TNRD_OK) return rc;
+        if ((rc = run_stage(c, a, phi, t - 1)) != TNRD_OK) return rc;
         src = dst;
     }
     if (u_T) TNRD_CUDA(cudaMemcpyAsync(u_T, src, n * sizeof(float), cudaMemcpyDeviceToDevice, st));
     // e_T = dl/du_T: given, or u_T - u_gt for the loss 1/2 ||u_T - u_gt||^2 (Supp. Eq. 3, 20)
     const float* e = e_T;
     if (u_gt) {
-        TNRD_CUDA(tnrd::launch_sub(src, u_gt, sc->bw_e[0].p, n, st, &g_launches));
+        TNRD_CUDA(tnrd::launch_sub(src, u_gt, sc->bw_e[0].p, n, st, &c.lc.n));
         e = sc->bw_e[0].p;
     }
     // backward recurrence (Supp. Eq. 21): e_{t-1} = (du_t/du_{t-1})^T e_t; parameter gradients of stage t from (u_{t-1}, e_t)
@@ -370,11 +493,11 @@ int tnrd_diffuse_backward(const float* f, const float* u0, const float* u_gt, co
         float* g_u;
         if (t == 1) g_u = grad_u0;                                   // may be null: not needed then
         else g_u = (e == sc->bw_e[0].p) ? sc->bw_e[1].p : sc->bw_e[0].p;
-        rc = run_stage_backward(sc, f, u_prev, e, B, H, W, N_k, ksize, sc->prm.p + (size_t)(t - 1) * rec,
+        rc = run_stage_backward(c, f, u_prev, e, B, H, W, N_k, ksize, sc->prm.p + (size_t)(t - 1) * rec,
                                 lambda + (t - 1), 0.0f, rbf_gamma, g_u,
                                 grad_filters ? grad_filters + (size_t)(t - 1) * N_k * KK : nullptr,
                                 grad_w ? grad_w + (size_t)(t - 1) * N_k * TNRD_NUM_RBF : nullptr,
-                                grad_lambda ? grad_lambda + (t - 1) : nullptr, st);
+                                grad_lambda ? grad_lambda + (t - 1) : nullptr);
         if (rc != TNRD_OK) return rc;
         e = g_u;
     }
@@ -398,7 +521,7 @@ int tnrd_plan_query(int B, int H, int W, int N_k, int ksize, int num_sms, long l
 
 int tnrd_set_kernel(int which)
 {
-    if (which < 0 || which > 2) return TNRD_ERR_UNSUPPORTED;
+    if (which < 0 || which > 3) return TNRD_ERR_UNSUPPORTED;
     g_kernel = which;
     return TNRD_OK;
 }
@@ -424,7 +547,8 @@ int tnrd_microbench(int which, double* rate, void* stream)
 {
     if (!rate) return TNRD_ERR_NULL;
     if (which < 0 || which > 7) return TNRD_ERR_UNSUPPORTED;
-    TNRD_CUDA(tnrd::run_microbench(which, rate, (cudaStream_t)stream, &g_launches));
+    LaunchCount lc;
+    TNRD_CUDA(tnrd::run_microbench(which, rate, (cudaStream_t)stream, &lc.n));
     return TNRD_OK;
 }
 
@@ -452,7 +576,7 @@ void tnrd_shutdown(void)
     (void)cudaGetDevice(&cur);
     for (Scratch* s : g_scratch) {
         (void)cudaSetDevice(s->dev);
-        Buf* bufs[] = {&s->prm, &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->refv, &s->split, &s->tab, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
+        Buf* bufs[] = {&s->pp, &s->tcws, &s->prm, &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->refv, &s->split, &s->tab, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
         for (Buf* b : bufs)
             if (b->p) (void)cudaFree(b->p);   // synchronising free: the stream may be gone by now
         delete s;

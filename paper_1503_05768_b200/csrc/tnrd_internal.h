@@ -127,6 +127,24 @@ cudaError_t launch_qcs_project(const float* y, const float* lo, const float* hi,
 cudaError_t launch_build_table(const float* rbf_w, const float* rbf_mu, float gamma, int TN, int basis, float* tab,
                                float* hdr, cudaStream_t st, unsigned long long* launches);
 cudaError_t fused_init();   // opt-in shared memory attributes; idempotent
+
+// ---- tensor-core stage kernel (tnrd_tc.cu): both filterings as tcgen05 implicit GEMMs, update fused in ----------
+// A unit = (image, row segment, strip of 256 - 2r output columns); one CTA per unit.
+struct TcPlan {
+    int nxs, nys, seg_rows;   // strips per image, row segments per image, output rows per segment
+    long long units;          // CTAs
+    double cost_rows;         // waves x (rows per CTA incl. recomputed ones + per-CTA constant), the planner's objective
+};
+bool tc_supported(int N_k, int ksize);                       // ksize 5 or 7, N_k <= 48
+size_t tc_workspace_bytes(int T, int N_k, int ksize);        // Toeplitz operands of T stages
+size_t tc_ws_stage_stride(int N_k, int ksize);               // bytes per stage inside that workspace
+TcPlan plan_stage_tc(int B, int H, int W, int ksize, int num_sms);
+// prm = staged records of T stages (launch_prep); ws receives the operands
+cudaError_t launch_tc_prep(const float* prm, int T, int N_k, int ksize, unsigned char* ws, cudaStream_t st,
+                           unsigned long long* launches);
+// one stage; a.u_out must not alias a.u_in (the kernel reads halos of u_in while other CTAs write u_out)
+cudaError_t launch_stage_tc(const StageArgs& a, const TcPlan& pl, const unsigned char* ws_t, cudaStream_t st,
+                            unsigned long long* launches);
 cudaError_t run_microbench(int which, double* rate, cudaStream_t st, unsigned long long* launches);
 
 }  // namespace tnrd

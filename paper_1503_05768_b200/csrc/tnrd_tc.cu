@@ -1,0 +1,592 @@
+// tnrd_tc.cu -- the stage kernel with both filterings on the 5th-generation tensor cores (tcgen05.mma, accumulators
+// in tensor memory) and the update fused in: rows a1-a5 of the hot path in ONE pass, u_t written by the same kernel.
+//
+//   u_t = u - ( sum_i kbar_i * phi_i(k_i * u~) + lambda (u - f) )          Main Eq. 7
+//
+// The two filterings are the only dense contractions of the path (PAPER.md:70 "K_i u <=> k_i * u", :125 the rot180
+// bank, :387-389 the patch-matrix form U k); everything else is the point-wise influence function.
+// One CTA owns a column strip of 256 phi columns (128 tensor-memory lanes x 2 pixels) and walks down it two phi rows
+// (one "batch" = 512 pixels) at a time:
+//
+//   a1  loader warps gather u rows through the mirror map into a ring of shared-memory rows,
+//       as 16-byte CELLS (row, g) = u~[row][2g .. 2g+3] -- every pixel twice, so that the 4-pixel window of ANY
+//       even column starts on a 16-byte boundary -- split x = hi + lo with hi = the top 19 bits (a TF32 number);
+//   a2  z = k * u~ as an implicit GEMM with NO im2col: M = 128 lanes (pixel pairs), K = (tap row a, window column
+//       c = 0..7) read straight from the cell ring by a K-major, unswizzled shared-memory descriptor whose two 16-byte
+//       chunks are the cells g and g + 2 (the window u~[row + a][2g .. 2g+7]), N = (filter i, pixel j of the pair) with
+//       the Toeplitz operand B[(a, c)][(i, j)] = k_i[K-1-a][K-1-(c-j)].  Three TF32 products hi*hi + hi*lo + lo*hi with
+//       fp32 accumulation in tensor memory: fp32-level accuracy (a single TF32 pass would not hold the tolerance).
+//   a3  phi warps read z from tensor memory (tcgen05.ld), evaluate all 63 Gaussians by the factorised form
+//       (tnrd_internal.h "fact": 3 ex2 per group of 13 centres, groups that are dead for the whole warp skipped), and
+//       write v = phi(z) back IN PLACE as BF16 pairs (hi, lo) (tcgen05.st);
+//   a4  the transposed bank as a SCATTER table, A = v straight from tensor memory (no shared-memory round trip):
+//       T[lane][(a, xo)] = sum_{i,j} v_i[pixel j of the lane] k_i[a][j + 2r - xo] is what the lane's two pixels add
+//       to output row py - a at columns 2g - 2r + xo.  The fold over a happens inside tensor memory (the two rows of
+//       a batch accumulate into the same table one 8-column block apart), the fold over neighbouring lanes and over
+//       batches in shared memory, in a fixed order (deterministic, no atomics);
+//   a5  the thread that completes an output pixel applies the reaction term and writes u_t.
+//
+// Strips overlap by 2r phi columns and row segments by 2r phi rows (recomputed) so that a CTA completes its own
+// outputs: no partial sums in HBM, no second kernel, 12 B of DRAM traffic per pixel-stage.
+// Warp roles: 16 phi warps (4 per tensor-memory lane quarter, each a quarter of the filters), 1 MMA-issuing warp,
+// 2 loader warps; mbarrier pipelines between them (u row pairs, z double-buffered, scatter table).
+#include <cuda_bf16.h>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+
+#include "tnrd_internal.h"
+#include "tnrd_device.cuh"
+
+namespace tnrd {
+
+namespace {
+
+constexpr int TC_PHI_WARPS = 16, TC_LOAD_WARPS = 2;
+constexpr int TC_MMA_WARP = TC_PHI_WARPS;                       // warp index of the MMA issuer
+constexpr int TC_THREADS = (TC_PHI_WARPS + 1 + TC_LOAD_WARPS) * 32;
+constexpr int TC_CW = 132;                                      // cells per ring row (130 used)
+constexpr int TC_CWU = 130;
+constexpr int TC_NP = 6;                                        // row pairs in the ring
+constexpr int TC_NKP_MAX = 48;                                  // filters (padded to a multiple of 8)
+constexpr int TC_TCOL = 8 * TC_NKP_MAX;                         // first tensor-memory column of the scatter table
+
+template <int KS>
+struct TcCfg {
+    static constexpr int R = (KS - 1) / 2;
+    static constexpr int OW = 256 - 2 * R;                      // output columns a strip completes
+    static constexpr int NSB = KS + 1;                          // 8-column blocks of one scatter MMA (the last one is padding)
+    static constexpr int NSC = 8 * NSB;                         // its N
+    static constexpr int XK = R + 1;                            // float2 slots per (block, lane) of the exchange buffer
+    static constexpr int PRM = prm_stride(KS);
+    // shared memory (bytes)
+    static constexpr int SM_UHI = 0;
+    static constexpr int U_BYTES = TC_NP * 2 * TC_CW * 16;
+    static constexpr int SM_ULO = SM_UHI + U_BYTES;
+    static constexpr int SM_BFH = SM_ULO + U_BYTES;
+    static constexpr int BF_BYTES = KS * 2 * (2 * TC_NKP_MAX) * 16;
+    static constexpr int SM_BFL = SM_BFH + BF_BYTES;
+    static constexpr int SM_BS = SM_BFL + BF_BYTES;
+    static constexpr int BS_BYTES = TC_NKP_MAX * NSC * 16;
+    static constexpr int SM_COEF = SM_BS + BS_BYTES;
+    static constexpr int COEF_BYTES = TC_NKP_MAX * TNRD_FG * TNRD_FSTRIDE * 4;
+    static constexpr int SM_X = SM_COEF + COEF_BYTES;
+    static constexpr int X_BYTES = (KS + 1) * XK * 128 * 8;
+    static constexpr int SM_O = SM_X + X_BYTES;
+    static constexpr int O_BYTES = 8 * 128 * 8;
+    static constexpr int SM_BAR = SM_O + O_BYTES;
+    static constexpr int SMEM = SM_BAR + 256;
+};
+
+// workspace of one stage (global memory, written by tc_prep_kernel): forward operand hi, lo (TF32), scatter operand
+__host__ __device__ constexpr size_t tc_ws_bf_bytes(int ks, int nkp) { return (size_t)ks * 2 * (2 * nkp) * 16; }
+__host__ __device__ constexpr size_t tc_ws_bs_bytes(int ks, int nkp) { return (size_t)nkp * (8 * (ks + 1)) * 16; }
+__host__ __device__ constexpr size_t tc_ws_stage_bytes(int ks, int nkp) { return 2 * tc_ws_bf_bytes(ks, nkp) + tc_ws_bs_bytes(ks, nkp); }
+
+// ---- PTX wrappers ----------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+// K-major, unswizzled operand: 8 rows of a core matrix 16 bytes apart, `sbo` between 8-row groups, `lbo` between
+// the two 16-byte K chunks of one MMA
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo)
+{
+    return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo >> 4) & 0x3FFF) << 16) |
+           ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) | ((uint64_t)1 << 46);
+}
+// instruction descriptor: fp32 accumulate, A and B K-major, fmt 1 = BF16, 2 = TF32
+__device__ __forceinline__ uint32_t umma_idesc(int fmt, int M, int N)
+{
+    return (1u << 4) | ((uint32_t)fmt << 7) | ((uint32_t)fmt << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+__device__ __forceinline__ void umma_tf32_ss(uint32_t d, uint64_t a, uint64_t b, uint32_t idesc, uint32_t acc)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}\n"
+                 :: "r"(d), "l"(a), "l"(b), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void umma_bf16_ts(uint32_t d, uint32_t a_tmem, uint64_t b, uint32_t idesc, uint32_t acc)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}\n"
+                 :: "r"(d), "r"(a_tmem), "l"(b), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t* bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\t"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+                 "@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}\n" :: "r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t (&r)[4])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                   "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                 : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t (&r)[4])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};"
+                 :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]) : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void bar_phi() { asm volatile("bar.sync 1, %0;" :: "n"(TC_PHI_WARPS * 32) : "memory"); }
+
+__device__ __forceinline__ float ex2f(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float clamp_nan(float x, float lim)          // NaN stays NaN
+{
+    float y;
+    asm("min.NaN.f32 %0, %1, %2;" : "=f"(y) : "f"(x), "f"(lim));
+    asm("max.NaN.f32 %0, %0, %1;" : "+f"(y) : "f"(-lim));
+    return y;
+}
+
+// Factorised influence function (tnrd_internal.h "fact"; PAPER.md:553 with equidistant centres, :117) of the two
+// response pairs z[0], z[1] of one filter; crec = the filter's TNRD_FG group records in shared memory (broadcast
+// loads).  A group whose Gaussian factor has flushed to zero for every response of the warp is skipped (its
+// contribution is an exact 0; NaN responses keep it live).
+__device__ __forceinline__ void tc_phi_fact(const float* __restrict__ crec, float kappa, float dmax, const float2 (&z)[2],
+                                            float2 (&v)[2])
+{
+    constexpr int S = TNRD_FS;
+#pragma unroll
+    for (int g = 0; g < TNRD_FG; ++g) {
+        float c[TNRD_FSTRIDE];
+        lds_vec(crec + g * TNRD_FSTRIDE, c);
+        const bool live = !(fabsf(z[0].x + c[0]) >= dmax) || !(fabsf(z[0].y + c[0]) >= dmax) ||
+                          !(fabsf(z[1].x + c[0]) >= dmax) || !(fabsf(z[1].y + c[0]) >= dmax);
+        if (!__any_sync(0xffffffffu, live)) continue;
+        float2 gg[2], rho[2], rhoi[2], h[2], hl[2];
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            float2 d = __fadd2_rn(z[p], make_float2(c[0], c[0]));
+            d = make_float2(clamp_nan(d.x, dmax), clamp_nan(d.y, dmax));
+            const float2 t = __fmul2_rn(d, d);
+            const float2 e = __fmul2_rn(d, make_float2(kappa, kappa));
+            gg[p] = make_float2(ex2f(-t.x), ex2f(-t.y));
+            rho[p] = make_float2(ex2f(e.x), ex2f(e.y));
+            rhoi[p] = make_float2(ex2f(-e.x), ex2f(-e.y));
+        }
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            h[p] = __ffma2_rn(make_float2(c[1], c[1]), rho[p], make_float2(c[2], c[2]));
+            hl[p] = __ffma2_rn(make_float2(c[S + 2], c[S + 2]), rhoi[p], make_float2(c[S + 3], c[S + 3]));
+        }
+#pragma unroll
+        for (int q = 2; q <= S; ++q)
+#pragma unroll
+            for (int p = 0; p < 2; ++p) h[p] = __ffma2_rn(h[p], rho[p], make_float2(c[1 + q], c[1 + q]));
+#pragma unroll
+        for (int q = 2; q < S; ++q)
+#pragma unroll
+            for (int p = 0; p < 2; ++p) hl[p] = __ffma2_rn(hl[p], rhoi[p], make_float2(c[S + 2 + q], c[S + 2 + q]));
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            h[p] = __ffma2_rn(hl[p], rhoi[p], h[p]);
+            v[p] = __ffma2_rn(gg[p], h[p], v[p]);
+        }
+    }
+}
+
+// Direct form (one ex2 per Gaussian) for centre sets the factorisation does not cover; (-mu', w') pairs from the
+// staged record in global memory (uniform loads).  Rare path.
+__device__ __forceinline__ void tc_phi_direct(const float* __restrict__ pairs, const float2 (&z)[2], float2 (&v)[2])
+{
+#pragma unroll 3
+    for (int j = 0; j < TNRD_M; ++j) {
+        const float2 mw = __ldg(reinterpret_cast<const float2*>(pairs) + j);
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            const float2 d = __fadd2_rn(z[p], make_float2(mw.x, mw.x));
+            const float2 t = __fmul2_rn(d, d);
+            v[p] = __ffma2_rn(make_float2(ex2f(-t.x), ex2f(-t.y)), make_float2(mw.y, mw.y), v[p]);
+        }
+    }
+}
+
+// v = (v.x, v.y) -> packed BF16 pairs: hi = (bf16(v.x) | bf16(v.y) << 16), lo = the same of the remainders
+__device__ __forceinline__ void split_bf16(float2 v, uint32_t& hi, uint32_t& lo)
+{
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(hi) : "f"(v.y), "f"(v.x));
+    const float hx = __uint_as_float(hi << 16), hy = __uint_as_float(hi & 0xFFFF0000u);
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(lo) : "f"(v.y - hy), "f"(v.x - hx));
+}
+
+// ---- operand staging kernel: Toeplitz operands of both banks from the staged records (scaled taps k' = s k) ------
+//   forward  BF[(2a + cc)][n = 2i + j][e]   = k'_i[K-1-a][K-1-(4cc + e - j)]   (TF32 hi / lo)
+//   scatter  BS[pass][kp / 8][n = 8 blk + xo][kp % 8],  kp = 4i + 2s + j  (s = 0: the hi half of v, 1: the lo half)
+//            = hi(k'_i[blk][j + 2r - xo]) for pass 0;  lo(k') for pass 1, s = 0;  0 for pass 1, s = 1
+__global__ void tc_prep_kernel(const float* __restrict__ prm, int T, int N_k, int nkp, int ks, unsigned char* __restrict__ ws)
+{
+    const int PRM = prm_stride(ks), R = (ks - 1) / 2, NSC = 8 * (ks + 1);
+    const size_t bfb = tc_ws_bf_bytes(ks, nkp), stb = tc_ws_stage_bytes(ks, nkp);
+    const int n_bf = ks * 2 * 2 * nkp * 4, n_bs = nkp * NSC * 8;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < T * (n_bf + n_bs); idx += gridDim.x * blockDim.x) {
+        const int t = idx / (n_bf + n_bs), q = idx - t * (n_bf + n_bs);
+        const float* rec = prm + (size_t)t * N_k * PRM;
+        unsigned char* wst = ws + (size_t)t * stb;
+        if (q < n_bf) {
+            const int e = q & 3, n = (q >> 2) % (2 * nkp), kc = (q >> 2) / (2 * nkp);
+            const int a = kc >> 1, cc = kc & 1, i = n >> 1, j = n & 1, b = 4 * cc + e - j;
+            float v = 0.0f;
+            if (i < N_k && b >= 0 && b < ks) v = rec[(size_t)i * PRM + prm_tap(ks, ks - 1 - a, ks - 1 - b)];
+            const float h = __uint_as_float(__float_as_uint(v) & 0xFFFFE000u);
+            reinterpret_cast<float*>(wst)[q] = h;
+            reinterpret_cast<float*>(wst + bfb)[q] = v - h;
+        } else {
+            const int qq = q - n_bf;
+            const int k8 = qq & 7, n = (qq >> 3) % NSC, kc = ((qq >> 3) / NSC) % (nkp / 2), pass = (qq >> 3) / NSC / (nkp / 2);
+            const int kp = 8 * kc + k8, i = kp >> 2, s = (kp >> 1) & 1, j = kp & 1, blk = n >> 3, xo = n & 7, b = j + 2 * R - xo;
+            float v = 0.0f;
+            if (i < N_k && blk < ks && b >= 0 && b < ks) v = rec[(size_t)i * PRM + prm_tap(ks, blk, b)];
+            const __nv_bfloat16 h = __float2bfloat16_rn(v);
+            const __nv_bfloat16 l = __float2bfloat16_rn(v - __bfloat162float(h));
+            reinterpret_cast<__nv_bfloat16*>(wst + 2 * bfb)[qq] = pass == 0 ? h : (s == 0 ? l : __float2bfloat16_rn(0.0f));
+        }
+    }
+}
+
+// ---- the stage kernel ------------------------------------------------------------------------------------------
+// grid: one CTA per unit = (image, row segment, strip); the unit completes output rows [ys0, ys1) x columns
+// [xs OW, xs OW + OW) from phi rows [ys0, ys1 + 2r) x phi columns [xs OW, xs OW + 256) (phi coordinates = image + r).
+template <int KS>
+__global__ void __launch_bounds__(TC_THREADS, 1)
+stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int nxs, int nys, int seg_rows)
+{
+    using C = TcCfg<KS>;
+    constexpr int R = C::R;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    __shared__ uint32_t tmem_base_s;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::SM_BAR);
+    uint64_t* pfull = bars;                     // [TC_NP] loader -> MMA: row pair landed
+    uint64_t* pempty = bars + TC_NP;            // [TC_NP] MMA -> loader: row pair no longer read
+    uint64_t* zfull = bars + 2 * TC_NP;         // [2] forward bank of a batch done
+    uint64_t* vdone = zfull + 2;                // [2] phi warps wrote v of a batch
+    uint64_t* tfull = vdone + 2;                // scatter table of a batch complete
+    uint64_t* tfree = tfull + 1;                // scatter table read out
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    int unit = blockIdx.x;
+    const int xs = unit % nxs; unit /= nxs;
+    const int ysg = unit % nys; unit /= nys;
+    const int img = unit;
+    const int X0 = xs * C::OW;                                  // phi column of lane 0, pixel 0 = image column X0 - r
+    const int ys0 = ysg * seg_rows, ys1 = min(a.H, ys0 + seg_rows);
+    const int rows_out = ys1 - ys0;
+    const int NB = (rows_out + 2 * R - 1) / 2 + 1;              // batches: phi rows ys0 .. ys0 + 2 NB - 1
+    const int NPAIRS = NB + R;                                  // u row pairs: u~ rows ys0 .. ys0 + 2 NB + 2r - 1
+    const float* __restrict__ u_img = a.u_in + (size_t)img * a.H * a.W;
+
+    // ---- setup: operands and coefficients to shared memory, barriers, tensor memory ----
+    {
+        const size_t bfb = tc_ws_bf_bytes(KS, nkp), bsb = tc_ws_bs_bytes(KS, nkp);
+        for (int i = tid; i < (int)(bfb / 16); i += TC_THREADS) {
+            cp_async16(reinterpret_cast<float*>(smem + C::SM_BFH) + 4 * i, reinterpret_cast<const float*>(ws) + 4 * i);
+            cp_async16(reinterpret_cast<float*>(smem + C::SM_BFL) + 4 * i, reinterpret_cast<const float*>(ws + bfb) + 4 * i);
+        }
+        for (int i = tid; i < (int)(bsb / 16); i += TC_THREADS)
+            cp_async16(reinterpret_cast<float*>(smem + C::SM_BS) + 4 * i, reinterpret_cast<const float*>(ws + 2 * bfb) + 4 * i);
+        constexpr int CF = TNRD_FG * TNRD_FSTRIDE;              // coefficient floats per filter
+        for (int i = tid; i < nkp * CF / 4; i += TC_THREADS) {
+            const int fi = (4 * i) / CF, o = 4 * i - fi * CF;
+            float* dst = reinterpret_cast<float*>(smem + C::SM_COEF) + 4 * i;
+            if (fi < a.N_k) cp_async16(dst, a.prm + (size_t)fi * C::PRM + prm_fact(KS) + o);
+            else *reinterpret_cast<float4*>(dst) = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+    }
+    if (tid == 0) {
+        for (int i = 0; i < TC_NP; ++i) { mbar_init(pfull + i, TC_LOAD_WARPS); mbar_init(pempty + i, 1); }
+        for (int i = 0; i < 2; ++i) { mbar_init(zfull + i, 1); mbar_init(vdone + i, TC_PHI_WARPS); }
+        mbar_init(tfull, 1);
+        mbar_init(tfree, TC_PHI_WARPS);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == TC_MMA_WARP) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "r"(512) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    cp_async_wait_all();
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = tmem_base_s;
+    const uint32_t sbase = smem_u32(smem);
+
+    if (warp < TC_PHI_WARPS) {
+        // =================================== phi warps ===================================
+        const int quarter = warp & 3, sub = warp >> 2;
+        const int L = quarter * 32 + lane;                       // tensor-memory lane = pixel pair
+        const uint32_t tl = tmem + ((uint32_t)(quarter * 32) << 16);
+        const int nf_sub = nkp >> 2, fbase = sub * nf_sub;       // this warp's filters
+        const float kappa = __ldg(a.prm + prm_hdr(KS) + 4), dmax = __ldg(a.prm + prm_hdr(KS) + 5);
+        const bool fact = __ldg(a.prm + prm_hdr(KS) + 6) != 0.0f;
+        const float* coef = reinterpret_cast<const float*>(smem + C::SM_COEF);
+        float2* xbuf = reinterpret_cast<float2*>(smem + C::SM_X);      // [q][k][128]
+        float2* oring = reinterpret_cast<float2*>(smem + C::SM_O);     // [8][128]
+        const float lambda = a.lambda_ptr ? __ldg(a.lambda_ptr) : a.lambda_val;
+        const int q0 = 2 * sub;                                  // this warp folds table blocks q0, q0 + 1
+        const bool has_q = q0 <= KS;
+        const int xcol = xs * C::OW + 2 * L;                     // image column of this lane's first pixel
+        const bool lane_out = L < 128 - R;                       // lanes whose output pixels this strip completes
+
+        auto drain = [&](int b) {
+            mbar_wait(tfull, b & 1);
+            tc_fence_after();
+            uint32_t t[16];
+            if (has_q) { tmem_ld16(tl + TC_TCOL + 8 * q0, t); tmem_ld_wait(); }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tfree);
+            bar_phi();                                           // the previous fold has finished reading xbuf
+            if (has_q) {
+#pragma unroll
+                for (int qq = 0; qq < 2; ++qq)
+#pragma unroll
+                    for (int k = 0; k < C::XK; ++k)
+                        xbuf[((q0 + qq) * C::XK + k) * 128 + L] =
+                            make_float2(__uint_as_float(t[8 * qq + 2 * k]), __uint_as_float(t[8 * qq + 2 * k + 1]));
+            }
+            bar_phi();
+            if (!has_q) return;
+#pragma unroll
+            for (int qq = 0; qq < 2; ++qq) {
+                const int q = q0 + qq;
+                float2 o = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int t2 = 0; t2 <= R; ++t2)                  // lanes L .. L + r reach this lane's pixel pair
+                    if (L + t2 < 128) {
+                        const float2 x = xbuf[(q * C::XK + (R - t2)) * 128 + L + t2];
+                        o.x += x.x; o.y += x.y;
+                    }
+                const int yrel = 2 * b + 1 - q;                  // output row (relative to ys0) block q belongs to
+                float2* slot = oring + (yrel & 7) * 128 + L;
+                if (q >= 2) { const float2 p = *slot; o.x += p.x; o.y += p.y; }
+                if (q < KS - 1) { *slot = o; continue; }
+                // a5: the row is complete
+                if (yrel < 0 || yrel >= rows_out || !lane_out) continue;
+                const size_t base = ((size_t)img * a.H + ys0 + yrel) * a.W;
+                if (xcol < a.W) {
+                    const float uu = __ldg(a.u_in + base + xcol), ff = __ldg(a.f + base + xcol);
+                    a.u_out[base + xcol] = uu - (o.x + lambda * (uu - ff));
+                }
+                if (xcol + 1 < a.W) {
+                    const float uu = __ldg(a.u_in + base + xcol + 1), ff = __ldg(a.f + base + xcol + 1);
+                    a.u_out[base + xcol + 1] = uu - (o.y + lambda * (uu - ff));
+                }
+            }
+        };
+
+        for (int b = 0; b < NB; ++b) {
+            const int bb = b & 1;
+            mbar_wait(zfull + bb, (b >> 1) & 1);
+            tc_fence_after();
+            const uint32_t zrow0 = tl + bb * 4 * nkp + 2 * fbase, zrow1 = zrow0 + 2 * nkp;
+            for (int fi = 0; fi < nf_sub; fi += 2) {
+                uint32_t z0[4], z1[4], o0[4], o1[4];
+                tmem_ld4(zrow0 + 2 * fi, z0);
+                tmem_ld4(zrow1 + 2 * fi, z1);
+                tmem_ld_wait();
+#pragma unroll
+                for (int f = 0; f < 2; ++f) {
+                    const float2 zc[2] = {make_float2(__uint_as_float(z0[2 * f]), __uint_as_float(z0[2 * f + 1])),
+                                          make_float2(__uint_as_float(z1[2 * f]), __uint_as_float(z1[2 * f + 1]))};
+                    float2 v[2] = {{0.f, 0.f}, {0.f, 0.f}};
+                    const int fidx = fbase + fi + f;
+                    if (fact) tc_phi_fact(coef + fidx * (TNRD_FG * TNRD_FSTRIDE), kappa, dmax, zc, v);
+                    else if (fidx < a.N_k) tc_phi_direct(a.prm + (size_t)fidx * C::PRM + prm_kkp(KS), zc, v);
+                    split_bf16(v[0], o0[2 * f], o0[2 * f + 1]);
+                    split_bf16(v[1], o1[2 * f], o1[2 * f + 1]);
+                }
+                tmem_st4(zrow0 + 2 * fi, o0);
+                tmem_st4(zrow1 + 2 * fi, o1);
+            }
+            tmem_st_wait();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(vdone + bb);
+            if (b > 0) drain(b - 1);
+        }
+        drain(NB - 1);
+    } else if (warp == TC_MMA_WARP) {
+        // =================================== MMA issuer ===================================
+        if (lane == 0) {
+            const uint32_t id_f = umma_idesc(2, 128, 2 * nkp), id_s = umma_idesc(1, 128, C::NSC);
+            const uint32_t lbo_f = 2 * nkp * 16;
+            auto forward = [&](int b) {
+                const int bb = b & 1;
+                for (int rr = 0; rr < 2; ++rr) {
+                    const uint32_t d = tmem + bb * 4 * nkp + rr * 2 * nkp;
+                    uint32_t acc = 0;
+                    for (int split = 0; split < 3; ++split) {            // hi*hi, hi*lo, lo*hi
+                        const uint32_t ab = sbase + (split == 2 ? C::SM_ULO : C::SM_UHI);
+                        const uint32_t bbase = sbase + (split == 1 ? C::SM_BFL : C::SM_BFH);
+                        for (int ta = 0; ta < KS; ++ta) {
+                            const int ring = (2 * b + rr + ta) % (2 * TC_NP);
+                            umma_tf32_ss(d, umma_desc(ab + ring * TC_CW * 16, 32, 128),
+                                         umma_desc(bbase + 2 * ta * lbo_f, lbo_f, 128), id_f, acc);
+                            acc = 1;
+                        }
+                    }
+                }
+                umma_commit(zfull + bb);
+                umma_commit(pempty + b % TC_NP);
+            };
+            auto wait_pair = [&](int p) { mbar_wait(pfull + p % TC_NP, (p / TC_NP) & 1); };
+            for (int p = 0; p <= R; ++p) wait_pair(p);
+            tc_fence_after();
+            forward(0);
+            if (NB > 1) { wait_pair(R + 1); tc_fence_after(); forward(1); }
+            for (int b = 0; b < NB; ++b) {
+                const int bb = b & 1;
+                mbar_wait(vdone + bb, (b >> 1) & 1);
+                if (b >= 1) mbar_wait(tfree, (b - 1) & 1);
+                tc_fence_after();
+                for (int rr = 1; rr >= 0; --rr) {                        // row 1 first: it initialises blocks 0 .. KS
+                    const uint32_t d = tmem + TC_TCOL + (rr == 0 ? 8 : 0);
+                    const uint32_t av = tmem + bb * 4 * nkp + rr * 2 * nkp;
+                    for (int pass = 0; pass < 2; ++pass)
+                        for (int ks = 0; ks < nkp / 4; ++ks)
+                            umma_bf16_ts(d, av + 8 * ks,
+                                         umma_desc(sbase + C::SM_BS + ((pass * (nkp / 2) + 2 * ks) * C::NSC) * 16, C::NSC * 16, 128),
+                                         id_s, (rr == 1 && pass == 0 && ks == 0) ? 0u : 1u);
+                }
+                umma_commit(tfull);
+                if (b + 2 < NB) { wait_pair(b + 2 + R); tc_fence_after(); forward(b + 2); }
+            }
+        }
+    } else {
+        // =================================== loader warps ===================================
+        const int lt = tid - (TC_MMA_WARP + 1) * 32;
+        for (int p = 0; p < NPAIRS; ++p) {
+            const int slot = p % TC_NP;
+            if (p >= TC_NP) mbar_wait(pempty + slot, ((p / TC_NP) - 1) & 1);
+            for (int idx = lt; idx < 2 * TC_CWU; idx += TC_LOAD_WARPS * 32) {
+                const int rrow = idx / TC_CWU, xg = idx - rrow * TC_CWU;
+                const float* __restrict__ grow = u_img + (size_t)mirror_clamp(ys0 + 2 * p + rrow - 2 * R, a.H) * a.W;
+                float v[4], h[4], l[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) v[e] = __ldg(grow + mirror_clamp(X0 + 2 * xg + e - 2 * R, a.W));
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    h[e] = __uint_as_float(__float_as_uint(v[e]) & 0xFFFFE000u);
+                    l[e] = v[e] - h[e];
+                }
+                const int cell = ((slot * 2 + rrow) * TC_CW + xg) * 16;
+                *reinterpret_cast<float4*>(smem + C::SM_UHI + cell) = make_float4(h[0], h[1], h[2], h[3]);
+                *reinterpret_cast<float4*>(smem + C::SM_ULO + cell) = make_float4(l[0], l[1], l[2], l[3]);
+            }
+            fence_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(pfull + slot);
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == TC_MMA_WARP)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "r"(512) : "memory");
+}
+
+inline int tc_env_int(const char* name)
+{
+    const char* e = getenv(name);
+    return e ? atoi(e) : 0;
+}
+
+}  // namespace
+
+bool tc_supported(int N_k, int ksize) { return (ksize == 7 || ksize == 5) && N_k >= 1 && N_k <= TC_NKP_MAX; }
+
+size_t tc_workspace_bytes(int T, int N_k, int ksize)
+{
+    const int nkp = (N_k + 7) / 8 * 8;
+    return (size_t)T * tc_ws_stage_bytes(ksize, nkp);
+}
+
+TcPlan plan_stage_tc(int B, int H, int W, int ksize, int num_sms)
+{
+    const int R = (ksize - 1) / 2, OW = 256 - 2 * R;
+    TcPlan pl;
+    pl.nxs = (W + OW - 1) / OW;
+    // row segments: minimise waves x (rows per segment + recomputed rows + a per-CTA constant, in rows)
+    const double c0 = 10.0;
+    double best = -1.0;
+    pl.nys = 1; pl.seg_rows = H;
+    const int forced = tc_env_int("TNRD_TC_SEG");
+    for (int nys = 1; nys <= (H + 3) / 4; ++nys) {
+        int seg = (H + nys - 1) / nys;
+        if (forced > 0) seg = forced < H ? forced : H;
+        const int n = (H + seg - 1) / seg;
+        const long long units = (long long)B * pl.nxs * n;
+        const double cost = (double)((units + num_sms - 1) / num_sms) * (seg + 2 * R + c0);
+        if (best < 0 || cost < best) { best = cost; pl.nys = n; pl.seg_rows = seg; }
+        if (forced > 0) break;
+    }
+    pl.units = (long long)B * pl.nxs * pl.nys;
+    pl.cost_rows = best;
+    return pl;
+}
+
+cudaError_t launch_tc_prep(const float* prm, int T, int N_k, int ksize, unsigned char* ws, cudaStream_t st,
+                           unsigned long long* launches)
+{
+    const int nkp = (N_k + 7) / 8 * 8;
+    const long long total = (long long)T * (ksize * 2 * 2 * nkp * 4 + nkp * 8 * (ksize + 1) * 8);
+    const int threads = 256;
+    long long blocks = (total + threads - 1) / threads;
+    if (blocks > 1184) blocks = 1184;
+    tc_prep_kernel<<<(int)blocks, threads, 0, st>>>(prm, T, N_k, nkp, ksize, ws);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+template <int KS>
+static cudaError_t launch_tc_ks(const StageArgs& a, const TcPlan& pl, const unsigned char* ws_t, int nkp, cudaStream_t st)
+{
+    using C = TcCfg<KS>;
+    cudaError_t e = cudaFuncSetAttribute(stage_tc_kernel<KS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    if (e != cudaSuccess) return e;
+    if (pl.units > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    stage_tc_kernel<KS><<<(unsigned)pl.units, TC_THREADS, C::SMEM, st>>>(a, ws_t, nkp, pl.nxs, pl.nys, pl.seg_rows);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_stage_tc(const StageArgs& a, const TcPlan& pl, const unsigned char* ws_t, cudaStream_t st,
+                            unsigned long long* launches)
+{
+    const int nkp = (a.N_k + 7) / 8 * 8;
+    cudaError_t e;
+    if (a.ksize == 7) e = launch_tc_ks<7>(a, pl, ws_t, nkp, st);
+    else if (a.ksize == 5) e = launch_tc_ks<5>(a, pl, ws_t, nkp, st);
+    else return cudaErrorInvalidValue;
+    ++*launches;
+    return e;
+}
+
+size_t tc_ws_stage_stride(int N_k, int ksize) { return tc_ws_stage_bytes(ksize, (N_k + 7) / 8 * 8); }
+
+}  // namespace tnrd
