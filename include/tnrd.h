@@ -24,9 +24,11 @@
  *   - "device pointer": memory of the CURRENT CUDA device (cudaMalloc / torch allocator), 4-byte aligned.
  *     "host pointer": ordinary or pinned host memory.
  *   - Ownership: the caller owns every buffer and keeps device buffers alive until the work queued on
- *     `stream` has completed.  The library owns only an internal per-(device, stream) scratch (the staged parameters
- *     and the partial sums of the tile kernel, about 4.5 bytes per pixel), grown on demand and released by
- *     tnrd_shutdown().
+ *     `stream` has completed.  The library owns only an internal per-(device, stream) scratch (the staged parameters,
+ *     and either the partial sums of the tile kernel, about 4.5 bytes per pixel, or the ping-pong plane of the
+ *     tensor-core kernel, 4 bytes per pixel), grown on demand and released by tnrd_shutdown().  The scratch grows
+ *     with cudaMallocAsync on `stream`; a call that would have to grow it while `stream` is being captured into a
+ *     CUDA graph returns TNRD_ERR_CUDA instead (run the shape once before capturing).
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device entry points
  *     are asynchronous on `stream` and never synchronise the device.
  *   - Every function returning int returns TNRD_OK (0) or a negative tnrd_status.  Nothing throws.
@@ -78,7 +80,8 @@ int tnrd_stage(const float* f, const float* u_in, int B, int H, int W, int N_k, 
  *   lambda      device, [T]  (device so that the call needs no host sync and can be graph-captured)
  *   out         device, [B][H][W]; receives u_T.  out may equal u0 (in place); out must not equal f.
  *   T = 0 copies u0 to out.
- * Every stage writes `out`, from the second one on in place; no image-sized scratch is needed.
+ * With the tile kernel every stage writes `out`, from the second one on in place; with the tensor-core kernel the
+ * stages alternate between `out` and one image-sized plane of the library scratch (tnrd_set_kernel).
  */
 int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, int N_k, int ksize,
                  const float* filters, const float* rbf_w, const float* rbf_mu, float rbf_gamma,
@@ -158,11 +161,32 @@ int tnrd_diffuse_backward(const float* f, const float* u0, const float* u_gt, co
                           float* grad_w, float* grad_lambda, void* stream);
 
 /*
- * Kernel selection, for tests and profiling.  which = 0: automatic (default); 1: the plain one-thread-per-
- * pixel reference kernel (global memory only); 2: the fused tiled stage kernel.  Returns TNRD_ERR_UNSUPPORTED
- * for other values.  Process-wide.
+ * Kernel selection, for tests and profiling.  Process-wide (read once at the entry of every call).
+ *   0  automatic (default): the tensor-core stage kernel where it applies and its work units fill the GPU
+ *      (tnrd_tc_plan_query), the tile kernel otherwise;
+ *   1  the plain one-thread-per-pixel reference kernel (global memory only);
+ *   2  the fused tile kernel: both filterings on the FP32 FMA pipe, partial sums + a point-wise update kernel;
+ *   3  the tensor-core stage kernel (csrc/tnrd_tc.cu): both filterings as tcgen05 implicit GEMMs (forward bank: three
+ *      TF32 products of hi/lo split operands; transposed bank: BF16 hi/lo pairs), accumulators in tensor memory,
+ *      factorised influence functions on the accumulators, u_t written by the same kernel.  It applies to the Gaussian
+ *      basis with TNRD_PHI_FACTORED, ksize 5 or 7 and N_k <= 48; any other call returns TNRD_ERR_UNSUPPORTED while 3 is
+ *      selected.  Results agree with kernel 2 to fp32 rounding (same distance from the double-precision definition).
+ *      It cannot run in place: tnrd_diffuse / tnrd_deblock_diffuse then keep one image-sized ping-pong plane in the
+ *      library scratch (and copy u0 into it when out == u0 and T is odd), tnrd_stage with u_out == u_in writes the
+ *      plane and copies it back.  A non-finite pixel reaches a slightly larger neighbourhood than the (2 ksize - 1)^2
+ *      footprint of the definition (0 x NaN inside the 8-column windows of the implicit GEMM).
+ * Returns TNRD_ERR_UNSUPPORTED for other values.
  */
 int tnrd_set_kernel(int which);
+
+/*
+ * Work decomposition of the tensor-core stage kernel for this shape on a device with `num_sms` multiprocessors (pure host
+ * logic).  plan[0..5] = {0: the kernel does not apply to (N_k, ksize); 1: applies, the automatic choice is the tile
+ * kernel; 2: applies and is the automatic choice}, strips per image (256 - 2r output columns each), row segments per
+ * image, output rows per segment, CTAs (= images x strips x segments), output columns per strip.  Honours the
+ * TNRD_TC_SEG environment knob (forces the rows per segment; tests).
+ */
+int tnrd_tc_plan_query(int B, int H, int W, int N_k, int ksize, int num_sms, long long* plan);
 
 /*
  * Influence-function evaluator of the fused kernel.  Process-wide.
@@ -228,19 +252,6 @@ void tnrd_reset_launch_count(void);
  *   which = 0: FP32 FFMA rate      -> *rate = FMA lane-operations per second (x2 = FLOP/s)
  *   which = 1: MUFU.EX2 rate       -> *rate = ex2 evaluations per second
  *   which = 2: the phi inner loop (FADD, FMUL, MUFU.EX2, FFMA per term) -> RBF terms per second
- *   which = 3: warp-level tensor path, mma.sync m16n8k8 TF32, fp32 accumulation -> multiply-adds per second (x2 = FLOP/s)
- *   which = 4: the same with m16n8k16 BF16
- *   which = 5: prototype of the forward filter bank (48 filters 7x7) as an implicit GEMM on that path: A fragments gathered tap
- *              by tap from a 128 x 128 tile in shared memory, operands split into BF16 halves, three products, fp32
- *              accumulation -> pixels (48 responses each) per second; checks itself against plain fp32 FMAs on the device
- *              and fails with TNRD_ERR_CUDA if the two differ by more than 0.05 (|z| ~ 75)
- *   which = 6: the same followed by the factorised phi evaluated on the accumulator fragments (two adjacent filters of a
- *              pixel per register pair, packed coefficient pairs from shared memory; synthetic coefficients) -> pixels per second
- *   which = 7: 6 followed by the transposed bank as a scatter table S[pixel][tap] = sum_f v_f K_f[tap] on the same path (the phi
- *              accumulators are the A fragments; BF16 halves, three products); the fold s(p) = sum_tap S[p + tap - r][tap]
- *              is NOT included -> pixels per second.  5 .. 7 all check the forward responses and the scatter table of one
- *              tile against plain fp32 sums on the device.
- * (3 .. 7 are not used by the product path: they size the filterings as an implicit GEMM.)
  * Any other value: TNRD_ERR_UNSUPPORTED.
  */
 int tnrd_microbench(int which, double* rate, void* stream);

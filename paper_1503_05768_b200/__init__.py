@@ -19,6 +19,7 @@ NUM_RBF = 63
 
 OK, ERR_NULL, ERR_SHAPE, ERR_UNSUPPORTED, ERR_ALIAS, ERR_CUDA, ERR_PARAM = 0, -1, -2, -3, -4, -5, -6
 PHI_DENSE, PHI_WINDOW, PHI_LUT, PHI_FACTORED = 0, 1, 2, 3          # tnrd_set_phi_mode (include/tnrd.h)
+KERNEL_AUTO, KERNEL_REF, KERNEL_TILE, KERNEL_TC = 0, 1, 2, 3        # tnrd_set_kernel (include/tnrd.h)
 
 _lib = None
 
@@ -69,6 +70,8 @@ def lib() -> ctypes.CDLL:
         L.tnrd_set_rbf_basis.restype = ci
         L.tnrd_plan_query.argtypes = [ci, ci, ci, ci, ci, ci, ctypes.POINTER(ctypes.c_longlong)]
         L.tnrd_plan_query.restype = ci
+        L.tnrd_tc_plan_query.argtypes = [ci, ci, ci, ci, ci, ci, ctypes.POINTER(ctypes.c_longlong)]
+        L.tnrd_tc_plan_query.restype = ci
         L.tnrd_launch_count.restype = ctypes.c_ulonglong
         L.tnrd_reset_launch_count.restype = None
         L.tnrd_microbench.argtypes = [ci, ctypes.POINTER(ctypes.c_double), vp]
@@ -186,6 +189,14 @@ def tnrd_plan_query(B, H, W, N_k, ksize, num_sms=148) -> dict:
     buf = (ctypes.c_longlong * 10)()
     _check(lib().tnrd_plan_query(B, H, W, N_k, ksize, num_sms, buf))
     keys = ("cfg", "ntx", "nty", "tw", "th", "n_full", "nsplit", "ctas", "cta_floats", "part_floats")
+    return dict(zip(keys, (int(v) for v in buf)))
+
+
+def tnrd_tc_plan_query(B, H, W, N_k, ksize, num_sms=148) -> dict:
+    """Work decomposition of the tensor-core stage kernel (include/tnrd.h: tnrd_tc_plan_query); host logic only."""
+    buf = (ctypes.c_longlong * 6)()
+    _check(lib().tnrd_tc_plan_query(B, H, W, N_k, ksize, num_sms, buf))
+    keys = ("applies", "nxs", "nys", "seg_rows", "units", "out_cols")
     return dict(zip(keys, (int(v) for v in buf)))
 
 

@@ -48,7 +48,8 @@ def build(verbose: bool = False, force: bool = False) -> str:
         obj = os.path.join(OBJ, os.path.basename(src)[:-3] + ".o")
         if not force and os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(src), newest_header):
             return obj, 0, ""
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+        extra = os.environ.get("TNRD_NVCC_EXTRA", "").split()      # tuning experiments only (e.g. -DTNRD_TC_PHI_WARPS=24)
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
         res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
         return obj, res.returncode, res.stdout + res.stderr
 

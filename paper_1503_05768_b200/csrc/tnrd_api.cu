@@ -121,6 +121,13 @@ struct Call {
     bool tc = false;   // this call runs the tensor-core stage kernel
 };
 
+// The automatic choice between the two stage kernels: strips of the tensor-core kernel are 256 - 2r columns wide and
+// every CTA recomputes 2r phi rows, so it pays once its units fill the GPU with segments of a few dozen rows.
+bool tc_auto(const tnrd::TcPlan& pl, int W, int num_sms)
+{
+    return pl.units * 10 >= (long long)num_sms * 6 && pl.seg_rows >= 24 && W >= 192;
+}
+
 // Which stage kernel a call uses.  kernel 3 forces the tensor-core kernel (TNRD_ERR_UNSUPPORTED where it does not apply),
 // 0 picks it when it applies and the image keeps its 128-lane strips busy: it needs the Gaussian basis with the
 // factorised evaluator, ksize 5 or 7 and N_k <= 48 (tnrd_tc.cu).
@@ -132,8 +139,7 @@ int pick_kernel(Call& c, int B, int H, int W, int N_k, int ksize, int phi)
         c.tc = true;
     } else if (c.o.kernel == 0 && can) {
         // strips are 256 - 2r columns wide and every CTA recomputes 2r phi rows: worth it once the units fill the GPU
-        const tnrd::TcPlan pl = tnrd::plan_stage_tc(B, H, W, ksize, c.sc->num_sms);
-        c.tc = pl.units >= c.sc->num_sms && pl.seg_rows >= 24 && W >= 192;
+        c.tc = tc_auto(tnrd::plan_stage_tc(B, H, W, ksize, c.sc->num_sms), W, c.sc->num_sms);
     }
     return TNRD_OK;
 }
@@ -519,6 +525,20 @@ int tnrd_plan_query(int B, int H, int W, int N_k, int ksize, int num_sms, long l
     return TNRD_OK;
 }
 
+int tnrd_tc_plan_query(int B, int H, int W, int N_k, int ksize, int num_sms, long long* plan)
+{
+    if (!plan) return TNRD_ERR_NULL;
+    int rc = check_shape(B, H, W, N_k, ksize);
+    if (rc != TNRD_OK) return rc;
+    if (num_sms < 1) return TNRD_ERR_SHAPE;
+    for (int i = 0; i < 6; ++i) plan[i] = 0;
+    if (!tnrd::tc_supported(N_k, ksize)) return TNRD_OK;
+    const tnrd::TcPlan pl = tnrd::plan_stage_tc(B, H, W, ksize, num_sms);
+    plan[0] = 1 + (tc_auto(pl, W, num_sms) ? 1 : 0);
+    plan[1] = pl.nxs; plan[2] = pl.nys; plan[3] = pl.seg_rows; plan[4] = pl.units; plan[5] = 256 - (ksize - 1);
+    return TNRD_OK;
+}
+
 int tnrd_set_kernel(int which)
 {
     if (which < 0 || which > 3) return TNRD_ERR_UNSUPPORTED;
@@ -546,7 +566,7 @@ void tnrd_reset_launch_count(void) { g_launches = 0; }
 int tnrd_microbench(int which, double* rate, void* stream)
 {
     if (!rate) return TNRD_ERR_NULL;
-    if (which < 0 || which > 7) return TNRD_ERR_UNSUPPORTED;
+    if (which < 0 || which > 2) return TNRD_ERR_UNSUPPORTED;
     LaunchCount lc;
     TNRD_CUDA(tnrd::run_microbench(which, rate, (cudaStream_t)stream, &lc.n));
     return TNRD_OK;

@@ -17,9 +17,11 @@
 // -- times the chunks of a split filter bank -- that reach the pixel + lambda (u - f)), point-wise, fixed order.
 // HBM traffic: 4 B read + ~4.5 B written per pixel-stage by the tile kernel, ~16.5 B by the update kernel.
 //
-// The path is bound by the XU (MUFU) pipe: 3024 ex2 per pixel-stage for the 48 x 7x7 model against 4704 FFMA of
-// filtering; tensor cores are not used.  Two things keep the XU pipe fed
-// (profiles/r01_*.md):
+// This is the TILE kernel (tnrd_set_kernel(2)): both filterings on the FP32 FMA pipe.  It serves the shapes the
+// tensor-core stage kernel (tnrd_tc.cu) does not take: 3x3 and 9x9 banks, more than 48 filters, the direct / windowed /
+// table evaluators, and images too small to fill that kernel's 128-lane strips.  With the default factorised evaluator
+// it is bound by the FMA pipe (8544 FMA-pipe operations per pixel-stage for 48 x 7x7), with the direct evaluator
+// (TNRD_PHI_DENSE) by the XU pipe (3024 ex2).  Two things keep the pipes fed (profiles/r01_*.md):
 //   * software pipelining inside a thread: the 63-term phi loop of block n is interleaved, row-step by row-step, with
 //     the forward filter of the NEXT block (a2) and the transposed filter of block n for the previous filter (a4), so
 //     every warp always carries a mix of MUFU and FMA work instead of all warps of a CTA filtering in lock-step;
@@ -31,12 +33,7 @@
 #include "tnrd_internal.h"
 #include "tnrd_device.cuh"
 
-#ifndef TNRD_SKIP_DEAD
-#define TNRD_SKIP_DEAD 0   // experiment: skip a phi group that is dead (Gaussian factor flushed to zero) for the whole warp
-#endif
-#ifndef TNRD_FACT_NP
-#define TNRD_FACT_NP 2   // pairs of responses per factorised-phi step (2 or 4)
-#endif
+#define TNRD_FACT_NP 2   // pairs of responses per factorised-phi step
 
 namespace tnrd {
 
@@ -198,6 +195,9 @@ __device__ __forceinline__ void fact_poly(const float (&c)[TNRD_FSTRIDE], const 
     }
 }
 
+// A group whose Gaussian factor has flushed to zero for EVERY response of the warp is skipped (fact_group_live): its
+// contribution is an exact 0 either way, so the result is bit-identical; the run time then depends on the responses
+// (bench.py reports the executed next to the defined phi work).
 // One block of the software pipeline with the factorised evaluator: phi of the block's 8 responses (TNRD_FG groups, two
 // pairs of responses at a time) with the KS + 1 window rows of both filterings riding along -- rows 1 .. KS-1 two per
 // group in the first (KS-1)/2 groups, the one-sided rows 0 and KS (rowstep_half) in the last group.  A window row of the
@@ -213,36 +213,9 @@ __device__ __forceinline__ void fact_block(const float* __restrict__ frec, float
     float fc[TNRD_FSTRIDE];
     FactState st;
     lds_vec(frec, fc);
-#if TNRD_FACT_NP == 4
-    const bool hasB = hasB_;
-#pragma unroll 1
-    for (int g = 0; g < NGR; ++g) {
-        if (hasB) fact_exp<0>(fc, kappa, dmax, zc, st);
-        if (hasN) rowstep<KS, false>(uwn + (2 * g + 1) * C::US, tapsN + (KS - 2 * g - 1) * TS, zn);
-        if (hasC) rowstep<KS, true, C::SHIFT>(vw + (2 * g + 1) * C::VS, recp + (2 * g + 1) * TS, acc);
-        if (hasB) fact_poly<0>(fc, st, v);
-        if (hasN) rowstep<KS, false>(uwn + (2 * g + 2) * C::US, tapsN + (KS - 2 * g - 2) * TS, zn);
-        if (hasC) rowstep<KS, true, C::SHIFT>(vw + (2 * g + 2) * C::VS, recp + (2 * g + 2) * TS, acc);
-        lds_vec(frec + (g + 1) * TNRD_FSTRIDE, fc);
-    }
-#pragma unroll 1
-    for (int g = NGR; g < TNRD_FG - 1; ++g) {
-        if (hasB) {
-            fact_exp<0>(fc, kappa, dmax, zc, st);
-            fact_poly<0>(fc, st, v);
-        }
-        lds_vec(frec + (g + 1) * TNRD_FSTRIDE, fc);
-    }
-    if (hasB) fact_exp<0>(fc, kappa, dmax, zc, st);
-    if (hasN) rowstep_half<KS, false, 0, 0>(uwn, tapsN + KS * TS, zn);                            // window row 0
-    if (hasC) rowstep_half<KS, true, C::SHIFT, 1>(vw, recp, acc);
-    if (hasB) fact_poly<0>(fc, st, v);
-    if (hasN) rowstep_half<KS, false, 0, 1>(uwn + KS * C::US, tapsN, zn);                         // window row KS
-    if (hasC) rowstep_half<KS, true, C::SHIFT, 0>(vw + KS * C::VS, recp + KS * TS, acc);
-#else
 #pragma unroll
     for (int g = 0; g < NGR; ++g) {
-        const bool hasB = TNRD_SKIP_DEAD ? fact_group_live(zc, fc[0], dmax, hasB_) : hasB_;
+        const bool hasB = fact_group_live(zc, fc[0], dmax, hasB_);
         if (hasB) fact_exp<0>(fc, kappa, dmax, zc, st);
         if (hasN) rowstep<KS, false>(uwn + (2 * g + 1) * C::US, tapsN + (KS - 2 * g - 1) * TS, zn);
         if (hasB) fact_poly<0>(fc, st, v);
@@ -255,7 +228,7 @@ __device__ __forceinline__ void fact_block(const float* __restrict__ frec, float
     }
 #pragma unroll 1
     for (int g = NGR; g < TNRD_FG - 1; ++g) {
-        const bool hasB = TNRD_SKIP_DEAD ? fact_group_live(zc, fc[0], dmax, hasB_) : hasB_;
+        const bool hasB = fact_group_live(zc, fc[0], dmax, hasB_);
         if (hasB) {
             fact_exp<0>(fc, kappa, dmax, zc, st);
             fact_poly<0>(fc, st, v);
@@ -264,7 +237,7 @@ __device__ __forceinline__ void fact_block(const float* __restrict__ frec, float
         }
         lds_vec(frec + (g + 1) * TNRD_FSTRIDE, fc);
     }
-    const bool hasB = TNRD_SKIP_DEAD ? fact_group_live(zc, fc[0], dmax, hasB_) : hasB_;
+    const bool hasB = fact_group_live(zc, fc[0], dmax, hasB_);
     if (hasB) fact_exp<0>(fc, kappa, dmax, zc, st);
     if (hasN) rowstep_half<KS, false, 0, 0>(uwn, tapsN + KS * TS, zn);                            // window row 0
     if (hasB) fact_poly<0>(fc, st, v);
@@ -273,7 +246,6 @@ __device__ __forceinline__ void fact_block(const float* __restrict__ frec, float
     if (hasN) rowstep_half<KS, false, 0, 1>(uwn + KS * C::US, tapsN, zn);                         // window row KS
     if (hasB) fact_poly<2>(fc, st, v);
     if (hasC) rowstep_half<KS, true, C::SHIFT, 0>(vw + KS * C::VS, recp + KS * TS, acc);
-#endif
 }
 
 template <int KS, int RW, int RH, int NT, int MINB, int PHI>

@@ -29,7 +29,8 @@ namespace tnrd {
 //            kappa = 2 delta', D and ok_f belong to the factorised evaluator (next item)
 //   fact     at offset prm_fact: TNRD_FG groups of TNRD_FSTRIDE floats for the factorised phi evaluator.  Group g has its
 //            anchor at centre a = g (2 S + 1) + S (S = TNRD_FS) and holds
-//            -mu'_a,  c_S, c_{S-1}, .., c_0,  c_{-S}, c_{-S+1}, .., c_{-1}  (then zeros up to TNRD_FSTRIDE)  with
+//            -mu'_a,  c_S, c_{S-1}, .., c_0,  c_{-S}, c_{-S+1}, .., c_{-1},  K_g, 1/K_g  (slots 14, 15: K_g = 2^{kappa (mu'_mid -
+//            mu'_a)}, mid = the middle group's anchor; used by the tensor-core kernel to derive rho of every group from one)  with
 //            c_j = w'_{i,a+j} 2^{-(j delta')^2} (0 where a + j is not a centre).  With d = z' - mu'_a and equidistant
 //            centres,  2^{-(d - j delta')^2} = 2^{-d^2} (2^{kappa d})^j 2^{-(j delta')^2},  so the 2S+1 terms of a group
 //            are  2^{-d^2} * (polynomial in rho = 2^{kappa d} for j >= 0, in 1/rho for j < 0): 3 ex2 instead of 2S+1.

@@ -71,6 +71,12 @@ __global__ void prep_params_kernel(const float* __restrict__ filters, const floa
                 const int j = o <= TNRD_FS + 1 ? TNRD_FS + 1 - o : o - 2 * TNRD_FS - 2;   // S .. 0, then -S .. -1
                 const int c = anchor + j;
                 if (c >= 0 && c < TNRD_M) val = rbf_w[(size_t)rec * TNRD_M + c] / s * exp2f(-(float)(j * j) * ds * ds);
+            } else if (o == TNRD_FSTRIDE - 2 || o == TNRD_FSTRIDE - 1) {
+                // K_g = 2^{kappa (d_g - d_mid)} = 2^{-2 delta'^2 (anchor_g - anchor_mid)} and 1 / K_g: rho of group g from the
+                // rho of the middle group (tensor-core kernel, tnrd_tc.cu)
+                const int mid = (TNRD_FG / 2) * TNRD_FM + TNRD_FS;
+                const float ex = -2.0f * ds * ds * (float)(anchor - mid);
+                val = exp2f(o == TNRD_FSTRIDE - 2 ? ex : -ex);
             }
         }
         prm[idx] = val;

@@ -28,8 +28,9 @@
 //
 // Strips overlap by 2r phi columns and row segments by 2r phi rows (recomputed) so that a CTA completes its own
 // outputs: no partial sums in HBM, no second kernel, 12 B of DRAM traffic per pixel-stage.
-// Warp roles: 16 phi warps (4 per tensor-memory lane quarter, each a quarter of the filters), 1 MMA-issuing warp,
-// 2 loader warps; mbarrier pipelines between them (u row pairs, z double-buffered, scatter table).
+// Warp roles: 16 phi warps (4 per tensor-memory lane quarter, sharing the quarter's filter pairs through a ticket
+// counter), 4 drain warps (fold + a5), 1 MMA-issuing warp, 1 loader warp; mbarrier pipelines between them (u row pairs,
+// z double-buffered, scatter table).
 #include <cuda_bf16.h>
 #include <cstdint>
 #include <cstdio>
@@ -42,9 +43,13 @@ namespace tnrd {
 
 namespace {
 
-constexpr int TC_PHI_WARPS = 16, TC_LOAD_WARPS = 2;
-constexpr int TC_MMA_WARP = TC_PHI_WARPS;                       // warp index of the MMA issuer
-constexpr int TC_THREADS = (TC_PHI_WARPS + 1 + TC_LOAD_WARPS) * 32;
+#ifndef TNRD_TC_PHI_WARPS
+#define TNRD_TC_PHI_WARPS 24
+#endif
+constexpr int TC_PHI_WARPS = TNRD_TC_PHI_WARPS, TC_LOAD_WARPS = 1;   // phi warps: a multiple of 4 (TC_PHI_WARPS / 4 per lane quarter)
+constexpr int TC_DRAIN_WARPS = 4;                               // one per lane quarter, right after the phi warps
+constexpr int TC_MMA_WARP = TC_PHI_WARPS + TC_DRAIN_WARPS;      // warp index of the MMA issuer
+constexpr int TC_THREADS = (TC_PHI_WARPS + TC_DRAIN_WARPS + 1 + TC_LOAD_WARPS) * 32;
 constexpr int TC_CW = 132;                                      // cells per ring row (130 used)
 constexpr int TC_CWU = 130;
 constexpr int TC_NP = 6;                                        // row pairs in the ring
@@ -127,12 +132,33 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
                  "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
                  "@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}\n" :: "r"(smem_u32(bar)), "r"(parity) : "memory");
 }
+// The same for the warps that wait most of the time (MMA issuer, loader, drain): a spinning try_wait loop takes issue
+// slots from the phi warps on its scheduler (20 % of all issued instructions in a profile), so back off between polls.
+__device__ __forceinline__ void mbar_wait_idle(uint64_t* bar, uint32_t parity)
+{
+    for (;;) {
+        uint32_t done;
+        asm volatile("{\n\t.reg .pred p;\n\t"
+                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}\n" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+        if (done) return;
+        __nanosleep(200);
+    }
+}
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t (&r)[4])
 {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld2(uint32_t taddr, uint32_t (&r)[2])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_st2(uint32_t taddr, const uint32_t (&r)[2])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" :: "r"(taddr), "r"(r[0]), "r"(r[1]) : "memory");
 }
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
 {
@@ -149,7 +175,7 @@ __device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t (&r)[4])
 }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void bar_phi() { asm volatile("bar.sync 1, %0;" :: "n"(TC_PHI_WARPS * 32) : "memory"); }
+__device__ __forceinline__ void bar_drain() { asm volatile("bar.sync 1, %0;" :: "n"(TC_DRAIN_WARPS * 32) : "memory"); }
 
 __device__ __forceinline__ float ex2f(float x)
 {
@@ -157,39 +183,68 @@ __device__ __forceinline__ float ex2f(float x)
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-__device__ __forceinline__ float clamp_nan(float x, float lim)          // NaN stays NaN
+__device__ __forceinline__ float fmin_nan(float x, float lim)           // NaN stays NaN
 {
     float y;
     asm("min.NaN.f32 %0, %1, %2;" : "=f"(y) : "f"(x), "f"(lim));
-    asm("max.NaN.f32 %0, %0, %1;" : "+f"(y) : "f"(-lim));
     return y;
 }
 
 // Factorised influence function (tnrd_internal.h "fact"; PAPER.md:553 with equidistant centres, :117) of the two
 // response pairs z[0], z[1] of one filter; crec = the filter's TNRD_FG group records in shared memory (broadcast
-// loads).  A group whose Gaussian factor has flushed to zero for every response of the warp is skipped (its
-// contribution is an exact 0; NaN responses keep it live).
-__device__ __forceinline__ void tc_phi_fact(const float* __restrict__ crec, float kappa, float dmax, const float2 (&z)[2],
-                                            float2 (&v)[2])
+// loads).  Per response: ONE pair rho0 = 2^{kappa d0}, 1/rho0 for the middle group; the other groups' rho_g =
+// 2^{kappa d_g} = rho0 K_g with the constants K_g = 2^{kappa (d_g - d0)} staged in the group record (anchors are a fixed
+// number of centres apart), capped at 2^{kappa D} (beyond |d_g| = D the Gaussian factor 2^{-d_g^2} has flushed to
+// zero, so the cap changes no value and keeps rho^S finite): 2 + TNRD_FG ex2 per response instead of 3 TNRD_FG.
+// A group is skipped when its Gaussian factor is zero for every response of the warp (an exact 0 either way): the
+// decision is warp-uniform, from the warp's smallest and largest response (NaN responses keep every group live).
+__device__ __forceinline__ uint32_t f2ord(float x)            // order-preserving map float -> uint32
 {
-    constexpr int S = TNRD_FS;
+    const uint32_t b = __float_as_uint(x);
+    return b ^ ((uint32_t)((int32_t)b >> 31) | 0x80000000u);
+}
+__device__ __forceinline__ float ord2f(uint32_t o)
+{
+    return __uint_as_float(o ^ ((o >> 31) - 1u | 0x80000000u));
+}
+__device__ __forceinline__ void tc_phi_fact(const float* __restrict__ crec, float kappa, float dmax, float rmax,
+                                            const float2 (&z)[2], float2 (&v)[2])
+{
+    constexpr int S = TNRD_FS, GC = TNRD_FG / 2;
+    // warp-wide range of the responses
+    float zlo, zhi;
+    asm("min.NaN.f32 %0, %1, %2;" : "=f"(zlo) : "f"(fminf(z[0].x, z[0].y)), "f"(fminf(z[1].x, z[1].y)));
+    asm("max.NaN.f32 %0, %1, %2;" : "=f"(zhi) : "f"(fmaxf(z[0].x, z[0].y)), "f"(fmaxf(z[1].x, z[1].y)));
+    const bool lane_nan = (z[0].x != z[0].x) || (z[0].y != z[0].y) || (z[1].x != z[1].x) || (z[1].y != z[1].y);
+    const float wlo = ord2f(__reduce_min_sync(0xffffffffu, f2ord(zlo)));
+    const float whi = ord2f(__reduce_max_sync(0xffffffffu, f2ord(zhi)));
+    const bool any_nan = __any_sync(0xffffffffu, lane_nan);
+    // the shared exponential pair (middle group)
+    float2 rho0[2], rhoi0[2];
+    {
+        const float c0 = crec[GC * TNRD_FSTRIDE];
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            const float2 e = __fmul2_rn(__fadd2_rn(z[p], make_float2(c0, c0)), make_float2(kappa, kappa));
+            rho0[p] = make_float2(ex2f(e.x), ex2f(e.y));
+            rhoi0[p] = make_float2(ex2f(-e.x), ex2f(-e.y));
+        }
+    }
 #pragma unroll
     for (int g = 0; g < TNRD_FG; ++g) {
         float c[TNRD_FSTRIDE];
         lds_vec(crec + g * TNRD_FSTRIDE, c);
-        const bool live = !(fabsf(z[0].x + c[0]) >= dmax) || !(fabsf(z[0].y + c[0]) >= dmax) ||
-                          !(fabsf(z[1].x + c[0]) >= dmax) || !(fabsf(z[1].y + c[0]) >= dmax);
-        if (!__any_sync(0xffffffffu, live)) continue;
+        if (!(any_nan || (wlo + c[0] < dmax && whi + c[0] > -dmax))) continue;    // dead for the whole warp
         float2 gg[2], rho[2], rhoi[2], h[2], hl[2];
 #pragma unroll
         for (int p = 0; p < 2; ++p) {
-            float2 d = __fadd2_rn(z[p], make_float2(c[0], c[0]));
-            d = make_float2(clamp_nan(d.x, dmax), clamp_nan(d.y, dmax));
+            const float2 d = __fadd2_rn(z[p], make_float2(c[0], c[0]));
             const float2 t = __fmul2_rn(d, d);
-            const float2 e = __fmul2_rn(d, make_float2(kappa, kappa));
             gg[p] = make_float2(ex2f(-t.x), ex2f(-t.y));
-            rho[p] = make_float2(ex2f(e.x), ex2f(e.y));
-            rhoi[p] = make_float2(ex2f(-e.x), ex2f(-e.y));
+            const float2 r = __fmul2_rn(rho0[p], make_float2(c[14], c[14]));
+            const float2 ri = __fmul2_rn(rhoi0[p], make_float2(c[15], c[15]));
+            rho[p] = make_float2(fmin_nan(r.x, rmax), fmin_nan(r.y, rmax));
+            rhoi[p] = make_float2(fmin_nan(ri.x, rmax), fmin_nan(ri.y, rmax));
         }
 #pragma unroll
         for (int p = 0; p < 2; ++p) {
@@ -322,7 +377,8 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
         for (int i = 0; i < TC_NP; ++i) { mbar_init(pfull + i, TC_LOAD_WARPS); mbar_init(pempty + i, 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(zfull + i, 1); mbar_init(vdone + i, TC_PHI_WARPS); }
         mbar_init(tfull, 1);
-        mbar_init(tfree, TC_PHI_WARPS);
+        mbar_init(tfree, TC_DRAIN_WARPS);
+        for (int i = 0; i < 4; ++i) reinterpret_cast<int*>(smem + C::SM_BAR + 192)[i] = 0;      // ticket counters
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == TC_MMA_WARP) {
@@ -339,43 +395,109 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
 
     if (warp < TC_PHI_WARPS) {
         // =================================== phi warps ===================================
-        const int quarter = warp & 3, sub = warp >> 2;
-        const int L = quarter * 32 + lane;                       // tensor-memory lane = pixel pair
+        // The warps of a lane quarter share the (batch, filter pair) tickets of that quarter through a counter in shared
+        // memory: dead-group skipping makes the cost of a filter pair vary, and a fixed split would make every batch
+        // wait for its slowest warp.  A warp arrives on vdone[b] once it holds a ticket beyond batch b (all its batch-b
+        // work is written back); z is double-buffered, so a fast warp runs at most one batch ahead of the slowest.
+        const int quarter = warp & 3;
         const uint32_t tl = tmem + ((uint32_t)(quarter * 32) << 16);
-        const int nf_sub = nkp >> 2, fbase = sub * nf_sub;       // this warp's filters
+        const int npairs = nkp >> 1;
         const float kappa = __ldg(a.prm + prm_hdr(KS) + 4), dmax = __ldg(a.prm + prm_hdr(KS) + 5);
         const bool fact = __ldg(a.prm + prm_hdr(KS) + 6) != 0.0f;
+        const float rmax = ex2f(kappa * dmax);                   // cap of rho, 1/rho (tc_phi_fact)
         const float* coef = reinterpret_cast<const float*>(smem + C::SM_COEF);
+        int* ticket = reinterpret_cast<int*>(smem + C::SM_BAR + 192) + quarter;
+        int cur = 0;                                             // batch this warp has not yet arrived for
+        bool ready = false;                                      // zfull of batch `cur` observed
+        for (;;) {
+            int t = 0;
+            if (lane == 0) t = atomicAdd(ticket, 1);
+            t = __shfl_sync(0xffffffffu, t, 0);
+            const int bt = t / npairs, pi = t - bt * npairs;
+            const int upto = bt < NB ? bt : NB;
+            if (cur < upto) {
+                tmem_st_wait();
+                tc_fence_before();
+                __syncwarp();
+                for (; cur < upto; ++cur)
+                    if (lane == 0) mbar_arrive(vdone + (cur & 1));
+                ready = false;
+            }
+            if (bt >= NB) break;
+            if (!ready) {
+                mbar_wait(zfull + (cur & 1), (cur >> 1) & 1);
+                tc_fence_after();
+                ready = true;
+            }
+            const uint32_t zrow0 = tl + (cur & 1) * 4 * nkp + 4 * pi, zrow1 = zrow0 + 2 * nkp;
+            uint32_t z0[4], z1[4], o0[4], o1[4];
+            tmem_ld4(zrow0, z0);
+            tmem_ld4(zrow1, z1);
+            tmem_ld_wait();
+#pragma unroll
+            for (int f = 0; f < 2; ++f) {
+                const float2 zc[2] = {make_float2(__uint_as_float(z0[2 * f]), __uint_as_float(z0[2 * f + 1])),
+                                      make_float2(__uint_as_float(z1[2 * f]), __uint_as_float(z1[2 * f + 1]))};
+                float2 v[2] = {{0.f, 0.f}, {0.f, 0.f}};
+                const int fidx = 2 * pi + f;
+                if (fact) tc_phi_fact(coef + fidx * (TNRD_FG * TNRD_FSTRIDE), kappa, dmax, rmax, zc, v);
+                else if (fidx < a.N_k) tc_phi_direct(a.prm + (size_t)fidx * C::PRM + prm_kkp(KS), zc, v);
+                split_bf16(v[0], o0[2 * f], o0[2 * f + 1]);
+                split_bf16(v[1], o1[2 * f], o1[2 * f + 1]);
+            }
+            tmem_st4(zrow0, o0);
+            tmem_st4(zrow1, o1);
+        }
+    } else if (warp < TC_PHI_WARPS + 4) {
+        // =================================== drain warps ===================================
+        // One warp per lane quarter: reads the scatter table of a batch, folds it over neighbouring lanes and over
+        // batches (shared memory, fixed order), and completes output rows (a5).
+        const int quarter = warp & 3;
+        const int L = quarter * 32 + lane;                       // tensor-memory lane = pixel pair
+        const uint32_t tl = tmem + ((uint32_t)(quarter * 32) << 16);
         float2* xbuf = reinterpret_cast<float2*>(smem + C::SM_X);      // [q][k][128]
         float2* oring = reinterpret_cast<float2*>(smem + C::SM_O);     // [8][128]
         const float lambda = a.lambda_ptr ? __ldg(a.lambda_ptr) : a.lambda_val;
-        const int q0 = 2 * sub;                                  // this warp folds table blocks q0, q0 + 1
-        const bool has_q = q0 <= KS;
         const int xcol = xs * C::OW + 2 * L;                     // image column of this lane's first pixel
         const bool lane_out = L < 128 - R;                       // lanes whose output pixels this strip completes
-
-        auto drain = [&](int b) {
-            mbar_wait(tfull, b & 1);
+        constexpr int NQ = KS + 1;                               // table blocks with content
+        for (int b = 0; b < NB; ++b) {
+            mbar_wait_idle(tfull, b & 1);
             tc_fence_after();
-            uint32_t t[16];
-            if (has_q) { tmem_ld16(tl + TC_TCOL + 8 * q0, t); tmem_ld_wait(); }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(tfree);
-            bar_phi();                                           // the previous fold has finished reading xbuf
-            if (has_q) {
+            bar_drain();                                         // the previous fold has finished reading xbuf
+#pragma unroll 1
+            for (int q = 0; q < NQ; q += 2) {                    // two table blocks at a time (register count)
+                uint32_t tt[16];
+                tmem_ld16(tl + TC_TCOL + 8 * q, tt);
+                tmem_ld_wait();
 #pragma unroll
                 for (int qq = 0; qq < 2; ++qq)
 #pragma unroll
                     for (int k = 0; k < C::XK; ++k)
-                        xbuf[((q0 + qq) * C::XK + k) * 128 + L] =
-                            make_float2(__uint_as_float(t[8 * qq + 2 * k]), __uint_as_float(t[8 * qq + 2 * k + 1]));
+                        xbuf[((q + qq) * C::XK + k) * 128 + L] =
+                            make_float2(__uint_as_float(tt[8 * qq + 2 * k]), __uint_as_float(tt[8 * qq + 2 * k + 1]));
             }
-            bar_phi();
-            if (!has_q) return;
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tfree);
+            bar_drain();
+            // prefetch u and f of the two rows this batch completes
+            float uu[2][2], ff[2][2];
+            bool okr[2];
 #pragma unroll
             for (int qq = 0; qq < 2; ++qq) {
-                const int q = q0 + qq;
+                const int yrel = 2 * b + 1 - (KS - 1 + qq);
+                okr[qq] = yrel >= 0 && yrel < rows_out && lane_out;
+                const size_t base = ((size_t)img * a.H + ys0 + (okr[qq] ? yrel : 0)) * a.W;
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const bool ok = okr[qq] && xcol + e < a.W;
+                    uu[qq][e] = ok ? __ldg(a.u_in + base + xcol + e) : 0.f;
+                    ff[qq][e] = ok ? __ldg(a.f + base + xcol + e) : 0.f;
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) {
                 float2 o = make_float2(0.f, 0.f);
 #pragma unroll
                 for (int t2 = 0; t2 <= R; ++t2)                  // lanes L .. L + r reach this lane's pixel pair
@@ -388,50 +510,13 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
                 if (q >= 2) { const float2 p = *slot; o.x += p.x; o.y += p.y; }
                 if (q < KS - 1) { *slot = o; continue; }
                 // a5: the row is complete
-                if (yrel < 0 || yrel >= rows_out || !lane_out) continue;
+                const int qq = q - (KS - 1);
+                if (!okr[qq]) continue;
                 const size_t base = ((size_t)img * a.H + ys0 + yrel) * a.W;
-                if (xcol < a.W) {
-                    const float uu = __ldg(a.u_in + base + xcol), ff = __ldg(a.f + base + xcol);
-                    a.u_out[base + xcol] = uu - (o.x + lambda * (uu - ff));
-                }
-                if (xcol + 1 < a.W) {
-                    const float uu = __ldg(a.u_in + base + xcol + 1), ff = __ldg(a.f + base + xcol + 1);
-                    a.u_out[base + xcol + 1] = uu - (o.y + lambda * (uu - ff));
-                }
+                if (xcol < a.W) a.u_out[base + xcol] = uu[qq][0] - (o.x + lambda * (uu[qq][0] - ff[qq][0]));
+                if (xcol + 1 < a.W) a.u_out[base + xcol + 1] = uu[qq][1] - (o.y + lambda * (uu[qq][1] - ff[qq][1]));
             }
-        };
-
-        for (int b = 0; b < NB; ++b) {
-            const int bb = b & 1;
-            mbar_wait(zfull + bb, (b >> 1) & 1);
-            tc_fence_after();
-            const uint32_t zrow0 = tl + bb * 4 * nkp + 2 * fbase, zrow1 = zrow0 + 2 * nkp;
-            for (int fi = 0; fi < nf_sub; fi += 2) {
-                uint32_t z0[4], z1[4], o0[4], o1[4];
-                tmem_ld4(zrow0 + 2 * fi, z0);
-                tmem_ld4(zrow1 + 2 * fi, z1);
-                tmem_ld_wait();
-#pragma unroll
-                for (int f = 0; f < 2; ++f) {
-                    const float2 zc[2] = {make_float2(__uint_as_float(z0[2 * f]), __uint_as_float(z0[2 * f + 1])),
-                                          make_float2(__uint_as_float(z1[2 * f]), __uint_as_float(z1[2 * f + 1]))};
-                    float2 v[2] = {{0.f, 0.f}, {0.f, 0.f}};
-                    const int fidx = fbase + fi + f;
-                    if (fact) tc_phi_fact(coef + fidx * (TNRD_FG * TNRD_FSTRIDE), kappa, dmax, zc, v);
-                    else if (fidx < a.N_k) tc_phi_direct(a.prm + (size_t)fidx * C::PRM + prm_kkp(KS), zc, v);
-                    split_bf16(v[0], o0[2 * f], o0[2 * f + 1]);
-                    split_bf16(v[1], o1[2 * f], o1[2 * f + 1]);
-                }
-                tmem_st4(zrow0 + 2 * fi, o0);
-                tmem_st4(zrow1 + 2 * fi, o1);
-            }
-            tmem_st_wait();
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(vdone + bb);
-            if (b > 0) drain(b - 1);
         }
-        drain(NB - 1);
     } else if (warp == TC_MMA_WARP) {
         // =================================== MMA issuer ===================================
         if (lane == 0) {
@@ -456,15 +541,15 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
                 umma_commit(zfull + bb);
                 umma_commit(pempty + b % TC_NP);
             };
-            auto wait_pair = [&](int p) { mbar_wait(pfull + p % TC_NP, (p / TC_NP) & 1); };
+            auto wait_pair = [&](int p) { mbar_wait_idle(pfull + p % TC_NP, (p / TC_NP) & 1); };
             for (int p = 0; p <= R; ++p) wait_pair(p);
             tc_fence_after();
             forward(0);
             if (NB > 1) { wait_pair(R + 1); tc_fence_after(); forward(1); }
             for (int b = 0; b < NB; ++b) {
                 const int bb = b & 1;
-                mbar_wait(vdone + bb, (b >> 1) & 1);
-                if (b >= 1) mbar_wait(tfree, (b - 1) & 1);
+                mbar_wait_idle(vdone + bb, (b >> 1) & 1);
+                if (b >= 1) mbar_wait_idle(tfree, (b - 1) & 1);
                 tc_fence_after();
                 for (int rr = 1; rr >= 0; --rr) {                        // row 1 first: it initialises blocks 0 .. KS
                     const uint32_t d = tmem + TC_TCOL + (rr == 0 ? 8 : 0);
@@ -484,7 +569,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
         const int lt = tid - (TC_MMA_WARP + 1) * 32;
         for (int p = 0; p < NPAIRS; ++p) {
             const int slot = p % TC_NP;
-            if (p >= TC_NP) mbar_wait(pempty + slot, ((p / TC_NP) - 1) & 1);
+            if (p >= TC_NP) mbar_wait_idle(pempty + slot, ((p / TC_NP) - 1) & 1);
             for (int idx = lt; idx < 2 * TC_CWU; idx += TC_LOAD_WARPS * 32) {
                 const int rrow = idx / TC_CWU, xg = idx - rrow * TC_CWU;
                 const float* __restrict__ grow = u_img + (size_t)mirror_clamp(ys0 + 2 * p + rrow - 2 * R, a.H) * a.W;

@@ -11,6 +11,10 @@ torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
 
 MAX_ABS, RMS = 1e-2, 1e-3
+# Regression bound for the EXACT evaluators (factorised, direct, windowed; tile and tensor-core kernels): they sit at
+# ~3e-5 / 6e-6 from the oracle (fp32 rounding + ex2.approx), so 10 x that catches a loss of accuracy that the north_star
+# tolerance above would let through.
+TIGHT_MAX_ABS, TIGHT_RMS = 3e-4, 5e-5
 
 
 @pytest.fixture(scope="module")
@@ -48,11 +52,13 @@ def run_oracle(c, T=None):
                           c["lambda"][:T])
 
 
-def check(got, want, what=""):
+def check(got, want, what="", tight=False):
     err = got - want
     mx, rms = float(np.max(np.abs(err))), float(np.sqrt(np.mean(err ** 2)))
     assert np.all(np.isfinite(got)), what
     assert mx <= MAX_ABS and rms <= RMS, f"{what}: max-abs {mx:.3e} rms {rms:.3e}"
+    if tight:
+        assert mx <= TIGHT_MAX_ABS and rms <= TIGHT_RMS, f"{what}: max-abs {mx:.3e} rms {rms:.3e} (regression bound)"
     return mx, rms
 
 
@@ -69,7 +75,7 @@ SMALL = [  # seed, B, H, W, T, N_k, ksize
 def test_small_cases_match_oracle(tnrd, case, kernel):
     seed, B, H, W, T, n_k, K = case
     c = tnrd_gen.make_small(seed, B, H, W, T, n_k, K)
-    check(run_gpu(tnrd, c, kernel=kernel), run_oracle(c), f"case {case} kernel {kernel}")
+    check(run_gpu(tnrd, c, kernel=kernel), run_oracle(c), f"case {case} kernel {kernel}", tight=True)
 
 
 # --- BASELINE.json configs 1-3 in full ------------------------------------------------------------------------
@@ -77,7 +83,7 @@ def test_small_cases_match_oracle(tnrd, case, kernel):
 def test_configs_1_to_3_full_image(tnrd, cfg):
     c = tnrd_gen.make_config(cfg)
     want = run_oracle(c)
-    mx, rms = check(run_gpu(tnrd, c), want, f"config {cfg}")
+    mx, rms = check(run_gpu(tnrd, c), want, f"config {cfg}", tight=True)
     print(f"config {cfg}: max-abs {mx:.3e} rms {rms:.3e}")
     if cfg == 2:   # transposed orientation of the stand-in image (reading S14)
         ct = dict(c, H=c["W"], W=c["H"], f=np.ascontiguousarray(c["f"].transpose(0, 2, 1)),
@@ -231,20 +237,9 @@ def test_microbench_rates_are_sane(tnrd):
     ffma, mufu, phi = (tnrd.tnrd_microbench(i) for i in range(3))
     print(f"FFMA {ffma / 1e12:.2f} T/s  MUFU.EX2 {mufu / 1e12:.2f} T/s  phi terms {phi / 1e12:.2f} T/s")
     assert 5e12 < ffma < 60e12 and 1e12 < mufu < 12e12 and 0.5e12 < phi <= mufu * 1.05
-    tf32, bf16 = tnrd.tnrd_microbench(3), tnrd.tnrd_microbench(4)     # mma.sync multiply-adds per second
-    print(f"mma.sync TF32 {2 * tf32 / 1e12:.0f} TFLOP/s  BF16 {2 * bf16 / 1e12:.0f} TFLOP/s")
-    assert ffma < tf32 < bf16 < 2e15
-    # prototype of the forward bank on that path (BF16 x3 split, A fragments gathered tap by tap); the call fails if its
-    # device-side comparison with plain fp32 FMAs does
-    fwd = tnrd.tnrd_microbench(5)
-    print(f"forward bank 48 x 7x7 by mma.sync BF16 x3: {fwd / 1e9:.1f} Gpixel/s (FFMA pipe alone: {ffma / 2352 / 1e9:.1f})")
-    assert 2e9 < fwd < bf16 / (48 * 64 * 3)
-    fwd_phi = tnrd.tnrd_microbench(6)      # ... followed by the factorised phi on the accumulator fragments
-    print(f"forward bank + factorised phi on the accumulators: {fwd_phi / 1e9:.2f} Gpixel/s (XU roofline {mufu / 720 / 1e9:.2f})")
-    assert 1e9 < fwd_phi < min(fwd, mufu / 720)
-    no_fold = tnrd.tnrd_microbench(7)      # ... followed by the transposed bank as a scatter table (fold not included)
-    print(f"forward bank + phi + scatter table (no fold): {no_fold / 1e9:.2f} Gpixel/s")
-    assert 1e9 < no_fold < fwd_phi
+    with pytest.raises(tnrd.TnrdError) as ei:
+        tnrd.tnrd_microbench(3)
+    assert ei.value.status == tnrd.ERR_UNSUPPORTED
 
 
 # --- windowed phi evaluator (tnrd_set_phi_mode(1)): same oracle, same tolerance ------------------------------------
