@@ -46,7 +46,7 @@ extern "C" {
 
 #define TNRD_NUM_RBF 63 /* M, PAPER.md:176 ("63 Gaussian RBFs") -- fixed by the model family */
 #define TNRD_MAX_FILTERS 128
-#define TNRD_VERSION 100 /* 0.1.0 */
+#define TNRD_VERSION 200 /* 0.2.0 */
 
 typedef enum {
     TNRD_OK = 0,
@@ -201,7 +201,7 @@ int tnrd_tc_plan_query(int B, int H, int W, int N_k, int ksize, int num_sms, lon
  *       rho would leave the fp32 range) the same kernel evaluates the direct form -- decided on the device, one launch.
  *       Weights with |w| * rbf_gamma beyond about 1e9 overflow in this form (the direct form holds up to ~1e38).
  *   TNRD_PHI_DENSE  (0): the direct form, one ex2 per Gaussian.
- *   TNRD_PHI_WINDOW (1): when rbf_mu is equidistant (|mu_j - mu_0 - j delta| <= 1e-4 delta, checked on the device by the
+ *   TNRD_PHI_WINDOW (1): when rbf_mu is equidistant to rounding (|mu_j - (mu_0 + j delta)| <= 1.5e-7 (|mu_0| + 62 delta), checked on the device by the
  *       staging kernel) and rbf_gamma <= delta, each response evaluates only the 14 consecutive centres around it that
  *       contain every centre within 6.5 gamma; the dropped terms are each below e^{-21.1} = 6.7e-10 of their weight, i.e.
  *       below fp32 rounding of the sum ("equidistant centers").  When the check
@@ -241,6 +241,19 @@ int tnrd_set_rbf_basis(int basis);
  * TNRD_NTY environment knobs.
  */
 int tnrd_plan_query(int B, int H, int W, int N_k, int ksize, int num_sms, long long* plan);
+
+/*
+ * Executed vs defined influence-function work of the tensor-core stage kernel.  The factorised evaluator skips a group
+ * of 13 centres when its Gaussian factor is exactly zero for every response of a warp (the result is bit-identical),
+ * so the run time depends on the responses; this call reports how much was skipped.  enable != 0 switches counting on
+ * for later calls on `stream` (process-wide flag, a few atomics per CTA), 0 switches it off; either way the counters
+ * gathered so far on this (device, stream) are returned and reset: *executed = (warp, filter, group) evaluations
+ * performed, *defined = evaluations the definition has (5 groups per filter and warp).  Synchronises `stream`.
+ * Either pointer may be NULL.  The tile kernel is not instrumented.  rbf_w must be finite: with a skipped group a
+ * non-finite weight does not turn the result into NaN (0 x Inf is never formed), so results for non-finite weights are
+ * unspecified.
+ */
+int tnrd_phi_stats(int enable, unsigned long long* executed, unsigned long long* defined, void* stream);
 
 /* Number of kernels this library has launched since load (or since the last tnrd_reset_launch_count). */
 unsigned long long tnrd_launch_count(void);

@@ -72,6 +72,8 @@ def lib() -> ctypes.CDLL:
         L.tnrd_plan_query.restype = ci
         L.tnrd_tc_plan_query.argtypes = [ci, ci, ci, ci, ci, ci, ctypes.POINTER(ctypes.c_longlong)]
         L.tnrd_tc_plan_query.restype = ci
+        L.tnrd_phi_stats.argtypes = [ci, ctypes.POINTER(ctypes.c_ulonglong), ctypes.POINTER(ctypes.c_ulonglong), vp]
+        L.tnrd_phi_stats.restype = ci
         L.tnrd_launch_count.restype = ctypes.c_ulonglong
         L.tnrd_reset_launch_count.restype = None
         L.tnrd_microbench.argtypes = [ci, ctypes.POINTER(ctypes.c_double), vp]
@@ -198,6 +200,14 @@ def tnrd_tc_plan_query(B, H, W, N_k, ksize, num_sms=148) -> dict:
     _check(lib().tnrd_tc_plan_query(B, H, W, N_k, ksize, num_sms, buf))
     keys = ("applies", "nxs", "nys", "seg_rows", "units", "out_cols")
     return dict(zip(keys, (int(v) for v in buf)))
+
+
+def tnrd_phi_stats(enable: bool, stream=None):
+    """(executed, defined) phi group evaluations of the tensor-core kernel since the last call; switches counting on or
+    off for later calls (include/tnrd.h: tnrd_phi_stats)."""
+    ex, de = ctypes.c_ulonglong(0), ctypes.c_ulonglong(0)
+    _check(lib().tnrd_phi_stats(int(bool(enable)), ctypes.byref(ex), ctypes.byref(de), _stream(stream)))
+    return int(ex.value), int(de.value)
 
 
 def tnrd_launch_count() -> int:

@@ -21,6 +21,7 @@ std::atomic<int> g_kernel{0};    // 0 auto, 1 reference, 2 fused tile kernel (FM
 std::atomic<int> g_phi_mode{3};  // 0 direct 63-term phi, 1 windowed evaluator (dense fallback decided on the device), 2 table,
                                  // 3 factorised 63-term phi (direct fallback inside the kernel)
 std::atomic<int> g_basis{0};     // 0 Gaussian radial basis, 1 triangular-shaped (table evaluator)
+std::atomic<int> g_stats{0};     // 1: the tensor-core kernel counts executed / defined phi group evaluations (tnrd_phi_stats)
 std::mutex g_mu;
 
 struct Opts {
@@ -61,6 +62,7 @@ struct Scratch {
     Buf split;                        // partial transposed-filter sums of the fused kernel's CTAs
     Buf pp;                           // ping-pong image plane of the tensor-core kernel (it cannot run in place)
     Buf tcws;                         // its Toeplitz operands, T stages
+    Buf stats;                        // two 64-bit counters (tnrd_phi_stats)
     Buf tab;                          // piecewise-linear phi tables [T][N_k][4096] float2 + 4 header floats
     Buf h_f, h_u, h_out, h_par;       // device staging of the host entry point
     Buf bw_maps, bw_part, bw_trace, bw_e[2];   // backward pass: P/V maps, per-CTA partial sums, iterates, dl/du planes
@@ -177,6 +179,14 @@ int run_stage(Call& c, tnrd::StageArgs a, int phi, int t)
     }
     if (c.tc) {
         if (a.u_out == a.u_in) return TNRD_ERR_ALIAS;        // callers ping-pong (run_stages)
+        if (g_stats.load()) {
+            if (!sc->stats.p) {
+                int rc = grow(sc->stats, 4, c.st);
+                if (rc != TNRD_OK) return rc;
+                TNRD_CUDA(cudaMemsetAsync(sc->stats.p, 0, 16, c.st));
+            }
+            a.stats = reinterpret_cast<unsigned long long*>(sc->stats.p);
+        }
         const tnrd::TcPlan pl = tnrd::plan_stage_tc(a.B, a.H, a.W, a.ksize, sc->num_sms);
         const unsigned char* ws = reinterpret_cast<const unsigned char*>(sc->tcws.p) +
                                   (size_t)t * tnrd::tc_ws_stage_stride(a.N_k, a.ksize);
@@ -539,6 +549,24 @@ int tnrd_tc_plan_query(int B, int H, int W, int N_k, int ksize, int num_sms, lon
     return TNRD_OK;
 }
 
+int tnrd_phi_stats(int enable, unsigned long long* executed, unsigned long long* defined, void* stream)
+{
+    g_stats = enable ? 1 : 0;
+    if (executed) *executed = 0;
+    if (defined) *defined = 0;
+    Scratch* sc = nullptr;
+    int rc = get_scratch((cudaStream_t)stream, &sc);
+    if (rc != TNRD_OK) return rc;
+    if (!sc->stats.p) return TNRD_OK;
+    unsigned long long h[2] = {0, 0};
+    TNRD_CUDA(cudaMemcpyAsync(h, sc->stats.p, 16, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    TNRD_CUDA(cudaMemsetAsync(sc->stats.p, 0, 16, (cudaStream_t)stream));
+    TNRD_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    if (executed) *executed = h[0];
+    if (defined) *defined = h[1];
+    return TNRD_OK;
+}
+
 int tnrd_set_kernel(int which)
 {
     if (which < 0 || which > 3) return TNRD_ERR_UNSUPPORTED;
@@ -596,7 +624,7 @@ void tnrd_shutdown(void)
     (void)cudaGetDevice(&cur);
     for (Scratch* s : g_scratch) {
         (void)cudaSetDevice(s->dev);
-        Buf* bufs[] = {&s->pp, &s->tcws, &s->prm, &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->refv, &s->split, &s->tab, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
+        Buf* bufs[] = {&s->pp, &s->tcws, &s->stats, &s->prm, &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->refv, &s->split, &s->tab, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
         for (Buf* b : bufs)
             if (b->p) (void)cudaFree(b->p);   // synchronising free: the stream may be gone by now
         delete s;

@@ -513,13 +513,11 @@ template <int KS, bool WANT_W, bool WANT_K>
 cudaError_t launch_bwd_cfg(const BwdArgs& a, const BwdPlan& pl, cudaStream_t st)
 {
     using C = BCfg<KS>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(stage_bwd_kernel<KS, WANT_W, WANT_K>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    // the opt-in is an attribute of the CURRENT device's copy of the kernel: set at every launch (cheap), so that a
+    // process that uses several devices works on each of them
+    cudaError_t e = cudaFuncSetAttribute(stage_bwd_kernel<KS, WANT_W, WANT_K>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    if (e != cudaSuccess) return e;
     stage_bwd_kernel<KS, WANT_W, WANT_K><<<(unsigned)pl.n_cta, C::NT, C::SMEM, st>>>(a, pl.ntx, pl.nty);
     return cudaGetLastError();
 }

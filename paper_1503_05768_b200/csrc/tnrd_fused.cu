@@ -502,8 +502,8 @@ stage_update_kernel(StageArgs a, const float* __restrict__ part, int tw, int th,
 #pragma unroll
     for (int q = 0; q < PX; ++q) {
         const bool ok = x0 + q < a.W;
-        uu[q] = ok ? __ldg(a.u_in + idx0 + q) : 0.f;
-        ff[q] = ok ? __ldg(a.f + idx0 + q) : 0.f;
+        uu[q] = ok ? a.u_in[idx0 + q] : 0.f;     // plain loads: u_out may be u_in (and f, deblocking) -- in place
+        ff[q] = ok ? a.f[idx0 + q] : 0.f;
         s[q] = 0.f;
     }
     for (int ty = tylo; ty <= tyhi; ++ty) {
@@ -651,13 +651,11 @@ template <int KS, int RW, int RH, int NT, int MINB, int PHI>
 cudaError_t launch_cfg(const StageArgs& a, const FusedPlan& pl, float* part, cudaStream_t st)
 {
     using C = Cfg<KS, RW, RH, NT, MINB>;
-    static bool attr_done = false;  // per-process; the attribute is per-function and sticky
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<KS, RW, RH, NT, MINB, PHI>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
+    // the opt-in is an attribute of the CURRENT device's copy of the kernel: set at every launch (cheap), so that a
+    // process that uses several devices works on each of them
+    cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<KS, RW, RH, NT, MINB, PHI>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    if (e != cudaSuccess) return e;
     const long long tiles = (long long)pl.ntx * pl.nty * a.B;
     const long long grid = pl.n_full + (tiles - pl.n_full) * pl.nsplit;
     if (grid > 0x7fffffffLL || pl.n_full > tiles || !part) return cudaErrorInvalidConfiguration;

@@ -24,8 +24,8 @@ namespace tnrd {
 //   pairs    at offset prm_kkp: 64 pairs (-mu'_j, w'_ij) = (-s * mu_j, w_ij / s), pair 63 = (0, 0)
 //   wplain   at offset prm_wplain: w'_ij, j = 0..63 (w'_i63 = 0), for the windowed phi evaluator's per-lane gathers
 //   hdr      at offset prm_hdr, 8 floats, the same in every record: (1/delta', mu'_0, delta', ok_w, kappa, D, ok_f, 0) --
-//            centre spacing in scaled units; ok_w = 1.0f when the centres are equidistant (|mu_j - mu_0 - j delta| <=
-//            1e-4 delta) and gamma <= delta (window of 14 centres then holds every centre within 6.5 gamma of any z);
+//            centre spacing in scaled units; ok_w = 1.0f when the centres are equidistant to rounding (|mu_j - (mu_0 +
+//            j delta)| <= 1.5e-7 (|mu_0| + 62 delta), a few ulp of the largest centre) and gamma <= delta (window of 14 centres then holds every centre within 6.5 gamma of any z);
 //            kappa = 2 delta', D and ok_f belong to the factorised evaluator (next item)
 //   fact     at offset prm_fact: TNRD_FG groups of TNRD_FSTRIDE floats for the factorised phi evaluator.  Group g has its
 //            anchor at centre a = g (2 S + 1) + S (S = TNRD_FS) and holds
@@ -69,6 +69,7 @@ struct StageArgs {
     int dense_is_fallback;  // set by the launcher: the dense kernel returns at once when the windowed one applies
     const float* tab;       // piecewise-linear phi tables of this stage [N_k][TNRD_TAB_NODES] float2 (phi evaluator 2)
     const float* tabhdr;    // their header (tnrd_table.cu), device
+    unsigned long long* stats;  // null, or device counters {phi group evaluations executed, defined} (tensor-core kernel)
 };
 
 // Launch plan of the fused stage kernel (tnrd_fused.cu: plan_stage_fused).  Tiles partition the phi region

@@ -49,7 +49,7 @@ __global__ void prep_params_kernel(const float* __restrict__ filters, const floa
                 bool ok = delta > 0.0f;
 #pragma unroll 9
                 for (int j = 0; j < TNRD_M; ++j)       // no early exit: the 63 loads are independent and overlap
-                    ok &= fabsf(__ldg(rbf_mu + j) - (mu0 + (float)j * delta)) <= 1e-4f * delta;
+                    ok &= fabsf(__ldg(rbf_mu + j) - fmaf((float)j, delta, mu0)) <= 1.5e-7f * (fabsf(mu0) + 62.0f * delta);   // a few ulp of the largest centre
                 if (h == 3) ok &= gamma <= delta * 1.000001f;
                 else {
                     const float reach = TNRD_FCLAMP - (float)TNRD_FS * ds;

@@ -33,7 +33,7 @@ build_phi_table_kernel(const float* __restrict__ rbf_w, const float* __restrict_
     for (int j = 0; j < TNRD_M; ++j) {
         const float mj = rbf_mu[j];
         lo = fminf(lo, mj); hi = fmaxf(hi, mj);
-        equi = equi && fabsf(mj - (mu0 + (float)j * delta)) <= 1e-4f * delta;
+        equi = equi && fabsf(mj - fmaf((float)j, delta, mu0)) <= 1.5e-7f * (fabsf(mu0) + 62.0f * delta);
     }
     const bool exact = basis == 1 && equi && fabsf(gamma - delta) <= 1e-5f * delta;
     int nodes;

@@ -207,9 +207,10 @@ __device__ __forceinline__ float ord2f(uint32_t o)
 {
     return __uint_as_float(o ^ ((o >> 31) - 1u | 0x80000000u));
 }
-__device__ __forceinline__ void tc_phi_fact(const float* __restrict__ crec, float kappa, float dmax, float rmax,
-                                            const float2 (&z)[2], float2 (&v)[2])
+__device__ __forceinline__ int tc_phi_fact(const float* __restrict__ crec, float kappa, float dmax, float rmax,
+                                           const float2 (&z)[2], float2 (&v)[2])
 {
+    int nlive = 0;                                               // groups evaluated (warp-uniform; statistics only)
     constexpr int S = TNRD_FS, GC = TNRD_FG / 2;
     // warp-wide range of the responses
     float zlo, zhi;
@@ -235,6 +236,7 @@ __device__ __forceinline__ void tc_phi_fact(const float* __restrict__ crec, floa
         float c[TNRD_FSTRIDE];
         lds_vec(crec + g * TNRD_FSTRIDE, c);
         if (!(any_nan || (wlo + c[0] < dmax && whi + c[0] > -dmax))) continue;    // dead for the whole warp
+        ++nlive;
         float2 gg[2], rho[2], rhoi[2], h[2], hl[2];
 #pragma unroll
         for (int p = 0; p < 2; ++p) {
@@ -265,6 +267,7 @@ __device__ __forceinline__ void tc_phi_fact(const float* __restrict__ crec, floa
             v[p] = __ffma2_rn(gg[p], h[p], v[p]);
         }
     }
+    return nlive;
 }
 
 // Direct form (one ex2 per Gaussian) for centre sets the factorisation does not cover; (-mu', w') pairs from the
@@ -328,7 +331,7 @@ __global__ void tc_prep_kernel(const float* __restrict__ prm, int T, int N_k, in
 // ---- the stage kernel ------------------------------------------------------------------------------------------
 // grid: one CTA per unit = (image, row segment, strip); the unit completes output rows [ys0, ys1) x columns
 // [xs OW, xs OW + OW) from phi rows [ys0, ys1 + 2r) x phi columns [xs OW, xs OW + 256) (phi coordinates = image + r).
-template <int KS>
+template <int KS, bool STATS>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int nxs, int nys, int seg_rows)
 {
@@ -407,6 +410,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
         const float rmax = ex2f(kappa * dmax);                   // cap of rho, 1/rho (tc_phi_fact)
         const float* coef = reinterpret_cast<const float*>(smem + C::SM_COEF);
         int* ticket = reinterpret_cast<int*>(smem + C::SM_BAR + 192) + quarter;
+        int nlive = 0, nfilt = 0;                                // statistics: groups evaluated, filters evaluated
         int cur = 0;                                             // batch this warp has not yet arrived for
         bool ready = false;                                      // zfull of batch `cur` observed
         for (;;) {
@@ -440,13 +444,21 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
                                       make_float2(__uint_as_float(z1[2 * f]), __uint_as_float(z1[2 * f + 1]))};
                 float2 v[2] = {{0.f, 0.f}, {0.f, 0.f}};
                 const int fidx = 2 * pi + f;
-                if (fact) tc_phi_fact(coef + fidx * (TNRD_FG * TNRD_FSTRIDE), kappa, dmax, rmax, zc, v);
+                if (fact) {
+                    const int nl = tc_phi_fact(coef + fidx * (TNRD_FG * TNRD_FSTRIDE), kappa, dmax, rmax, zc, v);
+                    if (STATS) nlive += nl;
+                }
                 else if (fidx < a.N_k) tc_phi_direct(a.prm + (size_t)fidx * C::PRM + prm_kkp(KS), zc, v);
                 split_bf16(v[0], o0[2 * f], o0[2 * f + 1]);
                 split_bf16(v[1], o1[2 * f], o1[2 * f + 1]);
             }
             tmem_st4(zrow0, o0);
             tmem_st4(zrow1, o1);
+            if (STATS) nfilt += 2;
+        }
+        if (STATS && a.stats && lane == 0 && fact) {
+            atomicAdd(a.stats, (unsigned long long)nlive);
+            atomicAdd(a.stats + 1, (unsigned long long)nfilt * TNRD_FG);
         }
     } else if (warp < TC_PHI_WARPS + 4) {
         // =================================== drain warps ===================================
@@ -624,6 +636,8 @@ TcPlan plan_stage_tc(int B, int H, int W, int ksize, int num_sms)
     const int forced = tc_env_int("TNRD_TC_SEG");
     for (int nys = 1; nys <= (H + 3) / 4; ++nys) {
         int seg = (H + nys - 1) / nys;
+        seg += seg & 1;                 // even: every segment then starts on an even row, so a pixel's arithmetic (the
+                                        // pairing of phi rows into batches) does not depend on how the rows are cut up
         if (forced > 0) seg = forced < H ? forced : H;
         const int n = (H + seg - 1) / seg;
         const long long units = (long long)B * pl.nxs * n;
@@ -653,10 +667,13 @@ template <int KS>
 static cudaError_t launch_tc_ks(const StageArgs& a, const TcPlan& pl, const unsigned char* ws_t, int nkp, cudaStream_t st)
 {
     using C = TcCfg<KS>;
-    cudaError_t e = cudaFuncSetAttribute(stage_tc_kernel<KS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+    // the opt-in shared-memory size is a per-device function attribute: set it at every launch (cheap) so that any
+    // device of the process works
+    auto kern = a.stats ? stage_tc_kernel<KS, true> : stage_tc_kernel<KS, false>;    // counting costs registers: own instance
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     if (e != cudaSuccess) return e;
     if (pl.units > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    stage_tc_kernel<KS><<<(unsigned)pl.units, TC_THREADS, C::SMEM, st>>>(a, ws_t, nkp, pl.nxs, pl.nys, pl.seg_rows);
+    kern<<<(unsigned)pl.units, TC_THREADS, C::SMEM, st>>>(a, ws_t, nkp, pl.nxs, pl.nys, pl.seg_rows);
     return cudaGetLastError();
 }
 

@@ -41,7 +41,7 @@ def test_python_binding_has_the_same_names():
 
 
 def test_version_and_strerror(L):
-    assert tnrd.tnrd_version() == 100
+    assert tnrd.tnrd_version() == 200
     assert tnrd.tnrd_strerror(0) == "ok"
     for code in range(-6, 0):
         assert tnrd.tnrd_strerror(code) not in ("", "unknown status")
@@ -84,7 +84,19 @@ def test_argument_validation_without_gpu(L):
     assert L.tnrd_set_phi_mode(tnrd.PHI_FACTORED) == tnrd.OK
     # options
     assert L.tnrd_set_kernel(7) == tnrd.ERR_UNSUPPORTED
-    assert L.tnrd_set_kernel(0) == tnrd.OK
+    assert L.tnrd_set_kernel(3) == tnrd.OK and L.tnrd_set_kernel(0) == tnrd.OK
+    # backward pass: the forward result may not overwrite what the gradients are formed from
+    bw = (1, 16, 16, 2, 4, 3, p, p, p, 10.0, p)
+    assert L.tnrd_diffuse_backward(p, p + 64, p + 128, n, *bw, p + 128, n, n, n, n, st) == tnrd.ERR_ALIAS    # u_T == u_gt
+    assert L.tnrd_diffuse_backward(p, p + 64, n, p + 128, *bw, p + 128, n, n, n, n, st) == tnrd.ERR_ALIAS    # u_T == e_T
+    assert L.tnrd_diffuse_backward(p, p + 64, p + 128, n, *bw, p + 192, p + 192, n, n, n, st) == tnrd.ERR_ALIAS  # u_T == grad_u0
+    assert L.tnrd_diffuse_backward(p, p + 64, p + 128, n, *bw, p + 64, n, n, n, n, st) == tnrd.ERR_ALIAS     # u_T == u0
+    # tensor-core plan query: pure host logic
+    q = (ctypes.c_longlong * 6)()
+    assert L.tnrd_tc_plan_query(1, 4096, 4096, 48, 7, 148, q) == tnrd.OK and q[0] == 2 and q[1] == 17 and q[5] == 250
+    assert q[4] == q[1] * q[2] and q[3] % 2 == 0
+    assert L.tnrd_tc_plan_query(1, 64, 64, 8, 3, 148, q) == tnrd.OK and q[0] == 0
+    assert L.tnrd_tc_plan_query(1, 64, 64, 8, 3, 148, None) == tnrd.ERR_NULL
     assert L.tnrd_microbench(0, None, st) == tnrd.ERR_NULL
     r = ctypes.c_double()
     assert L.tnrd_microbench(9, ctypes.byref(r), st) == tnrd.ERR_UNSUPPORTED

@@ -57,3 +57,27 @@ def test_diffuse_is_graph_capturable_and_replay_is_identical():
     flipped = np.ascontiguousarray(c["f"][:, ::-1, :])
     want = oracle.diffuse(flipped, flipped, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"], c["lambda"])
     assert np.max(np.abs(got - want)) <= 1e-2
+
+
+def test_scratch_growth_during_capture_is_refused():
+    """include/tnrd.h: a call that would have to grow the library scratch while its stream is being captured returns
+    TNRD_ERR_CUDA instead of caching a graph-owned allocation."""
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1503_05768_b200 as tnrd
+    tnrd.build(); tnrd.lib()
+    c = tnrd_gen.make_small(77, 1, 50, 60, 1, 4, 5)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()   # noqa: E731
+    f, k, w, mu, lam = d(c["f"]), d(c["filters"]), d(c["rbf_w"]), d(c["rbf_mu"]), d(c["lambda"])
+    out = torch.empty_like(f)
+    s = torch.cuda.Stream()                             # a fresh stream: no scratch yet for (device, stream)
+    with torch.cuda.stream(s):
+        g = torch.cuda.CUDAGraph()
+        with pytest.raises(tnrd.TnrdError) as ei:
+            with torch.cuda.graph(g, stream=s):
+                tnrd.tnrd_diffuse(f, f, 1, 50, 60, 1, 4, 5, k, w, mu, c["rbf_gamma"], lam, out, s)
+        assert ei.value.status == tnrd.ERR_CUDA and "capture" in str(ei.value)
+    s.synchronize()
+    tnrd.tnrd_diffuse(f, f, 1, 50, 60, 1, 4, 5, k, w, mu, c["rbf_gamma"], lam, out)     # the library is still usable
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(out).all())

@@ -234,3 +234,81 @@ def test_automatic_kernel_choice(tnrd):
     tnrd.tnrd_reset_launch_count()
     run_gpu(tnrd, c)
     assert tnrd.tnrd_launch_count() == 2 + c["T"]
+
+
+def test_nearly_equidistant_centres_take_the_direct_form(tnrd):
+    """Centres jittered by 5e-5 of their spacing are NOT equidistant to rounding: both stage kernels must evaluate the
+    direct form with the centres as given (the factorised identity would silently move them onto the ideal grid)."""
+    c = tnrd_gen.make_small(260, 1, 60, 270, 2, 8, 7)
+    r = np.random.default_rng(3)
+    mu = (c["rbf_mu"].astype(np.float64) + 5e-5 * 10.0 * r.uniform(-1, 1, 63)).astype(np.float32)
+    big = dict(c, rbf_mu=mu, rbf_w=(c["rbf_w"] * 40.0).astype(np.float32))      # large weights make a moved centre visible
+    want = run_oracle(big)
+    scale = float(np.max(np.abs(want - big["f"].astype(np.float64))))
+    for kernel in (2, 3):
+        got = run_gpu(tnrd, big, kernel=kernel)
+        assert np.max(np.abs(got - want)) <= 1.5e-5 * scale, kernel         # fp32 level, relative to the update
+    tnrd.tnrd_set_phi_mode(0)
+    try:
+        direct = run_gpu(tnrd, big, kernel=2)
+    finally:
+        tnrd.tnrd_set_phi_mode(tnrd.PHI_FACTORED)
+    assert np.array_equal(run_gpu(tnrd, big, kernel=2), direct), "same launch, direct form"
+
+
+def test_phi_statistics_counters(tnrd, monkeypatch):
+    """tnrd_phi_stats: executed <= defined, defined = 5 groups x filters x warps x stages; results unchanged by counting;
+    a constant image (z = 0) leaves 2 of 5 groups executed."""
+    c = tnrd_gen.make_small(261, 1, 64, 500, 2, 16, 7)
+    monkeypatch.setenv("TNRD_TC_SEG", "16")
+    ref = run_gpu(tnrd, c, kernel=3)
+    tnrd.tnrd_phi_stats(True)
+    got = run_gpu(tnrd, c, kernel=3)
+    ex, de = tnrd.tnrd_phi_stats(False)
+    assert np.array_equal(got, ref)
+    pl = tnrd.tnrd_tc_plan_query(1, 64, 500, 16, 7, num_sms())
+    batches = (pl["seg_rows"] + 6 + 1) // 2                    # per unit (every segment has seg_rows rows here)
+    assert 64 % pl["seg_rows"] == 0
+    assert de == 5 * 16 * 4 * batches * pl["units"] * c["T"], "5 groups x filters x lane quarters x batches x CTAs x stages"
+    assert 0 < ex <= de
+    flat = dict(c, f=np.full_like(c["f"], 100.0), u0=np.full_like(c["f"], 100.0))     # z = 0 everywhere
+    tnrd.tnrd_phi_stats(True)
+    run_gpu(tnrd, flat, kernel=3, T=1)
+    ex, de = tnrd.tnrd_phi_stats(False)
+    assert 5 * ex == 2 * de, "z = 0 is within reach (133) of the anchors at -110 and 20 only"
+    run_gpu(tnrd, c, kernel=3)
+    assert tnrd.tnrd_phi_stats(False) == (0, 0), "counting is off"
+
+
+def test_non_finite_weights_are_unspecified_but_harmless(tnrd):
+    """include/tnrd.h: rbf_w must be finite.  An infinite weight on a centre no response comes near is skipped with its
+    group, so every output pixel is either non-finite or the result with that weight zeroed; nothing faults."""
+    c = tnrd_gen.make_small(262, 1, 40, 260, 1, 8, 7)
+    w = c["rbf_w"].copy(); w[:, :, 62] = np.inf
+    w0 = c["rbf_w"].copy(); w0[:, :, 62] = 0.0
+    for kernel in (2, 3):
+        got = run_gpu(tnrd, dict(c, rbf_w=w), kernel=kernel)
+        ref = run_gpu(tnrd, dict(c, rbf_w=w0), kernel=kernel)
+        ok = ~np.isfinite(got) | (np.abs(got - ref) <= 1e-4)
+        assert ok.all(), kernel
+
+
+def test_two_devices_in_one_process(tnrd):
+    """The opt-in shared-memory attribute is per device: the first call on a second GPU must work."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    c = tnrd_gen.make_small(263, 1, 80, 300, 2, 8, 7)
+    want = run_oracle(c)
+    for kernel in (2, 3):
+        with torch.cuda.device(1):
+            tnrd.tnrd_set_kernel(kernel)
+            try:
+                f = torch.from_numpy(c["f"]).cuda(1)
+                out = torch.empty_like(f)
+                d1 = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda(1)   # noqa: E731
+                tnrd.tnrd_diffuse(f, f, 1, 80, 300, 2, 8, 7, d1(c["filters"]), d1(c["rbf_w"]), d1(c["rbf_mu"]),
+                                  c["rbf_gamma"], d1(c["lambda"]), out)
+                torch.cuda.synchronize()
+            finally:
+                tnrd.tnrd_set_kernel(0)
+            check(out.cpu().numpy().astype(np.float64), want, f"device 1 kernel {kernel}", tight=True)
