@@ -197,7 +197,8 @@ __device__ __forceinline__ float fmin_nan(float x, float lim)           // NaN s
 // number of centres apart), capped at 2^{kappa D} (beyond |d_g| = D the Gaussian factor 2^{-d_g^2} has flushed to
 // zero, so the cap changes no value and keeps rho^S finite): 2 + TNRD_FG ex2 per response instead of 3 TNRD_FG.
 // A group is skipped when its Gaussian factor is zero for every response of the warp (an exact 0 either way): the
-// decision is warp-uniform, from the warp's smallest and largest response (NaN responses keep every group live).
+// loop runs over the groups within reach D of the warp's smallest .. largest response (NaN responses keep every
+// group live); ganch = mu' of the first group's anchor, ginv = 1 / (anchor spacing).
 __device__ __forceinline__ uint32_t f2ord(float x)            // order-preserving map float -> uint32
 {
     const uint32_t b = __float_as_uint(x);
@@ -208,18 +209,24 @@ __device__ __forceinline__ float ord2f(uint32_t o)
     return __uint_as_float(o ^ ((o >> 31) - 1u | 0x80000000u));
 }
 __device__ __forceinline__ int tc_phi_fact(const float* __restrict__ crec, float kappa, float dmax, float rmax,
-                                           const float2 (&z)[2], float2 (&v)[2])
+                                           float ganch, float ginv, const float2 (&z)[2], float2 (&v)[2])
 {
-    int nlive = 0;                                               // groups evaluated (warp-uniform; statistics only)
     constexpr int S = TNRD_FS, GC = TNRD_FG / 2;
-    // warp-wide range of the responses
+    // warp-wide range of the responses -> the range of groups that are live for some response of the warp: group g
+    // (anchor mu'_0a + g * spacing) is live iff  wlo - mu'_g < D  and  whi - mu'_g > -D
     float zlo, zhi;
     asm("min.NaN.f32 %0, %1, %2;" : "=f"(zlo) : "f"(fminf(z[0].x, z[0].y)), "f"(fminf(z[1].x, z[1].y)));
     asm("max.NaN.f32 %0, %1, %2;" : "=f"(zhi) : "f"(fmaxf(z[0].x, z[0].y)), "f"(fmaxf(z[1].x, z[1].y)));
     const bool lane_nan = (z[0].x != z[0].x) || (z[0].y != z[0].y) || (z[1].x != z[1].x) || (z[1].y != z[1].y);
     const float wlo = ord2f(__reduce_min_sync(0xffffffffu, f2ord(zlo)));
     const float whi = ord2f(__reduce_max_sync(0xffffffffu, f2ord(zhi)));
-    const bool any_nan = __any_sync(0xffffffffu, lane_nan);
+    int g0 = 0, g1 = TNRD_FG - 1;
+    if (!__any_sync(0xffffffffu, lane_nan)) {
+        // float -> int conversions saturate, so far-away responses (or an empty range) need no special case
+        g0 = max(0, __float2int_rd((wlo - dmax - ganch) * ginv) + 1);
+        g1 = min(TNRD_FG - 1, __float2int_ru((whi + dmax - ganch) * ginv) - 1);
+    }
+    if (g0 > g1) return 0;
     // the shared exponential pair (middle group)
     float2 rho0[2], rhoi0[2];
     {
@@ -231,12 +238,10 @@ __device__ __forceinline__ int tc_phi_fact(const float* __restrict__ crec, float
             rhoi0[p] = make_float2(ex2f(-e.x), ex2f(-e.y));
         }
     }
-#pragma unroll
-    for (int g = 0; g < TNRD_FG; ++g) {
+#pragma unroll 1
+    for (int g = g0; g <= g1; ++g) {
         float c[TNRD_FSTRIDE];
         lds_vec(crec + g * TNRD_FSTRIDE, c);
-        if (!(any_nan || (wlo + c[0] < dmax && whi + c[0] > -dmax))) continue;    // dead for the whole warp
-        ++nlive;
         float2 gg[2], rho[2], rhoi[2], h[2], hl[2];
 #pragma unroll
         for (int p = 0; p < 2; ++p) {
@@ -267,7 +272,7 @@ __device__ __forceinline__ int tc_phi_fact(const float* __restrict__ crec, float
             v[p] = __ffma2_rn(gg[p], h[p], v[p]);
         }
     }
-    return nlive;
+    return g1 - g0 + 1;
 }
 
 // Direct form (one ex2 per Gaussian) for centre sets the factorisation does not cover; (-mu', w') pairs from the
@@ -408,6 +413,8 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
         const float kappa = __ldg(a.prm + prm_hdr(KS) + 4), dmax = __ldg(a.prm + prm_hdr(KS) + 5);
         const bool fact = __ldg(a.prm + prm_hdr(KS) + 6) != 0.0f;
         const float rmax = ex2f(kappa * dmax);                   // cap of rho, 1/rho (tc_phi_fact)
+        const float dsp = __ldg(a.prm + prm_hdr(KS) + 2);        // centre spacing in scaled units
+        const float ganch = __ldg(a.prm + prm_hdr(KS) + 1) + (float)TNRD_FS * dsp, ginv = 1.0f / ((float)TNRD_FM * dsp);
         const float* coef = reinterpret_cast<const float*>(smem + C::SM_COEF);
         int* ticket = reinterpret_cast<int*>(smem + C::SM_BAR + 192) + quarter;
         int nlive = 0, nfilt = 0;                                // statistics: groups evaluated, filters evaluated
@@ -445,7 +452,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
                 float2 v[2] = {{0.f, 0.f}, {0.f, 0.f}};
                 const int fidx = 2 * pi + f;
                 if (fact) {
-                    const int nl = tc_phi_fact(coef + fidx * (TNRD_FG * TNRD_FSTRIDE), kappa, dmax, rmax, zc, v);
+                    const int nl = tc_phi_fact(coef + fidx * (TNRD_FG * TNRD_FSTRIDE), kappa, dmax, rmax, ganch, ginv, zc, v);
                     if (STATS) nlive += nl;
                 }
                 else if (fidx < a.N_k) tc_phi_direct(a.prm + (size_t)fidx * C::PRM + prm_kkp(KS), zc, v);
