@@ -110,21 +110,20 @@ class ClockSampler:
 
 def measured_traffic(kernel_substr: str, lib_version: int):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the kernels whose name contains kernel_substr, from the
-    CSV the committed ncu command wrote (profiles/r02_launches.md).  None unless the file exists and its first line names
-    this library version."""
+    CSV the committed ncu command wrote (profiles/r02_dram_stage.csv; the command and the library version it profiled are
+    in profiles/r02_launches.md).  None unless both files exist and the .md names this library version."""
     try:
         import csv
-        lines = open(TRAFFIC_CSV).read().splitlines()
-        if not lines or f"tnrd_version={lib_version}" not in lines[0]:
+        md = open(os.path.join(ROOT, "profiles", "r02_launches.md")).read()
+        if f"tnrd_version={lib_version}" not in md:
             return None
-        rows = list(csv.DictReader([ln for ln in lines if ln.startswith('"')]))
+        lines = [ln for ln in open(TRAFFIC_CSV).read().splitlines() if ln.startswith('"')]
         per = {}
-        for r in rows:
+        for r in csv.DictReader(lines):
             if kernel_substr in r.get("Kernel Name", "") and r.get("Metric Name", "").startswith("dram__bytes_"):
                 v = float(r["Metric Value"].replace(",", ""))
                 v *= {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}.get(r.get("Metric Unit", "byte"), 1.0)
-                per.setdefault(r["ID"], 0.0)
-                per[r["ID"]] += v
+                per[r["ID"]] = per.get(r["ID"], 0.0) + v
         return float(np.mean(list(per.values()))) if per else None
     except Exception:
         return None
@@ -185,6 +184,8 @@ def main():
     ap.add_argument("--T", type=int, default=5)
     ap.add_argument("--ref-seconds", type=float, default=10.0, help="CPU seconds per oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "tile", "tc"],
+                    help="stage kernel (tnrd_set_kernel): auto (default), the tile kernel, the tensor-core kernel; profiling")
     ap.add_argument("--no-window", action="store_true", help="skip the extra windowed-phi measurement")
     ap.add_argument("--shard", default="images", choices=["images", "slab"],
                     help="N > 1: 'images' = one image per GPU (weak scaling, default); 'slab' = ONE image split into row "
@@ -208,6 +209,8 @@ def main():
         raise SystemExit("bench.py needs a CUDA device: the TNRD hot path has no CPU fallback")
     tnrd.build()
     tnrd.lib()
+    kernel_sel = {"auto": tnrd.KERNEL_AUTO, "tile": tnrd.KERNEL_TILE, "tc": tnrd.KERNEL_TC}[args.kernel]
+    tnrd.tnrd_set_kernel(kernel_sel)
     torch.cuda.set_device(local_rank)
     devs = torch.device("cuda", local_rank)
     if world > 1:
@@ -353,7 +356,7 @@ def main():
         tnrd.tnrd_set_kernel(tnrd.KERNEL_TILE)
         ms_t = timed()
         tile_out = out.clone()
-        tnrd.tnrd_set_kernel(tnrd.KERNEL_AUTO)
+        tnrd.tnrd_set_kernel(kernel_sel)
         tile = px_stages_all / (ms_t * 1e-3) / 1e6
         tnrd.tnrd_set_phi_mode(0)
         for _ in range(warmup):
@@ -411,7 +414,7 @@ def main():
     # formulation each implements give one time per pipe, the largest is the roofline (SURVEY.md 8d accounting rule).
     sms = torch.cuda.get_device_properties(devs).multi_processor_count
     tcq = tnrd.tnrd_tc_plan_query(B, H, W, N_K, KSIZE, sms)
-    use_tc = tcq["applies"] == 2
+    use_tc = (tcq["applies"] == 2 and args.kernel == "auto") or (tcq["applies"] >= 1 and args.kernel == "tc")
     launch_s = (ms * 1e-3) / (args.steps * T)           # step time / T: the staging kernels (~us) are charged too
     fma_peak = NOMINAL_SMS * FMA_PER_CLK_SM * NOMINAL_SM_MHZ * 1e6 / 1e12
     xu_peak = NOMINAL_SMS * MUFU_PER_CLK_SM * NOMINAL_SM_MHZ * 1e6 / 1e12

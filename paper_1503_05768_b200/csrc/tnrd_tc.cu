@@ -152,14 +152,6 @@ __device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t (&r)[4])
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(taddr));
 }
-__device__ __forceinline__ void tmem_ld2(uint32_t taddr, uint32_t (&r)[2])
-{
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "r"(taddr));
-}
-__device__ __forceinline__ void tmem_st2(uint32_t taddr, const uint32_t (&r)[2])
-{
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" :: "r"(taddr), "r"(r[0]), "r"(r[1]) : "memory");
-}
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
 {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
@@ -183,19 +175,16 @@ __device__ __forceinline__ float ex2f(float x)
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-__device__ __forceinline__ float fmin_nan(float x, float lim)           // NaN stays NaN
-{
-    float y;
-    asm("min.NaN.f32 %0, %1, %2;" : "=f"(y) : "f"(x), "f"(lim));
-    return y;
-}
 
 // Factorised influence function (tnrd_internal.h "fact"; PAPER.md:553 with equidistant centres, :117) of the two
 // response pairs z[0], z[1] of one filter; crec = the filter's TNRD_FG group records in shared memory (broadcast
-// loads).  Per response: ONE pair rho0 = 2^{kappa d0}, 1/rho0 for the middle group; the other groups' rho_g =
-// 2^{kappa d_g} = rho0 K_g with the constants K_g = 2^{kappa (d_g - d0)} staged in the group record (anchors are a fixed
-// number of centres apart), capped at 2^{kappa D} (beyond |d_g| = D the Gaussian factor 2^{-d_g^2} has flushed to
-// zero, so the cap changes no value and keeps rho^S finite): 2 + TNRD_FG ex2 per response instead of 3 TNRD_FG.
+// loads; scaled at kernel start, see there).  Per response: ONE pair rho0 = 2^{kappa d0}, 1/rho0 for the middle
+// group; the other groups' rho_g = 2^{kappa d_g} = rho0 K_g with the constants K_g = 2^{kappa (d_g - d0)} staged in
+// the group record (anchors are a fixed number of centres apart), capped at R = 2^{kappa D} (beyond |d_g| = D the
+// Gaussian factor 2^{-d_g^2} has flushed to zero, so the cap changes no value and keeps rho^S finite): 2 + TNRD_FG
+// ex2 per response instead of 3 TNRD_FG.  The shared FMA / ALU dispatch is what binds this kernel, so
+// the scaling and the cap are ONE single-cycle instruction per value, x = sat(rho0 K_g / R) (a NaN response is
+// flushed to 0 here and comes back through the Gaussian factor).
 // A group is skipped when its Gaussian factor is zero for every response of the warp (an exact 0 either way): the
 // loop runs over the groups within reach D of the warp's smallest .. largest response (NaN responses keep every
 // group live); ganch = mu' of the first group's anchor, ginv = 1 / (anchor spacing).
@@ -208,7 +197,7 @@ __device__ __forceinline__ float ord2f(uint32_t o)
 {
     return __uint_as_float(o ^ ((o >> 31) - 1u | 0x80000000u));
 }
-__device__ __forceinline__ int tc_phi_fact(const float* __restrict__ crec, float kappa, float dmax, float rmax,
+__device__ __forceinline__ int tc_phi_fact(const float* __restrict__ crec, float kappa, float dmax,
                                            float ganch, float ginv, const float2 (&z)[2], float2 (&v)[2])
 {
     constexpr int S = TNRD_FS, GC = TNRD_FG / 2;
@@ -248,10 +237,9 @@ __device__ __forceinline__ int tc_phi_fact(const float* __restrict__ crec, float
             const float2 d = __fadd2_rn(z[p], make_float2(c[0], c[0]));
             const float2 t = __fmul2_rn(d, d);
             gg[p] = make_float2(ex2f(-t.x), ex2f(-t.y));
-            const float2 r = __fmul2_rn(rho0[p], make_float2(c[14], c[14]));
-            const float2 ri = __fmul2_rn(rhoi0[p], make_float2(c[15], c[15]));
-            rho[p] = make_float2(fmin_nan(r.x, rmax), fmin_nan(r.y, rmax));
-            rhoi[p] = make_float2(fmin_nan(ri.x, rmax), fmin_nan(ri.y, rmax));
+            // x = min(rho_g, R) / R, rho_g = rho0 K_g: c[14] = K_g / R, and the saturation to [0, 1] IS the cap
+            rho[p] = make_float2(__saturatef(rho0[p].x * c[14]), __saturatef(rho0[p].y * c[14]));
+            rhoi[p] = make_float2(__saturatef(rhoi0[p].x * c[15]), __saturatef(rhoi0[p].y * c[15]));
         }
 #pragma unroll
         for (int p = 0; p < 2; ++p) {
@@ -268,8 +256,9 @@ __device__ __forceinline__ int tc_phi_fact(const float* __restrict__ crec, float
             for (int p = 0; p < 2; ++p) hl[p] = __ffma2_rn(hl[p], rhoi[p], make_float2(c[S + 2 + q], c[S + 2 + q]));
 #pragma unroll
         for (int p = 0; p < 2; ++p) {
-            h[p] = __ffma2_rn(hl[p], rhoi[p], h[p]);
-            v[p] = __ffma2_rn(gg[p], h[p], v[p]);
+            // three register-pair operands make a packed FMA take 3.3 issue cycles instead of 2: two scalar FMAs here
+            h[p] = make_float2(fmaf(hl[p].x, rhoi[p].x, h[p].x), fmaf(hl[p].y, rhoi[p].y, h[p].y));
+            v[p] = make_float2(fmaf(gg[p].x, h[p].x, v[p].x), fmaf(gg[p].y, h[p].y, v[p].y));
         }
     }
     return g1 - g0 + 1;
@@ -381,6 +370,10 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
             else *reinterpret_cast<float4*>(dst) = make_float4(0.f, 0.f, 0.f, 0.f);
         }
     }
+    // The phi warps run Horner's rule in x = min(rho, R) / R with R = 2^{kappa D} (one saturating multiply does the
+    // scaling by K_g AND the cap, tc_phi_fact), so the coefficient of rho^j is scaled by R^|j| and K_g, 1/K_g by 1/R.
+    // |c_j| R^|j| <= |w'| 2^92 by the staging kernel's range check (tnrd_internal.h "fact").
+    const float tc_kappa = __ldg(a.prm + prm_hdr(KS) + 4), tc_dmax = __ldg(a.prm + prm_hdr(KS) + 5);
     if (tid == 0) {
         for (int i = 0; i < TC_NP; ++i) { mbar_init(pfull + i, TC_LOAD_WARPS); mbar_init(pempty + i, 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(zfull + i, 1); mbar_init(vdone + i, TC_PHI_WARPS); }
@@ -394,6 +387,22 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     cp_async_wait_all();
+    {
+        constexpr int CF = TNRD_FG * TNRD_FSTRIDE, S = TNRD_FS;
+        float* cf = reinterpret_cast<float*>(smem + C::SM_COEF);
+        for (int i = tid; i < nkp * CF / 4; i += TC_THREADS) {   // the same 16-byte pieces this thread copied above
+            if ((4 * i) / CF >= a.N_k) continue;
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int o = (4 * i + e) % TNRD_FSTRIDE;        // slot inside the group record
+                int pw = 0;                                      // power of R
+                if (o >= 1 && o <= S + 1) pw = S + 1 - o;        // c_S .. c_0
+                else if (o >= S + 2 && o <= 2 * S + 1) pw = 2 * S + 2 - o;   // c_-S .. c_-1
+                else if (o >= TNRD_FSTRIDE - 2) pw = -1;         // K_g, 1 / K_g
+                if (pw != 0) cf[4 * i + e] *= exp2f((float)pw * tc_kappa * tc_dmax);
+            }
+        }
+    }
     fence_async_smem();
     tc_fence_before();
     __syncthreads();
@@ -412,7 +421,6 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
         const int npairs = nkp >> 1;
         const float kappa = __ldg(a.prm + prm_hdr(KS) + 4), dmax = __ldg(a.prm + prm_hdr(KS) + 5);
         const bool fact = __ldg(a.prm + prm_hdr(KS) + 6) != 0.0f;
-        const float rmax = ex2f(kappa * dmax);                   // cap of rho, 1/rho (tc_phi_fact)
         const float dsp = __ldg(a.prm + prm_hdr(KS) + 2);        // centre spacing in scaled units
         const float ganch = __ldg(a.prm + prm_hdr(KS) + 1) + (float)TNRD_FS * dsp, ginv = 1.0f / ((float)TNRD_FM * dsp);
         const float* coef = reinterpret_cast<const float*>(smem + C::SM_COEF);
@@ -452,7 +460,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
                 float2 v[2] = {{0.f, 0.f}, {0.f, 0.f}};
                 const int fidx = 2 * pi + f;
                 if (fact) {
-                    const int nl = tc_phi_fact(coef + fidx * (TNRD_FG * TNRD_FSTRIDE), kappa, dmax, rmax, ganch, ginv, zc, v);
+                    const int nl = tc_phi_fact(coef + fidx * (TNRD_FG * TNRD_FSTRIDE), kappa, dmax, ganch, ginv, zc, v);
                     if (STATS) nlive += nl;
                 }
                 else if (fidx < a.N_k) tc_phi_direct(a.prm + (size_t)fidx * C::PRM + prm_kkp(KS), zc, v);
