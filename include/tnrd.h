@@ -265,6 +265,10 @@ void tnrd_reset_launch_count(void);
  *   which = 0: FP32 FFMA rate      -> *rate = FMA lane-operations per second (x2 = FLOP/s)
  *   which = 1: MUFU.EX2 rate       -> *rate = ex2 evaluations per second
  *   which = 2: the phi inner loop (FADD, FMUL, MUFU.EX2, FFMA per term) -> RBF terms per second
+ *   which = 3: FFMA2 (FMA pipe) and FMNMX (ALU pipe) interleaved 1:1 on independent registers -> WARP instructions per
+ *              second of the two together.  Each occupies its pipe for 2 cycles per warp; pipes that issued side by side
+ *              would give 148 x 4 x clock, one shared dispatch half of that; B200 measures 0.66 of it (DESIGN.md "Roofline":
+ *              the sum of FMA-pipe and ALU-pipe cycles is what the tensor-core stage kernel runs against)
  * Any other value: TNRD_ERR_UNSUPPORTED.
  */
 int tnrd_microbench(int which, double* rate, void* stream);

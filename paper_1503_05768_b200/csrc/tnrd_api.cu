@@ -594,7 +594,7 @@ void tnrd_reset_launch_count(void) { g_launches = 0; }
 int tnrd_microbench(int which, double* rate, void* stream)
 {
     if (!rate) return TNRD_ERR_NULL;
-    if (which < 0 || which > 2) return TNRD_ERR_UNSUPPORTED;
+    if (which < 0 || which > 3) return TNRD_ERR_UNSUPPORTED;
     LaunchCount lc;
     TNRD_CUDA(tnrd::run_microbench(which, rate, (cudaStream_t)stream, &lc.n));
     return TNRD_OK;

@@ -80,6 +80,36 @@ __global__ void __launch_bounds__(MB_THREADS, 1) mb_phi(float* out, int iters)
     if (s == 123.456f) out[0] = s;
 }
 
+// FFMA2 (FMA pipe, 2 cycles per warp) and FMNMX (ALU pipe, 2 cycles per warp) interleaved 1:1 on independent registers,
+// 6 warps per scheduler.  Pipes that issued side by side would sustain 1.0 warp instructions per clock per scheduler
+// (0.5 each), one fully shared dispatch 0.5; B200 measures 0.66: the FMA and ALU pipes overlap only in part.  The
+// tensor-core stage kernel runs with FMA-pipe cycles + ALU-pipe cycles = 87 % of the time.
+__global__ void __launch_bounds__(768, 1) mb_dispatch(float* out, int iters, float x, float y)
+{
+    float2 h[4], r[4];
+    float m[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        h[k] = make_float2((float)(threadIdx.x + k), 1.0f);
+        r[k] = make_float2(x + 1e-7f * (float)threadIdx.x, x);
+        m[k] = (float)(threadIdx.x * 3 + k);
+    }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int rep = 0; rep < 16; ++rep)
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                h[k] = __ffma2_rn(h[k], r[k], make_float2(y, y));
+                m[k] = fminf(m[k], m[(k + 1) & 3]);
+                asm volatile("" : "+f"(m[k]));                   // keep every FMNMX
+            }
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) s += h[k].x + h[k].y + m[k];
+    if (s == 123.456f) out[0] = s;
+}
+
 }  // namespace
 
 cudaError_t run_microbench(int which, double* rate, cudaStream_t st, unsigned long long* launches)
@@ -89,14 +119,15 @@ cudaError_t run_microbench(int which, double* rate, cudaStream_t st, unsigned lo
     if (e != cudaSuccess) return e;
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) return e;
-    if (which < 0 || which > 2) return cudaErrorInvalidValue;
+    if (which < 0 || which > 3) return cudaErrorInvalidValue;
     float* d_out = nullptr;
     e = cudaMalloc(&d_out, sizeof(float));
     if (e != cudaSuccess) return e;
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
-    const int grid = sms * 2;   // 2 waves of 1 CTA/SM x 512 threads
+    const int grid = which == 3 ? sms : sms * 2;   // 2 waves of 1 CTA/SM x 512 threads (the dispatch probe: 1 x 768)
+    int threads = MB_THREADS;
     double ops_per_thread = 0.0;
     float best_ms = 1e30f;
     for (int rep = 0; rep < 4; ++rep) {   // rep 0 = warm-up
@@ -109,10 +140,15 @@ cudaError_t run_microbench(int which, double* rate, cudaStream_t st, unsigned lo
             const int iters = 1024;
             mb_mufu<<<grid, MB_THREADS, 0, st>>>(d_out, iters);
             ops_per_thread = (double)iters * 16 * MB_ILP;
-        } else {
+        } else if (which == 2) {
             const int iters = 256;
             mb_phi<<<grid, MB_THREADS, 0, st>>>(d_out, iters);
             ops_per_thread = (double)iters * TNRD_MP * MB_ILP;
+        } else {
+            const int iters = 2048;
+            threads = 768;
+            mb_dispatch<<<grid, threads, 0, st>>>(d_out, iters, 0.9999f, 1e-9f);
+            ops_per_thread = (double)iters * 16 * 4 * 2 / 32.0;     // WARP instructions (FFMA2 + FMNMX) per thread / 32
         }
         ++*launches;
         cudaEventRecord(e1, st);
@@ -128,7 +164,7 @@ cudaError_t run_microbench(int which, double* rate, cudaStream_t st, unsigned lo
     if (e != cudaSuccess) return e;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    *rate = ops_per_thread * (double)grid * MB_THREADS / ((double)best_ms * 1e-3);
+    *rate = ops_per_thread * (double)grid * threads / ((double)best_ms * 1e-3);
     return cudaSuccess;
 }
 

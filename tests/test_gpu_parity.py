@@ -237,8 +237,12 @@ def test_microbench_rates_are_sane(tnrd):
     ffma, mufu, phi = (tnrd.tnrd_microbench(i) for i in range(3))
     print(f"FFMA {ffma / 1e12:.2f} T/s  MUFU.EX2 {mufu / 1e12:.2f} T/s  phi terms {phi / 1e12:.2f} T/s")
     assert 5e12 < ffma < 60e12 and 1e12 < mufu < 12e12 and 0.5e12 < phi <= mufu * 1.05
+    disp = tnrd.tnrd_microbench(3)          # FFMA2 + FMNMX warp instructions per second (1.0 per clock per scheduler if the pipes issued side by side)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    print(f"FFMA2 + FMNMX mixed: {disp / 1e9:.0f} G warp-instr/s = {disp / (sms * 4 * 1.965e9):.2f} per clock per scheduler")
+    assert 0.45 < disp / (sms * 4 * 1.965e9) < 1.05
     with pytest.raises(tnrd.TnrdError) as ei:
-        tnrd.tnrd_microbench(3)
+        tnrd.tnrd_microbench(4)
     assert ei.value.status == tnrd.ERR_UNSUPPORTED
 
 
