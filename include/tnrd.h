@@ -175,6 +175,12 @@ int tnrd_diffuse_backward(const float* f, const float* u0, const float* u_gt, co
  *      library scratch (and copy u0 into it when out == u0 and T is odd), tnrd_stage with u_out == u_in writes the
  *      plane and copies it back.  A non-finite pixel reaches a slightly larger neighbourhood than the (2 ksize - 1)^2
  *      footprint of the definition (0 x NaN inside the 8-column windows of the implicit GEMM).
+ *   4  the small-image kernel (csrc/tnrd_small.cu): ALL T stages of tnrd_diffuse (or the one of tnrd_stage) in ONE launch,
+ *      parameter staging included, for images that fit a thread-block cluster of 8 or 16 CTAs (B*H*W <= 32768 and a row
+ *      band's working set -- its u tile and N_k influence maps -- within 200 KB of shared memory): the automatic choice for such images with the
+ *      Gaussian basis and TNRD_PHI_FACTORED / TNRD_PHI_DENSE (64 x 64, T = 2: 39 us -> about a quarter of that per
+ *      call).  Iterates alternate between `out` and the ping-pong plane.  Other entry points and shapes return
+ *      TNRD_ERR_UNSUPPORTED while 4 is selected.
  * Returns TNRD_ERR_UNSUPPORTED for other values.
  */
 int tnrd_set_kernel(int which);

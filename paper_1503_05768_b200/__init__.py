@@ -19,7 +19,7 @@ NUM_RBF = 63
 
 OK, ERR_NULL, ERR_SHAPE, ERR_UNSUPPORTED, ERR_ALIAS, ERR_CUDA, ERR_PARAM = 0, -1, -2, -3, -4, -5, -6
 PHI_DENSE, PHI_WINDOW, PHI_LUT, PHI_FACTORED = 0, 1, 2, 3          # tnrd_set_phi_mode (include/tnrd.h)
-KERNEL_AUTO, KERNEL_REF, KERNEL_TILE, KERNEL_TC = 0, 1, 2, 3        # tnrd_set_kernel (include/tnrd.h)
+KERNEL_AUTO, KERNEL_REF, KERNEL_TILE, KERNEL_TC, KERNEL_SMALL = 0, 1, 2, 3, 4     # tnrd_set_kernel (include/tnrd.h)
 
 _lib = None
 

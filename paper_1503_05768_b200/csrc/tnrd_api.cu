@@ -121,6 +121,7 @@ struct Call {
     Scratch* sc = nullptr;
     cudaStream_t st = nullptr;
     bool tc = false;   // this call runs the tensor-core stage kernel
+    bool small = false; // this call runs the small-image kernel (all stages in one launch)
 };
 
 // The automatic choice between the two stage kernels: strips of the tensor-core kernel are 256 - 2r columns wide and
@@ -133,8 +134,45 @@ bool tc_auto(const tnrd::TcPlan& pl, int W, int num_sms)
 // Which stage kernel a call uses.  kernel 3 forces the tensor-core kernel (TNRD_ERR_UNSUPPORTED where it does not apply),
 // 0 picks it when it applies and the image keeps its 128-lane strips busy: it needs the Gaussian basis with the
 // factorised evaluator, ksize 5 or 7 and N_k <= 48 (tnrd_tc.cu).
+// The small-image kernel (kernel 4, or the automatic choice for images that fit a cluster; tnrd_small.cu) serves the
+// Gaussian basis with the factorised or the direct evaluator.
+int pick_small(Call& c, int B, int H, int W, int N_k, int ksize, int phi)
+{
+    const bool can = tnrd::small_supported(B, H, W, N_k, ksize) && (phi == 3 || phi == 0) && c.o.basis == 0;
+    if (c.o.kernel == 4) {
+        if (!can) return TNRD_ERR_UNSUPPORTED;
+        c.small = true;
+    } else if (c.o.kernel == 0) {
+        c.small = can;
+    }
+    return TNRD_OK;
+}
+
+// All T stages through the small-image kernel.  Iterates alternate between `out` and the ping-pong plane so that stage T
+// lands in `out`; when stage 1 would write the buffer it reads (out == u0 and T odd) u0 is copied to the plane first.
+int run_small(Call& c, const float* f, const float* u0, int B, int H, int W, int T, int N_k, int ksize, const float* filters,
+              const float* rbf_w, const float* rbf_mu, float gamma, const float* lambda, float lambda_val, float* out, int phi)
+{
+    const size_t n = (size_t)B * H * W;
+    float* pp = nullptr;
+    const float* src = u0;
+    if (T > 1 || out == u0) {
+        int rc = grow(c.sc->pp, n, c.st);
+        if (rc != TNRD_OK) return rc;
+        pp = c.sc->pp.p;
+        if (out == u0 && (T & 1)) {
+            TNRD_CUDA(cudaMemcpyAsync(pp, u0, n * sizeof(float), cudaMemcpyDeviceToDevice, c.st));
+            src = pp;
+        }
+    }
+    TNRD_CUDA(tnrd::launch_small_diffuse(f, src, out, pp, filters, rbf_w, rbf_mu, gamma, lambda, lambda_val, B, H, W, T, N_k,
+                                         ksize, phi == 0 ? 1 : 0, c.st, &c.lc.n));
+    return TNRD_OK;
+}
+
 int pick_kernel(Call& c, int B, int H, int W, int N_k, int ksize, int phi)
 {
+    if (c.o.kernel == 4) return TNRD_ERR_UNSUPPORTED;     // the small-image kernel serves tnrd_stage / tnrd_diffuse only
     const bool can = tnrd::tc_supported(N_k, ksize) && phi == 3 && c.o.basis == 0;
     if (c.o.kernel == 3) {
         if (!can) return TNRD_ERR_UNSUPPORTED;
@@ -243,6 +281,9 @@ int tnrd_stage(const float* f, const float* u_in, int B, int H, int W, int N_k, 
     Call c;
     if ((rc = open_call(c, stream)) != TNRD_OK) return rc;
     const int phi = c.o.phi();
+    if ((rc = pick_small(c, B, H, W, N_k, ksize, phi)) != TNRD_OK) return rc;
+    if (c.small)
+        return run_small(c, f, u_in, B, H, W, 1, N_k, ksize, filters_t, rbf_w_t, rbf_mu, rbf_gamma, nullptr, lambda_t, u_out, phi);
     if ((rc = pick_kernel(c, B, H, W, N_k, ksize, phi)) != TNRD_OK) return rc;
     if ((rc = stage_params(c, filters_t, rbf_w_t, rbf_mu, rbf_gamma, 1, N_k, ksize, phi)) != TNRD_OK) return rc;
     tnrd::StageArgs a{f, u_in, u_out, c.sc->prm.p, nullptr, lambda_t, B, H, W, N_k, ksize};
@@ -270,6 +311,9 @@ int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, in
     if ((rc = open_call(c, stream)) != TNRD_OK) return rc;
     const size_t rec = (size_t)N_k * tnrd::prm_stride(ksize);
     const int phi = c.o.phi();
+    if ((rc = pick_small(c, B, H, W, N_k, ksize, phi)) != TNRD_OK) return rc;
+    if (c.small)
+        return run_small(c, f, u0, B, H, W, T, N_k, ksize, filters, rbf_w, rbf_mu, rbf_gamma, lambda, 0.0f, out, phi);
     if ((rc = pick_kernel(c, B, H, W, N_k, ksize, phi)) != TNRD_OK) return rc;
     if ((rc = stage_params(c, filters, rbf_w, rbf_mu, rbf_gamma, T, N_k, ksize, phi)) != TNRD_OK) return rc;
     const float* src = u0;
@@ -569,7 +613,7 @@ int tnrd_phi_stats(int enable, unsigned long long* executed, unsigned long long*
 
 int tnrd_set_kernel(int which)
 {
-    if (which < 0 || which > 3) return TNRD_ERR_UNSUPPORTED;
+    if (which < 0 || which > 4) return TNRD_ERR_UNSUPPORTED;
     g_kernel = which;
     return TNRD_OK;
 }

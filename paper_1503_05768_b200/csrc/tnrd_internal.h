@@ -123,6 +123,14 @@ FusedPlan plan_stage_fused(const StageArgs& a, int num_sms);
 // plan.part_floats floats.
 cudaError_t launch_stage_fused(const StageArgs& a, const FusedPlan& plan, float* part, int phi_mode, cudaStream_t st,
                                unsigned long long* launches);
+// ---- small-image kernel (tnrd_small.cu): all T stages of an image that fits a cluster of 8 CTAs in one launch ----
+bool small_supported(int B, int H, int W, int N_k, int ksize);
+// pp: ping-pong plane [B][H][W] (needed when T > 1); u0 must not be the buffer stage 1 writes (out when T is odd, pp else);
+// lambda: device [T], or null -> lambda_val for every stage; force_direct: one ex2 per Gaussian (TNRD_PHI_DENSE)
+cudaError_t launch_small_diffuse(const float* f, const float* u0, float* out, float* pp, const float* filters,
+                                 const float* rbf_w, const float* rbf_mu, float gamma, const float* lambda, float lambda_val,
+                                 int B, int H, int W, int T, int N_k, int ksize, int force_direct, cudaStream_t st,
+                                 unsigned long long* launches);
 cudaError_t launch_qcs_project(const float* y, const float* lo, const float* hi, float* u, int B, int H, int W,
                                cudaStream_t st, unsigned long long* launches);   // u may alias y
 // phi tables: [TN][TNRD_TAB_NODES] float2 + 4 header floats; basis 0 Gaussian, 1 triangular

@@ -211,9 +211,9 @@ __device__ __forceinline__ int tc_phi_fact(const float* __restrict__ crec, float
     const float whi = ord2f(__reduce_max_sync(0xffffffffu, f2ord(zhi)));
     int g0 = 0, g1 = TNRD_FG - 1;
     if (!__any_sync(0xffffffffu, lane_nan)) {
-        // float -> int conversions saturate, so far-away responses (or an empty range) need no special case
-        g0 = max(0, __float2int_rd((wlo - dmax - ganch) * ginv) + 1);
-        g1 = min(TNRD_FG - 1, __float2int_ru((whi + dmax - ganch) * ginv) - 1);
+        // clamped BEFORE the conversion: infinite responses must not overflow the + 1
+        g0 = max(0, __float2int_rd(fminf(fmaxf((wlo - dmax - ganch) * ginv, -8.0f), 8.0f)) + 1);
+        g1 = min(TNRD_FG - 1, __float2int_ru(fminf(fmaxf((whi + dmax - ganch) * ginv, -8.0f), 8.0f)) - 1);
     }
     if (g0 > g1) return 0;
     // the shared exponential pair (middle group)

@@ -67,6 +67,7 @@ def test_scratch_growth_during_capture_is_refused():
     import paper_1503_05768_b200 as tnrd
     tnrd.build(); tnrd.lib()
     c = tnrd_gen.make_small(77, 1, 50, 60, 1, 4, 5)
+    tnrd.tnrd_set_kernel(2)                             # the tile kernel keeps partial sums in the library scratch
     d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()   # noqa: E731
     f, k, w, mu, lam = d(c["f"]), d(c["filters"]), d(c["rbf_w"]), d(c["rbf_mu"]), d(c["lambda"])
     out = torch.empty_like(f)
@@ -78,6 +79,7 @@ def test_scratch_growth_during_capture_is_refused():
                 tnrd.tnrd_diffuse(f, f, 1, 50, 60, 1, 4, 5, k, w, mu, c["rbf_gamma"], lam, out, s)
         assert ei.value.status == tnrd.ERR_CUDA and "capture" in str(ei.value)
     s.synchronize()
+    tnrd.tnrd_set_kernel(0)
     tnrd.tnrd_diffuse(f, f, 1, 50, 60, 1, 4, 5, k, w, mu, c["rbf_gamma"], lam, out)     # the library is still usable
     torch.cuda.synchronize()
     assert bool(torch.isfinite(out).all())

@@ -228,7 +228,10 @@ def test_side_stream_and_launch_count(tnrd):
     with torch.cuda.stream(s):
         got = run_gpu(tnrd, c)
     assert np.array_equal(got, ref)
-    assert tnrd.tnrd_launch_count() == 1 + 2 * c["T"]      # one staging kernel + (fused kernel, update kernel) per stage
+    assert tnrd.tnrd_launch_count() == 1                   # the small-image kernel: all stages in one launch
+    tnrd.tnrd_reset_launch_count()
+    assert np.max(np.abs(run_gpu(tnrd, c, kernel=2) - ref)) <= 2e-4
+    assert tnrd.tnrd_launch_count() == 1 + 2 * c["T"]      # tile kernel: one staging kernel + (tile, update) per stage
     tnrd.tnrd_shutdown()
     assert np.array_equal(run_gpu(tnrd, c), ref)            # usable after shutdown
 
@@ -288,7 +291,7 @@ def test_window_phi_falls_back_to_dense(tnrd):
             mu = c["rbf_mu"].copy(); mu[10] += 2.0; d["rbf_mu"] = mu
         else:                                       # gamma > delta: 14 centres no longer cover 6.5 gamma
             d["rbf_gamma"] = 14.0
-        dense = run_gpu_mode(tnrd, d, phi_mode=0)
+        dense = run_gpu_mode(tnrd, d, phi_mode=0, kernel=2)
         tnrd.tnrd_reset_launch_count()
         got = run_gpu_window(tnrd, d)
         assert tnrd.tnrd_launch_count() == 1 + 3 * d["T"]      # both fused kernels launched (one returns at once) + update
@@ -364,10 +367,10 @@ def test_factorised_phi_other_centres_and_widths(tnrd, change):
         d["rbf_gamma"] = {"narrow": 8.0, "wide": 14.0, "wider": 30.0}[change]
     want = run_oracle(d)
     tnrd.tnrd_reset_launch_count()
-    got = run_gpu_mode(tnrd, d, phi_mode=3)
+    got = run_gpu_mode(tnrd, d, phi_mode=3, kernel=2)
     assert tnrd.tnrd_launch_count() == 1 + 2 * d["T"]
     check(got, want, f"factorised {change}")
-    direct = run_gpu_mode(tnrd, d, phi_mode=0)
+    direct = run_gpu_mode(tnrd, d, phi_mode=0, kernel=2)
     if change in ("jitter", "narrow"):
         assert np.array_equal(got, direct), "the direct form inside the factorised kernel is the direct kernel's"
     else:
