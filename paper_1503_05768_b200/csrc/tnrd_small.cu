@@ -31,7 +31,7 @@ namespace tnrd {
 namespace {
 
 constexpr int SM_CS = 8;        // CTAs per cluster = row bands per image (16 for images of 32 rows and more)
-constexpr int SM_NT = 512;      // threads per CTA
+constexpr int SM_NT = 1024;     // threads per CTA (64 registers each)
 constexpr int SM_REC = TNRD_FG * TNRD_FSTRIDE;   // floats per filter: factorised records (or w' of the direct form)
 
 struct SmallArgs {
@@ -48,6 +48,7 @@ struct SmallArgs {
     int B, H, W, T, N_k;
     int rpc;                    // rows per CTA
     int force_direct;           // phi mode 0
+    int all_stages;             // 1: the parameters of all T stages are staged at once (they fit shared memory)
 };
 
 __device__ __forceinline__ float ex2a(float x)
@@ -128,9 +129,12 @@ __global__ void __launch_bounds__(SM_NT, 1) small_diffuse_kernel(SmallArgs a)
     float* us = sm;                                        // [UH][UW]
     float* vs = us + ((UH * UW + 3) & ~3);                 // [N_k][vplane]
     const int vplane = (VH * VW + 3) & ~3;
-    float* taps = vs + (size_t)a.N_k * vplane;             // [N_k][KK] scaled taps k' = s k
-    float* recs = taps + ((a.N_k * KK + 3) & ~3);          // [N_k][SM_REC]
-    float* mun = recs + a.N_k * SM_REC;                    // [64] -mu'_j (direct form)
+    const int tstride = (a.N_k * KK + 3) & ~3;             // floats of one stage's taps
+    const int nst = a.all_stages ? a.T : 1;                // parameter sets resident at once
+    float* taps = vs + (size_t)a.N_k * vplane;             // [nst][N_k][KK] scaled taps k' = s k
+    float* recs = taps + (size_t)nst * tstride;            // [nst][N_k][SM_REC]
+    float* mun = recs + (size_t)nst * a.N_k * SM_REC;      // [64] -mu'_j (direct form)
+    int* poff = reinterpret_cast<int*>(mun + 64);          // [VH * VW] offset of an influence pixel's window in the u tile
     __shared__ int s_okf;
 
     const float s = sqrtf(1.4426950408889634f / (2.0f * a.gamma * a.gamma));
@@ -150,6 +154,7 @@ __global__ void __launch_bounds__(SM_NT, 1) small_diffuse_kernel(SmallArgs a)
         if (tid == 0) s_okf = ok ? 1 : 0;
     }
     if (tid < 64) mun[tid] = tid < TNRD_M ? -s * __ldg(a.rbf_mu + tid) : 0.0f;
+    for (int p = tid; p < VH * VW; p += SM_NT) poff[p] = (p / VW) * UW + (p % VW);
     __syncthreads();
     const bool fact = s_okf != 0;
     const float ganch = s * mu0 + (float)TNRD_FS * ds, ginv = 1.0f / ((float)TNRD_FM * ds);
@@ -175,42 +180,48 @@ __global__ void __launch_bounds__(SM_NT, 1) small_diffuse_kernel(SmallArgs a)
                 const int uy = i / UW, ux = i - uy * UW;
                 us[i] = __ldcg(src + (size_t)mirror_clamp(row0 - 2 * R + uy, H) * W + mirror_clamp(ux - 2 * R, W));
             }
-        // ---- parameters of stage t ----
-        const float* kt = a.filters + (size_t)(t - 1) * a.N_k * KK;
-        const float* wt = a.rbf_w + (size_t)(t - 1) * a.N_k * TNRD_M;
-        for (int i = tid; i < a.N_k * KK; i += SM_NT) taps[i] = s * __ldg(kt + i);
-        for (int i = tid; i < a.N_k * SM_REC; i += SM_NT) {
-            const int fi = i / SM_REC, o = i - fi * SM_REC;
-            float val = 0.0f;
-            if (!fact) {
-                if (o < TNRD_M) val = __ldg(wt + fi * TNRD_M + o) / s;
-            } else {
-                const int g = o / TNRD_FSTRIDE, q = o - g * TNRD_FSTRIDE, anchor = g * TNRD_FM + TNRD_FS;
-                if (q == 0) val = -s * (mu0 + (float)anchor * delta);
-                else if (q <= TNRD_FM) {
-                    const int j = q <= TNRD_FS + 1 ? TNRD_FS + 1 - q : q - 2 * TNRD_FS - 2;     // S .. 0, then -S .. -1
-                    const int c = anchor + j;
-                    if (c >= 0 && c < TNRD_M)
-                        val = __ldg(wt + fi * TNRD_M + c) / s * exp2f(-(float)(j * j) * ds * ds + (float)abs(j) * lR);
-                } else if (q >= TNRD_FSTRIDE - 2) {
-                    const int mid = (TNRD_FG / 2) * TNRD_FM + TNRD_FS;
-                    const float ex = -2.0f * ds * ds * (float)(anchor - mid);
-                    val = exp2f((q == TNRD_FSTRIDE - 2 ? ex : -ex) - lR);
+        // ---- parameters: of every stage before the first one when they fit shared memory, else of stage t ----
+        if (t == 1 || !a.all_stages)
+            for (int ts = (a.all_stages ? 0 : t - 1); ts < (a.all_stages ? a.T : t); ++ts) {
+                const float* kt = a.filters + (size_t)ts * a.N_k * KK;
+                const float* wt = a.rbf_w + (size_t)ts * a.N_k * TNRD_M;
+                float* tdst = taps + (size_t)(a.all_stages ? ts : 0) * tstride;
+                float* rdst = recs + (size_t)(a.all_stages ? ts : 0) * a.N_k * SM_REC;
+                for (int i = tid; i < a.N_k * KK; i += SM_NT) tdst[i] = s * __ldg(kt + i);
+                for (int i = tid; i < a.N_k * SM_REC; i += SM_NT) {
+                    const int fi = i / SM_REC, o = i - fi * SM_REC;
+                    float val = 0.0f;
+                    if (!fact) {
+                        if (o < TNRD_M) val = __ldg(wt + fi * TNRD_M + o) / s;
+                    } else {
+                        const int g = o / TNRD_FSTRIDE, q = o - g * TNRD_FSTRIDE, anchor = g * TNRD_FM + TNRD_FS;
+                        if (q == 0) val = -s * (mu0 + (float)anchor * delta);
+                        else if (q <= TNRD_FM) {
+                            const int j = q <= TNRD_FS + 1 ? TNRD_FS + 1 - q : q - 2 * TNRD_FS - 2;     // S .. 0, then -S .. -1
+                            const int c = anchor + j;
+                            if (c >= 0 && c < TNRD_M)
+                                val = __ldg(wt + fi * TNRD_M + c) / s * exp2f(-(float)(j * j) * ds * ds + (float)abs(j) * lR);
+                        } else if (q >= TNRD_FSTRIDE - 2) {
+                            const int mid = (TNRD_FG / 2) * TNRD_FM + TNRD_FS;
+                            const float ex = -2.0f * ds * ds * (float)(anchor - mid);
+                            val = exp2f((q == TNRD_FSTRIDE - 2 ? ex : -ex) - lR);
+                        }
+                    }
+                    rdst[i] = val;
                 }
             }
-            recs[i] = val;
-        }
+        const float* taps_t = taps + (size_t)(a.all_stages ? t - 1 : 0) * tstride;
+        const float* recs_t = recs + (size_t)(a.all_stages ? t - 1 : 0) * a.N_k * SM_REC;
         __syncthreads();
         // ---- a2 + a3: every (filter, chunk of 32 influence pixels) is one warp's item: responses and influence values
         // in registers, written to the filter's map.  No synchronisation between filters.
         for (int it = warp; it < a.N_k * nchunk; it += SM_NT / 32) {
             const int i = it / nchunk, p = (it - i * nchunk) * 32 + lane;
             const bool active = p < npx_phi;
-            const float* tp = taps + i * KK;
+            const float* tp = taps_t + i * KK;
             float z = 0.0f;
             if (active) {
-                const int py = p / VW, px = p - py * VW;           // phi pixel = image (row0 - r + py, px - r)
-                const float* uw = us + py * UW + px;               // its window in the u tile
+                const float* uw = us + poff[p];                    // window of phi pixel p = image (row0 - r + p / VW, p % VW - r)
 #pragma unroll
                 for (int ka = 0; ka < KS; ++ka)
 #pragma unroll
@@ -218,8 +229,8 @@ __global__ void __launch_bounds__(SM_NT, 1) small_diffuse_kernel(SmallArgs a)
                         z = fmaf(tp[ka * KS + kb], uw[(KS - 1 - ka) * UW + (KS - 1 - kb)], z);
             }
             float v;
-            if (fact) v = small_phi_fact(recs + i * SM_REC, kappa, dmax, ganch, ginv, z, active);
-            else v = small_phi_direct(recs + i * SM_REC, mun, z);
+            if (fact) v = small_phi_fact(recs_t + i * SM_REC, kappa, dmax, ganch, ginv, z, active);
+            else v = small_phi_direct(recs_t + i * SM_REC, mun, z);
             if (active) vs[(size_t)i * vplane + p] = v;
         }
         __syncthreads();
@@ -233,7 +244,7 @@ __global__ void __launch_bounds__(SM_NT, 1) small_diffuse_kernel(SmallArgs a)
             if (q < npx_out) {
                 oy = q / W; ox = q - oy * W;                       // output pixel = image (row0 + oy, ox)
                 for (int i = part; i < a.N_k; i += nsplit) {
-                    const float* tp = taps + i * KK;
+                    const float* tp = taps_t + i * KK;
                     const float* vw = vs + (size_t)i * vplane + oy * VW + ox;    // phi pixel (oy + a, ox + b)
 #pragma unroll
                     for (int ka = 0; ka < KS; ++ka)
@@ -254,12 +265,14 @@ __global__ void __launch_bounds__(SM_NT, 1) small_diffuse_kernel(SmallArgs a)
     }
 }
 
-size_t small_smem_bytes(int W, int N_k, int ksize, int rpc)
+// nst = parameter sets resident at once (T, or 1)
+size_t small_smem_bytes(int W, int N_k, int ksize, int rpc, int nst)
 {
     const int R = (ksize - 1) / 2, KK = ksize * ksize;
     const size_t us = ((size_t)(rpc + 4 * R) * (W + 4 * R) + 3) & ~(size_t)3;
-    const size_t vp = ((size_t)(rpc + 2 * R) * (W + 2 * R) + 3) & ~(size_t)3;
-    return sizeof(float) * (us + (size_t)N_k * vp + (((size_t)N_k * KK + 3) & ~(size_t)3) + (size_t)N_k * SM_REC + 64);
+    const size_t vpx = (size_t)(rpc + 2 * R) * (W + 2 * R), vp = (vpx + 3) & ~(size_t)3;
+    return sizeof(float) * (us + (size_t)N_k * vp + (size_t)nst * ((((size_t)N_k * KK + 3) & ~(size_t)3) + (size_t)N_k * SM_REC)
+                            + 64 + vpx);
 }
 
 template <int KS>
@@ -298,7 +311,7 @@ bool small_supported(int B, int H, int W, int N_k, int ksize)
 {
     if (B > 65535 || (long long)B * H * W > 32768) return false;
     const int cs = small_cluster(H), rpc = (H + cs - 1) / cs;
-    return small_smem_bytes(W, N_k, ksize, rpc) <= 200 * 1024;
+    return small_smem_bytes(W, N_k, ksize, rpc, 1) <= 200 * 1024;
 }
 
 cudaError_t launch_small_diffuse(const float* f, const float* u0, float* out, float* pp, const float* filters,
@@ -308,8 +321,9 @@ cudaError_t launch_small_diffuse(const float* f, const float* u0, float* out, fl
 {
     const int cs = small_cluster(H);
     SmallArgs a{f, u0, out, pp, filters, rbf_w, rbf_mu, lambda, lambda_val, gamma, B, H, W, T, N_k, (H + cs - 1) / cs,
-                force_direct};
-    const size_t smem = small_smem_bytes(W, N_k, ksize, a.rpc);
+                force_direct, 0};
+    a.all_stages = small_smem_bytes(W, N_k, ksize, a.rpc, T) <= 96 * 1024 ? 1 : 0;
+    const size_t smem = small_smem_bytes(W, N_k, ksize, a.rpc, a.all_stages ? T : 1);
     cudaError_t e;
     switch (ksize) {
         case 3: e = launch_small_ks<3>(a, cs, smem, st); break;
