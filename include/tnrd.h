@@ -89,9 +89,12 @@ int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, in
 
 /*
  * End-to-end variant with HOST buffers: every pointer below is a host pointer (pinned memory makes the
- * copies asynchronous).  Copies f, u0 and the parameters to the device, runs tnrd_diffuse on `stream`,
- * copies u_T back to `out` and synchronises `stream` before returning.  f == u0 (same host pointer) is
- * uploaded once.  Device staging buffers are cached in the library scratch.
+ * copies asynchronous).  Copies f, u0 and the parameters (packed, one copy) to the device, runs the T stages on
+ * `stream`, copies u_T back to `out` and synchronises before returning.  f == u0 (same host pointer) is uploaded once.
+ * Device staging buffers are cached in the library scratch.  With the tensor-core kernel (tnrd_set_kernel) the first
+ * and the last stage are cut in two halves (the images of a batch, or the rows of a single image at an even row) and
+ * the copies run on two internal streams, so that half of the upload and half of the download overlap the arithmetic;
+ * the result is bit-identical to tnrd_diffuse on device buffers.
  */
 int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int T, int N_k, int ksize,
                       const float* filters, const float* rbf_w, const float* rbf_mu, float rbf_gamma,

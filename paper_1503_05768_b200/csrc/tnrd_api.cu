@@ -63,6 +63,11 @@ struct Scratch {
     Buf pp;                           // ping-pong image plane of the tensor-core kernel (it cannot run in place)
     Buf tcws;                         // its Toeplitz operands, T stages
     Buf stats;                        // two 64-bit counters (tnrd_phi_stats)
+    // host entry point: copy streams and events of the pipelined path, pinned staging of the packed parameters
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    float* h_par_pinned = nullptr;
+    size_t h_par_cap = 0;
     Buf tab;                          // piecewise-linear phi tables [T][N_k][4096] float2 + 4 header floats
     Buf h_f, h_u, h_out, h_par;       // device staging of the host entry point
     Buf bw_maps, bw_part, bw_trace, bw_e[2];   // backward pass: P/V maps, per-CTA partial sums, iterates, dl/du planes
@@ -225,7 +230,8 @@ int run_stage(Call& c, tnrd::StageArgs a, int phi, int t)
             }
             a.stats = reinterpret_cast<unsigned long long*>(sc->stats.p);
         }
-        const tnrd::TcPlan pl = tnrd::plan_stage_tc(a.B, a.H, a.W, a.ksize, sc->num_sms);
+        const int rows = a.row_hi > 0 ? a.row_hi - a.row_lo : a.H;
+        const tnrd::TcPlan pl = tnrd::plan_stage_tc(a.B, rows, a.W, a.ksize, sc->num_sms);
         const unsigned char* ws = reinterpret_cast<const unsigned char*>(sc->tcws.p) +
                                   (size_t)t * tnrd::tc_ws_stage_stride(a.N_k, a.ksize);
         TNRD_CUDA(tnrd::launch_stage_tc(a, pl, ws, c.st, &c.lc.n));
@@ -346,6 +352,24 @@ int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, in
     return TNRD_OK;
 }
 
+// Copy streams, events and the pinned parameter staging of the host entry point (created on first use).
+static int host_pipe_init(Scratch* sc, size_t npar)
+{
+    if (!sc->s_in) {
+        TNRD_CUDA(cudaStreamCreateWithFlags(&sc->s_in, cudaStreamNonBlocking));
+        TNRD_CUDA(cudaStreamCreateWithFlags(&sc->s_out, cudaStreamNonBlocking));
+        for (auto& e : sc->ev) TNRD_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    if (npar > sc->h_par_cap) {
+        if (sc->h_par_pinned) TNRD_CUDA(cudaFreeHost(sc->h_par_pinned));
+        sc->h_par_pinned = nullptr;
+        sc->h_par_cap = 0;
+        TNRD_CUDA(cudaHostAlloc(&sc->h_par_pinned, npar * sizeof(float), cudaHostAllocDefault));
+        sc->h_par_cap = npar;
+    }
+    return TNRD_OK;
+}
+
 int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int T, int N_k, int ksize,
                       const float* filters, const float* rbf_w, const float* rbf_mu, float rbf_gamma,
                       const float* lambda, float* out, void* stream)
@@ -356,9 +380,10 @@ int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int 
     int rc = check_shape(B, H, W, N_k, ksize);
     if (rc != TNRD_OK) return rc;
     if ((rc = check_gamma(rbf_gamma)) != TNRD_OK) return rc;
-    cudaStream_t st = (cudaStream_t)stream;
-    Scratch* sc = nullptr;
-    if ((rc = get_scratch(st, &sc)) != TNRD_OK) return rc;
+    Call c;
+    if ((rc = open_call(c, stream)) != TNRD_OK) return rc;
+    Scratch* sc = c.sc;
+    cudaStream_t st = c.st;
     const size_t n = (size_t)B * H * W;
     const size_t nk = (size_t)T * N_k * ksize * ksize, nw = (size_t)T * N_k * TNRD_NUM_RBF;
     const size_t npar = nk + nw + TNRD_NUM_RBF + (size_t)T;
@@ -366,25 +391,94 @@ int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int 
     if (u0 != f && (rc = grow(sc->h_u, n, st)) != TNRD_OK) return rc;
     if ((rc = grow(sc->h_out, n, st)) != TNRD_OK) return rc;
     if ((rc = grow(sc->h_par, npar > 0 ? npar : 1, st)) != TNRD_OK) return rc;
+    if ((rc = host_pipe_init(sc, npar > 0 ? npar : 1)) != TNRD_OK) return rc;
     float* d_k = sc->h_par.p;
     float* d_w = d_k + nk;
     float* d_mu = d_w + nw;
     float* d_lam = d_mu + TNRD_NUM_RBF;
-    TNRD_CUDA(cudaMemcpyAsync(sc->h_f.p, f, n * sizeof(float), cudaMemcpyHostToDevice, st));
-    const float* d_u0 = sc->h_f.p;
-    if (u0 != f) {
-        TNRD_CUDA(cudaMemcpyAsync(sc->h_u.p, u0, n * sizeof(float), cudaMemcpyHostToDevice, st));
-        d_u0 = sc->h_u.p;
+    float* d_f = sc->h_f.p;
+    float* d_u0 = (u0 != f) ? sc->h_u.p : sc->h_f.p;
+    float* d_out = sc->h_out.p;
+    if (T > 0) {        // the parameters: packed on the host, ONE copy
+        float* hp = sc->h_par_pinned;
+        memcpy(hp, filters, nk * sizeof(float));
+        memcpy(hp + nk, rbf_w, nw * sizeof(float));
+        memcpy(hp + nk + nw, rbf_mu, TNRD_NUM_RBF * sizeof(float));
+        memcpy(hp + nk + nw + TNRD_NUM_RBF, lambda, (size_t)T * sizeof(float));
+        TNRD_CUDA(cudaMemcpyAsync(d_k, hp, npar * sizeof(float), cudaMemcpyHostToDevice, st));
     }
+    const int phi = c.o.phi();
+    bool piped = false;
     if (T > 0) {
-        TNRD_CUDA(cudaMemcpyAsync(d_k, filters, nk * sizeof(float), cudaMemcpyHostToDevice, st));
-        TNRD_CUDA(cudaMemcpyAsync(d_w, rbf_w, nw * sizeof(float), cudaMemcpyHostToDevice, st));
-        TNRD_CUDA(cudaMemcpyAsync(d_mu, rbf_mu, TNRD_NUM_RBF * sizeof(float), cudaMemcpyHostToDevice, st));
-        TNRD_CUDA(cudaMemcpyAsync(d_lam, lambda, (size_t)T * sizeof(float), cudaMemcpyHostToDevice, st));
+        if ((rc = pick_small(c, B, H, W, N_k, ksize, phi)) != TNRD_OK) return rc;
+        if (!c.small && (rc = pick_kernel(c, B, H, W, N_k, ksize, phi)) != TNRD_OK) return rc;
+        piped = c.tc && (B >= 2 || H >= 256);
     }
-    rc = tnrd_diffuse(sc->h_f.p, d_u0, B, H, W, T, N_k, ksize, d_k, d_w, d_mu, rbf_gamma, d_lam, sc->h_out.p, stream);
-    if (rc != TNRD_OK) return rc;
-    TNRD_CUDA(cudaMemcpyAsync(out, sc->h_out.p, n * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (!piped) {
+        // serial: upload, all stages, download (small images, the tile kernel)
+        TNRD_CUDA(cudaMemcpyAsync(d_f, f, n * sizeof(float), cudaMemcpyHostToDevice, st));
+        if (u0 != f) TNRD_CUDA(cudaMemcpyAsync(d_u0, u0, n * sizeof(float), cudaMemcpyHostToDevice, st));
+        rc = tnrd_diffuse(d_f, d_u0, B, H, W, T, N_k, ksize, d_k, d_w, d_mu, rbf_gamma, d_lam, d_out, stream);
+        if (rc != TNRD_OK) return rc;
+        TNRD_CUDA(cudaMemcpyAsync(out, d_out, n * sizeof(float), cudaMemcpyDeviceToHost, st));
+        TNRD_CUDA(cudaStreamSynchronize(st));
+        return TNRD_OK;
+    }
+    // Pipelined (tensor-core kernel): the work of the FIRST and the LAST stage is cut in two halves -- the two halves of
+    // the batch, or of the rows of a single image (an even row, so that every pixel sees the arithmetic of the un-cut
+    // launch and the result is bit-identical) -- so that the first half computes while the second half of the input
+    // arrives, and the first half of the result leaves while the second half computes.  Copies run on two internal
+    // streams ordered against `stream` by events.
+    if ((rc = stage_params(c, d_k, d_w, d_mu, rbf_gamma, T, N_k, ksize, phi)) != TNRD_OK) return rc;
+    const bool by_img = B >= 2;
+    const int R = (ksize - 1) / 2;
+    const int b_mid = B / 2, r_mid = (H / 2) & ~1;
+    const size_t plane = (size_t)H * W;
+    // elements [0, cutA) must have arrived before the first half starts: its images, or its rows plus the 2r halo
+    const size_t cutA = by_img ? (size_t)b_mid * plane : (size_t)(r_mid + 2 * R < H ? r_mid + 2 * R : H) * W;
+    const size_t cutO = by_img ? (size_t)b_mid * plane : (size_t)r_mid * W;       // first half of the result
+    TNRD_CUDA(cudaEventRecord(sc->ev[0], st));
+    TNRD_CUDA(cudaStreamWaitEvent(sc->s_in, sc->ev[0], 0));
+    TNRD_CUDA(cudaMemcpyAsync(d_f, f, cutA * sizeof(float), cudaMemcpyHostToDevice, sc->s_in));
+    if (u0 != f) TNRD_CUDA(cudaMemcpyAsync(d_u0, u0, cutA * sizeof(float), cudaMemcpyHostToDevice, sc->s_in));
+    TNRD_CUDA(cudaEventRecord(sc->ev[1], sc->s_in));
+    TNRD_CUDA(cudaMemcpyAsync(d_f + cutA, f + cutA, (n - cutA) * sizeof(float), cudaMemcpyHostToDevice, sc->s_in));
+    if (u0 != f) TNRD_CUDA(cudaMemcpyAsync(d_u0 + cutA, u0 + cutA, (n - cutA) * sizeof(float), cudaMemcpyHostToDevice, sc->s_in));
+    TNRD_CUDA(cudaEventRecord(sc->ev[2], sc->s_in));
+    if (T > 1 && (rc = grow(sc->pp, n, st)) != TNRD_OK) return rc;
+    float* pp = sc->pp.p;
+    const size_t rec = (size_t)N_k * tnrd::prm_stride(ksize);
+    const float* src = d_u0;
+    for (int t = 1; t <= T; ++t) {
+        float* dst = ((T - t) & 1) ? pp : d_out;
+        tnrd::StageArgs a{d_f, src, dst, sc->prm.p + (size_t)(t - 1) * rec, d_lam + (t - 1), 0.0f, B, H, W, N_k, ksize};
+        const bool first = t == 1, last = t == T;
+        if (!first && !last) {
+            if ((rc = run_stage(c, a, phi, t - 1)) != TNRD_OK) return rc;
+        } else {
+            for (int half = 0; half < 2; ++half) {
+                tnrd::StageArgs h = a;
+                if (by_img) {
+                    const size_t off = half ? (size_t)b_mid * plane : 0;
+                    h.f += off; h.u_in += off; h.u_out += off;
+                    h.B = half ? B - b_mid : b_mid;
+                } else {
+                    h.row_lo = half ? r_mid : 0;
+                    h.row_hi = half ? H : r_mid;
+                }
+                if (first) TNRD_CUDA(cudaStreamWaitEvent(st, sc->ev[1 + half], 0));
+                if ((rc = run_stage(c, h, phi, t - 1)) != TNRD_OK) return rc;
+                if (last) {
+                    TNRD_CUDA(cudaEventRecord(sc->ev[3 + half], st));
+                    TNRD_CUDA(cudaStreamWaitEvent(sc->s_out, sc->ev[3 + half], 0));
+                    const size_t o0 = half ? cutO : 0, cnt = half ? n - cutO : cutO;
+                    TNRD_CUDA(cudaMemcpyAsync(out + o0, d_out + o0, cnt * sizeof(float), cudaMemcpyDeviceToHost, sc->s_out));
+                }
+            }
+        }
+        src = dst;
+    }
+    TNRD_CUDA(cudaStreamSynchronize(sc->s_out));
     TNRD_CUDA(cudaStreamSynchronize(st));
     return TNRD_OK;
 }
@@ -671,6 +765,9 @@ void tnrd_shutdown(void)
         Buf* bufs[] = {&s->pp, &s->tcws, &s->stats, &s->prm, &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->refv, &s->split, &s->tab, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
         for (Buf* b : bufs)
             if (b->p) (void)cudaFree(b->p);   // synchronising free: the stream may be gone by now
+        if (s->s_in) { (void)cudaStreamDestroy(s->s_in); (void)cudaStreamDestroy(s->s_out); }
+        for (cudaEvent_t e : s->ev) if (e) (void)cudaEventDestroy(e);
+        if (s->h_par_pinned) (void)cudaFreeHost(s->h_par_pinned);
         delete s;
     }
     g_scratch.clear();

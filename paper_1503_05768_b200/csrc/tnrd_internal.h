@@ -70,6 +70,7 @@ struct StageArgs {
     const float* tab;       // piecewise-linear phi tables of this stage [N_k][TNRD_TAB_NODES] float2 (phi evaluator 2)
     const float* tabhdr;    // their header (tnrd_table.cu), device
     unsigned long long* stats;  // null, or device counters {phi group evaluations executed, defined} (tensor-core kernel)
+    int row_lo, row_hi;         // tensor-core kernel: this launch completes output rows [row_lo, row_hi) only; 0, 0 = all rows
 };
 
 // Launch plan of the fused stage kernel (tnrd_fused.cu: plan_stage_fused).  Tiles partition the phi region
@@ -148,7 +149,7 @@ struct TcPlan {
 bool tc_supported(int N_k, int ksize);                       // ksize 5 or 7, N_k <= 48
 size_t tc_workspace_bytes(int T, int N_k, int ksize);        // Toeplitz operands of T stages
 size_t tc_ws_stage_stride(int N_k, int ksize);               // bytes per stage inside that workspace
-TcPlan plan_stage_tc(int B, int H, int W, int ksize, int num_sms);
+TcPlan plan_stage_tc(int B, int H, int W, int ksize, int num_sms);   // H = number of output rows of the launch
 // prm = staged records of T stages (launch_prep); ws receives the operands
 cudaError_t launch_tc_prep(const float* prm, int T, int N_k, int ksize, unsigned char* ws, cudaStream_t st,
                            unsigned long long* launches);

@@ -347,7 +347,8 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
     const int ysg = unit % nys; unit /= nys;
     const int img = unit;
     const int X0 = xs * C::OW;                                  // phi column of lane 0, pixel 0 = image column X0 - r
-    const int ys0 = ysg * seg_rows, ys1 = min(a.H, ys0 + seg_rows);
+    const int row_hi = a.row_hi > 0 ? a.row_hi : a.H;
+    const int ys0 = a.row_lo + ysg * seg_rows, ys1 = min(row_hi, ys0 + seg_rows);
     const int rows_out = ys1 - ys0;
     const int NB = (rows_out + 2 * R - 1) / 2 + 1;              // batches: phi rows ys0 .. ys0 + 2 NB - 1
     const int NPAIRS = NB + R;                                  // u row pairs: u~ rows ys0 .. ys0 + 2 NB + 2r - 1

@@ -312,3 +312,26 @@ def test_two_devices_in_one_process(tnrd):
             finally:
                 tnrd.tnrd_set_kernel(0)
             check(out.cpu().numpy().astype(np.float64), want, f"device 1 kernel {kernel}", tight=True)
+
+
+@pytest.mark.parametrize("shape", [(1, 600, 520), (1, 257, 300), (5, 130, 300), (2, 64, 512)], ids=lambda s: "x".join(map(str, s)))
+@pytest.mark.parametrize("T", [1, 2, 3])
+def test_host_entry_point_pipelined_is_bit_identical(tnrd, shape, T):
+    """tnrd_diffuse_host with the tensor-core kernel cuts the first and the last stage in two halves (images of a batch, or
+    rows of a single image at an even row) to overlap the copies: the result must be bit-identical to the device call."""
+    B, H, W = shape
+    c = tnrd_gen.make_small(270 + T, B, H, W, T, 8, 7)
+    ref = run_gpu(tnrd, c, kernel=3)
+    tnrd.tnrd_set_kernel(3)
+    try:
+        out = torch.empty(c["f"].shape).pin_memory()
+        f = torch.from_numpy(c["f"]).pin_memory()
+        tnrd.tnrd_diffuse_host(f, f, B, H, W, T, 8, 7, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"], c["lambda"], out)
+        assert np.array_equal(out.numpy().astype(np.float64), ref)
+        out2 = np.empty_like(c["f"])                                 # pageable buffers, u0 distinct from f
+        u0 = c["u0"].copy()
+        tnrd.tnrd_diffuse_host(c["f"], u0, B, H, W, T, 8, 7, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"],
+                               c["lambda"], out2)
+        assert np.array_equal(out2.astype(np.float64), ref)
+    finally:
+        tnrd.tnrd_set_kernel(0)
