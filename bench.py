@@ -415,6 +415,10 @@ def main():
     sms = torch.cuda.get_device_properties(devs).multi_processor_count
     tcq = tnrd.tnrd_tc_plan_query(B, H, W, N_K, KSIZE, sms)
     use_tc = (tcq["applies"] == 2 and args.kernel == "auto") or (tcq["applies"] >= 1 and args.kernel == "tc")
+    # one launch per tnrd_diffuse call = the small-image kernel (all stages in one launch; include/tnrd.h tnrd_set_kernel)
+    use_small = (not deblock and not backward) and launches == args.steps
+    if use_small:
+        use_tc = False
     launch_s = (ms * 1e-3) / (args.steps * T)           # step time / T: the staging kernels (~us) are charged too
     fma_peak = NOMINAL_SMS * FMA_PER_CLK_SM * NOMINAL_SM_MHZ * 1e6 / 1e12
     xu_peak = NOMINAL_SMS * MUFU_PER_CLK_SM * NOMINAL_SM_MHZ * 1e6 / 1e12
@@ -474,6 +478,11 @@ def main():
         "launch_ms": launch_s * 1e3,
     }
     roofline.update(tensor_extra)
+    if use_small:
+        roofline.update({"kernel": "small_diffuse_kernel", "achieved": None, "frac": None, "x_defined_work_roofline": None,
+                         "formulation": "small-image kernel: all T stages in one launch (cluster of 8 / 16 CTAs per image)",
+                         "us_per_call": 1e3 * ms / args.steps,
+                         "note": "latency-bound: reported as microseconds per call, not as a roofline fraction (SURVEY.md 8d)"})
     if backward:
         roofline["note"] = "no roofline statement for the joint-training step: its three kernels have no single declared count"
     peak_nominal = xu_peak                               # the opt-in evaluators below are quoted against the XU roofline
