@@ -190,10 +190,12 @@ int tnrd_set_kernel(int which);
 
 /*
  * Work decomposition of the tensor-core stage kernel for this shape on a device with `num_sms` multiprocessors (pure host
- * logic).  plan[0..5] = {0: the kernel does not apply to (N_k, ksize); 1: applies, the automatic choice is the tile
+ * logic).  plan[0..6] = {0: the kernel does not apply to (N_k, ksize); 1: applies, the automatic choice is the tile
  * kernel; 2: applies and is the automatic choice}, strips per image (256 - 2r output columns each), row segments per
- * image, output rows per segment, CTAs (= images x strips x segments), output columns per strip.  Honours the
- * TNRD_TC_SEG environment knob (forces the rows per segment; tests).
+ * image, output rows per segment, CTAs (= images x filter chunks x segments x strips), output columns per strip, filter
+ * chunks (> 1 for images that would not fill the GPU otherwise: each CTA takes a chunk of the filter bank and a point-wise
+ * kernel adds the chunks' partial sums and applies the reaction term).  Honours the TNRD_TC_SEG / TNRD_TC_CHUNK environment
+ * knobs (force the rows per segment / the number of chunks; tests).
  */
 int tnrd_tc_plan_query(int B, int H, int W, int N_k, int ksize, int num_sms, long long* plan);
 

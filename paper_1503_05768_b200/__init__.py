@@ -196,9 +196,9 @@ def tnrd_plan_query(B, H, W, N_k, ksize, num_sms=148) -> dict:
 
 def tnrd_tc_plan_query(B, H, W, N_k, ksize, num_sms=148) -> dict:
     """Work decomposition of the tensor-core stage kernel (include/tnrd.h: tnrd_tc_plan_query); host logic only."""
-    buf = (ctypes.c_longlong * 6)()
+    buf = (ctypes.c_longlong * 7)()
     _check(lib().tnrd_tc_plan_query(B, H, W, N_k, ksize, num_sms, buf))
-    keys = ("applies", "nxs", "nys", "seg_rows", "units", "out_cols")
+    keys = ("applies", "nxs", "nys", "seg_rows", "units", "out_cols", "nchunk")
     return dict(zip(keys, (int(v) for v in buf)))
 
 

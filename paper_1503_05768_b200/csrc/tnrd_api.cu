@@ -131,9 +131,9 @@ struct Call {
 
 // The automatic choice between the two stage kernels: strips of the tensor-core kernel are 256 - 2r columns wide and
 // every CTA recomputes 2r phi rows, so it pays once its units fill the GPU with segments of a few dozen rows.
-bool tc_auto(const tnrd::TcPlan& pl, int W, int num_sms)
+bool tc_auto(const tnrd::TcPlan& pl, int W, int num_sms, int ksize)
 {
-    return pl.units * 10 >= (long long)num_sms * 6 && pl.seg_rows >= 24 && W >= 192;
+    return pl.units * 10 >= (long long)num_sms * 6 && pl.seg_rows > ksize && W >= 192;
 }
 
 // Which stage kernel a call uses.  kernel 3 forces the tensor-core kernel (TNRD_ERR_UNSUPPORTED where it does not apply),
@@ -184,7 +184,7 @@ int pick_kernel(Call& c, int B, int H, int W, int N_k, int ksize, int phi)
         c.tc = true;
     } else if (c.o.kernel == 0 && can) {
         // strips are 256 - 2r columns wide and every CTA recomputes 2r phi rows: worth it once the units fill the GPU
-        c.tc = tc_auto(tnrd::plan_stage_tc(B, H, W, ksize, c.sc->num_sms), W, c.sc->num_sms);
+        c.tc = tc_auto(tnrd::plan_stage_tc(B, H, W, N_k, ksize, c.sc->num_sms), W, c.sc->num_sms, ksize);
     }
     return TNRD_OK;
 }
@@ -231,10 +231,14 @@ int run_stage(Call& c, tnrd::StageArgs a, int phi, int t)
             a.stats = reinterpret_cast<unsigned long long*>(sc->stats.p);
         }
         const int rows = a.row_hi > 0 ? a.row_hi - a.row_lo : a.H;
-        const tnrd::TcPlan pl = tnrd::plan_stage_tc(a.B, rows, a.W, a.ksize, sc->num_sms);
+        const tnrd::TcPlan pl = tnrd::plan_stage_tc(a.B, rows, a.W, a.N_k, a.ksize, sc->num_sms);
+        if (pl.nchunk > 1) {
+            int rc = grow(sc->split, (size_t)pl.nchunk * a.B * a.H * a.W, c.st);
+            if (rc != TNRD_OK) return rc;
+        }
         const unsigned char* ws = reinterpret_cast<const unsigned char*>(sc->tcws.p) +
                                   (size_t)t * tnrd::tc_ws_stage_stride(a.N_k, a.ksize);
-        TNRD_CUDA(tnrd::launch_stage_tc(a, pl, ws, c.st, &c.lc.n));
+        TNRD_CUDA(tnrd::launch_stage_tc(a, pl, ws, sc->split.p, c.st, &c.lc.n));
     } else if (c.o.kernel == 1) {
         if (c.o.basis == 1) return TNRD_ERR_UNSUPPORTED;     // the reference kernel knows the Gaussian basis only
         int rc = grow(sc->refv, tnrd::ref_scratch_floats(a.B, a.H, a.W, a.N_k, a.ksize), c.st);
@@ -679,11 +683,11 @@ int tnrd_tc_plan_query(int B, int H, int W, int N_k, int ksize, int num_sms, lon
     int rc = check_shape(B, H, W, N_k, ksize);
     if (rc != TNRD_OK) return rc;
     if (num_sms < 1) return TNRD_ERR_SHAPE;
-    for (int i = 0; i < 6; ++i) plan[i] = 0;
+    for (int i = 0; i < 7; ++i) plan[i] = 0;
     if (!tnrd::tc_supported(N_k, ksize)) return TNRD_OK;
-    const tnrd::TcPlan pl = tnrd::plan_stage_tc(B, H, W, ksize, num_sms);
-    plan[0] = 1 + (tc_auto(pl, W, num_sms) ? 1 : 0);
-    plan[1] = pl.nxs; plan[2] = pl.nys; plan[3] = pl.seg_rows; plan[4] = pl.units; plan[5] = 256 - (ksize - 1);
+    const tnrd::TcPlan pl = tnrd::plan_stage_tc(B, H, W, N_k, ksize, num_sms);
+    plan[0] = 1 + (tc_auto(pl, W, num_sms, ksize) ? 1 : 0);
+    plan[1] = pl.nxs; plan[2] = pl.nys; plan[3] = pl.seg_rows; plan[4] = pl.units; plan[5] = 256 - (ksize - 1); plan[6] = pl.nchunk;
     return TNRD_OK;
 }
 

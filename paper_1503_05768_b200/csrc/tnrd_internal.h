@@ -143,18 +143,20 @@ cudaError_t fused_init();   // opt-in shared memory attributes; idempotent
 // A unit = (image, row segment, strip of 256 - 2r output columns); one CTA per unit.
 struct TcPlan {
     int nxs, nys, seg_rows;   // strips per image, row segments per image, output rows per segment
+    int nchunk;               // filter chunks per (image, segment, strip): > 1 = partial sums + tc_update_kernel
     long long units;          // CTAs
-    double cost_rows;         // waves x (rows per CTA incl. recomputed ones + per-CTA constant), the planner's objective
+    double cost_clk;          // the planner's objective: waves x modelled clocks of a unit
 };
 bool tc_supported(int N_k, int ksize);                       // ksize 5 or 7, N_k <= 48
 size_t tc_workspace_bytes(int T, int N_k, int ksize);        // Toeplitz operands of T stages
 size_t tc_ws_stage_stride(int N_k, int ksize);               // bytes per stage inside that workspace
-TcPlan plan_stage_tc(int B, int H, int W, int ksize, int num_sms);   // H = number of output rows of the launch
+TcPlan plan_stage_tc(int B, int H, int W, int N_k, int ksize, int num_sms);   // H = number of output rows of the launch
 // prm = staged records of T stages (launch_prep); ws receives the operands
 cudaError_t launch_tc_prep(const float* prm, int T, int N_k, int ksize, unsigned char* ws, cudaStream_t st,
                            unsigned long long* launches);
 // one stage; a.u_out must not alias a.u_in (the kernel reads halos of u_in while other CTAs write u_out)
-cudaError_t launch_stage_tc(const StageArgs& a, const TcPlan& pl, const unsigned char* ws_t, cudaStream_t st,
+// part: scratch of nchunk * B * H * W floats when pl.nchunk > 1 (then a point-wise update kernel follows), else unused
+cudaError_t launch_stage_tc(const StageArgs& a, const TcPlan& pl, const unsigned char* ws_t, float* part, cudaStream_t st,
                             unsigned long long* launches);
 cudaError_t run_microbench(int which, double* rate, cudaStream_t st, unsigned long long* launches);
 

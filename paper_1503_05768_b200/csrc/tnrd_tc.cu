@@ -28,10 +28,11 @@
 //
 // Strips overlap by 2r phi columns and row segments by 2r phi rows (recomputed) so that a CTA completes its own
 // outputs: no partial sums in HBM, no second kernel, 12 B of DRAM traffic per pixel-stage.
-// Warp roles: 16 phi warps (4 per tensor-memory lane quarter, sharing the quarter's filter pairs through a ticket
+// Warp roles: 24 phi warps (4 per tensor-memory lane quarter, sharing the quarter's filter pairs through a ticket
 // counter), 4 drain warps (fold + a5), 1 MMA-issuing warp, 1 loader warp; mbarrier pipelines between them (u row pairs,
 // z double-buffered, scatter table).
 #include <cuda_bf16.h>
+#include <cmath>
 #include <cstdint>
 #include <cstdio>
 #include <cstdlib>
@@ -288,6 +289,27 @@ __device__ __forceinline__ void split_bf16(float2 v, uint32_t& hi, uint32_t& lo)
     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(lo) : "f"(v.y - hy), "f"(v.x - hx));
 }
 
+// One 16-byte cell (row, g) = u~[row][2g .. 2g+3] of the u ring, through the mirror map, split
+// x = hi + lo with hi = the top 19 bits (a TF32 number; lo is exact): the four loads ...
+__device__ __forceinline__ void tc_cell_load(const float* __restrict__ u_img, int H, int W, int urow, int ucol, float (&v)[4])
+{
+    const float* __restrict__ grow = u_img + (size_t)mirror_clamp(urow, H) * W;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) v[e] = __ldg(grow + mirror_clamp(ucol + e, W));
+}
+// ... and the two stores
+__device__ __forceinline__ void tc_cell_store(unsigned char* smem_hi, unsigned char* smem_lo, int cell_byte, const float (&v)[4])
+{
+    float h[4], l[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        h[e] = __uint_as_float(__float_as_uint(v[e]) & 0xFFFFE000u);
+        l[e] = v[e] - h[e];
+    }
+    *reinterpret_cast<float4*>(smem_hi + cell_byte) = make_float4(h[0], h[1], h[2], h[3]);
+    *reinterpret_cast<float4*>(smem_lo + cell_byte) = make_float4(l[0], l[1], l[2], l[3]);
+}
+
 // ---- operand staging kernel: Toeplitz operands of both banks from the staged records (scaled taps k' = s k) ------
 //   forward  BF[(2a + cc)][n = 2i + j][e]   = k'_i[K-1-a][K-1-(4cc + e - j)]   (TF32 hi / lo)
 //   scatter  BS[pass][kp / 8][n = 8 blk + xo][kp % 8],  kp = 4i + 2s + j  (s = 0: the hi half of v, 1: the lo half)
@@ -327,7 +349,8 @@ __global__ void tc_prep_kernel(const float* __restrict__ prm, int T, int N_k, in
 // [xs OW, xs OW + OW) from phi rows [ys0, ys1 + 2r) x phi columns [xs OW, xs OW + 256) (phi coordinates = image + r).
 template <int KS, bool STATS>
 __global__ void __launch_bounds__(TC_THREADS, 1)
-stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int nxs, int nys, int seg_rows)
+stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, int nxs, int nys, int seg_rows, int nchunk,
+                float* __restrict__ part)
 {
     using C = TcCfg<KS>;
     constexpr int R = C::R;
@@ -342,10 +365,15 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
     uint64_t* tfree = tfull + 1;                // scatter table read out
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // a unit = (image, filter chunk, row segment, strip).  nchunk > 1 (images too small to fill the GPU otherwise): the CTA
+    // takes filters [f0, f0 + nkp) of the bank and stores its partial transposed-bank sums to part[chunk][image][H][W];
+    // tc_update_kernel adds the chunks in fixed order and applies the reaction term.
     int unit = blockIdx.x;
     const int xs = unit % nxs; unit /= nxs;
     const int ysg = unit % nys; unit /= nys;
+    const int chunk = unit % nchunk; unit /= nchunk;
     const int img = unit;
+    const int nkp = nkp_all / nchunk, f0 = chunk * nkp;         // this CTA's filters (a multiple of 8)
     const int X0 = xs * C::OW;                                  // phi column of lane 0, pixel 0 = image column X0 - r
     const int row_hi = a.row_hi > 0 ? a.row_hi : a.H;
     const int ys0 = a.row_lo + ysg * seg_rows, ys1 = min(row_hi, ys0 + seg_rows);
@@ -356,16 +384,23 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
 
     // ---- setup: operands and coefficients to shared memory, barriers, tensor memory ----
     {
-        const size_t bfb = tc_ws_bf_bytes(KS, nkp), bsb = tc_ws_bs_bytes(KS, nkp);
-        for (int i = tid; i < (int)(bfb / 16); i += TC_THREADS) {
-            cp_async16(reinterpret_cast<float*>(smem + C::SM_BFH) + 4 * i, reinterpret_cast<const float*>(ws) + 4 * i);
-            cp_async16(reinterpret_cast<float*>(smem + C::SM_BFL) + 4 * i, reinterpret_cast<const float*>(ws + bfb) + 4 * i);
+        // forward operand: cells [2 KS chunks][2 nkp_all columns] -> this CTA's 2 nkp columns, compact
+        const size_t bfb = tc_ws_bf_bytes(KS, nkp_all);
+        for (int i = tid; i < 2 * KS * 2 * nkp; i += TC_THREADS) {
+            const int kc = i / (2 * nkp), n = i - kc * 2 * nkp;
+            const size_t src = ((size_t)kc * 2 * nkp_all + 2 * f0 + n) * 4;
+            cp_async16(reinterpret_cast<float*>(smem + C::SM_BFH) + 4 * i, reinterpret_cast<const float*>(ws) + src);
+            cp_async16(reinterpret_cast<float*>(smem + C::SM_BFL) + 4 * i, reinterpret_cast<const float*>(ws + bfb) + src);
         }
-        for (int i = tid; i < (int)(bsb / 16); i += TC_THREADS)
-            cp_async16(reinterpret_cast<float*>(smem + C::SM_BS) + 4 * i, reinterpret_cast<const float*>(ws + 2 * bfb) + 4 * i);
+        // scatter operand: cells [2 passes][nkp_all / 2 K chunks][NSC] -> the K chunks of this CTA's filters
+        for (int i = tid; i < 2 * (nkp / 2) * C::NSC; i += TC_THREADS) {
+            const int pass = i / ((nkp / 2) * C::NSC), r = i - pass * (nkp / 2) * C::NSC;
+            const size_t src = ((size_t)(pass * (nkp_all / 2) + f0 / 2) * C::NSC + r) * 4;
+            cp_async16(reinterpret_cast<float*>(smem + C::SM_BS) + 4 * i, reinterpret_cast<const float*>(ws + 2 * bfb) + src);
+        }
         constexpr int CF = TNRD_FG * TNRD_FSTRIDE;              // coefficient floats per filter
         for (int i = tid; i < nkp * CF / 4; i += TC_THREADS) {
-            const int fi = (4 * i) / CF, o = 4 * i - fi * CF;
+            const int fi = f0 + (4 * i) / CF, o = (4 * i) % CF;
             float* dst = reinterpret_cast<float*>(smem + C::SM_COEF) + 4 * i;
             if (fi < a.N_k) cp_async16(dst, a.prm + (size_t)fi * C::PRM + prm_fact(KS) + o);
             else *reinterpret_cast<float4*>(dst) = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -387,12 +422,23 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "r"(512) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
+    // The first R + 1 row pairs (what the first batch needs) are gathered by ALL threads: left to the loader warp alone
+    // they would cost R + 1 round trips to L2 per thread chain before the first MMA can issue.
+    {
+        const int npre = min(NPAIRS, R + 1) * 2 * TC_CWU;
+        for (int idx = tid; idx < npre; idx += TC_THREADS) {
+            const int prow = idx / TC_CWU, xg = idx - prow * TC_CWU;         // prow = ring row = pair * 2 + row of the pair
+            float v[4];
+            tc_cell_load(u_img, a.H, a.W, ys0 + prow - 2 * R, X0 + 2 * xg - 2 * R, v);
+            tc_cell_store(smem + C::SM_UHI, smem + C::SM_ULO, (prow * TC_CW + xg) * 16, v);
+        }
+    }
     cp_async_wait_all();
     {
         constexpr int CF = TNRD_FG * TNRD_FSTRIDE, S = TNRD_FS;
         float* cf = reinterpret_cast<float*>(smem + C::SM_COEF);
         for (int i = tid; i < nkp * CF / 4; i += TC_THREADS) {   // the same 16-byte pieces this thread copied above
-            if ((4 * i) / CF >= a.N_k) continue;
+            if (f0 + (4 * i) / CF >= a.N_k) continue;
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
                 const int o = (4 * i + e) % TNRD_FSTRIDE;        // slot inside the group record
@@ -410,6 +456,9 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
     tc_fence_after();
     const uint32_t tmem = tmem_base_s;
     const uint32_t sbase = smem_u32(smem);
+    if (tid == 0)                                               // the pre-filled pairs: phase 0 of their barriers is complete
+        for (int p = 0; p < min(NPAIRS, R + 1); ++p)
+            for (int k = 0; k < TC_LOAD_WARPS; ++k) mbar_arrive(pfull + p);
 
     if (warp < TC_PHI_WARPS) {
         // =================================== phi warps ===================================
@@ -464,7 +513,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
                     const int nl = tc_phi_fact(coef + fidx * (TNRD_FG * TNRD_FSTRIDE), kappa, dmax, ganch, ginv, zc, v);
                     if (STATS) nlive += nl;
                 }
-                else if (fidx < a.N_k) tc_phi_direct(a.prm + (size_t)fidx * C::PRM + prm_kkp(KS), zc, v);
+                else if (f0 + fidx < a.N_k) tc_phi_direct(a.prm + (size_t)(f0 + fidx) * C::PRM + prm_kkp(KS), zc, v);
                 split_bf16(v[0], o0[2 * f], o0[2 * f + 1]);
                 split_bf16(v[1], o1[2 * f], o1[2 * f + 1]);
             }
@@ -519,7 +568,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
                 const size_t base = ((size_t)img * a.H + ys0 + (okr[qq] ? yrel : 0)) * a.W;
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
-                    const bool ok = okr[qq] && xcol + e < a.W;
+                    const bool ok = okr[qq] && xcol + e < a.W && part == nullptr;
                     uu[qq][e] = ok ? __ldg(a.u_in + base + xcol + e) : 0.f;
                     ff[qq][e] = ok ? __ldg(a.f + base + xcol + e) : 0.f;
                 }
@@ -541,6 +590,12 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
                 const int qq = q - (KS - 1);
                 if (!okr[qq]) continue;
                 const size_t base = ((size_t)img * a.H + ys0 + yrel) * a.W;
+                if (part) {                                      // a filter chunk: its partial sums, for tc_update_kernel
+                    float* pc = part + (size_t)chunk * a.B * a.H * a.W + base;
+                    if (xcol < a.W) __stcg(pc + xcol, o.x);
+                    if (xcol + 1 < a.W) __stcg(pc + xcol + 1, o.y);
+                    continue;
+                }
                 if (xcol < a.W) a.u_out[base + xcol] = uu[qq][0] - (o.x + lambda * (uu[qq][0] - ff[qq][0]));
                 if (xcol + 1 < a.W) a.u_out[base + xcol + 1] = uu[qq][1] - (o.y + lambda * (uu[qq][1] - ff[qq][1]));
             }
@@ -595,23 +650,28 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
     } else {
         // =================================== loader warps ===================================
         const int lt = tid - (TC_MMA_WARP + 1) * 32;
-        for (int p = 0; p < NPAIRS; ++p) {
+        for (int p = R + 1; p < NPAIRS; ++p) {
             const int slot = p % TC_NP;
             if (p >= TC_NP) mbar_wait_idle(pempty + slot, ((p / TC_NP) - 1) & 1);
-            for (int idx = lt; idx < 2 * TC_CWU; idx += TC_LOAD_WARPS * 32) {
-                const int rrow = idx / TC_CWU, xg = idx - rrow * TC_CWU;
-                const float* __restrict__ grow = u_img + (size_t)mirror_clamp(ys0 + 2 * p + rrow - 2 * R, a.H) * a.W;
-                float v[4], h[4], l[4];
+            constexpr int NL = TC_LOAD_WARPS * 32, UNR = 4;      // UNR cells' loads in flight per thread
+            for (int idx0 = lt; idx0 < 2 * TC_CWU; idx0 += NL * UNR) {
+                float v[UNR][4];
 #pragma unroll
-                for (int e = 0; e < 4; ++e) v[e] = __ldg(grow + mirror_clamp(X0 + 2 * xg + e - 2 * R, a.W));
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    h[e] = __uint_as_float(__float_as_uint(v[e]) & 0xFFFFE000u);
-                    l[e] = v[e] - h[e];
+                for (int k = 0; k < UNR; ++k) {
+                    const int idx = idx0 + k * NL;
+                    if (idx < 2 * TC_CWU) {
+                        const int rrow = idx / TC_CWU, xg = idx - rrow * TC_CWU;
+                        tc_cell_load(u_img, a.H, a.W, ys0 + 2 * p + rrow - 2 * R, X0 + 2 * xg - 2 * R, v[k]);
+                    }
                 }
-                const int cell = ((slot * 2 + rrow) * TC_CW + xg) * 16;
-                *reinterpret_cast<float4*>(smem + C::SM_UHI + cell) = make_float4(h[0], h[1], h[2], h[3]);
-                *reinterpret_cast<float4*>(smem + C::SM_ULO + cell) = make_float4(l[0], l[1], l[2], l[3]);
+#pragma unroll
+                for (int k = 0; k < UNR; ++k) {
+                    const int idx = idx0 + k * NL;
+                    if (idx < 2 * TC_CWU) {
+                        const int rrow = idx / TC_CWU, xg = idx - rrow * TC_CWU;
+                        tc_cell_store(smem + C::SM_UHI, smem + C::SM_ULO, ((slot * 2 + rrow) * TC_CW + xg) * 16, v[k]);
+                    }
+                }
             }
             fence_async_smem();
             __syncwarp();
@@ -622,6 +682,19 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp, int 
     __syncthreads();
     if (warp == TC_MMA_WARP)
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem), "r"(512) : "memory");
+}
+
+// a5 for the filter-chunk mode: u_t = u - (sum of the chunks' partial sums, in chunk order + lambda (u - f))
+__global__ void __launch_bounds__(256) tc_update_kernel(StageArgs a, const float* __restrict__ part, int nchunk)
+{
+    const size_t n = (size_t)a.B * a.H * a.W;
+    const float lambda = a.lambda_ptr ? __ldg(a.lambda_ptr) : a.lambda_val;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        float s = 0.0f;
+        for (int c = 0; c < nchunk; ++c) s += __ldcg(part + (size_t)c * n + i);
+        const float uu = a.u_in[i];
+        a.u_out[i] = uu - (s + lambda * (uu - a.f[i]));
+    }
 }
 
 inline int tc_env_int(const char* name)
@@ -640,29 +713,39 @@ size_t tc_workspace_bytes(int T, int N_k, int ksize)
     return (size_t)T * tc_ws_stage_bytes(ksize, nkp);
 }
 
-TcPlan plan_stage_tc(int B, int H, int W, int ksize, int num_sms)
+TcPlan plan_stage_tc(int B, int H, int W, int N_k, int ksize, int num_sms)
 {
-    const int R = (ksize - 1) / 2, OW = 256 - 2 * R;
+    const int R = (ksize - 1) / 2, OW = 256 - 2 * R, nkp = (N_k + 7) / 8 * 8;
     TcPlan pl;
     pl.nxs = (W + OW - 1) / OW;
-    // row segments: minimise waves x (rows per segment + recomputed rows + a per-CTA constant, in rows)
-    const double c0 = 10.0;
+    // Units = images x filter chunks x row segments x strips.  Time of a unit in SM clocks (fitted on B200): a constant
+    // (operands to shared memory, tensor-memory allocation, pipeline fill and drain) + batches x the larger of the phi
+    // time of the chunk's filters and the per-batch floor of the MMA / drain pipeline.  Minimise waves x unit time (+ the
+    // update kernel when the bank is split).  Even segment heights: every segment then starts on an even row, so a pixel's
+    // arithmetic (the pairing of phi rows into batches) does not depend on how the rows are cut up.
     double best = -1.0;
-    pl.nys = 1; pl.seg_rows = H;
-    const int forced = tc_env_int("TNRD_TC_SEG");
-    for (int nys = 1; nys <= (H + 3) / 4; ++nys) {
-        int seg = (H + nys - 1) / nys;
-        seg += seg & 1;                 // even: every segment then starts on an even row, so a pixel's arithmetic (the
-                                        // pairing of phi rows into batches) does not depend on how the rows are cut up
-        if (forced > 0) seg = forced < H ? forced : H;
-        const int n = (H + seg - 1) / seg;
-        const long long units = (long long)B * pl.nxs * n;
-        const double cost = (double)((units + num_sms - 1) / num_sms) * (seg + 2 * R + c0);
-        if (best < 0 || cost < best) { best = cost; pl.nys = n; pl.seg_rows = seg; }
-        if (forced > 0) break;
+    pl.nys = 1; pl.seg_rows = H; pl.nchunk = 1;
+    const int forced = tc_env_int("TNRD_TC_SEG"), forced_chunk = tc_env_int("TNRD_TC_CHUNK");
+    for (int nchunk = 1; nchunk <= nkp / 8; ++nchunk) {
+        if (nkp % (8 * nchunk)) continue;
+        if (forced_chunk > 0 && nchunk != forced_chunk && nkp % (8 * forced_chunk) == 0) continue;
+        const double per_batch = 2900.0 + 408.0 * (nkp / nchunk);      // measured: 22.5 k clocks at 48 filters, 12.7 k at 24
+        for (int nys = 1; nys <= (H + 3) / 4; ++nys) {
+            int seg = (H + nys - 1) / nys;
+            seg += seg & 1;
+            if (forced > 0) seg = forced < H ? forced : H;
+            const int n = (H + seg - 1) / seg;
+            const long long units = (long long)B * nchunk * pl.nxs * n;
+            const double unit_clk = 14000.0 + ((seg + 2 * R) / 2 + 1) * per_batch;
+            // split bank: the update kernel (launch + (nchunk + 3) planes of traffic) and the doubled drain work
+            const double upd = nchunk > 1 ? 14000.0 + 0.004 * (double)B * H * W * (nchunk + 3) : 0.0;
+            const double cost = (double)((units + num_sms - 1) / num_sms) * unit_clk * (nchunk > 1 ? 1.06 : 1.0) + upd;
+            if (best < 0 || cost < best) { best = cost; pl.nys = n; pl.seg_rows = seg; pl.nchunk = nchunk; }
+            if (forced > 0) break;
+        }
     }
-    pl.units = (long long)B * pl.nxs * pl.nys;
-    pl.cost_rows = best;
+    pl.units = (long long)B * pl.nchunk * pl.nxs * pl.nys;
+    pl.cost_clk = best;
     return pl;
 }
 
@@ -680,7 +763,8 @@ cudaError_t launch_tc_prep(const float* prm, int T, int N_k, int ksize, unsigned
 }
 
 template <int KS>
-static cudaError_t launch_tc_ks(const StageArgs& a, const TcPlan& pl, const unsigned char* ws_t, int nkp, cudaStream_t st)
+static cudaError_t launch_tc_ks(const StageArgs& a, const TcPlan& pl, const unsigned char* ws_t, int nkp, float* part,
+                                cudaStream_t st)
 {
     using C = TcCfg<KS>;
     // the opt-in shared-memory size is a per-device function attribute: set it at every launch (cheap) so that any
@@ -689,20 +773,28 @@ static cudaError_t launch_tc_ks(const StageArgs& a, const TcPlan& pl, const unsi
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     if (e != cudaSuccess) return e;
     if (pl.units > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    kern<<<(unsigned)pl.units, TC_THREADS, C::SMEM, st>>>(a, ws_t, nkp, pl.nxs, pl.nys, pl.seg_rows);
+    kern<<<(unsigned)pl.units, TC_THREADS, C::SMEM, st>>>(a, ws_t, nkp, pl.nxs, pl.nys, pl.seg_rows, pl.nchunk,
+                                                          pl.nchunk > 1 ? part : nullptr);
     return cudaGetLastError();
 }
 
-cudaError_t launch_stage_tc(const StageArgs& a, const TcPlan& pl, const unsigned char* ws_t, cudaStream_t st,
+cudaError_t launch_stage_tc(const StageArgs& a, const TcPlan& pl, const unsigned char* ws_t, float* part, cudaStream_t st,
                             unsigned long long* launches)
 {
     const int nkp = (a.N_k + 7) / 8 * 8;
+    if (pl.nchunk > 1 && !part) return cudaErrorInvalidValue;
     cudaError_t e;
-    if (a.ksize == 7) e = launch_tc_ks<7>(a, pl, ws_t, nkp, st);
-    else if (a.ksize == 5) e = launch_tc_ks<5>(a, pl, ws_t, nkp, st);
+    if (a.ksize == 7) e = launch_tc_ks<7>(a, pl, ws_t, nkp, part, st);
+    else if (a.ksize == 5) e = launch_tc_ks<5>(a, pl, ws_t, nkp, part, st);
     else return cudaErrorInvalidValue;
     ++*launches;
-    return e;
+    if (e != cudaSuccess || pl.nchunk == 1) return e;
+    const size_t n = (size_t)a.B * a.H * a.W;
+    size_t blocks = (n + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    tc_update_kernel<<<(unsigned)blocks, 256, 0, st>>>(a, part, pl.nchunk);
+    ++*launches;
+    return cudaGetLastError();
 }
 
 size_t tc_ws_stage_stride(int N_k, int ksize) { return tc_ws_stage_bytes(ksize, (N_k + 7) / 8 * 8); }

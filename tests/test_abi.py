@@ -92,9 +92,9 @@ def test_argument_validation_without_gpu(L):
     assert L.tnrd_diffuse_backward(p, p + 64, p + 128, n, *bw, p + 192, p + 192, n, n, n, st) == tnrd.ERR_ALIAS  # u_T == grad_u0
     assert L.tnrd_diffuse_backward(p, p + 64, p + 128, n, *bw, p + 64, n, n, n, n, st) == tnrd.ERR_ALIAS     # u_T == u0
     # tensor-core plan query: pure host logic
-    q = (ctypes.c_longlong * 6)()
+    q = (ctypes.c_longlong * 7)()
     assert L.tnrd_tc_plan_query(1, 4096, 4096, 48, 7, 148, q) == tnrd.OK and q[0] == 2 and q[1] == 17 and q[5] == 250
-    assert q[4] == q[1] * q[2] and q[3] % 2 == 0
+    assert q[4] == q[1] * q[2] * q[6] and q[3] % 2 == 0 and q[6] == 1
     assert L.tnrd_tc_plan_query(1, 64, 64, 8, 3, 148, q) == tnrd.OK and q[0] == 0
     assert L.tnrd_tc_plan_query(1, 64, 64, 8, 3, 148, None) == tnrd.ERR_NULL
     assert L.tnrd_microbench(0, None, st) == tnrd.ERR_NULL

@@ -227,13 +227,48 @@ def test_automatic_kernel_choice(tnrd):
     n = num_sms()
     assert tnrd.tnrd_tc_plan_query(1, 4096, 4096, 48, 7, n)["applies"] == 2
     assert tnrd.tnrd_tc_plan_query(128, 321, 481, 48, 7, n)["applies"] == 2
-    assert tnrd.tnrd_tc_plan_query(1, 321, 481, 48, 7, n)["applies"] == 1       # one small image: the tile kernel
+    q = tnrd.tnrd_tc_plan_query(1, 321, 481, 48, 7, n)                          # one small image: the bank cut in chunks
+    assert q["applies"] == 2 and q["nchunk"] > 1 and q["units"] == q["nxs"] * q["nys"] * q["nchunk"]
+    assert tnrd.tnrd_tc_plan_query(1, 1024, 1024, 48, 7, n)["nchunk"] == 1
+    assert tnrd.tnrd_tc_plan_query(1, 200, 150, 48, 7, n)["applies"] == 1       # narrower than a strip: the tile kernel
     assert tnrd.tnrd_tc_plan_query(1, 64, 64, 8, 3, n)["applies"] == 0
     # launch count: one staging kernel + the operand kernel + one stage kernel per stage
     c = tnrd_gen.make_config(4, size=1024, T=5)
     tnrd.tnrd_reset_launch_count()
     run_gpu(tnrd, c)
     assert tnrd.tnrd_launch_count() == 2 + c["T"]
+    # with a split bank each stage is the tensor-core kernel plus the kernel that sums the chunks' partial updates
+    c = tnrd_gen.make_small(262, 1, 321, 481, 3, 48, 7)
+    tnrd.tnrd_reset_launch_count()
+    run_gpu(tnrd, c)
+    assert tnrd.tnrd_launch_count() == 2 + 2 * c["T"]
+
+
+@pytest.mark.parametrize("nchunk,N_k,ksize", [(2, 48, 7), (3, 48, 7), (6, 48, 7), (3, 24, 5), (2, 16, 7)])
+def test_filter_chunks(tnrd, monkeypatch, nchunk, N_k, ksize):
+    """The filter bank cut into chunks (units = chunks x segments x strips, partial updates summed by a second kernel):
+    same bound against the oracle as the whole bank, identical from run to run, equal to the whole bank up to the order
+    of the sum over filters, and legal in place (the partial sums live in scratch)."""
+    B, H, W, T = 2, 77, 300, 3
+    c = tnrd_gen.make_small(263 + nchunk, B, H, W, T, N_k, ksize)
+    want = run_oracle(c)
+    monkeypatch.setenv("TNRD_TC_CHUNK", "1")
+    whole = run_gpu(tnrd, c, kernel=3)
+    monkeypatch.setenv("TNRD_TC_CHUNK", str(nchunk))
+    got = run_gpu(tnrd, c, kernel=3)
+    assert np.array_equal(got, run_gpu(tnrd, c, kernel=3))
+    check(got, want, f"tc chunks {nchunk}", tight=True)
+    assert np.max(np.abs(got - whole)) <= 6.2e-5          # 4 ulp at 255: only the order of the sum over filters differs
+    tnrd.tnrd_set_kernel(3)
+    try:
+        f, v = dev(c["f"]), dev(c["u0"])
+        k, w, mu = dev(c["filters"]), dev(c["rbf_w"]), dev(c["rbf_mu"])
+        for t in range(T):
+            tnrd.tnrd_stage(f, v, B, H, W, N_k, ksize, k[t], w[t], mu, c["rbf_gamma"], float(c["lambda"][t]), v)
+        torch.cuda.synchronize()
+        assert np.array_equal(v.cpu().numpy().astype(np.float64), got), "in-place stage with chunks differs"
+    finally:
+        tnrd.tnrd_set_kernel(0)
 
 
 def test_nearly_equidistant_centres_take_the_direct_form(tnrd):
