@@ -28,7 +28,10 @@
 //
 // Strips overlap by 2r phi columns and row segments by 2r phi rows (recomputed) so that a CTA completes its own
 // outputs: no partial sums in HBM, no second kernel, 12 B of DRAM traffic per pixel-stage.
-// Warp roles: 24 phi warps (4 per tensor-memory lane quarter, sharing the quarter's filter pairs through a ticket
+// When one stage of a call has too few such units to fill the GPU (a single 321x481 image), the filter bank is cut into
+// chunks as well (plan_stage_tc): a unit then evaluates only its chunk's filters and writes the partial sum of Eq. 7's
+// diffusion term to scratch, and tc_update_kernel adds the chunks in a fixed order and applies the reaction term.
+// Warp roles: 24 phi warps (6 per tensor-memory lane quarter, sharing the quarter's filter pairs through a ticket
 // counter), 4 drain warps (fold + a5), 1 MMA-issuing warp, 1 loader warp; mbarrier pipelines between them (u row pairs,
 // z double-buffered, scatter table).
 #include <cuda_bf16.h>
