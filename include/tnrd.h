@@ -91,10 +91,16 @@ int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, in
  * End-to-end variant with HOST buffers: every pointer below is a host pointer (pinned memory makes the
  * copies asynchronous).  Copies f, u0 and the parameters (packed, one copy) to the device, runs the T stages on
  * `stream`, copies u_T back to `out` and synchronises before returning.  f == u0 (same host pointer) is uploaded once.
- * Device staging buffers are cached in the library scratch.  With the tensor-core kernel (tnrd_set_kernel) the first
- * and the last stage are cut in two halves (the images of a batch, or the rows of a single image at an even row) and
- * the copies run on two internal streams, so that half of the upload and half of the download overlap the arithmetic;
- * the result is bit-identical to tnrd_diffuse on device buffers.
+ * Device staging buffers are cached in the library scratch.  With the tensor-core kernel (tnrd_set_kernel) the copies
+ * overlap the arithmetic, on internal streams:
+ *   - a batch is cut into up to four groups of images, each taken through all T stages on a stream of its own, so that a
+ *     group computes while the next one arrives and the previous one leaves;
+ *   - a single image arrives in blocks of 32 rows, the rows of the first wave of CTAs first; the first stage's loader
+ *     warps wait for the block they are about to read (one device word per block, written by the copy stream; a wait
+ *     that lasts two seconds ends the call with TNRD_ERR_CUDA), and when `out` is pinned (or otherwise device-mapped)
+ *     host memory the last stage stores u_T into it directly; a pageable `out` gets one copy after the last stage.
+ * Either way the result is bit-identical to tnrd_diffuse on device buffers.  The buffers must stay valid and unchanged
+ * until the call returns (it synchronises `stream`).
  */
 int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int T, int N_k, int ksize,
                       const float* filters, const float* rbf_w, const float* rbf_mu, float rbf_gamma,

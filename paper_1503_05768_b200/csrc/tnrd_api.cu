@@ -54,6 +54,8 @@ struct Buf {
     size_t cap = 0;  // floats
 };
 
+constexpr int HOST_BANDS = 4;
+
 struct Scratch {
     int dev = -1;
     cudaStream_t st = nullptr;
@@ -65,9 +67,14 @@ struct Scratch {
     Buf stats;                        // two 64-bit counters (tnrd_phi_stats)
     // host entry point: copy streams and events of the pipelined path, pinned staging of the packed parameters
     cudaStream_t s_in = nullptr, s_out = nullptr;
-    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    cudaStream_t s_band[HOST_BANDS] = {};       // one compute stream per group of images, falling priority
+    cudaEvent_t ev[5 + 2 * HOST_BANDS] = {};
     float* h_par_pinned = nullptr;
     size_t h_par_cap = 0;
+    Buf arrive;                       // single-image path: {time-out, one word per block of 32 rows}
+    unsigned* h_word = nullptr;       // pinned: the time-out word read back
+    unsigned* h_flags = nullptr;      // pinned: snapshots of the block words, one per pass / piece of the copy schedule
+    size_t h_flags_cap = 0;
     Buf tab;                          // piecewise-linear phi tables [T][N_k][4096] float2 + 4 header floats
     Buf h_f, h_u, h_out, h_par;       // device staging of the host entry point
     Buf bw_maps, bw_part, bw_trace, bw_e[2];   // backward pass: P/V maps, per-CTA partial sums, iterates, dl/du planes
@@ -127,6 +134,7 @@ struct Call {
     cudaStream_t st = nullptr;
     bool tc = false;   // this call runs the tensor-core stage kernel
     bool small = false; // this call runs the small-image kernel (all stages in one launch)
+    int nchunk_fixed = 0, seg_mult = 2;   // handed to plan_stage_tc by run_stage (the host entry point's first stage)
 };
 
 // The automatic choice between the two stage kernels: strips of the tensor-core kernel are 256 - 2r columns wide and
@@ -231,7 +239,7 @@ int run_stage(Call& c, tnrd::StageArgs a, int phi, int t)
             a.stats = reinterpret_cast<unsigned long long*>(sc->stats.p);
         }
         const int rows = a.row_hi > 0 ? a.row_hi - a.row_lo : a.H;
-        const tnrd::TcPlan pl = tnrd::plan_stage_tc(a.B, rows, a.W, a.N_k, a.ksize, sc->num_sms);
+        const tnrd::TcPlan pl = tnrd::plan_stage_tc(a.B, rows, a.W, a.N_k, a.ksize, sc->num_sms, c.nchunk_fixed, c.seg_mult);
         if (pl.nchunk > 1) {
             int rc = grow(sc->split, (size_t)pl.nchunk * a.B * a.H * a.W, c.st);
             if (rc != TNRD_OK) return rc;
@@ -362,7 +370,14 @@ static int host_pipe_init(Scratch* sc, size_t npar)
     if (!sc->s_in) {
         TNRD_CUDA(cudaStreamCreateWithFlags(&sc->s_in, cudaStreamNonBlocking));
         TNRD_CUDA(cudaStreamCreateWithFlags(&sc->s_out, cudaStreamNonBlocking));
+        int pr_least = 0, pr_greatest = 0;      // numerically lower = more urgent
+        TNRD_CUDA(cudaDeviceGetStreamPriorityRange(&pr_least, &pr_greatest));
+        for (int g = 0; g < HOST_BANDS; ++g) {
+            const int pr = pr_greatest + g < pr_least ? pr_greatest + g : pr_least;
+            TNRD_CUDA(cudaStreamCreateWithPriority(&sc->s_band[g], cudaStreamNonBlocking, pr));
+        }
         for (auto& e : sc->ev) TNRD_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        TNRD_CUDA(cudaHostAlloc(&sc->h_word, sizeof(unsigned), cudaHostAllocDefault));
     }
     if (npar > sc->h_par_cap) {
         if (sc->h_par_pinned) TNRD_CUDA(cudaFreeHost(sc->h_par_pinned));
@@ -372,6 +387,25 @@ static int host_pipe_init(Scratch* sc, size_t npar)
         sc->h_par_cap = npar;
     }
     return TNRD_OK;
+}
+
+static int host_flags_reserve(Scratch* sc, size_t words)
+{
+    if (words <= sc->h_flags_cap) return TNRD_OK;
+    if (sc->h_flags) TNRD_CUDA(cudaFreeHost(sc->h_flags));
+    sc->h_flags = nullptr;
+    sc->h_flags_cap = 0;
+    TNRD_CUDA(cudaHostAlloc(&sc->h_flags, words * sizeof(unsigned), cudaHostAllocDefault));
+    sc->h_flags_cap = words;
+    return TNRD_OK;
+}
+
+// experiments with the host entry point: 1 = a single image takes the two-halves path as well, 2 = never store to host
+// memory from a kernel, 3 = the input strictly top to bottom
+static int host_mode_env()
+{
+    const char* e = getenv("TNRD_HOST_MODE");
+    return e ? atoi(e) : 0;
 }
 
 int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int T, int N_k, int ksize,
@@ -428,6 +462,186 @@ int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int 
         TNRD_CUDA(cudaStreamSynchronize(st));
         return TNRD_OK;
     }
+    if (B == 1 && host_mode_env() != 1) {
+        // One image: the stage launches are those of the device call (the first with segment heights that are a multiple
+        // of 32).  The input arrives in blocks of 32 whole rows (they end on 128-byte lines) on a copy stream, and one
+        // word per block says so; the loader warps of the FIRST stage poll the word of a block before they read its
+        // first row, so the stage starts with the first blocks instead of the last.  When `out` is pinned host memory
+        // the LAST stage stores u_T straight into it (posted writes over PCIe while the stage computes), otherwise one
+        // copy follows.  Same arithmetic per pixel whatever the segments: bit-identical to the device call.
+        if ((rc = stage_params(c, d_k, d_w, d_mu, rbf_gamma, T, N_k, ksize, phi)) != TNRD_OK) return rc;
+        const int nblk = (H + 31) / 32;
+        if ((rc = grow(sc->arrive, (size_t)nblk + 4, st)) != TNRD_OK) return rc;
+        if (T > 1 && (rc = grow(sc->pp, n, st)) != TNRD_OK) return rc;
+        float* out_dev = nullptr;
+        {
+            cudaPointerAttributes pa;
+            if (cudaPointerGetAttributes(&pa, out) == cudaSuccess && pa.type == cudaMemoryTypeHost && pa.devicePointer &&
+                host_mode_env() != 2)
+                out_dev = static_cast<float*>(pa.devicePointer);
+            (void)cudaGetLastError();
+        }
+        unsigned* arrived = reinterpret_cast<unsigned*>(sc->arrive.p);
+        TNRD_CUDA(cudaEventRecord(sc->ev[0], st));
+        TNRD_CUDA(cudaStreamWaitEvent(sc->s_in, sc->ev[0], 0));
+        TNRD_CUDA(cudaMemsetAsync(arrived, 0, ((size_t)nblk + 1) * sizeof(unsigned), sc->s_in));
+        TNRD_CUDA(cudaEventRecord(sc->ev[1], sc->s_in));
+        // The copy schedule.  The first stage's CTAs each walk down a segment of S rows, and the first wave of CTAs
+        // covers the top `nreg` segments: their rows go first, INTERLEAVED -- pass k brings rows [32 k, 32 k + 32) of
+        // every region (region j = the rows segment j reads first, [j S - 32, (j + 1) S - 32); one strided copy per
+        // pass) -- so that every CTA of the first wave starts after the first pass and the data then stays ahead of
+        // it.  The rest of the image follows top to bottom in pieces of about 4 MB.  After every pass / piece the
+        // block words are refreshed with one small copy from a pinned snapshot.
+        const int nchunk_dev = tnrd::plan_stage_tc(1, H, W, N_k, ksize, sc->num_sms).nchunk;     // as the device call cuts the bank
+        const tnrd::TcPlan pl1 = tnrd::plan_stage_tc(1, H, W, N_k, ksize, sc->num_sms, nchunk_dev, 32);
+        const int S = pl1.seg_rows;
+        int nreg = (sc->num_sms + pl1.nxs * pl1.nchunk - 1) / (pl1.nxs * pl1.nchunk);
+        if (nreg > pl1.nys) nreg = pl1.nys;
+        const bool inter = S % 32 == 0 && S >= 64 && nreg >= 2 && host_mode_env() != 3;
+        const int E = !inter ? 0 : ((long long)nreg * S - 32 > H ? H : nreg * S - 32);   // rows [0, E) are interleaved
+        int piece = (int)(((1u << 20) / (size_t)W + 31) & ~(size_t)31);       // rows per piece of the linear part
+        if (piece < 32) piece = 32;
+        {
+            int ops = (inter ? S / 32 : 0) + 8;
+            for (int r = E, pc = inter ? piece : 32; r < H; r += pc, ++ops) if (!inter && pc < piece) pc *= 2;
+            if ((rc = host_flags_reserve(sc, (size_t)ops * nblk)) != TNRD_OK) return rc;
+        }
+        std::vector<unsigned> ok((size_t)nblk, 0u);
+        int op = 0;
+        auto copy_rows = [&](int r0, int r1) -> int {
+            const size_t o = (size_t)r0 * W, cnt = (size_t)(r1 - r0) * W;
+            TNRD_CUDA(cudaMemcpyAsync(d_f + o, f + o, cnt * sizeof(float), cudaMemcpyHostToDevice, sc->s_in));
+            if (u0 != f) TNRD_CUDA(cudaMemcpyAsync(d_u0 + o, u0 + o, cnt * sizeof(float), cudaMemcpyHostToDevice, sc->s_in));
+            for (int bk = r0 / 32; bk < (r1 + 31) / 32; ++bk) ok[bk] = 1u;
+            return TNRD_OK;
+        };
+        auto flush = [&]() -> int {
+            unsigned* snap = sc->h_flags + (size_t)op * nblk;
+            memcpy(snap, ok.data(), (size_t)nblk * sizeof(unsigned));
+            TNRD_CUDA(cudaMemcpyAsync(arrived + 1, snap, (size_t)nblk * sizeof(unsigned), cudaMemcpyHostToDevice, sc->s_in));
+            ++op;
+            return TNRD_OK;
+        };
+        if (inter) {
+            const int npass = S / 32;
+            for (int k = 0; k < npass; ++k) {
+                if (k <= npass - 2 && 32 * k < E)         // region 0 = rows [0, S - 32)
+                    if ((rc = copy_rows(32 * k, 32 * k + 32 < E ? 32 * k + 32 : E)) != TNRD_OK) return rc;
+                int jfull = 0;                            // regions 1 .. jfull have this block whole
+                for (int j = 1; j < nreg && j * S + 32 * k <= E; ++j) jfull = j;
+                if (jfull >= 1) {
+                    const size_t o = (size_t)(S - 32 + 32 * k) * W, pitch = (size_t)S * W * sizeof(float);
+                    const size_t width = (size_t)32 * W * sizeof(float);
+                    TNRD_CUDA(cudaMemcpy2DAsync(d_f + o, pitch, f + o, pitch, width, (size_t)jfull, cudaMemcpyHostToDevice, sc->s_in));
+                    if (u0 != f)
+                        TNRD_CUDA(cudaMemcpy2DAsync(d_u0 + o, pitch, u0 + o, pitch, width, (size_t)jfull, cudaMemcpyHostToDevice, sc->s_in));
+                    for (int j = 1; j <= jfull; ++j) ok[(j * S - 32 + 32 * k) / 32] = 1u;
+                }
+                const int tail = (jfull + 1) * S - 32 + 32 * k;      // a last block cut short by the end of the image
+                if (jfull + 1 < nreg && tail < E)
+                    if ((rc = copy_rows(tail, E)) != TNRD_OK) return rc;
+                if ((rc = flush()) != TNRD_OK) return rc;
+            }
+        }
+        for (int r0 = E, pc = inter ? piece : 32; r0 < H;) {
+            const int r1 = r0 + pc < H ? r0 + pc : H;
+            if ((rc = copy_rows(r0, r1)) != TNRD_OK) return rc;
+            if ((rc = flush()) != TNRD_OK) return rc;
+            r0 = r1;
+            if (!inter && pc < piece) pc *= 2;
+        }
+        TNRD_CUDA(cudaStreamWaitEvent(st, sc->ev[1], 0));          // the block words are zero before the first stage starts
+        const size_t rec = (size_t)N_k * tnrd::prm_stride(ksize);
+        const float* src = d_u0;
+        for (int t = 1; t <= T; ++t) {
+            float* dst = ((T - t) & 1) ? sc->pp.p : (t == T && out_dev ? out_dev : d_out);
+            tnrd::StageArgs a{d_f, src, dst, sc->prm.p + (size_t)(t - 1) * rec, d_lam + (t - 1), 0.0f, B, H, W, N_k, ksize};
+            if (t == 1) {                           // the plan the copy schedule was made for
+                a.arrived = arrived;
+                c.nchunk_fixed = nchunk_dev;
+                c.seg_mult = 32;
+            } else {
+                c.nchunk_fixed = 0;
+                c.seg_mult = 2;
+            }
+            if ((rc = run_stage(c, a, phi, t - 1)) != TNRD_OK) return rc;
+            src = dst;
+        }
+        if (!out_dev) TNRD_CUDA(cudaMemcpyAsync(out, d_out, n * sizeof(float), cudaMemcpyDeviceToHost, st));
+        *sc->h_word = 0;
+        TNRD_CUDA(cudaMemcpyAsync(sc->h_word, arrived, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
+        TNRD_CUDA(cudaStreamSynchronize(st));
+        TNRD_CUDA(cudaStreamSynchronize(sc->s_in));
+        if (*sc->h_word) return cuda_fail(cudaErrorLaunchTimeout, "tnrd_diffuse_host: the first stage gave up waiting for its input");
+        return TNRD_OK;
+    }
+    // the filter chunks of the device call: every launch below cuts the bank the same way (the order of the sum over
+    // filters), whatever part of the batch it covers
+    const int nchunk_call = tnrd::plan_stage_tc(B, H, W, N_k, ksize, sc->num_sms).nchunk;
+    if (B >= 2 && nchunk_call == 1 && host_mode_env() != 1) {
+        // A batch: up to four GROUPS of images, each taken through all T stages on a stream of its own (falling priority,
+        // so that the groups finish one after the other; the SMs a group's last wave leaves idle take units of the next
+        // group).  Group g computes while the input of group g+1 arrives and the result of group g-1 leaves.  The first
+        // and the last group are small (their copies are the ones nothing hides).  Images are independent: bit-identical.
+        if ((rc = stage_params(c, d_k, d_w, d_mu, rbf_gamma, T, N_k, ksize, phi)) != TNRD_OK) return rc;
+        if (g_stats.load() && !sc->stats.p) {
+            if ((rc = grow(sc->stats, 4, st)) != TNRD_OK) return rc;
+            TNRD_CUDA(cudaMemsetAsync(sc->stats.p, 0, 16, st));
+        }
+        if (T > 1 && (rc = grow(sc->pp, n, st)) != TNRD_OK) return rc;
+        int lo[HOST_BANDS], hi[HOST_BANDS], G = 0;
+        {
+            const int want = B < HOST_BANDS ? B : HOST_BANDS;
+            const long long wsum = want >= 2 ? 2 + 3LL * (want - 2) : 1;
+            long long acc = 0;
+            int prev = 0;
+            for (int g = 0; g < want; ++g) {
+                acc += (g == 0 || g == want - 1) ? 1 : 3;
+                const int cut = g == want - 1 ? B : (int)((B * acc + wsum / 2) / wsum);
+                if (cut <= prev) continue;
+                lo[G] = prev; hi[G] = cut; prev = cut; ++G;
+            }
+        }
+        const size_t plane = (size_t)H * W;
+        cudaEvent_t* ev_in = sc->ev + 5;
+        cudaEvent_t* ev_done = sc->ev + 5 + HOST_BANDS;
+        TNRD_CUDA(cudaEventRecord(sc->ev[0], st));
+        TNRD_CUDA(cudaStreamWaitEvent(sc->s_in, sc->ev[0], 0));
+        TNRD_CUDA(cudaStreamWaitEvent(sc->s_out, sc->ev[0], 0));
+        for (int g = 0; g < G; ++g) {
+            const size_t o = (size_t)lo[g] * plane, cnt = (size_t)(hi[g] - lo[g]) * plane;
+            TNRD_CUDA(cudaMemcpyAsync(d_f + o, f + o, cnt * sizeof(float), cudaMemcpyHostToDevice, sc->s_in));
+            if (u0 != f) TNRD_CUDA(cudaMemcpyAsync(d_u0 + o, u0 + o, cnt * sizeof(float), cudaMemcpyHostToDevice, sc->s_in));
+            TNRD_CUDA(cudaEventRecord(ev_in[g], sc->s_in));
+        }
+        const size_t rec = (size_t)N_k * tnrd::prm_stride(ksize);
+        c.nchunk_fixed = 1;                 // concurrent launches must not share the partial-sum scratch
+        for (int g = 0; g < G; ++g) {
+            cudaStream_t bs = sc->s_band[g];
+            TNRD_CUDA(cudaStreamWaitEvent(bs, sc->ev[0], 0));
+            TNRD_CUDA(cudaStreamWaitEvent(bs, ev_in[g], 0));
+            const size_t o = (size_t)lo[g] * plane, cnt = (size_t)(hi[g] - lo[g]) * plane;
+            const float* src = d_u0 + o;
+            c.st = bs;
+            for (int t = 1; t <= T && rc == TNRD_OK; ++t) {
+                float* dst = (((T - t) & 1) ? sc->pp.p : d_out) + o;
+                tnrd::StageArgs a{d_f + o, src, dst, sc->prm.p + (size_t)(t - 1) * rec, d_lam + (t - 1), 0.0f,
+                                  hi[g] - lo[g], H, W, N_k, ksize};
+                rc = run_stage(c, a, phi, t - 1);
+                src = dst;
+            }
+            c.st = st;
+            if (rc != TNRD_OK) return rc;
+            TNRD_CUDA(cudaEventRecord(ev_done[g], bs));
+            TNRD_CUDA(cudaStreamWaitEvent(sc->s_out, ev_done[g], 0));
+            TNRD_CUDA(cudaMemcpyAsync(out + o, d_out + o, cnt * sizeof(float), cudaMemcpyDeviceToHost, sc->s_out));
+            TNRD_CUDA(cudaStreamWaitEvent(st, ev_done[g], 0));     // later work on the caller's stream comes after the groups
+        }
+        TNRD_CUDA(cudaStreamSynchronize(sc->s_out));
+        TNRD_CUDA(cudaStreamSynchronize(st));
+        return TNRD_OK;
+    }
+    c.nchunk_fixed = nchunk_call;
     // Pipelined (tensor-core kernel): the work of the FIRST and the LAST stage is cut in two halves -- the two halves of
     // the batch, or of the rows of a single image (an even row, so that every pixel sees the arithmetic of the un-cut
     // launch and the result is bit-identical) -- so that the first half computes while the second half of the input
@@ -766,12 +980,15 @@ void tnrd_shutdown(void)
     (void)cudaGetDevice(&cur);
     for (Scratch* s : g_scratch) {
         (void)cudaSetDevice(s->dev);
-        Buf* bufs[] = {&s->pp, &s->tcws, &s->stats, &s->prm, &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->refv, &s->split, &s->tab, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
+        Buf* bufs[] = {&s->pp, &s->arrive, &s->tcws, &s->stats, &s->prm, &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->refv, &s->split, &s->tab, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
         for (Buf* b : bufs)
             if (b->p) (void)cudaFree(b->p);   // synchronising free: the stream may be gone by now
         if (s->s_in) { (void)cudaStreamDestroy(s->s_in); (void)cudaStreamDestroy(s->s_out); }
+        for (cudaStream_t b : s->s_band) if (b) (void)cudaStreamDestroy(b);
         for (cudaEvent_t e : s->ev) if (e) (void)cudaEventDestroy(e);
         if (s->h_par_pinned) (void)cudaFreeHost(s->h_par_pinned);
+        if (s->h_word) (void)cudaFreeHost(s->h_word);
+        if (s->h_flags) (void)cudaFreeHost(s->h_flags);
         delete s;
     }
     g_scratch.clear();

@@ -71,6 +71,10 @@ struct StageArgs {
     const float* tabhdr;    // their header (tnrd_table.cu), device
     unsigned long long* stats;  // null, or device counters {phi group evaluations executed, defined} (tensor-core kernel)
     int row_lo, row_hi;         // tensor-core kernel: this launch completes output rows [row_lo, row_hi) only; 0, 0 = all rows
+    // tensor-core kernel, one image, host entry point: null, or device words {set to 1 by a poll that timed out, then one
+    // word per block of 32 rows: non-zero once the block of f / u_in has arrived} -- copied by another stream while the
+    // kernel runs; the loader polls the word of a block before it reads its first row
+    unsigned* arrived;
 };
 
 // Launch plan of the fused stage kernel (tnrd_fused.cu: plan_stage_fused).  Tiles partition the phi region
@@ -150,7 +154,9 @@ struct TcPlan {
 bool tc_supported(int N_k, int ksize);                       // ksize 5 or 7, N_k <= 48
 size_t tc_workspace_bytes(int T, int N_k, int ksize);        // Toeplitz operands of T stages
 size_t tc_ws_stage_stride(int N_k, int ksize);               // bytes per stage inside that workspace
-TcPlan plan_stage_tc(int B, int H, int W, int N_k, int ksize, int num_sms);   // H = number of output rows of the launch
+// H = number of output rows of the launch; nchunk_fixed > 0: that many filter chunks, no choice; seg_mult: segment heights
+// are a multiple of it (even; the host entry point asks for 32, the rows of an arrival block)
+TcPlan plan_stage_tc(int B, int H, int W, int N_k, int ksize, int num_sms, int nchunk_fixed = 0, int seg_mult = 2);
 // prm = staged records of T stages (launch_prep); ws receives the operands
 cudaError_t launch_tc_prep(const float* prm, int T, int N_k, int ksize, unsigned char* ws, cudaStream_t st,
                            unsigned long long* launches);

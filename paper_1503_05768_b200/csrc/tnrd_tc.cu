@@ -292,6 +292,26 @@ __device__ __forceinline__ void split_bf16(float2 v, uint32_t& hi, uint32_t& lo)
     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(lo) : "f"(v.y - hy), "f"(v.x - hx));
 }
 
+// Host entry point, one image: the input plane is still arriving (copy engine, in blocks of 32 whole rows, so every
+// block ends on a 128-byte line and no line is read into L1 before all of it is there) while the first stage runs.
+// arrived[1 + b] != 0 once block b is there.  A CTA reads its rows top to bottom, so it checks each block as it enters
+// it: waits until the block of row `need - 1` is there and returns the first row of the next block; gives up after
+// about two seconds (word 0, reported by the entry point) rather than hang the GPU.
+__device__ __forceinline__ int tc_wait_rows(unsigned* arrived, int need, int have)
+{
+    if (have >= need) return have;
+    const int blk = (need - 1) >> 5;
+    int spins = 0;
+    for (;;) {
+        unsigned v;
+        asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(arrived + 1 + blk) : "memory");
+        if (v) break;
+        __nanosleep(500);
+        if (++spins > (1 << 22)) { atomicExch(arrived, 1u); break; }
+    }
+    return (blk + 1) << 5;
+}
+
 // One 16-byte cell (row, g) = u~[row][2g .. 2g+3] of the u ring, through the mirror map, split
 // x = hi + lo with hi = the top 19 bits (a TF32 number; lo is exact): the four loads ...
 __device__ __forceinline__ void tc_cell_load(const float* __restrict__ u_img, int H, int W, int urow, int ucol, float (&v)[4])
@@ -427,6 +447,13 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
     }
     // The first R + 1 row pairs (what the first batch needs) are gathered by ALL threads: left to the loader warp alone
     // they would cost R + 1 round trips to L2 per thread chain before the first MMA can issue.
+    if (a.arrived) {       // the first R + 1 pairs: rows ys0 - 2r .. ys0 + 1 (mirrored rows above the image: rows up to 2r)
+        if (tid == 0) {
+            tc_wait_rows(a.arrived, max(ys0 - 2 * R, 0) + 1, 0);
+            tc_wait_rows(a.arrived, min(a.H, max(ys0 + 2, 2 * R + 1)), 0);
+        }
+        __syncthreads();
+    }
     {
         const int npre = min(NPAIRS, R + 1) * 2 * TC_CWU;
         for (int idx = tid; idx < npre; idx += TC_THREADS) {
@@ -653,9 +680,11 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
     } else {
         // =================================== loader warps ===================================
         const int lt = tid - (TC_MMA_WARP + 1) * 32;
+        int have = 0;
         for (int p = R + 1; p < NPAIRS; ++p) {
             const int slot = p % TC_NP;
             if (p >= TC_NP) mbar_wait_idle(pempty + slot, ((p / TC_NP) - 1) & 1);
+            if (a.arrived) have = tc_wait_rows(a.arrived, min(a.H, max(ys0 + 2 * p + 2 - 2 * R, 2 * R + 1)), have);
             constexpr int NL = TC_LOAD_WARPS * 32, UNR = 4;      // UNR cells' loads in flight per thread
             for (int idx0 = lt; idx0 < 2 * TC_CWU; idx0 += NL * UNR) {
                 float v[UNR][4];
@@ -716,7 +745,7 @@ size_t tc_workspace_bytes(int T, int N_k, int ksize)
     return (size_t)T * tc_ws_stage_bytes(ksize, nkp);
 }
 
-TcPlan plan_stage_tc(int B, int H, int W, int N_k, int ksize, int num_sms)
+TcPlan plan_stage_tc(int B, int H, int W, int N_k, int ksize, int num_sms, int nchunk_fixed, int seg_mult)
 {
     const int R = (ksize - 1) / 2, OW = 256 - 2 * R, nkp = (N_k + 7) / 8 * 8;
     TcPlan pl;
@@ -731,11 +760,12 @@ TcPlan plan_stage_tc(int B, int H, int W, int N_k, int ksize, int num_sms)
     const int forced = tc_env_int("TNRD_TC_SEG"), forced_chunk = tc_env_int("TNRD_TC_CHUNK");
     for (int nchunk = 1; nchunk <= nkp / 8; ++nchunk) {
         if (nkp % (8 * nchunk)) continue;
-        if (forced_chunk > 0 && nchunk != forced_chunk && nkp % (8 * forced_chunk) == 0) continue;
+        if (nchunk_fixed > 0 && nchunk != nchunk_fixed) continue;
+        if (nchunk_fixed <= 0 && forced_chunk > 0 && nchunk != forced_chunk && nkp % (8 * forced_chunk) == 0) continue;
         const double per_batch = 2900.0 + 408.0 * (nkp / nchunk);      // measured: 22.5 k clocks at 48 filters, 12.7 k at 24
         for (int nys = 1; nys <= (H + 3) / 4; ++nys) {
             int seg = (H + nys - 1) / nys;
-            seg += seg & 1;
+            seg = (seg + seg_mult - 1) / seg_mult * seg_mult;
             if (forced > 0) seg = forced < H ? forced : H;
             const int n = (H + seg - 1) / seg;
             const long long units = (long long)B * nchunk * pl.nxs * n;

@@ -304,7 +304,8 @@ def test_phi_statistics_counters(tnrd, monkeypatch):
     pl = tnrd.tnrd_tc_plan_query(1, 64, 500, 16, 7, num_sms())
     batches = (pl["seg_rows"] + 6 + 1) // 2                    # per unit (every segment has seg_rows rows here)
     assert 64 % pl["seg_rows"] == 0
-    assert de == 5 * 16 * 4 * batches * pl["units"] * c["T"], "5 groups x filters x lane quarters x batches x CTAs x stages"
+    assert pl["units"] == pl["nxs"] * pl["nys"] * pl["nchunk"]      # a unit of a split bank counts its own filters only
+    assert de == 5 * 16 * 4 * batches * pl["nxs"] * pl["nys"] * c["T"], "5 groups x filters x lane quarters x batches x strips x segments x stages"
     assert 0 < ex <= de
     flat = dict(c, f=np.full_like(c["f"], 100.0), u0=np.full_like(c["f"], 100.0))     # z = 0 everywhere
     tnrd.tnrd_phi_stats(True)
@@ -349,24 +350,44 @@ def test_two_devices_in_one_process(tnrd):
             check(out.cpu().numpy().astype(np.float64), want, f"device 1 kernel {kernel}", tight=True)
 
 
-@pytest.mark.parametrize("shape", [(1, 600, 520), (1, 257, 300), (5, 130, 300), (2, 64, 512)], ids=lambda s: "x".join(map(str, s)))
-@pytest.mark.parametrize("T", [1, 2, 3])
-def test_host_entry_point_pipelined_is_bit_identical(tnrd, shape, T):
-    """tnrd_diffuse_host with the tensor-core kernel cuts the first and the last stage in two halves (images of a batch, or
-    rows of a single image at an even row) to overlap the copies: the result must be bit-identical to the device call."""
+@pytest.mark.parametrize("shape", [(1, 600, 520), (1, 257, 300), (5, 130, 300), (2, 64, 512), (1, 1500, 700), (1, 1024, 1024)],
+                         ids=lambda s: "x".join(map(str, s)))
+@pytest.mark.parametrize("T,ksize,mode", [(1, 7, 0), (2, 7, 0), (3, 7, 0), (3, 5, 0), (2, 7, 1), (2, 7, 2), (2, 7, 3)])
+def test_host_entry_point_pipelined_is_bit_identical(tnrd, shape, T, ksize, mode, monkeypatch):
+    """tnrd_diffuse_host with the tensor-core kernel overlaps the copies with the first and the last stage: a batch is cut
+    in two halves; a single image arrives in blocks of 32 rows that the first stage's loaders wait for (arrival words),
+    and the last stage stores into pinned host memory itself.  The result must be bit-identical to the device call.
+    TNRD_HOST_MODE selects the variants (1: halves for a single image, 2: no stores to host memory, 3: input top to
+    bottom)."""
     B, H, W = shape
-    c = tnrd_gen.make_small(270 + T, B, H, W, T, 8, 7)
+    if mode:
+        monkeypatch.setenv("TNRD_HOST_MODE", str(mode))
+    c = tnrd_gen.make_small(270 + T, B, H, W, T, 8, ksize)
     ref = run_gpu(tnrd, c, kernel=3)
     tnrd.tnrd_set_kernel(3)
     try:
         out = torch.empty(c["f"].shape).pin_memory()
         f = torch.from_numpy(c["f"]).pin_memory()
-        tnrd.tnrd_diffuse_host(f, f, B, H, W, T, 8, 7, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"], c["lambda"], out)
-        assert np.array_equal(out.numpy().astype(np.float64), ref)
+        for _ in range(2):                                           # the arrival words are reset by every call
+            out.zero_()
+            tnrd.tnrd_diffuse_host(f, f, B, H, W, T, 8, ksize, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"], c["lambda"], out)
+            assert np.array_equal(out.numpy().astype(np.float64), ref)
         out2 = np.empty_like(c["f"])                                 # pageable buffers, u0 distinct from f
         u0 = c["u0"].copy()
-        tnrd.tnrd_diffuse_host(c["f"], u0, B, H, W, T, 8, 7, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"],
+        tnrd.tnrd_diffuse_host(c["f"], u0, B, H, W, T, 8, ksize, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"],
                                c["lambda"], out2)
         assert np.array_equal(out2.astype(np.float64), ref)
     finally:
         tnrd.tnrd_set_kernel(0)
+
+
+def test_host_entry_point_single_image_with_a_split_bank(tnrd):
+    """A single image small enough for the planner to cut the filter bank: the first stage of the host call must cut it
+    the way the device call does (the order of the sum over filters), so the two stay bit-identical."""
+    c = tnrd_gen.make_small(281, 1, 321, 481, 3, 48, 7)
+    assert tnrd.tnrd_tc_plan_query(1, 321, 481, 48, 7, num_sms())["nchunk"] > 1
+    ref = run_gpu(tnrd, c)
+    out = torch.empty(c["f"].shape).pin_memory()
+    f = torch.from_numpy(c["f"]).pin_memory()
+    tnrd.tnrd_diffuse_host(f, f, 1, 321, 481, 3, 48, 7, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"], c["lambda"], out)
+    assert np.array_equal(out.numpy().astype(np.float64), ref)
