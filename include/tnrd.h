@@ -55,7 +55,8 @@ typedef enum {
     TNRD_ERR_UNSUPPORTED = -3, /* ksize not in {3,5,7,9}; unknown option */
     TNRD_ERR_ALIAS = -4,       /* output aliases an input it must not alias */
     TNRD_ERR_CUDA = -5,        /* a CUDA call failed; see tnrd_last_cuda_error() */
-    TNRD_ERR_PARAM = -6        /* rbf_gamma not finite or <= 0 */
+    TNRD_ERR_PARAM = -6,       /* rbf_gamma not finite or <= 0 */
+    TNRD_ERR_TOO_LARGE = -7    /* tnrd_stage_static: the call needs more than TNRD_STATIC_SCRATCH_BYTES of scratch */
 } tnrd_status;
 
 /*
@@ -72,6 +73,26 @@ typedef enum {
 int tnrd_stage(const float* f, const float* u_in, int B, int H, int W, int N_k, int ksize,
                const float* filters_t, const float* rbf_w_t, const float* rbf_mu, float rbf_gamma,
                float lambda_t, float* u_out, void* stream);
+
+/*
+ * tnrd_stage for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): the same operation (Main Eq. 7), arguments, layouts and aliasing rules as tnrd_stage, always
+ * with the tile kernel and the factorised Gaussian evaluator (the process-wide options of tnrd_set_kernel /
+ * tnrd_set_phi_mode / tnrd_set_basis do not apply).  Its scratch -- the staged parameters and the per-CTA partial sums
+ * -- is a fixed device array of TNRD_STATIC_SCRATCH_BYTES that every GPU loading the library holds until exit; the call
+ * makes no cudaMalloc / cudaFree / host allocation.
+ *   Limit: TNRD_ERR_TOO_LARGE, and nothing launched, when the stage needs more: 1 MiB holds the parameters, the rest
+ *   the partial sums, 4 x part_floats bytes of tnrd_plan_query's plan (64 KiB per CTA of the tile kernel for 7x7
+ *   filters, so at most 1008 CTAs).  That covers e.g. one 2560 x 2560 image or 36 images of 321 x 481 with 48 filters of
+ *   7x7, not 4096 x 4096 (1756 CTAs): cut larger batches into several calls.
+ *   Sharing: every call uses the same array and finds the last call's contents in it (nothing has to start at zero:
+ *   each call writes all it reads).  Calls on one stream are ordered; calls that overlap on the GPU (several streams or
+ *   host threads) race on it and give garbage -- serialise them.
+ */
+#define TNRD_STATIC_SCRATCH_BYTES (64u << 20)
+int tnrd_stage_static(const float* f, const float* u_in, int B, int H, int W, int N_k, int ksize,
+                      const float* filters_t, const float* rbf_w_t, const float* rbf_mu, float rbf_gamma,
+                      float lambda_t, float* u_out, void* stream);
 
 /*
  * T stages with per-stage parameters Theta_t = {lambda^t, phi_i^t, k_i^t} (row a6).

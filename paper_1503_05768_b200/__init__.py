@@ -17,7 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtnrd.so")
 NUM_RBF = 63
 
-OK, ERR_NULL, ERR_SHAPE, ERR_UNSUPPORTED, ERR_ALIAS, ERR_CUDA, ERR_PARAM = 0, -1, -2, -3, -4, -5, -6
+OK, ERR_NULL, ERR_SHAPE, ERR_UNSUPPORTED, ERR_ALIAS, ERR_CUDA, ERR_PARAM, ERR_TOO_LARGE = 0, -1, -2, -3, -4, -5, -6, -7
+STATIC_SCRATCH_BYTES = 64 << 20                                     # TNRD_STATIC_SCRATCH_BYTES (include/tnrd.h)
 PHI_DENSE, PHI_WINDOW, PHI_LUT, PHI_FACTORED = 0, 1, 2, 3          # tnrd_set_phi_mode (include/tnrd.h)
 KERNEL_AUTO, KERNEL_REF, KERNEL_TILE, KERNEL_TC, KERNEL_SMALL = 0, 1, 2, 3, 4     # tnrd_set_kernel (include/tnrd.h)
 
@@ -48,6 +49,8 @@ def lib() -> ctypes.CDLL:
         vp, ci, cf = ctypes.c_void_p, ctypes.c_int, ctypes.c_float
         L.tnrd_stage.argtypes = [vp, vp, ci, ci, ci, ci, ci, vp, vp, vp, cf, cf, vp, vp]
         L.tnrd_stage.restype = ci
+        L.tnrd_stage_static.argtypes = L.tnrd_stage.argtypes
+        L.tnrd_stage_static.restype = ci
         dargs = [vp, vp, ci, ci, ci, ci, ci, ci, vp, vp, vp, cf, vp, vp, vp]
         L.tnrd_diffuse.argtypes = dargs
         L.tnrd_diffuse.restype = ci
@@ -123,6 +126,14 @@ def tnrd_stage(f, u_in, B, H, W, N_k, ksize, filters_t, rbf_w_t, rbf_mu, rbf_gam
     """One stage on device buffers (include/tnrd.h: tnrd_stage)."""
     _check(lib().tnrd_stage(_ptr(f), _ptr(u_in), B, H, W, N_k, ksize, _ptr(filters_t), _ptr(rbf_w_t),
                             _ptr(rbf_mu), float(rbf_gamma), float(lambda_t), _ptr(u_out), _stream(stream)))
+    return u_out
+
+
+def tnrd_stage_static(f, u_in, B, H, W, N_k, ksize, filters_t, rbf_w_t, rbf_mu, rbf_gamma, lambda_t, u_out,
+                      stream=None):
+    """One stage on device buffers without any allocation (include/tnrd.h: tnrd_stage_static)."""
+    _check(lib().tnrd_stage_static(_ptr(f), _ptr(u_in), B, H, W, N_k, ksize, _ptr(filters_t), _ptr(rbf_w_t),
+                                   _ptr(rbf_mu), float(rbf_gamma), float(lambda_t), _ptr(u_out), _stream(stream)))
     return u_out
 
 

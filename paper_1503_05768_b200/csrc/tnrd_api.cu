@@ -285,6 +285,11 @@ int open_call(Call& c, void* stream)
 
 }  // namespace
 
+namespace tnrd {
+int api_cuda_fail(cudaError_t e, const char* what) { return cuda_fail(e, what); }
+void api_count_launches(unsigned long long n) { g_launches.fetch_add(n); }
+}  // namespace tnrd
+
 extern "C" {
 
 int tnrd_stage(const float* f, const float* u_in, int B, int H, int W, int N_k, int ksize,
@@ -966,6 +971,7 @@ const char* tnrd_strerror(int status)
         case TNRD_ERR_ALIAS: return "output aliases an input it must not alias";
         case TNRD_ERR_CUDA: return "a CUDA call failed (see tnrd_last_cuda_error)";
         case TNRD_ERR_PARAM: return "rbf_gamma must be finite and > 0";
+        case TNRD_ERR_TOO_LARGE: return "the call needs more than the fixed scratch of tnrd_stage_static (TNRD_STATIC_SCRATCH_BYTES)";
         default: return "unknown status";
     }
 }

@@ -117,6 +117,11 @@ cudaError_t launch_reduce_partials(const float* part_w, long long n_cta, const f
                                    unsigned long long* launches);
 cudaError_t launch_sub(const float* x, const float* y, float* out, size_t n, cudaStream_t st, unsigned long long* launches);
 
+// tnrd_api.cu, for entry points that live in other files (tnrd_static.cu): record a CUDA failure for
+// tnrd_last_cuda_error and return TNRD_ERR_CUDA; add to the process-wide launch counter
+int api_cuda_fail(cudaError_t e, const char* what);
+void api_count_launches(unsigned long long n);
+
 // launchers (each returns the cudaError_t of the launch; *launches += kernels launched)
 cudaError_t launch_prep(const float* filters, const float* rbf_w, const float* rbf_mu, float gamma,
                         int T, int N_k, int ksize, float* prm, cudaStream_t st, unsigned long long* launches);
