@@ -192,33 +192,28 @@ __device__ __forceinline__ float ex2f(float x)
 // A group is skipped when its Gaussian factor is zero for every response of the warp (an exact 0 either way): the
 // loop runs over the groups within reach D of the warp's smallest .. largest response (NaN responses keep every
 // group live); ganch = mu' of the first group's anchor, ginv = 1 / (anchor spacing).
-__device__ __forceinline__ uint32_t f2ord(float x)            // order-preserving map float -> uint32
-{
-    const uint32_t b = __float_as_uint(x);
-    return b ^ ((uint32_t)((int32_t)b >> 31) | 0x80000000u);
-}
-__device__ __forceinline__ float ord2f(uint32_t o)
-{
-    return __uint_as_float(o ^ ((o >> 31) - 1u | 0x80000000u));
-}
-__device__ __forceinline__ int tc_phi_fact(const float* __restrict__ crec, float kappa, float dmax,
-                                           float ganch, float ginv, const float2 (&z)[2], float2 (&v)[2])
+// The range is taken per lane first -- x = (z -+ D - ganch) * ginv as ONE fused multiply-add with the offsets
+// olo = -(D + ganch) ginv, ohi = (D - ganch) ginv, clamped, rounded down / up -- and then reduced over the warp as small
+// integers (floor and ceil are monotone: the same range as rounding the warp's extreme responses).  The min / max over a
+// lane's four responses propagate NaN, and the order of the two clamps sends a NaN to the full range on either side.
+// D leaves a margin (the factor flushes to zero from d^2 = 126 on, D^2 = 127.7), so the rounding of the fused form
+// cannot cut a group that still contributes.
+__device__ __forceinline__ int tc_phi_fact(const float* __restrict__ crec, float kappa, float olo, float ohi, float ginv,
+                                           const float2 (&z)[2], float2 (&v)[2])
 {
     constexpr int S = TNRD_FS, GC = TNRD_FG / 2;
-    // warp-wide range of the responses -> the range of groups that are live for some response of the warp: group g
-    // (anchor mu'_0a + g * spacing) is live iff  wlo - mu'_g < D  and  whi - mu'_g > -D
-    float zlo, zhi;
-    asm("min.NaN.f32 %0, %1, %2;" : "=f"(zlo) : "f"(fminf(z[0].x, z[0].y)), "f"(fminf(z[1].x, z[1].y)));
-    asm("max.NaN.f32 %0, %1, %2;" : "=f"(zhi) : "f"(fmaxf(z[0].x, z[0].y)), "f"(fmaxf(z[1].x, z[1].y)));
-    const bool lane_nan = (z[0].x != z[0].x) || (z[0].y != z[0].y) || (z[1].x != z[1].x) || (z[1].y != z[1].y);
-    const float wlo = ord2f(__reduce_min_sync(0xffffffffu, f2ord(zlo)));
-    const float whi = ord2f(__reduce_max_sync(0xffffffffu, f2ord(zhi)));
-    int g0 = 0, g1 = TNRD_FG - 1;
-    if (!__any_sync(0xffffffffu, lane_nan)) {
-        // clamped BEFORE the conversion: infinite responses must not overflow the + 1
-        g0 = max(0, __float2int_rd(fminf(fmaxf((wlo - dmax - ganch) * ginv, -8.0f), 8.0f)) + 1);
-        g1 = min(TNRD_FG - 1, __float2int_ru(fminf(fmaxf((whi + dmax - ganch) * ginv, -8.0f), 8.0f)) - 1);
-    }
+    float zlo, zhi, t0, t1;
+    asm("min.NaN.f32 %0, %1, %2;" : "=f"(t0) : "f"(z[0].x), "f"(z[0].y));
+    asm("min.NaN.f32 %0, %1, %2;" : "=f"(t1) : "f"(z[1].x), "f"(z[1].y));
+    asm("min.NaN.f32 %0, %1, %2;" : "=f"(zlo) : "f"(t0), "f"(t1));
+    asm("max.NaN.f32 %0, %1, %2;" : "=f"(t0) : "f"(z[0].x), "f"(z[0].y));
+    asm("max.NaN.f32 %0, %1, %2;" : "=f"(t1) : "f"(z[1].x), "f"(z[1].y));
+    asm("max.NaN.f32 %0, %1, %2;" : "=f"(zhi) : "f"(t0), "f"(t1));
+    // clamped BEFORE the conversion (infinite responses must not overflow the + 1); NaN -> -8 resp. +8
+    const float xl = fminf(fmaxf(fmaf(zlo, ginv, olo), -8.0f), 8.0f);
+    const float xh = fmaxf(fminf(fmaf(zhi, ginv, ohi), 8.0f), -8.0f);
+    const int g0 = max(0, __reduce_min_sync(0xffffffffu, __float2int_rd(xl)) + 1);
+    const int g1 = min(TNRD_FG - 1, __reduce_max_sync(0xffffffffu, __float2int_ru(xh)) - 1);
     if (g0 > g1) return 0;
     // the shared exponential pair (middle group)
     float2 rho0[2], rhoi0[2];
@@ -503,6 +498,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
         const bool fact = __ldg(a.prm + prm_hdr(KS) + 6) != 0.0f;
         const float dsp = __ldg(a.prm + prm_hdr(KS) + 2);        // centre spacing in scaled units
         const float ganch = __ldg(a.prm + prm_hdr(KS) + 1) + (float)TNRD_FS * dsp, ginv = 1.0f / ((float)TNRD_FM * dsp);
+        const float olo = -(dmax + ganch) * ginv, ohi = (dmax - ganch) * ginv;     // tc_phi_fact: group range of a response
         const float* coef = reinterpret_cast<const float*>(smem + C::SM_COEF);
         int* ticket = reinterpret_cast<int*>(smem + C::SM_BAR + 192) + quarter;
         int nlive = 0, nfilt = 0;                                // statistics: groups evaluated, filters evaluated
@@ -540,7 +536,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
                 float2 v[2] = {{0.f, 0.f}, {0.f, 0.f}};
                 const int fidx = 2 * pi + f;
                 if (fact) {
-                    const int nl = tc_phi_fact(coef + fidx * (TNRD_FG * TNRD_FSTRIDE), kappa, dmax, ganch, ginv, zc, v);
+                    const int nl = tc_phi_fact(coef + fidx * (TNRD_FG * TNRD_FSTRIDE), kappa, olo, ohi, ginv, zc, v);
                     if (STATS) nlive += nl;
                 }
                 else if (f0 + fidx < a.N_k) tc_phi_direct(a.prm + (size_t)(f0 + fidx) * C::PRM + prm_kkp(KS), zc, v);
