@@ -406,7 +406,7 @@ static int host_flags_reserve(Scratch* sc, size_t words)
 }
 
 // experiments with the host entry point: 1 = a single image takes the two-halves path as well, 2 = never store to host
-// memory from a kernel, 3 = the input strictly top to bottom
+// memory from a kernel, 3 = the input strictly top to bottom, 4 = serial (upload, stages, download)
 static int host_mode_env()
 {
     const char* e = getenv("TNRD_HOST_MODE");
@@ -455,7 +455,11 @@ int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int 
     if (T > 0) {
         if ((rc = pick_small(c, B, H, W, N_k, ksize, phi)) != TNRD_OK) return rc;
         if (!c.small && (rc = pick_kernel(c, B, H, W, N_k, ksize, phi)) != TNRD_OK) return rc;
-        piped = c.tc && (B >= 2 || H >= 256);
+        // below about two million pixels the dozen extra copies and events of the pipelined paths cost more than they hide
+        // (1024^2: 1.43 ms serial, 1.53 ms pipelined; 2048^2: 4.35 / 3.96); TNRD_HOST_PIPE_MIN (pixels) for the tests
+        const char* pm = getenv("TNRD_HOST_PIPE_MIN");
+        const size_t pipe_min = pm ? (size_t)atoll(pm) : ((size_t)1 << 21);
+        piped = c.tc && (B >= 2 || H >= 256) && n >= pipe_min && host_mode_env() != 4;
     }
     if (!piped) {
         // serial: upload, all stages, download (small images, the tile kernel)

@@ -138,6 +138,12 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 }
 // The same for the warps that wait most of the time (MMA issuer, loader, drain): a spinning try_wait loop takes issue
 // slots from the phi warps on its scheduler (20 % of all issued instructions in a profile), so back off between polls.
+#ifndef TNRD_TC_SLEEP_DRAIN
+#define TNRD_TC_SLEEP_DRAIN 200      // 200 .. 2000 ns: no difference in the stage time (measured)
+#define TNRD_TC_SLEEP_LOAD 200
+#define TNRD_TC_SLEEP_MMA 200
+#endif
+template <unsigned NS>
 __device__ __forceinline__ void mbar_wait_idle(uint64_t* bar, uint32_t parity)
 {
     for (;;) {
@@ -146,7 +152,7 @@ __device__ __forceinline__ void mbar_wait_idle(uint64_t* bar, uint32_t parity)
                      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
                      "selp.u32 %0, 1, 0, p;\n\t}\n" : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
         if (done) return;
-        __nanosleep(200);
+        __nanosleep(NS);
     }
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -565,7 +571,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
         const bool lane_out = L < 128 - R;                       // lanes whose output pixels this strip completes
         constexpr int NQ = KS + 1;                               // table blocks with content
         for (int b = 0; b < NB; ++b) {
-            mbar_wait_idle(tfull, b & 1);
+            mbar_wait_idle<TNRD_TC_SLEEP_DRAIN>(tfull, b & 1);
             tc_fence_after();
             bar_drain();                                         // the previous fold has finished reading xbuf
 #pragma unroll 1
@@ -650,15 +656,15 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
                 umma_commit(zfull + bb);
                 umma_commit(pempty + b % TC_NP);
             };
-            auto wait_pair = [&](int p) { mbar_wait_idle(pfull + p % TC_NP, (p / TC_NP) & 1); };
+            auto wait_pair = [&](int p) { mbar_wait_idle<TNRD_TC_SLEEP_MMA>(pfull + p % TC_NP, (p / TC_NP) & 1); };
             for (int p = 0; p <= R; ++p) wait_pair(p);
             tc_fence_after();
             forward(0);
             if (NB > 1) { wait_pair(R + 1); tc_fence_after(); forward(1); }
             for (int b = 0; b < NB; ++b) {
                 const int bb = b & 1;
-                mbar_wait_idle(vdone + bb, (b >> 1) & 1);
-                if (b >= 1) mbar_wait_idle(tfree, (b - 1) & 1);
+                mbar_wait_idle<TNRD_TC_SLEEP_MMA>(vdone + bb, (b >> 1) & 1);
+                if (b >= 1) mbar_wait_idle<TNRD_TC_SLEEP_MMA>(tfree, (b - 1) & 1);
                 tc_fence_after();
                 for (int rr = 1; rr >= 0; --rr) {                        // row 1 first: it initialises blocks 0 .. KS
                     const uint32_t d = tmem + TC_TCOL + (rr == 0 ? 8 : 0);
@@ -679,7 +685,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
         int have = 0;
         for (int p = R + 1; p < NPAIRS; ++p) {
             const int slot = p % TC_NP;
-            if (p >= TC_NP) mbar_wait_idle(pempty + slot, ((p / TC_NP) - 1) & 1);
+            if (p >= TC_NP) mbar_wait_idle<TNRD_TC_SLEEP_LOAD>(pempty + slot, ((p / TC_NP) - 1) & 1);
             if (a.arrived) have = tc_wait_rows(a.arrived, min(a.H, max(ys0 + 2 * p + 2 - 2 * R, 2 * R + 1)), have);
             constexpr int NL = TC_LOAD_WARPS * 32, UNR = 4;      // UNR cells' loads in flight per thread
             for (int idx0 = lt; idx0 < 2 * TC_CWU; idx0 += NL * UNR) {

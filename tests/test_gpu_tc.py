@@ -360,6 +360,7 @@ def test_host_entry_point_pipelined_is_bit_identical(tnrd, shape, T, ksize, mode
     TNRD_HOST_MODE selects the variants (1: halves for a single image, 2: no stores to host memory, 3: input top to
     bottom)."""
     B, H, W = shape
+    monkeypatch.setenv("TNRD_HOST_PIPE_MIN", "0")                    # small images take the serial path otherwise
     if mode:
         monkeypatch.setenv("TNRD_HOST_MODE", str(mode))
     c = tnrd_gen.make_small(270 + T, B, H, W, T, 8, ksize)
@@ -381,9 +382,10 @@ def test_host_entry_point_pipelined_is_bit_identical(tnrd, shape, T, ksize, mode
         tnrd.tnrd_set_kernel(0)
 
 
-def test_host_entry_point_single_image_with_a_split_bank(tnrd):
+def test_host_entry_point_single_image_with_a_split_bank(tnrd, monkeypatch):
     """A single image small enough for the planner to cut the filter bank: the first stage of the host call must cut it
     the way the device call does (the order of the sum over filters), so the two stay bit-identical."""
+    monkeypatch.setenv("TNRD_HOST_PIPE_MIN", "0")
     c = tnrd_gen.make_small(281, 1, 321, 481, 3, 48, 7)
     assert tnrd.tnrd_tc_plan_query(1, 321, 481, 48, 7, num_sms())["nchunk"] > 1
     ref = run_gpu(tnrd, c)
