@@ -220,6 +220,13 @@ __global__ void __launch_bounds__(SM_NT, 1) small_diffuse_kernel(SmallArgs a)
     float* psum = reinterpret_cast<float*>(poff + ((VH * VW + 3) & ~3));   // [parts][rows of the band][W] partial sums of a4
     __shared__ int s_okf;
 
+    // Programmatic dependent launch: let the next kernel of the stream (typically the next call of this one) be
+    // scheduled now -- it waits below, like this one, before it touches global memory -- so that its launch latency and
+    // cluster set-up overlap this kernel's run instead of following it.  The wait returns once the previous kernel of
+    // the stream has completed and its writes are visible: stream order is kept.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+
     // ---- loads nothing depends on yet, issued before the first barrier (one L2 round trip instead of three in a row):
     // f of this thread's output pixel (the same in every stage) and this thread's first element of the u_0 tile
     const size_t plane = (size_t)H * W;
@@ -415,13 +422,15 @@ cudaError_t launch_small_ks(const SmallArgs& a, int cs, size_t smem, cudaStream_
     cfg.blockDim = dim3(SM_NT, 1, 1);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = (unsigned)cs;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;     // see griddepcontrol in the kernel
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = 2;
     return cudaLaunchKernelEx(&cfg, small_diffuse_kernel<KS>, a);
 }
 
