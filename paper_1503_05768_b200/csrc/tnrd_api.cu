@@ -230,6 +230,7 @@ int run_stage(Call& c, tnrd::StageArgs a, int phi, int t)
     }
     if (c.tc) {
         if (a.u_out == a.u_in) return TNRD_ERR_ALIAS;        // callers ping-pong (run_stages)
+        a.pdl_early = t >= 1 ? 1 : 0;      // operands and records of stage t were staged before stage 0 of this call ran
         if (g_stats.load()) {
             if (!sc->stats.p) {
                 int rc = grow(sc->stats, 4, c.st);

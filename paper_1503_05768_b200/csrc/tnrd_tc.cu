@@ -406,6 +406,12 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
     const int NPAIRS = NB + R;                                  // u row pairs: u~ rows ys0 .. ys0 + 2 NB + 2r - 1
     const float* __restrict__ u_img = a.u_in + (size_t)img * a.H * a.W;
 
+    // Programmatic dependent launch (launch_tc_ks): the next kernel of the stream may be scheduled as soon as every CTA
+    // of this one is running -- its CTAs take SMs as ours leave them and set themselves up -- and this kernel waits for
+    // the previous one (complete, writes visible) before it touches anything that kernel may have written: at once when
+    // that includes our operands (first stage of a call), else after the set-up.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (!a.pdl_early) asm volatile("griddepcontrol.wait;" ::: "memory");
     // ---- setup: operands and coefficients to shared memory, barriers, tensor memory ----
     {
         // forward operand: cells [2 KS chunks][2 nkp_all columns] -> this CTA's 2 nkp columns, compact
@@ -446,6 +452,29 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "r"(512) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
+    auto finish_coefs = [&]() {
+        cp_async_wait_all();
+        {
+            constexpr int CF = TNRD_FG * TNRD_FSTRIDE, S = TNRD_FS;
+            float* cf = reinterpret_cast<float*>(smem + C::SM_COEF);
+            for (int i = tid; i < nkp * CF / 4; i += TC_THREADS) {   // the same 16-byte pieces this thread copied above
+                if (f0 + (4 * i) / CF >= a.N_k) continue;
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int o = (4 * i + e) % TNRD_FSTRIDE;        // slot inside the group record
+                    int pw = 0;                                      // power of R
+                    if (o >= 1 && o <= S + 1) pw = S + 1 - o;        // c_S .. c_0
+                    else if (o >= S + 2 && o <= 2 * S + 1) pw = 2 * S + 2 - o;   // c_-S .. c_-1
+                    else if (o >= TNRD_FSTRIDE - 2) pw = -1;         // K_g, 1 / K_g
+                    if (pw != 0) cf[4 * i + e] *= exp2f((float)pw * tc_kappa * tc_dmax);
+                }
+            }
+        }
+    };
+    if (a.pdl_early) {
+        finish_coefs();
+        asm volatile("griddepcontrol.wait;" ::: "memory");
+    }
     // The first R + 1 row pairs (what the first batch needs) are gathered by ALL threads: left to the loader warp alone
     // they would cost R + 1 round trips to L2 per thread chain before the first MMA can issue.
     if (a.arrived) {       // the first R + 1 pairs: rows ys0 - 2r .. ys0 + 1 (mirrored rows above the image: rows up to 2r)
@@ -464,23 +493,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
             tc_cell_store(smem + C::SM_UHI, smem + C::SM_ULO, (prow * TC_CW + xg) * 16, v);
         }
     }
-    cp_async_wait_all();
-    {
-        constexpr int CF = TNRD_FG * TNRD_FSTRIDE, S = TNRD_FS;
-        float* cf = reinterpret_cast<float*>(smem + C::SM_COEF);
-        for (int i = tid; i < nkp * CF / 4; i += TC_THREADS) {   // the same 16-byte pieces this thread copied above
-            if (f0 + (4 * i) / CF >= a.N_k) continue;
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const int o = (4 * i + e) % TNRD_FSTRIDE;        // slot inside the group record
-                int pw = 0;                                      // power of R
-                if (o >= 1 && o <= S + 1) pw = S + 1 - o;        // c_S .. c_0
-                else if (o >= S + 2 && o <= 2 * S + 1) pw = 2 * S + 2 - o;   // c_-S .. c_-1
-                else if (o >= TNRD_FSTRIDE - 2) pw = -1;         // K_g, 1 / K_g
-                if (pw != 0) cf[4 * i + e] *= exp2f((float)pw * tc_kappa * tc_dmax);
-            }
-        }
-    }
+    if (!a.pdl_early) finish_coefs();
     fence_async_smem();
     tc_fence_before();
     __syncthreads();
@@ -721,6 +734,8 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
 // a5 for the filter-chunk mode: u_t = u - (sum of the chunks' partial sums, in chunk order + lambda (u - f))
 __global__ void __launch_bounds__(256) tc_update_kernel(StageArgs a, const float* __restrict__ part, int nchunk)
 {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const size_t n = (size_t)a.B * a.H * a.W;
     const float lambda = a.lambda_ptr ? __ldg(a.lambda_ptr) : a.lambda_val;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
@@ -808,9 +823,18 @@ static cudaError_t launch_tc_ks(const StageArgs& a, const TcPlan& pl, const unsi
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
     if (e != cudaSuccess) return e;
     if (pl.units > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    kern<<<(unsigned)pl.units, TC_THREADS, C::SMEM, st>>>(a, ws_t, nkp, pl.nxs, pl.nys, pl.seg_rows, pl.nchunk,
-                                                          pl.nchunk > 1 ? part : nullptr);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)pl.units, 1, 1);
+    cfg.blockDim = dim3(TC_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = C::SMEM;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;     // see griddepcontrol in the kernel
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, a, ws_t, nkp, pl.nxs, pl.nys, pl.seg_rows, pl.nchunk,
+                              pl.nchunk > 1 ? part : (float*)nullptr);
 }
 
 cudaError_t launch_stage_tc(const StageArgs& a, const TcPlan& pl, const unsigned char* ws_t, float* part, cudaStream_t st,
@@ -827,9 +851,17 @@ cudaError_t launch_stage_tc(const StageArgs& a, const TcPlan& pl, const unsigned
     const size_t n = (size_t)a.B * a.H * a.W;
     size_t blocks = (n + 255) / 256;
     if (blocks > 148 * 8) blocks = 148 * 8;
-    tc_update_kernel<<<(unsigned)blocks, 256, 0, st>>>(a, part, pl.nchunk);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)blocks, 1, 1);
+    cfg.blockDim = dim3(256, 1, 1);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
     ++*launches;
-    return cudaGetLastError();
+    return cudaLaunchKernelEx(&cfg, tc_update_kernel, a, (const float*)part, pl.nchunk);
 }
 
 size_t tc_ws_stage_stride(int N_k, int ksize) { return tc_ws_stage_bytes(ksize, (N_k + 7) / 8 * 8); }
