@@ -135,6 +135,7 @@ struct Call {
     bool tc = false;   // this call runs the tensor-core stage kernel
     bool small = false; // this call runs the small-image kernel (all stages in one launch)
     int nchunk_fixed = 0, seg_mult = 2;   // handed to plan_stage_tc by run_stage (the host entry point's first stage)
+    bool no_pdl = false;                  // plain launches (StageArgs::pdl = 0)
 };
 
 // The automatic choice between the two stage kernels: strips of the tensor-core kernel are 256 - 2r columns wide and
@@ -230,7 +231,7 @@ int run_stage(Call& c, tnrd::StageArgs a, int phi, int t)
     }
     if (c.tc) {
         if (a.u_out == a.u_in) return TNRD_ERR_ALIAS;        // callers ping-pong (run_stages)
-        a.pdl_early = t >= 1 ? 1 : 0;      // operands and records of stage t were staged before stage 0 of this call ran
+        a.pdl = c.no_pdl ? 0 : (t >= 1 ? 2 : 1);   // operands and records of stage t were staged before stage 0 of this call ran
         if (g_stats.load()) {
             if (!sc->stats.p) {
                 int rc = grow(sc->stats, 4, c.st);
@@ -626,6 +627,7 @@ int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int 
         }
         const size_t rec = (size_t)N_k * tnrd::prm_stride(ksize);
         c.nchunk_fixed = 1;                 // concurrent launches must not share the partial-sum scratch
+        c.no_pdl = true;
         for (int g = 0; g < G; ++g) {
             cudaStream_t bs = sc->s_band[g];
             TNRD_CUDA(cudaStreamWaitEvent(bs, sc->ev[0], 0));

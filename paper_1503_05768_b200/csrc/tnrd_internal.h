@@ -75,10 +75,12 @@ struct StageArgs {
     // word per block of 32 rows: non-zero once the block of f / u_in has arrived} -- copied by another stream while the
     // kernel runs; the loader polls the word of a block before it reads its first row
     unsigned* arrived;
-    // tensor-core kernel: 1 = this launch's operands and records were complete before the PREVIOUS kernel of the stream
-    // started (stages after the first of a call), so under programmatic dependent launch the CTA may set itself up before
-    // it waits for that kernel
-    int pdl_early;
+    // tensor-core kernel, programmatic dependent launch: 0 = a plain launch (the host entry point's image groups: a CTA
+    // that sits on an SM waiting for its own stream's previous kernel would keep the other groups' CTAs off it);
+    // 1 = programmatic, the CTA waits for the previous kernel of the stream before anything else; 2 = programmatic, and
+    // this launch's operands and records were complete before that kernel started (stages after the first of a call),
+    // so the CTA sets itself up before it waits
+    int pdl;
 };
 
 // Launch plan of the fused stage kernel (tnrd_fused.cu: plan_stage_fused).  Tiles partition the phi region

@@ -411,7 +411,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
     // the previous one (complete, writes visible) before it touches anything that kernel may have written: at once when
     // that includes our operands (first stage of a call), else after the set-up.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    if (!a.pdl_early) asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (a.pdl != 2) asm volatile("griddepcontrol.wait;" ::: "memory");
     // ---- setup: operands and coefficients to shared memory, barriers, tensor memory ----
     {
         // forward operand: cells [2 KS chunks][2 nkp_all columns] -> this CTA's 2 nkp columns, compact
@@ -471,7 +471,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
             }
         }
     };
-    if (a.pdl_early) {
+    if (a.pdl == 2) {
         finish_coefs();
         asm volatile("griddepcontrol.wait;" ::: "memory");
     }
@@ -493,7 +493,7 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
             tc_cell_store(smem + C::SM_UHI, smem + C::SM_ULO, (prow * TC_CW + xg) * 16, v);
         }
     }
-    if (!a.pdl_early) finish_coefs();
+    if (a.pdl != 2) finish_coefs();
     fence_async_smem();
     tc_fence_before();
     __syncthreads();
@@ -832,7 +832,7 @@ static cudaError_t launch_tc_ks(const StageArgs& a, const TcPlan& pl, const unsi
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;     // see griddepcontrol in the kernel
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = a.pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kern, a, ws_t, nkp, pl.nxs, pl.nys, pl.seg_rows, pl.nchunk,
                               pl.nchunk > 1 ? part : (float*)nullptr);
 }
@@ -859,7 +859,7 @@ cudaError_t launch_stage_tc(const StageArgs& a, const TcPlan& pl, const unsigned
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = a.pdl ? 1 : 0;
     ++*launches;
     return cudaLaunchKernelEx(&cfg, tc_update_kernel, a, (const float*)part, pl.nchunk);
 }
