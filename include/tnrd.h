@@ -121,7 +121,8 @@ int tnrd_diffuse(const float* f, const float* u0, int B, int H, int W, int T, in
  *     that lasts two seconds ends the call with TNRD_ERR_CUDA), and when `out` is pinned (or otherwise device-mapped)
  *     host memory the last stage stores u_T into it directly; a pageable `out` gets one copy after the last stage.
  * Either way the result is bit-identical to tnrd_diffuse on device buffers.  The buffers must stay valid and unchanged
- * until the call returns (it synchronises `stream`).
+ * until the call returns (it synchronises `stream`).  `out` may be the host buffer of f / u0 (in place on the host; the
+ * direct stores are then replaced by a copy); partial overlap is undefined behaviour.
  */
 int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int T, int N_k, int ksize,
                       const float* filters, const float* rbf_w, const float* rbf_mu, float rbf_gamma,

@@ -487,7 +487,9 @@ int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int 
         float* out_dev = nullptr;
         {
             cudaPointerAttributes pa;
-            if (cudaPointerGetAttributes(&pa, out) == cudaSuccess && pa.type == cudaMemoryTypeHost && pa.devicePointer &&
+            // not when `out` overlaps an input: with T = 1 the stage that stores u_T runs while the input still arrives
+            const bool apart = (out + n <= f || f + n <= out) && (out + n <= u0 || u0 + n <= out);
+            if (apart && cudaPointerGetAttributes(&pa, out) == cudaSuccess && pa.type == cudaMemoryTypeHost && pa.devicePointer &&
                 host_mode_env() != 2)
                 out_dev = static_cast<float*>(pa.devicePointer);
             (void)cudaGetLastError();

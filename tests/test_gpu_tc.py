@@ -373,6 +373,9 @@ def test_host_entry_point_pipelined_is_bit_identical(tnrd, shape, T, ksize, mode
             out.zero_()
             tnrd.tnrd_diffuse_host(f, f, B, H, W, T, 8, ksize, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"], c["lambda"], out)
             assert np.array_equal(out.numpy().astype(np.float64), ref)
+        g = f.clone().pin_memory()                                   # in place on the host: out is the input buffer
+        tnrd.tnrd_diffuse_host(g, g, B, H, W, T, 8, ksize, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"], c["lambda"], g)
+        assert np.array_equal(g.numpy().astype(np.float64), ref)
         out2 = np.empty_like(c["f"])                                 # pageable buffers, u0 distinct from f
         u0 = c["u0"].copy()
         tnrd.tnrd_diffuse_host(c["f"], u0, B, H, W, T, 8, ksize, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"],
