@@ -102,6 +102,14 @@ __device__ __forceinline__ float warp_reduce8(const float (&S)[8], int lane)
     return c;     // term index of this lane: 4 * bit4 + 2 * bit3 + bit2
 }
 
+// order-preserving map float <-> uint32 (warp-wide min / max by redux.sync)
+__device__ __forceinline__ unsigned f2ord(float x)
+{
+    const unsigned b = __float_as_uint(x);
+    return b ^ ((unsigned)((int)b >> 31) | 0x80000000u);
+}
+__device__ __forceinline__ float ord2f(unsigned o) { return __uint_as_float(o ^ (((o >> 31) - 1u) | 0x80000000u)); }
+
 // origin (extended coordinate, >= -2r) of tile t of n over an axis of `len` image pixels
 __device__ __forceinline__ int tile_origin(int t, int n, int len, int R) { return (int)((long long)t * (len + 4 * R) / n) - 2 * R; }
 
@@ -118,6 +126,7 @@ stage_bwd_kernel(BwdArgs a, int ntx, int nty)
     float* ps = vs + 2 * C::VPLANE;                // [4][PRM]  staged records
     __shared__ float gws[2][NT / 32][64];          // per-warp g_w sums of filters i and i-1
     __shared__ float red[NT / 32];
+    __shared__ float crange[2 * BCfg<KS>::NG];     // smallest / largest scaled centre of every step of 8 terms
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     int t = blockIdx.x;
@@ -157,6 +166,14 @@ stage_bwd_kernel(BwdArgs a, int ntx, int nty)
     for (int idx = tid; idx < 2 * C::PRM; idx += NT)
         if (idx < N_k * C::PRM) ps[idx] = __ldg(a.prm + idx);
     for (int idx = tid; idx < 2 * (NT / 32) * 64; idx += NT) (&gws[0][0][0])[idx] = 0.0f;
+    if (tid < C::NG) {      // the centres are the same for every filter: record 0 holds (-mu'_j, w'_j) pairs
+        float lo = __int_as_float(0x7f800000), hi = __int_as_float(0xff800000);
+        for (int m = 0; m < 8 && 8 * tid + m < TNRD_M; ++m) {
+            const float mu = -__ldg(a.prm + KKP + 2 * (8 * tid + m));
+            lo = fminf(lo, mu); hi = fmaxf(hi, mu);
+        }
+        crange[2 * tid] = lo; crange[2 * tid + 1] = hi;
+    }
 
     int uoff[C::NB], voff[C::NB], coff[C::NB];
     unsigned own[C::NB];            // bit (4 j + p): pixel (row j, column p) of phi block n belongs to this tile
@@ -238,17 +255,40 @@ stage_bwd_kernel(BwdArgs a, int ntx, int nty)
 #pragma unroll
             for (int p = 0; p < 4; ++p)
                 qm[p] = make_float2((own[n] >> p) & 1 ? qc[p].x : 0.f, (own[n] >> (4 + p)) & 1 ? qc[p].y : 0.f);
+            // A step of 8 terms whose centres are all farther than D from every response of the warp contributes exact
+            // zeros to A, V and the g_w sums (2^{-d^2} has flushed to zero): skipped, as the forward kernels skip dead
+            // groups.  The warp's response range by redux over an order-preserving integer map; a NaN response keeps
+            // every step live (max.NaN makes the upper end NaN and both tests false).
+            float wlo, whi;
+            {
+                float zlo, zhi, t0, t1;
+                asm("min.NaN.f32 %0, %1, %2;" : "=f"(t0) : "f"(fminf(zc[0].x, zc[0].y)), "f"(fminf(zc[1].x, zc[1].y)));
+                asm("min.NaN.f32 %0, %1, %2;" : "=f"(t1) : "f"(fminf(zc[2].x, zc[2].y)), "f"(fminf(zc[3].x, zc[3].y)));
+                asm("min.NaN.f32 %0, %1, %2;" : "=f"(zlo) : "f"(t0), "f"(t1));
+                asm("max.NaN.f32 %0, %1, %2;" : "=f"(t0) : "f"(zc[0].x), "f"(zc[0].y));
+                asm("max.NaN.f32 %0, %1, %2;" : "=f"(t1) : "f"(zc[1].x), "f"(zc[1].y));
+                asm("max.NaN.f32 %0, %1, %2;" : "=f"(zhi) : "f"(t0), "f"(t1));
+                asm("max.NaN.f32 %0, %1, %2;" : "=f"(t0) : "f"(zc[2].x), "f"(zc[2].y));
+                asm("max.NaN.f32 %0, %1, %2;" : "=f"(t1) : "f"(zc[3].x), "f"(zc[3].y));
+                asm("max.NaN.f32 %0, %1, %2;" : "=f"(zhi) : "f"(zhi), "f"(t0));
+                asm("max.NaN.f32 %0, %1, %2;" : "=f"(zhi) : "f"(zhi), "f"(t1));
+                if (!hasB) { zlo = __int_as_float(0x7f800000); zhi = __int_as_float(0xff800000); }
+                wlo = ord2f(__reduce_min_sync(0xffffffffu, f2ord(zlo)));
+                whi = ord2f(__reduce_max_sync(0xffffffffu, f2ord(zhi)));
+            }
 #pragma unroll 1
             for (int g = 0; g < C::NG; ++g) {
                 float S[8];
-                if (hasB) {
+                const float cmin = crange[2 * g], cmax = crange[2 * g + 1];
+                const bool live = !((wlo - cmax > TNRD_FCLAMP && whi == whi) || cmin - whi > TNRD_FCLAMP);
+                if (hasB && live) {
                     if (g < C::NG - 1) phi_bwd_step<8, WANT_W, WANT_K>(rec + KKP + 16 * g, zc, qm, A, V, S);
                     else phi_bwd_step<TNRD_M - 8 * (C::NG - 1), WANT_W, WANT_K>(rec + KKP + 16 * g, zc, qm, A, V, S);
                 } else {
 #pragma unroll
                     for (int m = 0; m < 8; ++m) S[m] = 0.f;
                 }
-                if (WANT_W && warpB) {
+                if (WANT_W && warpB && live) {
                     const float tot = warp_reduce8(S, lane);
                     if ((lane & 3) == 0) gw_slot[8 * g + (lane >> 2)] += tot;
                 }
@@ -416,25 +456,42 @@ wgrad_kernel(BwdArgs a, int ntx, int nty, int G, float* __restrict__ part_k)
                 V[j][p] = ok ? __ldg(a.vmap + mb + (size_t)Y * Wz + X) : 0.f;
             }
         // source pixel of phi index (Y, X) and lag (a, b): image coordinate (Y - r) - a + r = Y - a  ->  rows PY0 - (KS-1) ..
-        // all loads of the fill are issued before the first store (a rolled loop would serialise on the load latency)
-        constexpr int NFILL = (C::SH * C::SW + NT - 1) / NT;
-        float fu[NFILL], fe[NFILL];
+        // all loads of the fill are issued before the first store (a rolled loop would serialise on the load latency).
+        // A warp takes rows sy = warp, warp + 8, ..., a lane columns sx = lane, lane + 32, ...: the mirror map and the
+        // range tests of a column are computed once per tile and those of a row once per row, not once per element
+        // (the per-element index arithmetic was what bound this kernel: ALU pipe 46 %, FMA pipe 37 %).
+        constexpr int NCOL = (C::SW + 31) / 32, NROW = (C::SH + NT / 32 - 1) / (NT / 32);
+        int xm[NCOL];
+        unsigned xfl = 0;               // bit c: column inside the extended image, bit 8 + c: inside the image
 #pragma unroll
-        for (int q = 0; q < NFILL; ++q) {
-            const int idx = tid + q * NT;
-            const int sy = idx / C::SW, sx = idx - sy * C::SW;
-            const int y = PY0 - (KS - 1) + sy, x = PX0 - (KS - 1) + sx;             // image coordinates
-            const bool in = idx < C::SH * C::SW && y >= 0 && y < a.H && x >= 0 && x < a.W;
-            const bool ext = idx < C::SH * C::SW && y >= -2 * R && y < a.H + 2 * R && x >= -2 * R && x < a.W + 2 * R;
-            fu[q] = ext ? __ldg(u_img + (size_t)mirror_clamp(y, a.H) * a.W + mirror_clamp(x, a.W)) : 0.f;
-            fe[q] = in ? __ldg(e_img + (size_t)y * a.W + x) : 0.f;
+        for (int c = 0; c < NCOL; ++c) {
+            const int sx = lane + 32 * c, x = PX0 - (KS - 1) + sx;
+            if (sx < C::SW && x >= -2 * R && x < a.W + 2 * R) xfl |= 1u << c;
+            if (sx < C::SW && x >= 0 && x < a.W) xfl |= 1u << (8 + c);
+            xm[c] = mirror_clamp(x, a.W);
+        }
+        float fu[NROW][NCOL], fe[NROW][NCOL];
+#pragma unroll
+        for (int q = 0; q < NROW; ++q) {
+            const int sy = warp + q * (NT / 32), y = PY0 - (KS - 1) + sy;
+            const bool yext = sy < C::SH && y >= -2 * R && y < a.H + 2 * R, yin = sy < C::SH && y >= 0 && y < a.H;
+            const float* urow = u_img + (size_t)mirror_clamp(y, a.H) * a.W;
+            const float* erow = e_img + (size_t)(yin ? y : 0) * a.W + (PX0 - (KS - 1) + lane);
+#pragma unroll
+            for (int c = 0; c < NCOL; ++c) {
+                fu[q][c] = (yext && ((xfl >> c) & 1)) ? __ldg(urow + xm[c]) : 0.f;
+                fe[q][c] = (yin && ((xfl >> (8 + c)) & 1)) ? __ldg(erow + 32 * c) : 0.f;
+            }
         }
         __syncthreads();                                        // the previous tile's source is no longer read
 #pragma unroll
-        for (int q = 0; q < NFILL; ++q) {
-            const int idx = tid + q * NT;
-            const int sy = idx / C::SW, sx = idx - sy * C::SW;
-            if (idx < C::SH * C::SW) { us[sy * C::SS + sx] = fu[q]; es[sy * C::SS + sx] = fe[q]; }
+        for (int q = 0; q < NROW; ++q) {
+            const int sy = warp + q * (NT / 32);
+#pragma unroll
+            for (int c = 0; c < NCOL; ++c) {
+                const int sx = lane + 32 * c;
+                if (sy < C::SH && sx < C::SW) { us[sy * C::SS + sx] = fu[q][c]; es[sy * C::SS + sx] = fe[q][c]; }
+            }
         }
         __syncthreads();
         // window rows wr = 0..KS: source row sy = by2 + wr serves lag a = j + (KS-1) - wr of block row j
