@@ -787,9 +787,9 @@ TcPlan plan_stage_tc(int B, int H, int W, int N_k, int ksize, int num_sms, int n
             const int n = (H + seg - 1) / seg;
             const long long units = (long long)B * nchunk * pl.nxs * n;
             const double unit_clk = 14000.0 + ((seg + 2 * R) / 2 + 1) * per_batch;
-            // split bank: the update kernel (launch + (nchunk + 3) planes of traffic) and the doubled drain work
-            const double upd = nchunk > 1 ? 14000.0 + 0.004 * (double)B * H * W * (nchunk + 3) : 0.0;
-            const double cost = (double)((units + num_sms - 1) / num_sms) * unit_clk * (nchunk > 1 ? 1.06 : 1.0) + upd;
+            // split bank: the update kernel ((nchunk + 3) planes of traffic; its launch overlaps the stage kernel's tail)
+            const double upd = nchunk > 1 ? 4000.0 + 0.002 * (double)B * H * W * (nchunk + 3) : 0.0;
+            const double cost = (double)((units + num_sms - 1) / num_sms) * unit_clk + upd;
             if (best < 0 || cost < best) { best = cost; pl.nys = n; pl.seg_rows = seg; pl.nchunk = nchunk; }
             if (forced > 0) break;
         }
