@@ -407,6 +407,19 @@ static int host_flags_reserve(Scratch* sc, size_t words)
     return TNRD_OK;
 }
 
+// The device address of a host result buffer the last stage may store into directly (pinned or otherwise device-mapped
+// memory), or null.  Not when `out` overlaps an input: with T = 1 the stage that stores u_T runs while the input arrives.
+static float* host_mapped_out(float* out, const float* f, const float* u0, size_t n)
+{
+    const bool apart = (out + n <= f || f + n <= out) && (out + n <= u0 || u0 + n <= out);
+    cudaPointerAttributes pa;
+    float* dev = nullptr;
+    if (apart && cudaPointerGetAttributes(&pa, out) == cudaSuccess && pa.type == cudaMemoryTypeHost && pa.devicePointer)
+        dev = static_cast<float*>(pa.devicePointer);
+    (void)cudaGetLastError();
+    return dev;
+}
+
 // experiments with the host entry point: 1 = a single image takes the two-halves path as well, 2 = never store to host
 // memory from a kernel, 3 = the input strictly top to bottom, 4 = serial (upload, stages, download)
 static int host_mode_env()
@@ -467,6 +480,22 @@ int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int 
         // serial: upload, all stages, download (small images, the tile kernel)
         TNRD_CUDA(cudaMemcpyAsync(d_f, f, n * sizeof(float), cudaMemcpyHostToDevice, st));
         if (u0 != f) TNRD_CUDA(cudaMemcpyAsync(d_u0, u0, n * sizeof(float), cudaMemcpyHostToDevice, st));
+        float* out_dev = (c.tc && T > 0 && host_mode_env() != 2) ? host_mapped_out(out, f, u0, n) : nullptr;
+        if (out_dev) {
+            // tensor-core kernel and a pinned result buffer: the last stage stores u_T into it, no copy back
+            if ((rc = stage_params(c, d_k, d_w, d_mu, rbf_gamma, T, N_k, ksize, phi)) != TNRD_OK) return rc;
+            if (T > 1 && (rc = grow(sc->pp, n, st)) != TNRD_OK) return rc;
+            const size_t rec = (size_t)N_k * tnrd::prm_stride(ksize);
+            const float* src = d_u0;
+            for (int t = 1; t <= T; ++t) {
+                float* dst = ((T - t) & 1) ? sc->pp.p : (t == T ? out_dev : d_out);
+                tnrd::StageArgs a{d_f, src, dst, sc->prm.p + (size_t)(t - 1) * rec, d_lam + (t - 1), 0.0f, B, H, W, N_k, ksize};
+                if ((rc = run_stage(c, a, phi, t - 1)) != TNRD_OK) return rc;
+                src = dst;
+            }
+            TNRD_CUDA(cudaStreamSynchronize(st));
+            return TNRD_OK;
+        }
         rc = tnrd_diffuse(d_f, d_u0, B, H, W, T, N_k, ksize, d_k, d_w, d_mu, rbf_gamma, d_lam, d_out, stream);
         if (rc != TNRD_OK) return rc;
         TNRD_CUDA(cudaMemcpyAsync(out, d_out, n * sizeof(float), cudaMemcpyDeviceToHost, st));
@@ -484,16 +513,7 @@ int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int 
         const int nblk = (H + 31) / 32;
         if ((rc = grow(sc->arrive, (size_t)nblk + 4, st)) != TNRD_OK) return rc;
         if (T > 1 && (rc = grow(sc->pp, n, st)) != TNRD_OK) return rc;
-        float* out_dev = nullptr;
-        {
-            cudaPointerAttributes pa;
-            // not when `out` overlaps an input: with T = 1 the stage that stores u_T runs while the input still arrives
-            const bool apart = (out + n <= f || f + n <= out) && (out + n <= u0 || u0 + n <= out);
-            if (apart && cudaPointerGetAttributes(&pa, out) == cudaSuccess && pa.type == cudaMemoryTypeHost && pa.devicePointer &&
-                host_mode_env() != 2)
-                out_dev = static_cast<float*>(pa.devicePointer);
-            (void)cudaGetLastError();
-        }
+        float* out_dev = host_mode_env() != 2 ? host_mapped_out(out, f, u0, n) : nullptr;
         unsigned* arrived = reinterpret_cast<unsigned*>(sc->arrive.p);
         TNRD_CUDA(cudaEventRecord(sc->ev[0], st));
         TNRD_CUDA(cudaStreamWaitEvent(sc->s_in, sc->ev[0], 0));

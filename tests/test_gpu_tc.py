@@ -396,3 +396,27 @@ def test_host_entry_point_single_image_with_a_split_bank(tnrd, monkeypatch):
     f = torch.from_numpy(c["f"]).pin_memory()
     tnrd.tnrd_diffuse_host(f, f, 1, 321, 481, 3, 48, 7, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"], c["lambda"], out)
     assert np.array_equal(out.numpy().astype(np.float64), ref)
+
+
+@pytest.mark.parametrize("shape,T", [((1, 321, 481), 3), ((3, 100, 260), 1), ((1, 600, 520), 2)], ids=lambda v: str(v))
+def test_host_entry_point_serial_path_stores_into_pinned_memory(tnrd, shape, T):
+    """Below the pipelining threshold the host call uploads, runs the stages and -- with the tensor-core kernel and a pinned
+    result buffer -- lets the last stage store u_T into host memory; pageable buffers get a copy.  Bit-identical."""
+    B, H, W = shape
+    c = tnrd_gen.make_small(290 + T, B, H, W, T, 16, 7)
+    ref = run_gpu(tnrd, c, kernel=3)
+    tnrd.tnrd_set_kernel(3)
+    try:
+        f = torch.from_numpy(c["f"]).pin_memory()
+        out = torch.zeros(c["f"].shape).pin_memory()
+        tnrd.tnrd_diffuse_host(f, f, B, H, W, T, 16, 7, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"], c["lambda"], out)
+        assert np.array_equal(out.numpy().astype(np.float64), ref)
+        out2 = np.zeros_like(c["f"])
+        tnrd.tnrd_diffuse_host(c["f"], c["u0"].copy(), B, H, W, T, 16, 7, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"],
+                               c["lambda"], out2)
+        assert np.array_equal(out2.astype(np.float64), ref)
+        g = f.clone().pin_memory()                                   # in place on the host
+        tnrd.tnrd_diffuse_host(g, g, B, H, W, T, 16, 7, c["filters"], c["rbf_w"], c["rbf_mu"], c["rbf_gamma"], c["lambda"], g)
+        assert np.array_equal(g.numpy().astype(np.float64), ref)
+    finally:
+        tnrd.tnrd_set_kernel(0)
