@@ -420,3 +420,25 @@ def test_host_entry_point_serial_path_stores_into_pinned_memory(tnrd, shape, T):
         assert np.array_equal(g.numpy().astype(np.float64), ref)
     finally:
         tnrd.tnrd_set_kernel(0)
+
+
+def test_host_entry_point_repeated_calls_of_changing_shapes(tnrd):
+    """The pipelined host paths at their natural sizes (above the two-million-pixel threshold), called again and again with
+    changing shapes: the arrival words, the pinned snapshots and the scratch planes are reused and regrown between calls, and
+    every result must equal the device call's bit for bit."""
+    shapes = [(1, 1500, 1500), (1, 1100, 2000), (2, 1024, 1100), (1, 2100, 1030), (6, 600, 640)]
+    cases = []
+    for k, (B, H, W) in enumerate(shapes):
+        c = tnrd_gen.make_small(300 + k, B, H, W, 2, 8, 7)
+        cases.append((c, run_gpu(tnrd, c, kernel=3)))
+    tnrd.tnrd_set_kernel(3)
+    try:
+        for rep in range(3):
+            for c, ref in cases:
+                f = torch.from_numpy(c["f"]).pin_memory()
+                out = torch.zeros(c["f"].shape).pin_memory()
+                tnrd.tnrd_diffuse_host(f, f, c["B"], c["H"], c["W"], 2, 8, 7, c["filters"], c["rbf_w"], c["rbf_mu"],
+                                       c["rbf_gamma"], c["lambda"], out)
+                assert np.array_equal(out.numpy().astype(np.float64), ref), (rep, c["B"], c["H"], c["W"])
+    finally:
+        tnrd.tnrd_set_kernel(0)
