@@ -442,3 +442,43 @@ def test_host_entry_point_repeated_calls_of_changing_shapes(tnrd):
                 assert np.array_equal(out.numpy().astype(np.float64), ref), (rep, c["B"], c["H"], c["W"])
     finally:
         tnrd.tnrd_set_kernel(0)
+
+
+@pytest.mark.parametrize("kernel", [0, 2], ids=["tensor-core", "tile"])
+def test_billion_pixel_image_sampled_windows(tnrd, kernel):
+    """The size limit B*H*W < 2^31: one 36000 x 32000 image (1.15 G pixels, 4.6 GB per plane -- byte offsets beyond 2^32), T = 2,
+    8 filters 7x7, on the tensor-core kernel and on the tile kernel (8 GB of partial sums); windows at the corners, the centre and beyond the 2^32-byte offset against the
+    oracle.  The image comes from tnrd_gen.hash_image in row chunks; the oracle gets crops of it with a 2rT margin."""
+    H, W, T, n_k, K = 36000, 32000, 2, 8, 7
+    free, _ = torch.cuda.mem_get_info()
+    if free < 24 * (1 << 30):
+        pytest.skip("needs 24 GB of device memory")
+    p = tnrd_gen.make_small(320, 1, 16, 16, T, n_k, K)              # parameters only
+    f = torch.empty((1, H, W), dtype=torch.float32, device="cuda")
+    for r0 in range(0, H, 2000):
+        f[0, r0:r0 + 2000] = torch.from_numpy(tnrd_gen.hash_image(H, W, r0, min(H, r0 + 2000))).cuda()
+    out = torch.empty_like(f)
+    k, w, mu, lam = dev(p["filters"]), dev(p["rbf_w"]), dev(p["rbf_mu"]), dev(p["lambda"])
+    tnrd.tnrd_set_kernel(kernel)
+    try:
+        tnrd.tnrd_diffuse(f, f, 1, H, W, T, n_k, K, k, w, mu, p["rbf_gamma"], lam, out)
+        torch.cuda.synchronize()
+    finally:
+        tnrd.tnrd_set_kernel(0)
+        tnrd.tnrd_shutdown()                                        # give the scratch (planes, partial sums) back
+    assert tnrd.tnrd_tc_plan_query(1, H, W, n_k, K, num_sms())["applies"] == 2
+    m = 2 * (K // 2) * T + 4
+    wins = _windows(H, W, 24, 2, 99) + [(H - 30, W // 2), (33555, 17000)]       # row 33555: byte offset 2^32 and a bit
+    worst = 0.0
+    for (y0, x0) in wins:
+        cy0, cy1, cx0, cx1 = max(0, y0 - m), min(H, y0 + 24 + m), max(0, x0 - m), min(W, x0 + 24 + m)
+        crop = tnrd_gen.hash_image(H, W, cy0, cy1)[:, cx0:cx1]
+        # the crop's border is the image border exactly where the window is within the margin of it
+        assert (cy0 == 0 or y0 - cy0 == m) and (cx0 == 0 or x0 - cx0 == m)
+        assert (cy1 == H or cy1 - (y0 + 24) == m) and (cx1 == W or cx1 - (x0 + 24) == m)
+        want = oracle.diffuse_window(crop, crop, p["filters"], p["rbf_w"], p["rbf_mu"], p["rbf_gamma"], p["lambda"],
+                                     y0 - cy0, x0 - cx0, 24, 24)
+        got = out[0, y0:y0 + 24, x0:x0 + 24].cpu().numpy().astype(np.float64)
+        mx, _ = check(got, want, f"billion-pixel window {(y0, x0)}", tight=True)
+        worst = max(worst, mx)
+    print(f"36000 x 32000, T = 2: worst window max-abs {worst:.3e}")

@@ -272,3 +272,16 @@ def make_deblock(seed: int, B: int, H: int, W: int, T: int, n_k: int, ksize: int
     out = dict(B=B, H=H, W=W, u0=f32(u0), qcs_lo=f32(lo), qcs_hi=f32(hi), clean=f32(clean))
     out.update(prm)
     return out
+
+
+def hash_image(H: int, W: int, y0: int = 0, y1: int | None = None) -> np.ndarray:
+    """Rows [y0, y1) of an H x W image given by an integer formula of (y, x) -- blocks of two grey levels plus hash noise,
+    values 0 .. 191, exactly representable -- so that a billion-pixel image (the `B*H*W < 2^31` edge case) can be made in row
+    chunks and any window of it again later, without keeping or copying the whole image.  float32 [y1 - y0][W]."""
+    y1 = H if y1 is None else y1
+    y = np.arange(y0, y1, dtype=np.uint64)[:, None]
+    x = np.arange(W, dtype=np.uint64)[None, :]
+    h = (y * np.uint64(2654435761) + x * np.uint64(40503)) ^ ((y * x) >> np.uint64(3))
+    h ^= h >> np.uint64(15)
+    v = (h & np.uint64(127)) + np.uint64(64) * (((y // np.uint64(97)) + (x // np.uint64(89))) & np.uint64(1))
+    return v.astype(np.float32)
