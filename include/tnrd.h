@@ -31,6 +31,9 @@
  *     CUDA graph returns TNRD_ERR_CUDA instead (run the shape once before capturing).
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device entry points
  *     are asynchronous on `stream` and never synchronise the device.
+ *     The stage kernels of the tensor-core and small-image paths are launched with programmatic stream serialisation
+ *     (they may be scheduled while the previous kernel of the stream drains, and wait for it before they touch global
+ *     memory): work the caller queues before or after a call on the same stream sees ordinary stream order.
  *   - Every function returning int returns TNRD_OK (0) or a negative tnrd_status.  Nothing throws.
  *     Errors found while validating or launching are returned; asynchronous faults surface at the
  *     caller's next synchronisation.  On error no output is written.
