@@ -676,8 +676,8 @@ int tnrd_diffuse_host(const float* f, const float* u0, int B, int H, int W, int 
         return TNRD_OK;
     }
     c.nchunk_fixed = nchunk_call;
-    // Pipelined (tensor-core kernel): the work of the FIRST and the LAST stage is cut in two halves -- the two halves of
-    // the batch, or of the rows of a single image (an even row, so that every pixel sees the arithmetic of the un-cut
+    // What is left (a batch whose stages cut the filter bank, TNRD_HOST_MODE = 1): the work of the FIRST and the LAST
+    // stage is cut in two halves -- the two halves of the batch, or of the rows of a single image (an even row, so that every pixel sees the arithmetic of the un-cut
     // launch and the result is bit-identical) -- so that the first half computes while the second half of the input
     // arrives, and the first half of the result leaves while the second half computes.  Copies run on two internal
     // streams ordered against `stream` by events.
