@@ -77,7 +77,9 @@ struct Scratch {
     size_t h_flags_cap = 0;
     Buf tab;                          // piecewise-linear phi tables [T][N_k][4096] float2 + 4 header floats
     Buf h_f, h_u, h_out, h_par;       // device staging of the host entry point
-    Buf bw_maps, bw_part, bw_trace, bw_e[2];   // backward pass: P/V maps, per-CTA partial sums, iterates, dl/du planes
+    Buf bw_maps, bw_part, bw_trace, bw_e[3];   // backward pass: P/V maps, per-CTA partial sums, iterates, dl/du planes
+    cudaStream_t s_bw = nullptr;               // tnrd_diffuse_backward: the lag-product kernel of stage t runs here, next to
+    cudaEvent_t ev_bw[4] = {};                 // the stage kernel of stage t - 1 (lowest priority; events: maps written / read)
 };
 std::vector<Scratch*> g_scratch;
 
@@ -795,9 +797,20 @@ int tnrd_deblock_diffuse(const float* u0, int B, int H, int W, int T, int N_k, i
 }
 
 // Backward pass of one stage on staged parameters (shared by tnrd_stage_backward and tnrd_diffuse_backward).
+// tnrd_diffuse_backward overlaps the lag-product kernel (g_k) of stage t with the stage kernel of stage t - 1: the stage
+// kernel's 1296 CTAs at 2048^2 are 4.4 waves of the 296 resident slots, so a fifth of the GPU idles in its last wave, and
+// the lag products of stage t are needed by nobody until the call returns.  The maps and the g_k partial sums are double
+// buffered by `parity`; evA[p] = maps p written, evB[p] = maps p (and the dl/du plane of that stage) no longer read.
+struct BwdSide {
+    cudaStream_t s2;
+    cudaEvent_t evA[2], evB[2];
+    int parity = 0;
+    bool used[2] = {false, false};
+};
+
 static int run_stage_backward(Call& c, const float* f, const float* u, const float* e, int B, int H, int W, int N_k,
                               int ksize, const float* prm, const float* lambda_ptr, float lambda_val, float gamma,
-                              float* g_u, float* g_k, float* g_w, float* g_l)
+                              float* g_u, float* g_k, float* g_w, float* g_l, BwdSide* side = nullptr)
 {
     Scratch* sc = c.sc;
     cudaStream_t st = c.st;
@@ -806,22 +819,40 @@ static int run_stage_backward(Call& c, const float* f, const float* u, const flo
     const bool want_k = g_k != nullptr, want_w = g_w != nullptr || want_k;
     const size_t n_w = want_w ? (size_t)pl.n_cta * N_k * 64 : 0, n_l = (size_t)pl.n_cta;
     const size_t n_k = want_k ? (size_t)pl.G * N_k * KK : 0;
-    int rc = grow(sc->bw_part, n_w + n_l + n_k + 4, st);
+    if (!want_k) side = nullptr;
+    const int p = side ? side->parity : 0;
+    int rc = grow(sc->bw_part, n_w + n_l + 2 * n_k + 4, st);
     if (rc != TNRD_OK) return rc;
     const size_t map = want_k ? (size_t)B * N_k * (H + 2 * R) * (W + 2 * R) : 0;
-    if (want_k && (rc = grow(sc->bw_maps, 2 * map, st)) != TNRD_OK) return rc;
+    if (want_k && (rc = grow(sc->bw_maps, (side ? 4 : 2) * map, st)) != TNRD_OK) return rc;
     float* part_w = sc->bw_part.p;
     float* part_l = part_w + n_w;
-    float* part_k = part_l + n_l;
+    float* part_k = part_l + n_l + (size_t)p * n_k;
+    float* maps = sc->bw_maps.p + (size_t)p * 2 * map;
     tnrd::BwdArgs a{f, u, e, g_u, prm, lambda_ptr, lambda_val, B, H, W, N_k, ksize,
-                    want_k ? sc->bw_maps.p : nullptr, want_k ? sc->bw_maps.p + map : nullptr,
+                    want_k ? maps : nullptr, want_k ? maps + map : nullptr,
                     want_w ? part_w : nullptr, g_l ? part_l : nullptr};
-    TNRD_CUDA(tnrd::launch_stage_bwd(a, pl, part_k, st, &c.lc.n));
-    if (want_w || g_l) {
-        const float s = sqrtf(1.4426950408889634f / (2.0f * gamma * gamma));
-        TNRD_CUDA(tnrd::launch_reduce_partials(part_w, pl.n_cta, part_k, pl.G, part_l, N_k, ksize, s, g_w, g_k, g_l, st,
-                                               &c.lc.n));
+    const float s = sqrtf(1.4426950408889634f / (2.0f * gamma * gamma));
+    if (!side) {
+        TNRD_CUDA(tnrd::launch_stage_bwd(a, pl, part_k, 3, st, &c.lc.n));
+        if (want_w || g_l)
+            TNRD_CUDA(tnrd::launch_reduce_partials(part_w, pl.n_cta, part_k, pl.G, part_l, N_k, ksize, s, g_w, g_k, g_l, st,
+                                                   &c.lc.n));
+        return TNRD_OK;
     }
+    if (side->used[p]) TNRD_CUDA(cudaStreamWaitEvent(st, side->evB[p], 0));     // two stages ago: done with these buffers
+    TNRD_CUDA(tnrd::launch_stage_bwd(a, pl, part_k, 1, st, &c.lc.n));
+    TNRD_CUDA(cudaEventRecord(side->evA[p], st));
+    if (g_w || g_l)
+        TNRD_CUDA(tnrd::launch_reduce_partials(part_w, pl.n_cta, nullptr, 0, part_l, N_k, ksize, s, g_w, nullptr, g_l, st,
+                                               &c.lc.n));
+    TNRD_CUDA(cudaStreamWaitEvent(side->s2, side->evA[p], 0));
+    TNRD_CUDA(tnrd::launch_stage_bwd(a, pl, part_k, 2, side->s2, &c.lc.n));
+    TNRD_CUDA(tnrd::launch_reduce_partials(nullptr, 0, part_k, pl.G, nullptr, N_k, ksize, s, nullptr, g_k, nullptr, side->s2,
+                                           &c.lc.n));
+    TNRD_CUDA(cudaEventRecord(side->evB[p], side->s2));
+    side->used[p] = true;
+    side->parity ^= 1;
     return TNRD_OK;
 }
 
@@ -869,8 +900,20 @@ int tnrd_diffuse_backward(const float* f, const float* u0, const float* u_gt, co
     const int phi = c.o.phi_mode == 2 ? 3 : c.o.phi_mode;
     if ((rc = pick_kernel(c, B, H, W, N_k, ksize, phi)) != TNRD_OK) return rc;
     if ((rc = grow(sc->bw_trace, (size_t)T * n, st)) != TNRD_OK) return rc;     // u_1 .. u_T
-    if ((rc = grow(sc->bw_e[0], n, st)) != TNRD_OK) return rc;
-    if ((rc = grow(sc->bw_e[1], n, st)) != TNRD_OK) return rc;
+    for (Buf& eb : sc->bw_e)
+        if ((rc = grow(eb, n, st)) != TNRD_OK) return rc;
+    BwdSide side;
+    if (grad_filters) {
+        if (!sc->s_bw) {
+            int pr_least = 0, pr_greatest = 0;
+            TNRD_CUDA(cudaDeviceGetStreamPriorityRange(&pr_least, &pr_greatest));
+            TNRD_CUDA(cudaStreamCreateWithPriority(&sc->s_bw, cudaStreamNonBlocking, pr_least));
+            for (auto& ev : sc->ev_bw) TNRD_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        }
+        side.s2 = sc->s_bw;
+        side.evA[0] = sc->ev_bw[0]; side.evA[1] = sc->ev_bw[1];
+        side.evB[0] = sc->ev_bw[2]; side.evB[1] = sc->ev_bw[3];
+    }
     {
         Opts keep = c.o;
         c.o.basis = 0;                                          // stage_params builds no table: phi != 2 here
@@ -898,15 +941,18 @@ int tnrd_diffuse_backward(const float* f, const float* u0, const float* u_gt, co
         const float* u_prev = (t == 1) ? u0 : sc->bw_trace.p + (size_t)(t - 2) * n;
         float* g_u;
         if (t == 1) g_u = grad_u0;                                   // may be null: not needed then
-        else g_u = (e == sc->bw_e[0].p) ? sc->bw_e[1].p : sc->bw_e[0].p;
+        else g_u = sc->bw_e[(T - t + 1) % 3].p;      // three planes in turn: stage t's dl/du is still read by its lag products
+                                                    // (side stream) while stage t - 1 writes the next one
         rc = run_stage_backward(c, f, u_prev, e, B, H, W, N_k, ksize, sc->prm.p + (size_t)(t - 1) * rec,
                                 lambda + (t - 1), 0.0f, rbf_gamma, g_u,
                                 grad_filters ? grad_filters + (size_t)(t - 1) * N_k * KK : nullptr,
                                 grad_w ? grad_w + (size_t)(t - 1) * N_k * TNRD_NUM_RBF : nullptr,
-                                grad_lambda ? grad_lambda + (t - 1) : nullptr);
+                                grad_lambda ? grad_lambda + (t - 1) : nullptr, grad_filters ? &side : nullptr);
         if (rc != TNRD_OK) return rc;
         e = g_u;
     }
+    for (int q = 0; q < 2; ++q)         // the caller's stream continues after the last lag products
+        if (side.used[q]) TNRD_CUDA(cudaStreamWaitEvent(st, side.evB[q], 0));
     return TNRD_OK;
 }
 
@@ -1015,11 +1061,13 @@ void tnrd_shutdown(void)
     (void)cudaGetDevice(&cur);
     for (Scratch* s : g_scratch) {
         (void)cudaSetDevice(s->dev);
-        Buf* bufs[] = {&s->pp, &s->arrive, &s->tcws, &s->stats, &s->prm, &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->refv, &s->split, &s->tab, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
+        Buf* bufs[] = {&s->pp, &s->arrive, &s->tcws, &s->stats, &s->prm, &s->bw_maps, &s->bw_part, &s->bw_trace, &s->bw_e[0], &s->bw_e[1], &s->bw_e[2], &s->refv, &s->split, &s->tab, &s->h_f, &s->h_u, &s->h_out, &s->h_par};
         for (Buf* b : bufs)
             if (b->p) (void)cudaFree(b->p);   // synchronising free: the stream may be gone by now
         if (s->s_in) { (void)cudaStreamDestroy(s->s_in); (void)cudaStreamDestroy(s->s_out); }
         for (cudaStream_t b : s->s_band) if (b) (void)cudaStreamDestroy(b);
+        if (s->s_bw) (void)cudaStreamDestroy(s->s_bw);
+        for (cudaEvent_t e : s->ev_bw) if (e) (void)cudaEventDestroy(e);
         for (cudaEvent_t e : s->ev) if (e) (void)cudaEventDestroy(e);
         if (s->h_par_pinned) (void)cudaFreeHost(s->h_par_pinned);
         if (s->h_word) (void)cudaFreeHost(s->h_word);

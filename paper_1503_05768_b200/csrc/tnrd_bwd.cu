@@ -589,17 +589,20 @@ cudaError_t launch_bwd_cfg(const BwdArgs& a, const BwdPlan& pl, cudaStream_t st)
     return cudaGetLastError();
 }
 
+// `what`: 1 = the stage kernel, 2 = the lag-product kernel (g_k from the maps the stage kernel wrote), 3 = both in turn
 template <int KS>
-cudaError_t launch_bwd_ks(const BwdArgs& a, const BwdPlan& pl, float* part_k, cudaStream_t st,
+cudaError_t launch_bwd_ks(const BwdArgs& a, const BwdPlan& pl, float* part_k, int what, cudaStream_t st,
                           unsigned long long* launches)
 {
     const bool want_w = a.part_w != nullptr, want_k = a.pmap != nullptr;
-    cudaError_t e;
-    if (want_k) e = launch_bwd_cfg<KS, true, true>(a, pl, st);          // g_k is only asked for together with g_w
-    else if (want_w) e = launch_bwd_cfg<KS, true, false>(a, pl, st);
-    else e = launch_bwd_cfg<KS, false, false>(a, pl, st);
-    ++*launches;
-    if (e != cudaSuccess || !want_k) return e;
+    cudaError_t e = cudaSuccess;
+    if (what & 1) {
+        if (want_k) e = launch_bwd_cfg<KS, true, true>(a, pl, st);          // g_k is only asked for together with g_w
+        else if (want_w) e = launch_bwd_cfg<KS, true, false>(a, pl, st);
+        else e = launch_bwd_cfg<KS, false, false>(a, pl, st);
+        ++*launches;
+    }
+    if (e != cudaSuccess || !want_k || !(what & 2)) return e;
     wgrad_kernel<KS><<<dim3((unsigned)a.N_k, (unsigned)pl.G), WCfg<KS>::NT, 0, st>>>(a, pl.wtx, pl.wty, pl.G, part_k);
     ++*launches;
     return cudaGetLastError();
@@ -617,22 +620,34 @@ BwdPlan plan_stage_bwd(int B, int H, int W, int N_k, int ksize, int num_sms)
     p.wtx = (W + 2 * R + 63) / 64;               // wgrad tiles of 64 x 32 phi pixels
     p.wty = (H + 2 * R + 31) / 32;
     const long long wt = (long long)p.wtx * p.wty * B;
-    long long G = (4LL * num_sms + N_k - 1) / N_k;      // ~4 CTAs per SM in total
-    if (G > wt) G = wt;
-    if (G < 1) G = 1;
+    // wgrad: N_k x G CTAs, each walking over its share of the tiles (a CTA lasts as long as its share).  G such that the
+    // CTAs fill whole waves of the resident slots (2 CTAs per SM, 1 for 9x9): 13 CTAs per filter for 48 filters were 624
+    // CTAs on 296 slots, 2.1 waves of work in the time of 3.
+    const long long slots = (long long)(ksize <= 7 ? 2 : 1) * num_sms;
+    long long G = 1;
+    double best = -1.0;
+    for (long long w = 12; w >= 1; --w) {      // many short CTAs rather than few long ones: they fill the gaps other kernels leave
+        long long g = slots * w / N_k;
+        if (g < 1) g = 1;
+        if (g > wt) g = wt;
+        const long long ctas = g * N_k, waves = (ctas + slots - 1) / slots;
+        // the tiles of a filter are dealt out in turn: a CTA takes ceil(wt / g) tiles at most
+        const double eff = (double)wt / (double)(((wt + g - 1) / g) * g) * (double)ctas / (double)(waves * slots);
+        if (eff > best + 1e-9) { best = eff; G = g; }
+    }
     p.G = (int)G;
     return p;
 }
 
-cudaError_t launch_stage_bwd(const BwdArgs& a, const BwdPlan& pl, float* part_k, cudaStream_t st,
+cudaError_t launch_stage_bwd(const BwdArgs& a, const BwdPlan& pl, float* part_k, int what, cudaStream_t st,
                              unsigned long long* launches)
 {
     if (pl.n_cta > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     switch (a.ksize) {
-        case 3: return launch_bwd_ks<3>(a, pl, part_k, st, launches);
-        case 5: return launch_bwd_ks<5>(a, pl, part_k, st, launches);
-        case 7: return launch_bwd_ks<7>(a, pl, part_k, st, launches);
-        case 9: return launch_bwd_ks<9>(a, pl, part_k, st, launches);
+        case 3: return launch_bwd_ks<3>(a, pl, part_k, what, st, launches);
+        case 5: return launch_bwd_ks<5>(a, pl, part_k, what, st, launches);
+        case 7: return launch_bwd_ks<7>(a, pl, part_k, what, st, launches);
+        case 9: return launch_bwd_ks<9>(a, pl, part_k, what, st, launches);
         default: return cudaErrorInvalidValue;
     }
 }

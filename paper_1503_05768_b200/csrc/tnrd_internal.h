@@ -116,7 +116,8 @@ struct BwdPlan {
     int wtx, wty, G;     // wgrad tiles per image; CTAs per filter
 };
 BwdPlan plan_stage_bwd(int B, int H, int W, int N_k, int ksize, int num_sms);
-cudaError_t launch_stage_bwd(const BwdArgs& a, const BwdPlan& pl, float* part_k /*[G][N_k][ks*ks]*/, cudaStream_t st,
+// what: 1 = stage_bwd_kernel, 2 = wgrad_kernel (reads the maps kernel 1 wrote), 3 = both in turn
+cudaError_t launch_stage_bwd(const BwdArgs& a, const BwdPlan& pl, float* part_k /*[G][N_k][ks*ks]*/, int what, cudaStream_t st,
                              unsigned long long* launches);
 cudaError_t launch_reduce_partials(const float* part_w, long long n_cta, const float* part_k, int G, const float* part_l,
                                    int N_k, int ksize, float s, float* g_w, float* g_k, float* g_lambda, cudaStream_t st,
