@@ -12,7 +12,8 @@
 // EXTENDED output domain [-2r, H+2r) x [-2r, W+2r) (K_i^T reaches 2r beyond the image; E^T folds that rim back).
 // Per filter i (streamed): z' = k'_i * u~ and q' = k'_i * e0 (e0 = e, zero outside the image: Kbar_i^T e is a true
 // convolution of the zero-extended e) in registers on the tile + r ring; the 63 exponentials E_j are evaluated ONCE
-// and feed  A = sum_j w'_j d'_j E_j  (phi'),  V = sum_j w'_j E_j  (phi, for g_k) and the g_w sums  sum_p E_j q'_p
+// and feed  V = sum_j w'_j E_j  (phi, for g_k),  U = sum_j w'_j mu'_j E_j  (A = z' V - U = sum_j w'_j d'_j E_j is phi')
+// and the g_w sums  sum_p E_j q'_p
 // (reduced over the warp with a halving butterfly, then one shared-memory reduction per centre);
 // P = -2 ln2 A q' (= Lambda_i Kbar_i^T e / s) goes to a double-buffered shared map, the k'_i taps are applied to the
 // map of filter i-1 (K_i^T is a correlation with k_i) into per-thread accumulators.  Epilogue: the accumulators go to
@@ -52,10 +53,13 @@ struct BCfg {
 };
 
 // 8 RBF terms (7 in the last step) for the 8 responses of a block.  z = z' (scaled responses), qm = q' of the pixels
-// this tile owns (0 elsewhere).  Accumulates A (phi'), V (phi) and, per term, S[m] = sum over the 8 pixels of E q'.
-template <int NTERM, bool WANT_W, bool WANT_K>
+// this tile owns (0 elsewhere).  Accumulates V = sum_j w'_j E_j (phi) and U = sum_j w'_j mu'_j E_j -- the caller forms
+// sum_j w'_j (z' - mu'_j) E_j (phi') as z' V - U, one packed instruction per term less than accumulating it directly; the
+// cancellation costs log2(|z'| / |z' - mu'_j|) < 5 bits where a term is not negligible -- and, per term, S[m] = sum over
+// the 8 pixels of E q'.
+template <int NTERM, bool WANT_W>
 __device__ __forceinline__ void phi_bwd_step(const float* __restrict__ mw, const float2 (&z)[4], const float2 (&qm)[4],
-                                             float2 (&A)[4], float2 (&V)[4], float (&S)[8])
+                                             float2 (&U)[4], float2 (&V)[4], float (&S)[8])
 {
     float c[16];
     lds_vec(mw, c);
@@ -63,14 +67,14 @@ __device__ __forceinline__ void phi_bwd_step(const float* __restrict__ mw, const
     for (int m = 0; m < 8; ++m) {
         if (m >= NTERM) { S[m] = 0.f; continue; }
         float2 s2 = make_float2(0.f, 0.f);
+        const float wmu = -c[2 * m] * c[2 * m + 1];           // c = (-mu', w')
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
             const float2 d = __fadd2_rn(z[p], make_float2(c[2 * m], c[2 * m]));
             const float2 t = __fmul2_rn(d, d);
             const float2 e = make_float2(ex2_neg(t.x), ex2_neg(t.y));
-            const float2 wd = __fmul2_rn(d, make_float2(c[2 * m + 1], c[2 * m + 1]));
-            A[p] = __ffma2_rn(e, wd, A[p]);
-            if (WANT_K) V[p] = __ffma2_rn(e, make_float2(c[2 * m + 1], c[2 * m + 1]), V[p]);
+            V[p] = __ffma2_rn(e, make_float2(c[2 * m + 1], c[2 * m + 1]), V[p]);
+            U[p] = __ffma2_rn(e, make_float2(wmu, wmu), U[p]);
             if (WANT_W) s2 = __ffma2_rn(e, qm[p], s2);
         }
         S[m] = s2.x + s2.y;
@@ -247,7 +251,7 @@ stage_bwd_kernel(BwdArgs a, int ntx, int nty)
             const float* uwn = us + (un >= 0 ? un : 0);
             const float* ewn = es + (un >= 0 ? un : 0);
             const float* vw = vprev + (coff[n] >= 0 ? coff[n] : 0);
-            float2 A[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
+            float2 U[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
             float2 V[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
             float2 zn[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
             float2 qn[4] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
@@ -282,8 +286,8 @@ stage_bwd_kernel(BwdArgs a, int ntx, int nty)
                 const float cmin = crange[2 * g], cmax = crange[2 * g + 1];
                 const bool live = !((wlo - cmax > TNRD_FCLAMP && whi == whi) || cmin - whi > TNRD_FCLAMP);
                 if (hasB && live) {
-                    if (g < C::NG - 1) phi_bwd_step<8, WANT_W, WANT_K>(rec + KKP + 16 * g, zc, qm, A, V, S);
-                    else phi_bwd_step<TNRD_M - 8 * (C::NG - 1), WANT_W, WANT_K>(rec + KKP + 16 * g, zc, qm, A, V, S);
+                    if (g < C::NG - 1) phi_bwd_step<8, WANT_W>(rec + KKP + 16 * g, zc, qm, U, V, S);
+                    else phi_bwd_step<TNRD_M - 8 * (C::NG - 1), WANT_W>(rec + KKP + 16 * g, zc, qm, U, V, S);
                 } else {
 #pragma unroll
                     for (int m = 0; m < 8; ++m) S[m] = 0.f;
@@ -313,7 +317,10 @@ stage_bwd_kernel(BwdArgs a, int ntx, int nty)
                 constexpr float C0 = -1.3862943611198906f;
                 float2 P[4];
 #pragma unroll
-                for (int p = 0; p < 4; ++p) P[p] = make_float2(C0 * A[p].x * qc[p].x, C0 * A[p].y * qc[p].y);
+                for (int p = 0; p < 4; ++p) {
+                    const float2 A = make_float2(fmaf(zc[p].x, V[p].x, -U[p].x), fmaf(zc[p].y, V[p].y, -U[p].y));   // phi' terms
+                    P[p] = make_float2(C0 * A.x * qc[p].x, C0 * A.y * qc[p].y);
+                }
                 *reinterpret_cast<float4*>(vcur + voff[n]) = make_float4(P[0].x, P[1].x, P[2].x, P[3].x);
                 *reinterpret_cast<float4*>(vcur + voff[n] + C::VS) = make_float4(P[0].y, P[1].y, P[2].y, P[3].y);
                 if (WANT_K && own[n]) {     // owned pixels go to the HBM maps of kernel 2 (phi-region coordinates)
