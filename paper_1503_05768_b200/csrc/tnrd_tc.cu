@@ -32,7 +32,7 @@
 // chunks as well (plan_stage_tc): a unit then evaluates only its chunk's filters and writes the partial sum of Eq. 7's
 // diffusion term to scratch, and tc_update_kernel adds the chunks in a fixed order and applies the reaction term.
 // Warp roles: 24 phi warps (6 per tensor-memory lane quarter, sharing the quarter's filter pairs through a ticket
-// counter), 4 drain warps (fold + a5), 1 MMA-issuing warp, 1 loader warp; mbarrier pipelines between them (u row pairs,
+// counter), 4 drain warps (fold + a5), 1 MMA-issuing warp, 2 loader warps; mbarrier pipelines between them (u row pairs,
 // z double-buffered, scatter table).
 #include <cuda_bf16.h>
 #include <cmath>
@@ -50,7 +50,10 @@ namespace {
 #ifndef TNRD_TC_PHI_WARPS
 #define TNRD_TC_PHI_WARPS 24
 #endif
-constexpr int TC_PHI_WARPS = TNRD_TC_PHI_WARPS, TC_LOAD_WARPS = 1;   // phi warps: a multiple of 4 (TC_PHI_WARPS / 4 per lane quarter)
+#ifndef TNRD_TC_LOAD_WARPS
+#define TNRD_TC_LOAD_WARPS 2    // one warp delivered a row pair in ~ 6 k clocks: the floor of a batch with few filters (a third: same)
+#endif
+constexpr int TC_PHI_WARPS = TNRD_TC_PHI_WARPS, TC_LOAD_WARPS = TNRD_TC_LOAD_WARPS;   // phi warps: a multiple of 4 (TC_PHI_WARPS / 4 per lane quarter)
 constexpr int TC_DRAIN_WARPS = 4;                               // one per lane quarter, right after the phi warps
 constexpr int TC_MMA_WARP = TC_PHI_WARPS + TC_DRAIN_WARPS;      // warp index of the MMA issuer
 constexpr int TC_THREADS = (TC_PHI_WARPS + TC_DRAIN_WARPS + 1 + TC_LOAD_WARPS) * 32;
@@ -767,30 +770,38 @@ TcPlan plan_stage_tc(int B, int H, int W, int N_k, int ksize, int num_sms, int n
     const int R = (ksize - 1) / 2, OW = 256 - 2 * R, nkp = (N_k + 7) / 8 * 8;
     TcPlan pl;
     pl.nxs = (W + OW - 1) / OW;
-    // Units = images x filter chunks x row segments x strips.  Time of a unit in SM clocks (fitted on B200): a constant
-    // (operands to shared memory, tensor-memory allocation, pipeline fill and drain) + batches x the larger of the phi
-    // time of the chunk's filters and the per-batch floor of the MMA / drain pipeline.  Minimise waves x unit time (+ the
+    // Units = images x filter chunks x row segments x strips.  Time of a unit in SM clocks (fitted on B200): set-up
+    // (operands to shared memory, tensor-memory allocation, pipeline fill and drain) + batches x (a floor of the MMA /
+    // drain pipeline + the phi time of the chunk's filters).  Minimise waves x unit time (+ the
     // update kernel when the bank is split).  Even segment heights: every segment then starts on an even row, so a pixel's
     // arithmetic (the pairing of phi rows into batches) does not depend on how the rows are cut up.
     double best = -1.0;
+    long long best_units = 0;
     pl.nys = 1; pl.seg_rows = H; pl.nchunk = 1;
     const int forced = tc_env_int("TNRD_TC_SEG"), forced_chunk = tc_env_int("TNRD_TC_CHUNK");
     for (int nchunk = 1; nchunk <= nkp / 8; ++nchunk) {
         if (nkp % (8 * nchunk)) continue;
         if (nchunk_fixed > 0 && nchunk != nchunk_fixed) continue;
         if (nchunk_fixed <= 0 && forced_chunk > 0 && nchunk != forced_chunk && nkp % (8 * forced_chunk) == 0) continue;
-        const double per_batch = 2900.0 + 408.0 * (nkp / nchunk);      // measured: 22.5 k clocks at 48 filters, 12.7 k at 24
+        const double nf = nkp / nchunk;
+        const double per_batch = 2400.0 + 380.0 * nf;       // measured (7x7): 5.8 k clocks at 8 filters, 8.3 k at 16, 10.9 k at 24, 20.6 k at 48
         for (int nys = 1; nys <= (H + 3) / 4; ++nys) {
             int seg = (H + nys - 1) / nys;
             seg = (seg + seg_mult - 1) / seg_mult * seg_mult;
             if (forced > 0) seg = forced < H ? forced : H;
             const int n = (H + seg - 1) / seg;
             const long long units = (long long)B * nchunk * pl.nxs * n;
-            const double unit_clk = 14000.0 + ((seg + 2 * R) / 2 + 1) * per_batch;
+            const double unit_clk = 12000.0 + 300.0 * nf + ((seg + 2 * R) / 2 + 1) * per_batch;
             // split bank: the update kernel ((nchunk + 3) planes of traffic; its launch overlaps the stage kernel's tail)
             const double upd = nchunk > 1 ? 4000.0 + 0.002 * (double)B * H * W * (nchunk + 3) : 0.0;
             const double cost = (double)((units + num_sms - 1) / num_sms) * unit_clk + upd;
-            if (best < 0 || cost < best) { best = cost; pl.nys = n; pl.seg_rows = seg; pl.nchunk = nchunk; }
+            // within 1 % the plan with more units wins: units are handed out as SMs become free, and short units even
+            // out the tail that the wave count does not see (4096^2: 442 units of 158 rows beat 289 of 242 by 0.4 %)
+            if (best < 0 || cost < 0.99 * best || (cost < 1.01 * best && units > best_units)) {
+                if (best < 0 || cost < best) best = cost;
+                best_units = units;
+                pl.nys = n; pl.seg_rows = seg; pl.nchunk = nchunk;
+            }
             if (forced > 0) break;
         }
     }
