@@ -97,29 +97,35 @@ __host__ __device__ constexpr size_t tc_ws_stage_bytes(int ks, int nkp) { return
 
 // ---- PTX wrappers ----------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-// K-major, unswizzled operand: 8 rows of a core matrix 16 bytes apart, `sbo` between 8-row groups, `lbo` between
-// the two 16-byte K chunks of one MMA
-__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo)
-{
-    return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo >> 4) & 0x3FFF) << 16) |
-           ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) | ((uint64_t)1 << 46);
-}
+// Shared-memory operand descriptor, K-major and unswizzled: 8 rows of a core matrix 16 bytes apart, `sbo` between 8-row
+// groups, `lbo` between the two 16-byte K chunks of one MMA.  64 bits: start >> 4 in bits 0-13, lbo >> 4 in 16-29,
+// sbo >> 4 in 32-45, version 1 in bit 46 -- kept as two words (umma_desc_lo / umma_desc_hi below).
 // instruction descriptor: fp32 accumulate, A and B K-major, fmt 1 = BF16, 2 = TF32
 __device__ __forceinline__ uint32_t umma_idesc(int fmt, int M, int N)
 {
     return (1u << 4) | ((uint32_t)fmt << 7) | ((uint32_t)fmt << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
-__device__ __forceinline__ void umma_tf32_ss(uint32_t d, uint64_t a, uint64_t b, uint32_t idesc, uint32_t acc)
+// MMAs with the descriptors as (low, high) words and the accumulate flag as a constant: the issuing thread adds an offset
+// to the low word (the 14-bit address field, no carry) instead of building a 64-bit descriptor per instruction.  What is
+// left of the issue time is the tensor pipe's: about 73 clocks per forward MMA (M 128, K 8: the A operand is read from
+// shared memory) and 240 per scatter MMA (A from tensor memory, every one into the accumulator of the last) -- 42 + nkp
+// MMAs per batch, 5 k clocks with 8 filters, which is what a batch of a small filter chunk costs at least.
+__device__ __forceinline__ uint32_t umma_desc_lo(uint32_t saddr, uint32_t lbo) { return ((saddr >> 4) & 0x3FFF) | (((lbo >> 4) & 0x3FFF) << 16); }
+__device__ __forceinline__ uint32_t umma_desc_hi(uint32_t sbo) { return ((sbo >> 4) & 0x3FFF) | (1u << 14); }
+template <bool ACC>
+__device__ __forceinline__ void umma_tf32_ss2(uint32_t d, uint32_t a_lo, uint32_t a_hi, uint32_t b_lo, uint32_t b_hi, uint32_t idesc)
 {
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}\n"
-                 :: "r"(d), "l"(a), "l"(b), "r"(idesc), "r"(acc) : "memory");
+    asm volatile("{\n\t.reg .b64 da, db;\n\t.reg .pred p;\n\tsetp.ne.b32 p, %6, 0;\n\t"
+                 "mov.b64 da, {%1, %2};\n\tmov.b64 db, {%3, %4};\n\t"
+                 "tcgen05.mma.cta_group::1.kind::tf32 [%0], da, db, %5, p;\n\t}\n"
+                 :: "r"(d), "r"(a_lo), "r"(a_hi), "r"(b_lo), "r"(b_hi), "r"(idesc), "n"(ACC ? 1 : 0) : "memory");
 }
-__device__ __forceinline__ void umma_bf16_ts(uint32_t d, uint32_t a_tmem, uint64_t b, uint32_t idesc, uint32_t acc)
+template <bool ACC>
+__device__ __forceinline__ void umma_bf16_ts2(uint32_t d, uint32_t a_tmem, uint32_t b_lo, uint32_t b_hi, uint32_t idesc)
 {
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                 "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}\n"
-                 :: "r"(d), "r"(a_tmem), "l"(b), "r"(idesc), "r"(acc) : "memory");
+    asm volatile("{\n\t.reg .b64 db;\n\t.reg .pred p;\n\tsetp.ne.b32 p, %5, 0;\n\tmov.b64 db, {%2, %3};\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], db, %4, p;\n\t}\n"
+                 :: "r"(d), "r"(a_tmem), "r"(b_lo), "r"(b_hi), "r"(idesc), "n"(ACC ? 1 : 0) : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint64_t* bar)
 {
@@ -653,19 +659,34 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
         if (lane == 0) {
             const uint32_t id_f = umma_idesc(2, 128, 2 * nkp), id_s = umma_idesc(1, 128, C::NSC);
             const uint32_t lbo_f = 2 * nkp * 16;
+            const uint32_t s_lo = umma_desc_lo(sbase + C::SM_BS, C::NSC * 16), s_hi = umma_desc_hi(128);
+            // descriptor words that do not change: high words (stride between 8-row groups, version), the low words of
+            // the ring and operand bases; per MMA one 32-bit add each for the ring row and the tap row
+            const uint32_t a_hi = umma_desc_hi(128), b_hi = umma_desc_hi(128);
+            const uint32_t a_lo_hi = umma_desc_lo(sbase + C::SM_UHI, 32), a_lo_lo = umma_desc_lo(sbase + C::SM_ULO, 32);
+            const uint32_t b_lo_hi = umma_desc_lo(sbase + C::SM_BFH, lbo_f), b_lo_lo = umma_desc_lo(sbase + C::SM_BFL, lbo_f);
+            constexpr uint32_t RING_STEP = (TC_CW * 16) >> 4;            // one ring row, in 16-byte units
+            const uint32_t tap_step = (2 * lbo_f) >> 4;                  // one tap row of the operand
             auto forward = [&](int b) {
                 const int bb = b & 1;
-                for (int rr = 0; rr < 2; ++rr) {
-                    const uint32_t d = tmem + bb * 4 * nkp + rr * 2 * nkp;
-                    uint32_t acc = 0;
-                    for (int split = 0; split < 3; ++split) {            // hi*hi, hi*lo, lo*hi
-                        const uint32_t ab = sbase + (split == 2 ? C::SM_ULO : C::SM_UHI);
-                        const uint32_t bbase = sbase + (split == 1 ? C::SM_BFL : C::SM_BFH);
-                        for (int ta = 0; ta < KS; ++ta) {
-                            const int ring = (2 * b + rr + ta) % (2 * TC_NP);
-                            umma_tf32_ss(d, umma_desc(ab + ring * TC_CW * 16, 32, 128),
-                                         umma_desc(bbase + 2 * ta * lbo_f, lbo_f, 128), id_f, acc);
-                            acc = 1;
+                const int r0 = (2 * b) % (2 * TC_NP);
+                // the two rows of the batch accumulate into different columns and alternate: two chains of dependent
+                // accumulations in flight (no measurable difference: the pipe is bound by reading A)
+#pragma unroll
+                for (int split = 0; split < 3; ++split) {                // hi*hi, hi*lo, lo*hi
+                    const uint32_t ab = split == 2 ? a_lo_lo : a_lo_hi;
+                    const uint32_t bbl = split == 1 ? b_lo_lo : b_lo_hi;
+#pragma unroll
+                    for (int ta = 0; ta < KS; ++ta) {
+#pragma unroll
+                        for (int rr = 0; rr < 2; ++rr) {
+                            const uint32_t d = tmem + bb * 4 * nkp + rr * 2 * nkp;
+                            int ring = r0 + rr + ta;
+                            if (ring >= 2 * TC_NP) ring -= 2 * TC_NP;
+                            if (split == 0 && ta == 0)
+                                umma_tf32_ss2<false>(d, ab + ring * RING_STEP, a_hi, bbl + ta * tap_step, b_hi, id_f);
+                            else
+                                umma_tf32_ss2<true>(d, ab + ring * RING_STEP, a_hi, bbl + ta * tap_step, b_hi, id_f);
                         }
                     }
                 }
@@ -685,11 +706,13 @@ stage_tc_kernel(StageArgs a, const unsigned char* __restrict__ ws, int nkp_all, 
                 for (int rr = 1; rr >= 0; --rr) {                        // row 1 first: it initialises blocks 0 .. KS
                     const uint32_t d = tmem + TC_TCOL + (rr == 0 ? 8 : 0);
                     const uint32_t av = tmem + bb * 4 * nkp + rr * 2 * nkp;
-                    for (int pass = 0; pass < 2; ++pass)
-                        for (int ks = 0; ks < nkp / 4; ++ks)
-                            umma_bf16_ts(d, av + 8 * ks,
-                                         umma_desc(sbase + C::SM_BS + ((pass * (nkp / 2) + 2 * ks) * C::NSC) * 16, C::NSC * 16, 128),
-                                         id_s, (rr == 1 && pass == 0 && ks == 0) ? 0u : 1u);
+                    for (int pass = 0; pass < 2; ++pass) {
+                        uint32_t bl = s_lo + ((pass * (nkp / 2)) * C::NSC);      // in 16-byte units: one K chunk = NSC cells
+                        for (int ks = 0; ks < nkp / 4; ++ks, bl += 2 * C::NSC) {
+                            if (rr == 1 && pass == 0 && ks == 0) umma_bf16_ts2<false>(d, av, bl, s_hi, id_s);
+                            else umma_bf16_ts2<true>(d, av + 8 * ks, bl, s_hi, id_s);
+                        }
+                    }
                 }
                 umma_commit(tfull);
                 if (b + 2 < NB) { wait_pair(b + 2 + R); tc_fence_after(); forward(b + 2); }
